@@ -1,0 +1,282 @@
+/*
+ * heeps_oracle.c -- plain, slow, fp64 CPU oracle of the raw-data generator hot path.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Nothing in the product path (paper_2405_09938_b200/) may
+ * include, link, import or execute this file; only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs call it.  It shares no code, header,
+ * table or constant generator with the CUDA path.
+ *
+ * What it computes (BASELINE.json north_star; scalar form of PAPER.md eq. (3) line 91 and
+ * eq. (16), with the range-slice sum of eq. (17) lines 204-209 written out as
+ * explicit chirp replicas -- the paper convolves the sliced impulse response with the
+ * waveform afterwards):
+ *
+ *   s_{c,p}[n] = sum_f a_f G_tx G_rx exp(-j 2 pi f0 tau_f)
+ *                      rect((t_n - tau_f)/T) exp(j pi K (t_n - tau_f)^2),   t_n = t0[p] + n/fs
+ *
+ * evaluated term by term in the order O1..O10 of SURVEY.md §8(c), every transcendental
+ * through libm in double (long double for frac(f0 tau)), one complex exponential per
+ * facet-sample, no recurrences, no tables, no blocking.  The only concession to run time
+ * is an OpenMP split of the facet loop with per-thread accumulators (a sum is a sum).
+ *
+ * Readings of the paper taken here are the G-numbered ones of SURVEY.md §8(c), listed in
+ * DESIGN.md §"Readings":  G1 t_n origin, G2 half-open rect and up-chirp, G3 carrier sign,
+ * G4 no 1/(r_t r_r), G5 signed field pattern sinc*sinc, G6 cull on |G_t G_r,ref| from the
+ * un-offset phase centre, G8 offsets along the Rx unit velocity, G9 stop-and-go,
+ * G10 current by advection, G11 linear waves (CWM by flag), G12 tilt factor clamped at 0,
+ * G15 A = d^2, G24 displaced point feeds the antenna direction.
+ *
+ * Pins: tests/test_oracle_pins.py (closed forms with mpmath, invariants, brute force by an
+ * independent numpy script).  No function here is "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORACLE_C0 299792458.0
+
+typedef struct {
+    /* instrument */
+    double f0_hz, chirp_rate, chirp_len_s, fs_hz;
+    int32_t n_samples, n_channels;
+    double tx_aperture[2], rx_aperture[2];      /* {azimuth length, elevation height} */
+    const double *channel_offset_m;             /* [C] */
+    double cull_two_way_db;                     /* <= -300 disables */
+    /* geometry */
+    int32_t n_pulses;
+    const double *t_pulse_s;                    /* [P] */
+    const double *tx_pos, *tx_vel, *rx_pos, *rx_vel;   /* [P][3] */
+    const double *tx_frame, *rx_frame;          /* [P][3][3] rows: boresight, azimuth, elevation */
+    const double *t0_s;                         /* [P] */
+    /* scene */
+    int32_t nx, ny;
+    double spacing_m, centre_m[3];
+    int32_t n_waves;
+    const double *kx, *ky, *amp, *omega, *phase;/* [Nw] */
+    int32_t choppy;
+    const float *sigma0_lin;  double sigma0_uniform;   /* [ny][nx] or NULL */
+    int32_t tilt_modulation;  double look_dir[2];
+    const float *current_mps; double current_uniform[2]; /* [ny][nx][2] or NULL */
+    const float *xi;                            /* [ny][nx][2], required */
+} oracle_desc;
+
+/* per-facet intermediates of one pulse (O2..O8), exposed for unit parity */
+typedef struct {
+    double *pos;      /* [F][3]  displaced facet position x_f                */
+    double *slope;    /* [F][2]  grad z                                      */
+    double *vel;      /* [F][3]  facet velocity (orbital + current)          */
+    double *tau;      /* [C][F]  bistatic delay                              */
+    double *g_tx;     /* [F]                                                 */
+    double *g_rx;     /* [C][F]                                              */
+    double *amp;      /* [C][F][2] complex A~ = a G_t G_r exp(-j2pi f0 tau)  */
+    int32_t *keep;    /* [F]     1 = survives the cull                       */
+} oracle_facets;
+
+static double sinc_pi(double x)
+{   /* sin(pi x)/(pi x), sinc(0) = 1  (O6) */
+    if (x == 0.0) return 1.0;
+    double a = M_PI * x;
+    return sin(a) / a;
+}
+
+static double dot3(const double *a, const double *b) { return a[0]*b[0] + a[1]*b[1] + a[2]*b[2]; }
+
+/* O6: G = sinc(La (u.a)/lambda) sinc(Le (u.e)/lambda), frame rows {b, a, e} */
+static double gain(const double *u, const double *frame, const double *aperture, double lambda)
+{
+    double ua = dot3(u, frame + 3), ue = dot3(u, frame + 6);
+    return sinc_pi(aperture[0] * ua / lambda) * sinc_pi(aperture[1] * ue / lambda);
+}
+
+typedef struct {
+    double pos[3], slope[2], vel[3];
+    double tau[8], g_tx, g_rx[8], amp_re[8], amp_im[8];
+    int keep;
+} facet_eval;
+
+/* O1..O8 for facet (i,j) at pulse p.  Channels limited to 8. */
+static void eval_facet(const oracle_desc *d, int p, int i, int j, facet_eval *o)
+{
+    const double t = d->t_pulse_s[p];
+    const double lambda = ORACLE_C0 / d->f0_hz;
+    /* O1 rest point */
+    double xb = d->centre_m[0] + (i - (d->nx - 1) / 2.0) * d->spacing_m;
+    double yb = d->centre_m[1] + (j - (d->ny - 1) / 2.0) * d->spacing_m;
+    /* O2 wave sums (linear surface, CWM horizontal displacement by flag) */
+    double z = 0, sx = 0, sy = 0, dx = 0, dy = 0, vx = 0, vy = 0, vz = 0;
+    for (int w = 0; w < d->n_waves; ++w) {
+        double k = hypot(d->kx[w], d->ky[w]);
+        double psi = d->kx[w] * xb + d->ky[w] * yb - d->omega[w] * t + d->phase[w];
+        double c = cos(psi), s = sin(psi), a = d->amp[w];
+        z  += a * c;
+        sx -= a * d->kx[w] * s;
+        sy -= a * d->ky[w] * s;
+        vz += a * d->omega[w] * s;
+        if (d->choppy && k > 0) {
+            dx -= a * d->kx[w] / k * s;
+            dy -= a * d->ky[w] / k * s;
+            vx += a * d->omega[w] * d->kx[w] / k * c;
+            vy += a * d->omega[w] * d->ky[w] / k * c;
+        }
+    }
+    double cx = d->current_uniform[0], cy = d->current_uniform[1];
+    if (d->current_mps) {
+        cx = d->current_mps[((size_t)j * d->nx + i) * 2 + 0];
+        cy = d->current_mps[((size_t)j * d->nx + i) * 2 + 1];
+    }
+    /* O3 displaced position; current by advection (G10; first order = eq. (4)) */
+    o->pos[0] = xb + dx + cx * t;
+    o->pos[1] = yb + dy + cy * t;
+    o->pos[2] = d->centre_m[2] + z;
+    o->slope[0] = sx; o->slope[1] = sy;
+    o->vel[0] = vx + cx; o->vel[1] = vy + cy; o->vel[2] = vz;
+    /* O4 transmit leg */
+    const double *ptx = d->tx_pos + 3 * p, *prx = d->rx_pos + 3 * p, *vrx = d->rx_vel + 3 * p;
+    double dt[3] = { o->pos[0] - ptx[0], o->pos[1] - ptx[1], o->pos[2] - ptx[2] };
+    double rt = sqrt(dot3(dt, dt));
+    double ut[3] = { dt[0] / rt, dt[1] / rt, dt[2] / rt };
+    o->g_tx = gain(ut, d->tx_frame + 9 * p, d->tx_aperture, lambda);
+    /* O7 cull on the un-offset receive phase centre (G6) */
+    double dr0[3] = { o->pos[0] - prx[0], o->pos[1] - prx[1], o->pos[2] - prx[2] };
+    double rr0 = sqrt(dot3(dr0, dr0));
+    double ur0[3] = { dr0[0] / rr0, dr0[1] / rr0, dr0[2] / rr0 };
+    double g_ref = gain(ur0, d->rx_frame + 9 * p, d->rx_aperture, lambda);
+    o->keep = 1;
+    if (d->cull_two_way_db > -300.0) {
+        double thr = pow(10.0, d->cull_two_way_db / 20.0);
+        if (fabs(o->g_tx * g_ref) < thr) o->keep = 0;
+    }
+    /* O8 amplitude a = sqrt(sigma d^2) xi   (G15, G12) */
+    double sigma = d->sigma0_lin ? (double)d->sigma0_lin[(size_t)j * d->nx + i] : d->sigma0_uniform;
+    if (d->tilt_modulation) {
+        double f = 1.0 + 2.0 * (sx * d->look_dir[0] + sy * d->look_dir[1]);
+        sigma *= (f > 0.0 ? f : 0.0);
+    }
+    double a0 = sqrt(sigma * d->spacing_m * d->spacing_m);
+    double xr = d->xi[((size_t)j * d->nx + i) * 2 + 0], xim = d->xi[((size_t)j * d->nx + i) * 2 + 1];
+    double vn = sqrt(dot3(vrx, vrx));
+    for (int c = 0; c < d->n_channels; ++c) {
+        /* O4 receive leg: phase centre offset along the Rx unit velocity (G8) */
+        double pc[3] = { prx[0] + d->channel_offset_m[c] * vrx[0] / vn,
+                         prx[1] + d->channel_offset_m[c] * vrx[1] / vn,
+                         prx[2] + d->channel_offset_m[c] * vrx[2] / vn };
+        double dr[3] = { o->pos[0] - pc[0], o->pos[1] - pc[1], o->pos[2] - pc[2] };
+        double rr = sqrt(dot3(dr, dr));
+        double ur[3] = { dr[0] / rr, dr[1] / rr, dr[2] / rr };
+        double gr = gain(ur, d->rx_frame + 9 * p, d->rx_aperture, lambda);
+        /* O5 */
+        double tau = (rt + rr) / ORACLE_C0;
+        /* carrier phase -2 pi frac(f0 tau), long double for the 2.8e7-cycle product (G3) */
+        long double cyc = (long double)d->f0_hz * (long double)tau;
+        double fr = (double)(cyc - floorl(cyc));
+        double ph = -2.0 * M_PI * fr;
+        double g = a0 * o->g_tx * gr;
+        double ar = g * xr, ai = g * xim;
+        o->tau[c] = tau;
+        o->g_rx[c] = gr;
+        o->amp_re[c] = ar * cos(ph) - ai * sin(ph);
+        o->amp_im[c] = ar * sin(ph) + ai * cos(ph);
+    }
+}
+
+/* O9: add one facet-echo into acc[Ns][2] (interleaved re, im). */
+static void add_echo(const oracle_desc *d, int p, double tau, double are, double aim, double *acc)
+{
+    const double T = d->chirp_len_s, K = d->chirp_rate, fs = d->fs_hz, t0 = d->t0_s[p];
+    /* candidate samples: everything within one sample of the replica support */
+    double centre = (tau - t0) * fs;
+    long n_lo = (long)floor(centre - 0.5 * T * fs) - 2;
+    long n_hi = (long)ceil(centre + 0.5 * T * fs) + 2;
+    if (n_lo < 0) n_lo = 0;
+    if (n_hi > d->n_samples - 1) n_hi = d->n_samples - 1;
+    for (long n = n_lo; n <= n_hi; ++n) {
+        double u = (t0 + (double)n / fs) - tau;
+        if (u >= -0.5 * T && u < 0.5 * T) {           /* rect, half-open (G2) */
+            double ph = M_PI * K * u * u;
+            double c = cos(ph), s = sin(ph);
+            acc[2 * n]     += are * c - aim * s;
+            acc[2 * n + 1] += are * s + aim * c;
+        }
+    }
+}
+
+/*
+ * heeps_oracle_generate: out[C][n_sel][Ns][2] (double re,im) for the listed pulses.
+ * Returns 0, or -1 on bad arguments.
+ */
+int heeps_oracle_generate(const oracle_desc *d, const int32_t *pulses, int32_t n_sel, double *out,
+                          int32_t n_threads)
+{
+    if (!d || !pulses || !out || d->n_channels < 1 || d->n_channels > 8 || !d->xi) return -1;
+    const int C = d->n_channels, Ns = d->n_samples;
+    const size_t vec = (size_t)Ns * 2;
+    memset(out, 0, sizeof(double) * vec * C * n_sel);
+#ifdef _OPENMP
+    if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+    for (int s = 0; s < n_sel; ++s) {
+        const int p = pulses[s];
+        if (p < 0 || p >= d->n_pulses) return -1;
+#pragma omp parallel
+        {
+            double *acc = (double *)calloc(vec * C, sizeof(double));
+#pragma omp for schedule(static)
+            for (int j = 0; j < d->ny; ++j) {
+                for (int i = 0; i < d->nx; ++i) {
+                    facet_eval fe;
+                    eval_facet(d, p, i, j, &fe);
+                    if (!fe.keep) continue;                       /* O7 */
+                    for (int c = 0; c < C; ++c)
+                        add_echo(d, p, fe.tau[c], fe.amp_re[c], fe.amp_im[c], acc + vec * c);
+                }
+            }
+#pragma omp critical
+            {
+                for (int c = 0; c < C; ++c) {
+                    double *o = out + ((size_t)c * n_sel + s) * vec;
+                    for (size_t k = 0; k < vec; ++k) o[k] += acc[vec * c + k];
+                }
+            }
+            free(acc);
+        }
+    }
+    return 0;
+}
+
+/* heeps_oracle_facets: O2..O8 intermediates of one pulse (any pointer may be NULL). */
+int heeps_oracle_facets(const oracle_desc *d, int32_t p, oracle_facets *o)
+{
+    if (!d || !o || p < 0 || p >= d->n_pulses || d->n_channels > 8 || !d->xi) return -1;
+    const size_t F = (size_t)d->nx * d->ny;
+#pragma omp parallel for schedule(static)
+    for (int j = 0; j < d->ny; ++j)
+        for (int i = 0; i < d->nx; ++i) {
+            facet_eval fe;
+            eval_facet(d, p, i, j, &fe);
+            size_t f = (size_t)j * d->nx + i;
+            if (o->pos)   for (int k = 0; k < 3; ++k) o->pos[3 * f + k] = fe.pos[k];
+            if (o->slope) for (int k = 0; k < 2; ++k) o->slope[2 * f + k] = fe.slope[k];
+            if (o->vel)   for (int k = 0; k < 3; ++k) o->vel[3 * f + k] = fe.vel[k];
+            if (o->g_tx)  o->g_tx[f] = fe.g_tx;
+            if (o->keep)  o->keep[f] = fe.keep;
+            for (int c = 0; c < d->n_channels; ++c) {
+                if (o->tau)  o->tau[c * F + f] = fe.tau[c];
+                if (o->g_rx) o->g_rx[c * F + f] = fe.g_rx[c];
+                if (o->amp) { o->amp[2 * (c * F + f)] = fe.amp_re[c]; o->amp[2 * (c * F + f) + 1] = fe.amp_im[c]; }
+            }
+        }
+    return 0;
+}
+
+int heeps_oracle_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
