@@ -1,0 +1,166 @@
+/*
+ * heeps_sim.h -- C ABI of the B200-native HEEPS/MARE raw-data generator hot path.
+ *
+ * The library computes, for every pulse p and receive phase-centre channel c, the complex
+ * IQ samples
+ *
+ *   s_{c,p}[n] = sum_f a_f G_tx G_rx exp(-j 2 pi f0 tau_f)
+ *                      rect((t_n - tau_f)/T) exp(j pi K (t_n - tau_f)^2),  t_n = t0[p] + n/fs
+ *
+ * (BASELINE.json north_star; scalar form of PAPER.md eq. (3) line 91 and eq. (16);
+ * the range-slice sum of eq. (17), with the waveform convolution written
+ * out).  Every step runs in hand-written CUDA kernels for sm_100a:
+ *   K1 facet kinematics            (PAPER.md:53-55   surface = sum of wave components)
+ *   K2 geometry + gains + amplitude + cull + tile bucketing
+ *                                  (PAPER.md:91-98 ranges/phase, :202 antenna patterns, :223 contributing subset)
+ *   K3 echo accumulation
+ *   K4 finalize                    (raw data output)
+ *
+ * Conventions
+ *   - All descriptor arrays are HOST pointers, C order, copied during sim_create (the caller
+ *     may free them after it returns).  Units: SI (m, s, Hz, m/s); sigma0 linear (not dB).
+ *   - Frame arrays are [P][3][3] with rows {boresight, azimuth axis, elevation axis}, unit,
+ *     mutually orthogonal (checked to 1e-6).
+ *   - Facet (i,j), i fastest, rest position centre + ((i-(nx-1)/2) d, (j-(ny-1)/2) d, 0).
+ *   - Output is complex64 [C][pulse_end-pulse_begin][Ns], interleaved (re,im) float32.
+ *   - Return value 0 on success, a negative SIM_E* code otherwise.  Nothing is printed, no
+ *     exception or abort crosses the boundary.  A handle is not thread-safe; distinct
+ *     handles are independent.  There is no CPU fallback: without a CUDA device every
+ *     compute entry point returns SIM_ECUDA.
+ *   - Echo samples falling outside [0, Ns) are clipped silently (not an error).
+ */
+#ifndef HEEPS_SIM_H
+#define HEEPS_SIM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SIM_OK        0
+#define SIM_EINVAL   (-1)   /* null pointer, bad size, NaN, non-orthonormal frame, > SIM_MAX_CHANNELS */
+#define SIM_ERANGE   (-2)   /* pulse range outside [0, P] or empty-inverted */
+#define SIM_ENOMEM   (-3)   /* host or device allocation failed */
+#define SIM_ECUDA    (-4)   /* CUDA runtime error; see sim_last_cuda_error */
+
+#define SIM_MAX_CHANNELS 8
+
+typedef struct sim_handle sim_handle;        /* opaque, owned by the library */
+
+/* Instrument (BASELINE.json north_star (d): carrier, chirp rate/length, fs, PRF, apertures, offsets) */
+typedef struct {
+    double f0_hz;                  /* carrier */
+    double chirp_rate_hz_per_s;    /* K = B/T, > 0 up-chirp; p(t) = rect(t/T) exp(j pi K t^2)  (reading G2) */
+    double chirp_len_s;            /* T */
+    double fs_hz;                  /* complex sampling rate */
+    double prf_hz;                 /* informational; pulse times come from sim_geometry */
+    int32_t n_samples;             /* Ns fast-time samples per pulse */
+    double tx_aperture_m[2];       /* {azimuth length, elevation height}; field pattern sinc*sinc (G5); 0 = isotropic */
+    double rx_aperture_m[2];
+    int32_t n_channels;            /* C, 1..SIM_MAX_CHANNELS */
+    const double *channel_offset_m;/* [C] host; along-track offsets about the Rx state vector (G8) */
+    double cull_two_way_db;        /* facet dropped for all channels iff 20log10|G_t G_r,ref| < this; <= -300 disables (G6) */
+} sim_instrument;
+
+/* Geometry: per-pulse Tx/Rx state vectors (stop-and-go, reading G9) */
+typedef struct {
+    int32_t n_pulses;              /* P */
+    const double *t_pulse_s;       /* [P] time at which the scene is frozen for pulse p */
+    const double *tx_pos_m, *tx_vel_mps, *rx_pos_m, *rx_vel_mps;   /* [P][3] each */
+    const double *tx_frame, *rx_frame;                             /* [P][3][3] */
+    const double *t0_s;            /* [P] time of sample 0 after the Tx chirp centre (G1) */
+} sim_geometry;
+
+/* Scene: facet grid, wave components, sigma0 / current / speckle fields */
+typedef struct {
+    int32_t nx, ny;
+    double spacing_m;              /* d; facet area A = d^2 (G15) */
+    double centre_m[3];
+    int32_t n_waves;               /* Nw >= 0 */
+    const double *kx, *ky, *amp, *omega, *phase;   /* [Nw] host; z = sum A cos(kx x + ky y - omega t + phase) */
+    int32_t choppy;                /* 0 linear surface; 1 Choppy Wave Model horizontal displacement */
+    const float *sigma0_lin;       /* [ny][nx] host or NULL -> sigma0_uniform */
+    double sigma0_uniform;
+    int32_t tilt_modulation;       /* sigma0 *= max(0, 1 + 2 grad z . look_dir)  (G12) */
+    double look_dir[2];            /* horizontal unit vector radar -> scene */
+    const float *current_mps;      /* [ny][nx][2] host or NULL -> current_uniform; applied by advection (G10) */
+    double current_uniform[2];
+    const float *xi;               /* [ny][nx][2] host complex speckle, or NULL -> derived from seed (G14) */
+    uint64_t seed;
+} sim_scene;
+
+/* Tunables; zero-initialise for defaults. */
+typedef struct {
+    int32_t tile_facets;           /* spatial tile side in facets (8..64, power of 2); 0 = auto from L and spacing */
+    int32_t pulses_per_batch;      /* 0 = auto from workspace_bytes */
+    int64_t workspace_bytes;       /* cap for per-batch device workspace; 0 = 4 GiB */
+    int32_t reserved[8];
+} sim_options;
+
+/*
+ * sim_create: validate descriptors, upload tables, allocate the per-batch workspace on CUDA
+ * device `device`.  *out receives the handle.  opts may be NULL.
+ */
+int sim_create(const sim_instrument *inst, const sim_geometry *geo, const sim_scene *scene,
+               const sim_options *opts, int device, sim_handle **out);
+
+/*
+ * sim_generate: IQ for pulses [pulse_begin, pulse_end) into caller-owned DEVICE memory
+ * iq_dev (complex64 [C][pulse_end-pulse_begin][Ns]); asynchronous on cuda_stream (a
+ * cudaStream_t, NULL = default stream); overwrites, never accumulates into, iq_dev;
+ * idempotent per pulse range (that is the restart story).
+ */
+int sim_generate(sim_handle *h, int32_t pulse_begin, int32_t pulse_end, void *iq_dev, void *cuda_stream);
+
+/*
+ * sim_generate_host: same, but iq_host is HOST memory (pinned memory gives an asynchronous
+ * copy); the device->host copy is issued on cuda_stream and the call returns after the
+ * stream has been synchronised.  Used for the end-to-end measurement.
+ */
+int sim_generate_host(sim_handle *h, int32_t pulse_begin, int32_t pulse_end, void *iq_host, void *cuda_stream);
+
+/*
+ * sim_update_scene: replace the per-facet maps from HOST arrays (any may be NULL = keep):
+ * sigma0 [ny][nx], current [ny][nx][2], xi [ny][nx][2]; host->device copies on cuda_stream.
+ * A map that was NULL (uniform) at sim_create cannot be introduced later (SIM_EINVAL).
+ */
+int sim_update_scene(sim_handle *h, const float *sigma0_lin, const float *current_mps, const float *xi,
+                     void *cuda_stream);
+
+/* sim_replica: the transmitted waveform samples exp(j pi K (m/fs - T/2)^2), m = 0..*n-1 (PAPER.md:209:
+ * "raw data are output together with the waveforms").  host_c64_out may be NULL to query *n. */
+int sim_replica(const sim_handle *h, float *host_c64_out, int32_t *n);
+
+/* Per-facet intermediates of one pulse for unit parity (host arrays, any may be NULL):
+ * pos [F][3], slope [F][2], tau [C][F], g_tx [F], g_rx [C][F], amp [C][F][2] (= a G_t G_r exp(-j2pi f0 tau)),
+ * keep [F] (int32).  Synchronous. */
+int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, double *tau, double *g_tx,
+                     double *g_rx, double *amp, int32_t *keep);
+
+/* Counters of the most recent sim_generate* call (after the stream has completed). */
+typedef struct {
+    int64_t facet_echoes_nominal;  /* F * pulses * C                                   */
+    int64_t facet_echoes_kept;     /* after the cull                                   */
+    int64_t facet_samples;         /* sum over kept facet-echoes of in-window samples  */
+    int64_t kernel_launches;       /* kernels launched by the call                     */
+    int32_t tile_facets, pulses_per_batch, n_tiles, accumulate_block_threads;
+    int32_t max_span_samples;      /* largest per-tile sample span seen                */
+    int32_t reserved[3];
+} sim_stats;
+int sim_get_stats(sim_handle *h, sim_stats *out);
+
+/* Per-kernel device time of the most recent call, measured with CUDA events on the caller's
+ * stream when enabled (adds event records only): ms[0..3] = K1, K2, K3, K4 totals. */
+int sim_set_profiling(sim_handle *h, int32_t enable);
+int sim_get_kernel_ms(sim_handle *h, float ms[4]);
+
+void sim_destroy(sim_handle *h);
+const char *sim_error_string(int code);
+/* Text of the last CUDA error seen by this handle ("" if none). Valid until the next call on h. */
+const char *sim_last_cuda_error(const sim_handle *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HEEPS_SIM_H */

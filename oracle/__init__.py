@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     build_oracle,
     oracle_generate,
     oracle_facets,
+    oracle_samples,
     oracle_max_threads,
     rel_l2_per_vector,
     ati_phase,

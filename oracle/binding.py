@@ -67,6 +67,8 @@ def _load():
         _lib.heeps_oracle_facets.restype = C.c_int
         _lib.heeps_oracle_facets.argtypes = [C.POINTER(_Desc), C.c_int32, C.POINTER(_Facets)]
         _lib.heeps_oracle_max_threads.restype = C.c_int
+        _lib.heeps_oracle_samples.restype = C.c_int
+        _lib.heeps_oracle_samples.argtypes = [C.POINTER(_Desc), C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32]
     return _lib
 
 
@@ -146,6 +148,19 @@ def oracle_generate(w, pulses=None, n_threads: int = 0) -> np.ndarray:
         raise ValueError(f"heeps_oracle_generate failed ({rc})")
     del keep
     return out
+
+
+def oracle_samples(w, pulse: int, samples, n_threads: int = 0) -> np.ndarray:
+    """complex128 [C][len(samples)]: the defined sum at the listed fast-time samples of one pulse."""
+    lib = _load()
+    d, keep = _marshal(w)
+    samples = np.ascontiguousarray(np.asarray(samples, dtype=np.int32))
+    out = np.zeros((d.n_channels, samples.size, 2), dtype=np.float64)
+    rc = lib.heeps_oracle_samples(C.byref(d), int(pulse), samples.ctypes.data, samples.size, out.ctypes.data, n_threads)
+    if rc != 0:
+        raise ValueError(f"heeps_oracle_samples failed ({rc})")
+    del keep
+    return out[..., 0] + 1j * out[..., 1]
 
 
 def oracle_facets(w, pulse: int) -> dict:

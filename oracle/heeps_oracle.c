@@ -247,6 +247,48 @@ int heeps_oracle_generate(const oracle_desc *d, const int32_t *pulses, int32_t n
     return 0;
 }
 
+/*
+ * heeps_oracle_samples: the same defined sum, but only for the listed output samples n_list[0..count)
+ * of one pulse: out[C][count][2].  Lets the tests check full-size configurations sample by sample
+ * (every facet is still evaluated; only the O9 loop is restricted to the listed n).
+ */
+int heeps_oracle_samples(const oracle_desc *d, int32_t p, const int32_t *n_list, int32_t count, double *out,
+                         int32_t n_threads)
+{
+    if (!d || !n_list || !out || p < 0 || p >= d->n_pulses || d->n_channels > 8 || !d->xi || count < 1) return -1;
+    const int C = d->n_channels;
+    const double T = d->chirp_len_s, K = d->chirp_rate, fs = d->fs_hz, t0 = d->t0_s[p];
+    memset(out, 0, sizeof(double) * 2 * C * count);
+#ifdef _OPENMP
+    if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+#pragma omp parallel
+    {
+        double *acc = (double *)calloc((size_t)2 * C * count, sizeof(double));
+#pragma omp for schedule(static)
+        for (int j = 0; j < d->ny; ++j)
+            for (int i = 0; i < d->nx; ++i) {
+                facet_eval fe;
+                eval_facet(d, p, i, j, &fe);
+                if (!fe.keep) continue;
+                for (int c = 0; c < C; ++c)
+                    for (int q = 0; q < count; ++q) {
+                        double u = (t0 + (double)n_list[q] / fs) - fe.tau[c];
+                        if (u >= -0.5 * T && u < 0.5 * T) {
+                            double ph = M_PI * K * u * u;
+                            double cs = cos(ph), sn = sin(ph);
+                            acc[2 * (c * count + q)]     += fe.amp_re[c] * cs - fe.amp_im[c] * sn;
+                            acc[2 * (c * count + q) + 1] += fe.amp_re[c] * sn + fe.amp_im[c] * cs;
+                        }
+                    }
+            }
+#pragma omp critical
+        for (int k = 0; k < 2 * C * count; ++k) out[k] += acc[k];
+        free(acc);
+    }
+    return 0;
+}
+
 /* heeps_oracle_facets: O2..O8 intermediates of one pulse (any pointer may be NULL). */
 int heeps_oracle_facets(const oracle_desc *d, int32_t p, oracle_facets *o)
 {

@@ -1,0 +1,62 @@
+// Shared device-side data layout of the raw-data generator kernels (K1..K4).
+// Nothing here is shared with oracle/ (the oracle is an independent C file).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace heeps {
+
+constexpr int kMaxChannels = 8;
+constexpr double kC0 = 299792458.0;
+
+// Per-pulse constants, computed on the host in fp64 at sim_create (stop-and-go, G9).
+struct PulseConst {
+    double t;                    // t_pulse[p]
+    double r0;                   // c0 * t0[p]: bistatic path length of sample 0
+    double tx_pos[3];
+    double tx_a[3], tx_e[3];     // Tx azimuth / elevation axes
+    double rx_a[3], rx_e[3];
+    double rx_ref[3];            // un-offset Rx phase centre (cull reference, G6)
+    double rx_pos[kMaxChannels][3];   // P_rx + o_c * v_rx/|v_rx|   (G8)
+};
+
+// One surviving facet-echo as the accumulation kernel consumes it (32 B, 16 B aligned).
+// Phase of sample n in turns:  phi + beta*(n - n_mid)  [+ kappa (n-n_mid)^2 applied in K4],
+// in 32-bit fixed point (2^-32 turn); valid for n in [b, b+cnt).
+struct __align__(16) Rec {
+    uint32_t phi;                // frac(-dR/lambda + kappa c'^2) * 2^32 + bias (geometry.cu kPhiBias),  c' = echo centre - n_mid [samples]
+    uint32_t beta;               // frac(-2 kappa c') * 2^32
+    float ar, ai;                // A~ = a_f G_tx G_rx,c  (complex, without the carrier phase)
+    float wr, wi;                // exp(j 2 pi beta): one-sample phase step
+    int32_t b;                   // first in-window sample n_first = ceil(nu)
+    int32_t cnt;                 // number of in-window samples (floor or ceil of T*fs)
+};
+static_assert(sizeof(Rec) == 32, "Rec must be 32 bytes");
+
+struct TileInfo {               // per (pulse-in-batch, tile)
+    int32_t nrec;               // surviving facets (same for every channel)
+};
+struct TileSpan {               // per (channel, pulse-in-batch, tile)
+    int32_t bmin, bmax_end;     // min b and max (b+cnt) over the tile's records
+};
+
+// Scalars every kernel needs.
+struct DevParams {
+    // grid / tiling
+    int32_t nx, ny, tile, tiles_x, tiles_y, n_tiles, tile_cap;
+    double spacing, cx, cy, cz;
+    // instrument
+    int32_t n_samples, n_channels, n_mid;
+    double inv_lambda;           // f0/c0
+    double fs_over_c0;           // samples per metre of bistatic path
+    double kappa;                // K/(2 fs^2) turns per sample^2
+    double half_len;             // T*fs/2 [samples]
+    double len;                  // T*fs [samples]
+    double ap_tx_a, ap_tx_e, ap_rx_a, ap_rx_e;   // aperture/lambda
+    float cull_thr;              // 10^(dB/20) or 0
+    // scene
+    int32_t n_waves, choppy, tilt, has_sigma0, has_current;
+    double sigma0_uniform, look_x, look_y, cur_ux, cur_uy;
+};
+
+}  // namespace heeps

@@ -1,0 +1,65 @@
+// Launch wrappers of the four hot-path kernels (implemented in the .cu files beside this header).
+#pragma once
+#include "heeps_common.cuh"
+
+namespace heeps {
+
+// K1 -- facet kinematics (kinematics.cu).  One launch covers `n_pl` pulses starting at pulse p0.
+struct KinematicsArgs {
+    const double2 *xt;      // [Nw][nx]  A_w exp(j kx_w x_i)
+    const double2 *yt;      // [Nw][ny]  exp(j (ky_w y_j + phase_w))
+    const double2 *tt;      // [Nw][P]   exp(-j omega_w t_p)
+    const float4 *wk;       // [Nw]      {kx, ky, kx/|k|, ky/|k|}
+    int32_t n_pulses_total; // P (row stride of tt)
+    double *z;              // [n_pl][F]            surface height above centre_z
+    float2 *slope;          // [n_pl][F] or null    grad z
+    double2 *dxy;           // [n_pl][F] or null    CWM horizontal displacement
+};
+cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a, int p0, int n_pl, cudaStream_t s);
+
+// K2 -- geometry, gains, amplitude, cull, tile bucketing (geometry.cu).
+struct GeometryArgs {
+    const PulseConst *pulses;   // [P]
+    const double *z;            // from K1
+    const float2 *slope;        // or null
+    const double2 *dxy;         // or null
+    const float *sigma0;        // [F] or null
+    const float2 *current;      // [F] or null
+    const float2 *xi;           // [F]
+    Rec *recs;                  // [C][n_pl][n_tiles][tile_cap]
+    TileInfo *tinfo;            // [n_pl][n_tiles]
+    TileSpan *tspan;            // [C][n_pl][n_tiles]
+    unsigned long long *counters;  // [2]: kept facet-echoes, facet-samples (in-window, clipped to [0,Ns))
+    // optional per-facet debug outputs (spatial order, single pulse): any may be null
+    double *dbg_pos, *dbg_tau, *dbg_gtx, *dbg_grx, *dbg_amp;
+    int32_t *dbg_keep;
+    const double *carrier_frac_t0;  // [P] frac(f0 t0[p]) (debug amp only)
+};
+cudaError_t launch_geometry(const DevParams &prm, const GeometryArgs &a, int p0, int n_pl, cudaStream_t s);
+
+// K3 -- echo accumulation, direct form (accumulate.cu).
+struct AccumulateArgs {
+    const Rec *recs;
+    const TileInfo *tinfo;
+    const TileSpan *tspan;
+    double2 *acc;               // [C][n_pl][Ns] complex128 accumulators (zeroed by the caller)
+    int block_threads;          // multiple of 32
+};
+cudaError_t launch_accumulate(const DevParams &prm, const AccumulateArgs &a, int n_pl, cudaStream_t s);
+
+// K4 -- finalize (finalize.cu): out = acc * exp(j 2 pi kappa (n-n_mid)^2) * exp(-j 2 pi f0 t0[p]) -> complex64
+struct FinalizeArgs {
+    const double2 *acc;         // [C][n_pl][Ns]
+    const double2 *chirp_n;     // [Ns]  exp(j 2 pi kappa (n - n_mid)^2)
+    const double2 *carrier_p;   // [P]   exp(-j 2 pi f0 t0[p])
+    float2 *out;                // [C][n_out_pulses][Ns]
+    int32_t n_out_pulses;       // pulse stride of `out`
+    int32_t out_pulse0;         // index in `out` of the batch's first pulse
+};
+cudaError_t launch_finalize(const DevParams &prm, const FinalizeArgs &a, int p0, int n_pl, cudaStream_t s);
+
+// Speckle from seed (G14): xi[f] = circular complex Gaussian, variance 1/2 per part, Philox4x32-10
+// keyed by seed, counter = facet index, Box-Muller.
+cudaError_t launch_speckle_from_seed(float2 *xi, int64_t n_facets, uint64_t seed, cudaStream_t s);
+
+}  // namespace heeps

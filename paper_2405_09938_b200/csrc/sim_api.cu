@@ -1,0 +1,589 @@
+// Host runtime + C ABI (include/heeps_sim.h) of the raw-data generator.
+// Owns the device tables and the per-batch workspace, and sequences K1..K4 per pulse batch on
+// the caller's stream with no host synchronisation inside sim_generate.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/heeps_sim.h"
+#include "kernels.cuh"
+
+using namespace heeps;
+
+namespace {
+
+constexpr int kAccumR = 8;           // samples per thread in K3 (must match accumulate.cu)
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; prev = -1; }
+        if (ok && prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+template <typename T>
+struct DevBuf {
+    T *p = nullptr;
+    size_t n = 0;
+    cudaError_t alloc(size_t count)
+    {
+        release();
+        if (count == 0) return cudaSuccess;
+        cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&p), count * sizeof(T));
+        if (e == cudaSuccess) n = count; else p = nullptr;
+        return e;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; n = 0; }
+};
+
+}  // namespace
+
+struct sim_handle {
+    int device = 0;
+    DevParams prm{};
+    int n_pulses = 0;
+    int64_t n_facets = 0;
+    double chirp_rate = 0, chirp_len = 0, fs = 0;
+    int pulses_per_batch = 1;
+    int accum_threads = 32;
+    bool need_slope = false;
+
+    // tables
+    DevBuf<double2> xt, yt, tt, chirp_n, carrier_p;
+    DevBuf<float4> wk;
+    DevBuf<double> carrier_frac;
+    DevBuf<PulseConst> pulses;
+    // maps
+    DevBuf<float> sigma0;
+    DevBuf<float2> current, xi;
+    // workspace
+    DevBuf<double> z;
+    DevBuf<float2> slope;
+    DevBuf<double2> dxy;
+    DevBuf<Rec> recs;
+    DevBuf<TileInfo> tinfo;
+    DevBuf<TileSpan> tspan;
+    DevBuf<double2> acc;
+    DevBuf<unsigned long long> counters;
+    DevBuf<float2> out_staging;
+
+    // bookkeeping
+    sim_stats stats{};
+    bool profiling = false;
+    std::vector<cudaEvent_t> events;     // 5 per batch when profiling
+    size_t events_used = 0;
+    std::string cuda_err;
+
+    ~sim_handle()
+    {
+        for (auto e : events) cudaEventDestroy(e);
+    }
+};
+
+namespace {
+
+int fail_cuda(sim_handle *h, cudaError_t e, const char *what)
+{
+    if (h) {
+        h->cuda_err = std::string(what) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")";
+    }
+    cudaGetLastError();   // clear the sticky-less error state
+    return (e == cudaErrorMemoryAllocation) ? SIM_ENOMEM : SIM_ECUDA;
+}
+
+#define CK(h, call)                                                   \
+    do {                                                              \
+        cudaError_t e__ = (call);                                     \
+        if (e__ != cudaSuccess) return fail_cuda((h), e__, #call);    \
+    } while (0)
+
+bool finite_all(const double *p, size_t n)
+{
+    for (size_t k = 0; k < n; ++k) if (!std::isfinite(p[k])) return false;
+    return true;
+}
+
+bool frame_ok(const double *f)
+{   // rows {b, a, e}: unit length, mutually orthogonal
+    for (int r = 0; r < 3; ++r) {
+        double n2 = f[3 * r] * f[3 * r] + f[3 * r + 1] * f[3 * r + 1] + f[3 * r + 2] * f[3 * r + 2];
+        if (!(std::fabs(n2 - 1.0) < 1e-6)) return false;
+        int q = (r + 1) % 3;
+        double d = f[3 * r] * f[3 * q] + f[3 * r + 1] * f[3 * q + 1] + f[3 * r + 2] * f[3 * q + 2];
+        if (!(std::fabs(d) < 1e-6)) return false;
+    }
+    return true;
+}
+
+int validate(const sim_instrument *in, const sim_geometry *g, const sim_scene *sc)
+{
+    if (!in || !g || !sc) return SIM_EINVAL;
+    if (in->n_channels < 1 || in->n_channels > SIM_MAX_CHANNELS || !in->channel_offset_m) return SIM_EINVAL;
+    if (in->n_samples < 1 || in->n_samples > (1 << 24)) return SIM_EINVAL;
+    const double sc_in[] = {in->f0_hz, in->chirp_rate_hz_per_s, in->chirp_len_s, in->fs_hz, in->cull_two_way_db,
+                            in->tx_aperture_m[0], in->tx_aperture_m[1], in->rx_aperture_m[0], in->rx_aperture_m[1]};
+    if (!finite_all(sc_in, sizeof(sc_in) / sizeof(double))) return SIM_EINVAL;
+    if (!(in->f0_hz > 0) || !(in->chirp_len_s > 0) || !(in->fs_hz > 0)) return SIM_EINVAL;
+    if (in->tx_aperture_m[0] < 0 || in->tx_aperture_m[1] < 0 || in->rx_aperture_m[0] < 0 || in->rx_aperture_m[1] < 0)
+        return SIM_EINVAL;
+    if (!(in->chirp_len_s * in->fs_hz < (double)(1 << 22))) return SIM_EINVAL;
+    if (!finite_all(in->channel_offset_m, in->n_channels)) return SIM_EINVAL;
+    if (g->n_pulses < 1) return SIM_EINVAL;
+    if (!g->t_pulse_s || !g->tx_pos_m || !g->tx_vel_mps || !g->rx_pos_m || !g->rx_vel_mps || !g->tx_frame ||
+        !g->rx_frame || !g->t0_s)
+        return SIM_EINVAL;
+    const size_t P = g->n_pulses;
+    if (!finite_all(g->t_pulse_s, P) || !finite_all(g->t0_s, P) || !finite_all(g->tx_pos_m, 3 * P) ||
+        !finite_all(g->rx_pos_m, 3 * P) || !finite_all(g->tx_vel_mps, 3 * P) || !finite_all(g->rx_vel_mps, 3 * P) ||
+        !finite_all(g->tx_frame, 9 * P) || !finite_all(g->rx_frame, 9 * P))
+        return SIM_EINVAL;
+    for (size_t p = 0; p < P; ++p) {
+        if (!frame_ok(g->tx_frame + 9 * p) || !frame_ok(g->rx_frame + 9 * p)) return SIM_EINVAL;
+        const double *v = g->rx_vel_mps + 3 * p;
+        if (!(v[0] * v[0] + v[1] * v[1] + v[2] * v[2] > 0)) return SIM_EINVAL;
+    }
+    if (sc->nx < 1 || sc->ny < 1 || (int64_t)sc->nx * sc->ny > ((int64_t)1 << 31)) return SIM_EINVAL;
+    if (!(sc->spacing_m > 0) || !std::isfinite(sc->spacing_m) || !finite_all(sc->centre_m, 3)) return SIM_EINVAL;
+    if (sc->n_waves < 0 || sc->n_waves > 4096) return SIM_EINVAL;
+    if (sc->n_waves > 0) {
+        if (!sc->kx || !sc->ky || !sc->amp || !sc->omega || !sc->phase) return SIM_EINVAL;
+        if (!finite_all(sc->kx, sc->n_waves) || !finite_all(sc->ky, sc->n_waves) || !finite_all(sc->amp, sc->n_waves) ||
+            !finite_all(sc->omega, sc->n_waves) || !finite_all(sc->phase, sc->n_waves))
+            return SIM_EINVAL;
+    }
+    if (!sc->sigma0_lin && !(sc->sigma0_uniform >= 0 && std::isfinite(sc->sigma0_uniform))) return SIM_EINVAL;
+    if (!finite_all(sc->look_dir, 2) || !finite_all(sc->current_uniform, 2)) return SIM_EINVAL;
+    return SIM_OK;
+}
+
+// Horizontal gradient magnitude bound of the bistatic path at the scene centre, mid dwell
+// (flat surface): |d(r_t+r_r)/dx| + |d(r_t+r_r)/dy|, used only to size tiles and CTAs.
+double path_gradient_l1(const sim_geometry *g, const sim_scene *sc)
+{
+    double worst = 0;
+    const int P = g->n_pulses;
+    const int picks[3] = {0, P / 2, P - 1};
+    for (int q = 0; q < 3; ++q) {
+        const double *tx = g->tx_pos_m + 3 * picks[q], *rx = g->rx_pos_m + 3 * picks[q];
+        // evaluate at centre and the four scene corners
+        for (int cx = -1; cx <= 1; ++cx)
+            for (int cy = -1; cy <= 1; ++cy) {
+                double x = sc->centre_m[0] + cx * 0.5 * sc->nx * sc->spacing_m;
+                double y = sc->centre_m[1] + cy * 0.5 * sc->ny * sc->spacing_m;
+                double z = sc->centre_m[2];
+                double dt[3] = {x - tx[0], y - tx[1], z - tx[2]}, dr[3] = {x - rx[0], y - rx[1], z - rx[2]};
+                double rt = std::sqrt(dt[0] * dt[0] + dt[1] * dt[1] + dt[2] * dt[2]);
+                double rr = std::sqrt(dr[0] * dr[0] + dr[1] * dr[1] + dr[2] * dr[2]);
+                double gx = dt[0] / rt + dr[0] / rr, gy = dt[1] / rt + dr[1] / rr;
+                worst = std::max(worst, std::fabs(gx) + std::fabs(gy));
+            }
+    }
+    return worst;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *sim_error_string(int code)
+{
+    switch (code) {
+        case SIM_OK: return "ok";
+        case SIM_EINVAL: return "invalid argument";
+        case SIM_ERANGE: return "pulse range out of bounds";
+        case SIM_ENOMEM: return "out of memory";
+        case SIM_ECUDA: return "CUDA error";
+        default: return "unknown error";
+    }
+}
+
+const char *sim_last_cuda_error(const sim_handle *h) { return h ? h->cuda_err.c_str() : ""; }
+
+void sim_destroy(sim_handle *h)
+{
+    if (!h) return;
+    DeviceGuard g(h->device);
+    h->xt.release(); h->yt.release(); h->tt.release(); h->chirp_n.release(); h->carrier_p.release();
+    h->wk.release(); h->carrier_frac.release(); h->pulses.release();
+    h->sigma0.release(); h->current.release(); h->xi.release();
+    h->z.release(); h->slope.release(); h->dxy.release(); h->recs.release(); h->tinfo.release();
+    h->tspan.release(); h->acc.release(); h->counters.release(); h->out_staging.release();
+    delete h;
+}
+
+int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene *sc, const sim_options *opts,
+               int device, sim_handle **out)
+{
+    if (!out) return SIM_EINVAL;
+    *out = nullptr;
+    int rc = validate(in, g, sc);
+    if (rc != SIM_OK) return rc;
+    if (opts && opts->tile_facets != 0) {
+        int t = opts->tile_facets;
+        if (t < 4 || t > 64 || (t & (t - 1))) return SIM_EINVAL;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return SIM_ECUDA;
+    }
+    sim_handle *h = new (std::nothrow) sim_handle();
+    if (!h) return SIM_ENOMEM;
+    h->device = device;
+    DeviceGuard guard(device);
+    if (!guard.ok) { delete h; return SIM_ECUDA; }
+
+    const int P = g->n_pulses, C = in->n_channels, Nw = sc->n_waves, nx = sc->nx, ny = sc->ny;
+    const int Ns = in->n_samples;
+    const double lambda = kC0 / in->f0_hz;
+    DevParams &prm = h->prm;
+    h->n_pulses = P;
+    h->n_facets = (int64_t)nx * ny;
+    h->chirp_rate = in->chirp_rate_hz_per_s; h->chirp_len = in->chirp_len_s; h->fs = in->fs_hz;
+    prm.nx = nx; prm.ny = ny; prm.spacing = sc->spacing_m;
+    prm.cx = sc->centre_m[0]; prm.cy = sc->centre_m[1]; prm.cz = sc->centre_m[2];
+    prm.n_samples = Ns; prm.n_channels = C; prm.n_mid = Ns / 2;
+    prm.inv_lambda = in->f0_hz / kC0;
+    prm.fs_over_c0 = in->fs_hz / kC0;
+    prm.kappa = in->chirp_rate_hz_per_s / (2.0 * in->fs_hz * in->fs_hz);
+    prm.len = in->chirp_len_s * in->fs_hz;
+    prm.half_len = 0.5 * prm.len;
+    prm.ap_tx_a = in->tx_aperture_m[0] / lambda; prm.ap_tx_e = in->tx_aperture_m[1] / lambda;
+    prm.ap_rx_a = in->rx_aperture_m[0] / lambda; prm.ap_rx_e = in->rx_aperture_m[1] / lambda;
+    prm.cull_thr = (in->cull_two_way_db > -300.0) ? (float)std::pow(10.0, in->cull_two_way_db / 20.0) : 0.f;
+    prm.n_waves = Nw; prm.choppy = sc->choppy ? 1 : 0; prm.tilt = sc->tilt_modulation ? 1 : 0;
+    prm.has_sigma0 = sc->sigma0_lin ? 1 : 0; prm.has_current = sc->current_mps ? 1 : 0;
+    prm.sigma0_uniform = sc->sigma0_uniform; prm.look_x = sc->look_dir[0]; prm.look_y = sc->look_dir[1];
+    prm.cur_ux = sc->current_uniform[0]; prm.cur_uy = sc->current_uniform[1];
+    h->need_slope = prm.tilt != 0;
+
+    // ---- tiling: a spatial tile must stay narrow in delay compared with the replica ----
+    const double grad = std::max(0.25, path_gradient_l1(g, sc));
+    const double samples_per_facet = sc->spacing_m * grad * prm.fs_over_c0;   // delay spread per facet step
+    int tile = opts ? opts->tile_facets : 0;
+    if (tile == 0) {
+        tile = 64;
+        const double budget = std::max(16.0, prm.len / 12.0);     // spread <= ~8 % of the replica
+        while (tile > 8 && tile * samples_per_facet > budget) tile >>= 1;
+    }
+    prm.tile = tile;
+    prm.tiles_x = (nx + tile - 1) / tile; prm.tiles_y = (ny + tile - 1) / tile;
+    prm.n_tiles = prm.tiles_x * prm.tiles_y;
+    prm.tile_cap = tile * tile;
+    double wave_sum = 0;
+    for (int w = 0; w < Nw; ++w) wave_sum += std::fabs(sc->amp[w]);
+    const double span_est = prm.len + tile * samples_per_facet + 2.0 * 2.0 * wave_sum * prm.fs_over_c0 + 3.0;
+    int threads = 32 * (int)std::ceil(span_est / (32.0 * kAccumR));
+    h->accum_threads = std::max(32, std::min(1024, threads));
+
+    // ---- batch size ----
+    const int64_t fcap = (int64_t)prm.n_tiles * prm.tile_cap;
+    const int64_t per_pulse = (int64_t)C * fcap * (int64_t)sizeof(Rec) + h->n_facets * 8 +
+                              (h->need_slope ? h->n_facets * 8 : 0) + (prm.choppy ? h->n_facets * 16 : 0) +
+                              (int64_t)C * Ns * 16 + (int64_t)prm.n_tiles * (4 + 8 * C);
+    int64_t ws = (opts && opts->workspace_bytes > 0) ? opts->workspace_bytes : ((int64_t)4 << 30);
+    int pb = (int)std::max<int64_t>(1, std::min<int64_t>(ws / std::max<int64_t>(per_pulse, 1), 256));
+    if (opts && opts->pulses_per_batch > 0) pb = opts->pulses_per_batch;
+    pb = std::min(pb, P);
+    h->pulses_per_batch = pb;
+
+    // ---- host tables (fp64) ----
+    std::vector<double2> xt((size_t)Nw * nx), yt((size_t)Nw * ny), tt((size_t)Nw * P);
+    std::vector<float4> wk(Nw);
+    for (int w = 0; w < Nw; ++w) {
+        for (int i = 0; i < nx; ++i) {
+            double x = sc->centre_m[0] + (i - 0.5 * (nx - 1)) * sc->spacing_m;
+            double a = sc->kx[w] * x;
+            xt[(size_t)w * nx + i] = make_double2(sc->amp[w] * std::cos(a), sc->amp[w] * std::sin(a));
+        }
+        for (int j = 0; j < ny; ++j) {
+            double y = sc->centre_m[1] + (j - 0.5 * (ny - 1)) * sc->spacing_m;
+            double a = sc->ky[w] * y + sc->phase[w];
+            yt[(size_t)w * ny + j] = make_double2(std::cos(a), std::sin(a));
+        }
+        for (int p = 0; p < P; ++p) {
+            double a = -sc->omega[w] * g->t_pulse_s[p];
+            tt[(size_t)w * P + p] = make_double2(std::cos(a), std::sin(a));
+        }
+        double k = std::hypot(sc->kx[w], sc->ky[w]);
+        wk[w] = make_float4((float)sc->kx[w], (float)sc->ky[w], k > 0 ? (float)(sc->kx[w] / k) : 0.f,
+                            k > 0 ? (float)(sc->ky[w] / k) : 0.f);
+    }
+    std::vector<PulseConst> pcs(P);
+    std::vector<double2> carrier(P);
+    std::vector<double> cfrac(P);
+    for (int p = 0; p < P; ++p) {
+        PulseConst &pc = pcs[p];
+        std::memset(&pc, 0, sizeof(pc));
+        pc.t = g->t_pulse_s[p];
+        pc.r0 = kC0 * g->t0_s[p];
+        const double *v = g->rx_vel_mps + 3 * p;
+        const double vn = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+        for (int k = 0; k < 3; ++k) {
+            pc.tx_pos[k] = g->tx_pos_m[3 * p + k];
+            pc.tx_a[k] = g->tx_frame[9 * p + 3 + k]; pc.tx_e[k] = g->tx_frame[9 * p + 6 + k];
+            pc.rx_a[k] = g->rx_frame[9 * p + 3 + k]; pc.rx_e[k] = g->rx_frame[9 * p + 6 + k];
+            pc.rx_ref[k] = g->rx_pos_m[3 * p + k];
+            for (int c = 0; c < C; ++c) pc.rx_pos[c][k] = g->rx_pos_m[3 * p + k] + in->channel_offset_m[c] * v[k] / vn;
+        }
+        // carrier phase of the reference path: f0 * (r0/c0), reduced in long double
+        long double cyc = (long double)pc.r0 * ((long double)in->f0_hz / (long double)kC0);
+        long double fr = cyc - floorl(cyc);
+        cfrac[p] = (double)fr;
+        carrier[p] = make_double2(std::cos(-2.0 * M_PI * (double)fr), std::sin(-2.0 * M_PI * (double)fr));
+    }
+    std::vector<double2> chirp(Ns);
+    for (int n = 0; n < Ns; ++n) {
+        long double m = (long double)(n - prm.n_mid);
+        long double turns = (long double)prm.kappa * m * m;
+        turns -= floorl(turns);
+        chirp[n] = make_double2(std::cos(2.0 * M_PI * (double)turns), std::sin(2.0 * M_PI * (double)turns));
+    }
+
+    // ---- device allocation + upload ----
+    auto bail = [&](int code) { sim_destroy(h); return code; };
+#define CKC(call)                                                                 \
+    do {                                                                          \
+        cudaError_t e__ = (call);                                                 \
+        if (e__ != cudaSuccess) { int c__ = fail_cuda(h, e__, #call); return bail(c__); } \
+    } while (0)
+    CKC(h->xt.alloc(xt.size())); CKC(h->yt.alloc(yt.size())); CKC(h->tt.alloc(tt.size()));
+    CKC(h->wk.alloc(wk.size())); CKC(h->pulses.alloc(P)); CKC(h->carrier_p.alloc(P));
+    CKC(h->carrier_frac.alloc(P)); CKC(h->chirp_n.alloc(Ns));
+    if (Nw) {
+        CKC(cudaMemcpy(h->xt.p, xt.data(), xt.size() * sizeof(double2), cudaMemcpyHostToDevice));
+        CKC(cudaMemcpy(h->yt.p, yt.data(), yt.size() * sizeof(double2), cudaMemcpyHostToDevice));
+        CKC(cudaMemcpy(h->tt.p, tt.data(), tt.size() * sizeof(double2), cudaMemcpyHostToDevice));
+        CKC(cudaMemcpy(h->wk.p, wk.data(), wk.size() * sizeof(float4), cudaMemcpyHostToDevice));
+    }
+    CKC(cudaMemcpy(h->pulses.p, pcs.data(), (size_t)P * sizeof(PulseConst), cudaMemcpyHostToDevice));
+    CKC(cudaMemcpy(h->carrier_p.p, carrier.data(), (size_t)P * sizeof(double2), cudaMemcpyHostToDevice));
+    CKC(cudaMemcpy(h->carrier_frac.p, cfrac.data(), (size_t)P * sizeof(double), cudaMemcpyHostToDevice));
+    CKC(cudaMemcpy(h->chirp_n.p, chirp.data(), (size_t)Ns * sizeof(double2), cudaMemcpyHostToDevice));
+    const size_t F = (size_t)h->n_facets;
+    if (sc->sigma0_lin) {
+        CKC(h->sigma0.alloc(F));
+        CKC(cudaMemcpy(h->sigma0.p, sc->sigma0_lin, F * sizeof(float), cudaMemcpyHostToDevice));
+    }
+    if (sc->current_mps) {
+        CKC(h->current.alloc(F));
+        CKC(cudaMemcpy(h->current.p, sc->current_mps, F * sizeof(float2), cudaMemcpyHostToDevice));
+    }
+    CKC(h->xi.alloc(F));
+    if (sc->xi) {
+        CKC(cudaMemcpy(h->xi.p, sc->xi, F * sizeof(float2), cudaMemcpyHostToDevice));
+    } else {
+        CKC(launch_speckle_from_seed(h->xi.p, (int64_t)F, sc->seed, nullptr));
+        CKC(cudaDeviceSynchronize());
+    }
+    CKC(h->z.alloc(F * pb));
+    if (h->need_slope) CKC(h->slope.alloc(F * pb));
+    if (prm.choppy) CKC(h->dxy.alloc(F * pb));
+    CKC(h->recs.alloc((size_t)C * pb * fcap));
+    CKC(h->tinfo.alloc((size_t)pb * prm.n_tiles));
+    CKC(h->tspan.alloc((size_t)C * pb * prm.n_tiles));
+    CKC(h->acc.alloc((size_t)C * pb * Ns));
+    CKC(h->counters.alloc(2));
+    CKC(cudaMemset(h->counters.p, 0, 2 * sizeof(unsigned long long)));
+#undef CKC
+    h->stats.tile_facets = tile; h->stats.pulses_per_batch = pb; h->stats.n_tiles = prm.n_tiles;
+    h->stats.accumulate_block_threads = h->accum_threads;
+    *out = h;
+    return SIM_OK;
+}
+
+static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cudaStream_t s)
+{
+    const DevParams &prm = h->prm;
+    const int n_out = pb1 - pb0;
+    int64_t launches = 0;
+    CK(h, cudaMemsetAsync(h->counters.p, 0, 2 * sizeof(unsigned long long), s));
+    h->events_used = 0;
+    auto mark = [&]() -> cudaError_t {
+        if (!h->profiling) return cudaSuccess;
+        if (h->events_used == h->events.size()) {
+            cudaEvent_t e;
+            cudaError_t rc = cudaEventCreate(&e);
+            if (rc != cudaSuccess) return rc;
+            h->events.push_back(e);
+        }
+        return cudaEventRecord(h->events[h->events_used++], s);
+    };
+    for (int p0 = pb0; p0 < pb1; p0 += h->pulses_per_batch) {
+        const int n_pl = std::min(h->pulses_per_batch, pb1 - p0);
+        CK(h, cudaMemsetAsync(h->acc.p, 0, (size_t)prm.n_channels * n_pl * prm.n_samples * sizeof(double2), s));
+        CK(h, mark());
+        KinematicsArgs ka{h->xt.p, h->yt.p, h->tt.p, h->wk.p, h->n_pulses, h->z.p, h->slope.p, h->dxy.p};
+        CK(h, launch_kinematics(prm, ka, p0, n_pl, s));
+        CK(h, mark());
+        GeometryArgs ga{};
+        ga.pulses = h->pulses.p; ga.z = h->z.p; ga.slope = h->slope.p; ga.dxy = h->dxy.p;
+        ga.sigma0 = h->sigma0.p; ga.current = h->current.p; ga.xi = h->xi.p;
+        ga.recs = h->recs.p; ga.tinfo = h->tinfo.p; ga.tspan = h->tspan.p; ga.counters = h->counters.p;
+        ga.carrier_frac_t0 = h->carrier_frac.p;
+        CK(h, launch_geometry(prm, ga, p0, n_pl, s));
+        CK(h, mark());
+        AccumulateArgs aa{h->recs.p, h->tinfo.p, h->tspan.p, h->acc.p, h->accum_threads};
+        CK(h, launch_accumulate(prm, aa, n_pl, s));
+        CK(h, mark());
+        FinalizeArgs fa{h->acc.p, h->chirp_n.p, h->carrier_p.p, out, n_out, p0 - pb0};
+        CK(h, launch_finalize(prm, fa, p0, n_pl, s));
+        CK(h, mark());
+        launches += 4;
+    }
+    h->stats.kernel_launches = launches;
+    h->stats.facet_echoes_nominal = h->n_facets * (int64_t)n_out * prm.n_channels;
+    return SIM_OK;
+}
+
+int sim_generate(sim_handle *h, int32_t pulse_begin, int32_t pulse_end, void *iq_dev, void *cuda_stream)
+{
+    if (!h) return SIM_EINVAL;
+    if (pulse_begin < 0 || pulse_end > h->n_pulses || pulse_begin >= pulse_end) return SIM_ERANGE;
+    if (!iq_dev) return SIM_EINVAL;
+    DeviceGuard g(h->device);
+    if (!g.ok) return SIM_ECUDA;
+    return run_batches(h, pulse_begin, pulse_end, static_cast<float2 *>(iq_dev), static_cast<cudaStream_t>(cuda_stream));
+}
+
+int sim_generate_host(sim_handle *h, int32_t pulse_begin, int32_t pulse_end, void *iq_host, void *cuda_stream)
+{
+    if (!h) return SIM_EINVAL;
+    if (pulse_begin < 0 || pulse_end > h->n_pulses || pulse_begin >= pulse_end) return SIM_ERANGE;
+    if (!iq_host) return SIM_EINVAL;
+    DeviceGuard g(h->device);
+    if (!g.ok) return SIM_ECUDA;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const size_t n = (size_t)h->prm.n_channels * (pulse_end - pulse_begin) * h->prm.n_samples;
+    if (h->out_staging.n < n) CK(h, h->out_staging.alloc(n));
+    int rc = run_batches(h, pulse_begin, pulse_end, h->out_staging.p, s);
+    if (rc != SIM_OK) return rc;
+    CK(h, cudaMemcpyAsync(iq_host, h->out_staging.p, n * sizeof(float2), cudaMemcpyDeviceToHost, s));
+    CK(h, cudaStreamSynchronize(s));
+    return SIM_OK;
+}
+
+int sim_update_scene(sim_handle *h, const float *sigma0_lin, const float *current_mps, const float *xi, void *cuda_stream)
+{
+    if (!h) return SIM_EINVAL;
+    if ((sigma0_lin && !h->sigma0.p) || (current_mps && !h->current.p)) return SIM_EINVAL;
+    DeviceGuard g(h->device);
+    if (!g.ok) return SIM_ECUDA;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const size_t F = (size_t)h->n_facets;
+    if (sigma0_lin) CK(h, cudaMemcpyAsync(h->sigma0.p, sigma0_lin, F * sizeof(float), cudaMemcpyHostToDevice, s));
+    if (current_mps) CK(h, cudaMemcpyAsync(h->current.p, current_mps, F * sizeof(float2), cudaMemcpyHostToDevice, s));
+    if (xi) CK(h, cudaMemcpyAsync(h->xi.p, xi, F * sizeof(float2), cudaMemcpyHostToDevice, s));
+    return SIM_OK;
+}
+
+int sim_replica(const sim_handle *h, float *host_c64_out, int32_t *n)
+{
+    if (!h || !n) return SIM_EINVAL;
+    // samples m with -T/2 <= m/fs - T/2 < T/2  <=>  0 <= m < T fs
+    const int32_t L = (int32_t)std::ceil(h->chirp_len * h->fs - 1e-9);
+    *n = L;
+    if (!host_c64_out) return SIM_OK;
+    for (int32_t m = 0; m < L; ++m) {
+        const double u = m / h->fs - 0.5 * h->chirp_len;
+        const double ph = M_PI * h->chirp_rate * u * u;
+        host_c64_out[2 * m] = (float)std::cos(ph);
+        host_c64_out[2 * m + 1] = (float)std::sin(ph);
+    }
+    return SIM_OK;
+}
+
+int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, double *tau, double *g_tx,
+                     double *g_rx, double *amp, int32_t *keep)
+{
+    if (!h) return SIM_EINVAL;
+    if (pulse < 0 || pulse >= h->n_pulses) return SIM_ERANGE;
+    DeviceGuard g(h->device);
+    if (!g.ok) return SIM_ECUDA;
+    const DevParams &prm = h->prm;
+    const size_t F = (size_t)h->n_facets, C = prm.n_channels;
+    DevBuf<double> d_pos, d_tau, d_gtx, d_grx, d_amp;
+    DevBuf<int32_t> d_keep;
+    DevBuf<float2> d_slope;
+    int rc = SIM_OK;
+    auto run = [&]() -> int {
+        CK(h, d_pos.alloc(3 * F)); CK(h, d_tau.alloc(C * F)); CK(h, d_gtx.alloc(F));
+        CK(h, d_grx.alloc(C * F)); CK(h, d_amp.alloc(2 * C * F)); CK(h, d_keep.alloc(F));
+        float2 *slope_buf = h->slope.p;
+        if (!slope_buf) { CK(h, d_slope.alloc(F)); slope_buf = d_slope.p; }
+        KinematicsArgs ka{h->xt.p, h->yt.p, h->tt.p, h->wk.p, h->n_pulses, h->z.p, slope_buf, h->dxy.p};
+        CK(h, launch_kinematics(prm, ka, pulse, 1, nullptr));
+        GeometryArgs ga{};
+        ga.pulses = h->pulses.p; ga.z = h->z.p; ga.slope = h->need_slope ? slope_buf : nullptr; ga.dxy = h->dxy.p;
+        ga.sigma0 = h->sigma0.p; ga.current = h->current.p; ga.xi = h->xi.p;
+        ga.recs = h->recs.p; ga.tinfo = h->tinfo.p; ga.tspan = h->tspan.p; ga.counters = nullptr;
+        ga.dbg_pos = d_pos.p; ga.dbg_tau = d_tau.p; ga.dbg_gtx = d_gtx.p; ga.dbg_grx = d_grx.p;
+        ga.dbg_amp = d_amp.p; ga.dbg_keep = d_keep.p; ga.carrier_frac_t0 = h->carrier_frac.p;
+        CK(h, launch_geometry(prm, ga, pulse, 1, nullptr));
+        CK(h, cudaDeviceSynchronize());
+        if (pos) CK(h, cudaMemcpy(pos, d_pos.p, 3 * F * sizeof(double), cudaMemcpyDeviceToHost));
+        if (tau) CK(h, cudaMemcpy(tau, d_tau.p, C * F * sizeof(double), cudaMemcpyDeviceToHost));
+        if (g_tx) CK(h, cudaMemcpy(g_tx, d_gtx.p, F * sizeof(double), cudaMemcpyDeviceToHost));
+        if (g_rx) CK(h, cudaMemcpy(g_rx, d_grx.p, C * F * sizeof(double), cudaMemcpyDeviceToHost));
+        if (amp) CK(h, cudaMemcpy(amp, d_amp.p, 2 * C * F * sizeof(double), cudaMemcpyDeviceToHost));
+        if (keep) CK(h, cudaMemcpy(keep, d_keep.p, F * sizeof(int32_t), cudaMemcpyDeviceToHost));
+        if (slope) {
+            std::vector<float2> tmp(F);
+            CK(h, cudaMemcpy(tmp.data(), slope_buf, F * sizeof(float2), cudaMemcpyDeviceToHost));
+            for (size_t f = 0; f < F; ++f) { slope[2 * f] = tmp[f].x; slope[2 * f + 1] = tmp[f].y; }
+        }
+        return SIM_OK;
+    };
+    rc = run();
+    d_pos.release(); d_tau.release(); d_gtx.release(); d_grx.release(); d_amp.release(); d_keep.release();
+    d_slope.release();
+    return rc;
+}
+
+int sim_get_stats(sim_handle *h, sim_stats *out)
+{
+    if (!h || !out) return SIM_EINVAL;
+    DeviceGuard g(h->device);
+    if (!g.ok) return SIM_ECUDA;
+    unsigned long long c[2] = {0, 0};
+    CK(h, cudaMemcpy(c, h->counters.p, sizeof(c), cudaMemcpyDeviceToHost));   // synchronises with prior work
+    h->stats.facet_echoes_kept = (int64_t)c[0];
+    h->stats.facet_samples = (int64_t)c[1];
+    *out = h->stats;
+    return SIM_OK;
+}
+
+int sim_set_profiling(sim_handle *h, int32_t enable)
+{
+    if (!h) return SIM_EINVAL;
+    h->profiling = enable != 0;
+    return SIM_OK;
+}
+
+int sim_get_kernel_ms(sim_handle *h, float ms[4])
+{
+    if (!h || !ms) return SIM_EINVAL;
+    DeviceGuard g(h->device);
+    if (!g.ok) return SIM_ECUDA;
+    for (int k = 0; k < 4; ++k) ms[k] = 0.f;
+    if (h->events_used == 0) return SIM_OK;
+    CK(h, cudaEventSynchronize(h->events[h->events_used - 1]));
+    for (size_t b = 0; b + 5 <= h->events_used; b += 5) {
+        for (int k = 0; k < 4; ++k) {
+            float t = 0.f;
+            CK(h, cudaEventElapsedTime(&t, h->events[b + k], h->events[b + k + 1]));
+            ms[k] += t;
+        }
+    }
+    return SIM_OK;
+}
+
+}  // extern "C"

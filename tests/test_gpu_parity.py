@@ -1,0 +1,334 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle, element by element on
+the same seeded inputs.  Bars (BASELINE.json north_star): relative L2 <= 1e-4 per
+(channel, pulse) vector; RMS inter-channel ATI phase error <= 1e-3 rad; integer decisions
+(window membership, cull) identical except where the deciding quantity sits within rounding of
+the threshold (reading G18).
+"""
+import numpy as np
+import pytest
+
+from oracle import (ati_phase_rms_error, oracle_facets, oracle_generate, oracle_samples,
+                    rel_l2_per_vector)
+from workloads import make_workload, make_sweep_point
+from helpers import custom_workload
+
+pytestmark = pytest.mark.gpu
+
+REL_L2_BAR = 1e-4
+ATI_BAR = 1e-3
+
+
+def _sim(w, **opts):
+    from paper_2405_09938_b200 import Simulator
+    return Simulator(w, 0, **opts)
+
+
+def _gpu(w, p0=0, p1=None, **opts):
+    import torch
+    with _sim(w, **opts) as sim:
+        out = sim.generate(p0, p1)
+        torch.cuda.synchronize()
+        return out.cpu().numpy()
+
+
+def _assert_parity(got, ref, what=""):
+    err = rel_l2_per_vector(got, ref)
+    assert np.all(err <= REL_L2_BAR), f"{what}: worst rel-L2 {err.max():.3e} at {np.unravel_index(err.argmax(), err.shape)}"
+    if got.shape[0] > 1:
+        rms = ati_phase_rms_error(got, ref)
+        assert rms <= ATI_BAR, f"{what}: ATI phase RMS error {rms:.3e} rad"
+    return err.max()
+
+
+# ----------------------------------------------------------------------------- Tiny, in full
+
+def test_tiny_all_pulses():
+    w = make_workload("tiny")
+    got = _gpu(w)
+    ref = oracle_generate(w)
+    assert got.shape == (1, 32, 256) and got.dtype == np.complex64
+    worst = _assert_parity(got, ref, "tiny")
+    assert worst < 2e-5            # headroom: the budget is not being eaten by the kernel
+    # samples outside every echo window are exactly zero on both sides
+    assert np.array_equal(got == 0, ref == 0)
+
+
+@pytest.mark.parametrize("tile", [4, 8, 16, 32, 64])
+def test_tiny_tile_sizes_and_batches(tile):
+    w = make_workload("tiny", n_pulses=7)
+    ref = oracle_generate(w)
+    got = _gpu(w, tile_facets=tile, pulses_per_batch=3)      # ragged last batch
+    _assert_parity(got, ref, f"tile {tile}")
+
+
+def test_pulse_ranges_are_idempotent_and_consistent():
+    import torch
+    w = make_workload("tiny", n_pulses=9)
+    with _sim(w) as sim:
+        full = sim.generate().cpu().numpy()
+        part = sim.generate(3, 8).cpu().numpy()
+        again = sim.generate(3, 8).cpu().numpy()
+        torch.cuda.synchronize()
+    ref = oracle_generate(w)
+    _assert_parity(part, ref[:, 3:8], "range")
+    _assert_parity(again, ref[:, 3:8], "range again")
+    # fp32 atomics order may differ run to run only inside the tolerance
+    assert np.max(np.abs(part - full[:, 3:8])) <= 1e-5 * np.abs(full).max()
+
+
+# ----------------------------------------------------------------------------- per-kernel unit parity (T1)
+
+@pytest.mark.parametrize("name", ["tiny", "hetero_small"])
+def test_facet_intermediates(name):
+    if name == "tiny":
+        w = make_workload("tiny", n_pulses=4)
+    else:
+        w = _hetero_small()
+    p = w.n_pulses - 1
+    with _sim(w) as sim:
+        g = sim.debug_facets(p)
+    o = oracle_facets(w, p)
+    assert np.max(np.abs(g["pos"] - o["pos"])) < 2e-9                 # metres, fp64 phasor tables
+    assert np.max(np.abs(g["slope"] - o["slope"])) < 2e-6              # fp32 slopes
+    assert np.max(np.abs(g["tau"] - o["tau"])) < 1e-17 + 2e-16 * np.abs(o["tau"]).max()
+    assert np.max(np.abs(g["g_tx"] - o["g_tx"])) < 2e-6
+    assert np.max(np.abs(g["g_rx"] - o["g_rx"])) < 2e-6
+    # cull: identical except facets within rounding of the threshold
+    thr = 10 ** (w.instrument["cull_two_way_db"] / 20)
+    margin = np.abs(np.abs(o["g_tx"] * o["g_rx"][w.n_channels // 2]) - thr) < 1e-5
+    assert np.array_equal(g["keep"][~margin], o["keep"][~margin])
+    kept = o["keep"].astype(bool) & ~margin
+    scale = np.abs(o["amp"][:, kept]).max()
+    assert np.max(np.abs(g["amp"][:, kept] - o["amp"][:, kept])) < 5e-6 * scale
+
+
+# ----------------------------------------------------------------------------- edge cases
+
+def _hetero_small(nx=150, ny=90, n_pulses=3):
+    """The Heterogeneous recipe (sigma0 field, tilt, current front, 256 components) cropped."""
+    w = make_workload("hetero", n_pulses=n_pulses)
+    sc = w.scene
+    j0, i0 = 1024 - ny // 2, 1024 - nx // 2
+    sc["sigma0_lin"] = np.ascontiguousarray(sc["sigma0_lin"][j0:j0 + ny, i0:i0 + nx])
+    sc["current_mps"] = np.ascontiguousarray(sc["current_mps"][j0:j0 + ny, i0:i0 + nx])
+    sc["xi"] = np.ascontiguousarray(sc["xi"][j0:j0 + ny, i0:i0 + nx])
+    sc["nx"], sc["ny"] = nx, ny
+    return w
+
+
+def test_hetero_recipe_ragged_grid():
+    """sigma0 map + tilt modulation + current front + 256 components, grid not a tile multiple."""
+    w = _hetero_small()
+    got = _gpu(w)
+    ref = oracle_generate(w)
+    _assert_parity(got, ref, "hetero_small")
+
+
+def test_choppy_wave_model_flag():
+    w = make_workload("tiny", n_pulses=3)
+    w.scene["choppy"] = 1
+    _assert_parity(_gpu(w), oracle_generate(w), "choppy")
+
+
+def test_cull_active_and_window_clipping():
+    """Wide patch: part of the facets fall below -30 dB two-way (culled), and the delay spread
+    exceeds the sampling window so echoes are clipped at both ends (silently)."""
+    w = make_workload("tiny", n_pulses=2)
+    w.scene["spacing_m"] = 220.0
+    o = oracle_facets(w, 0)
+    assert 0.1 < o["keep"].mean() < 0.95
+    ref = oracle_generate(w)
+    assert np.abs(ref[0, 0, 0]) > 0 and np.abs(ref[0, 0, -1]) > 0      # window is full edge to edge
+    got = _gpu(w)
+    _assert_parity(got, ref, "cull+clip")
+    with _sim(w) as sim:
+        sim.generate()
+        st = sim.stats()
+    assert st["facet_echoes_nominal"] == 4096 * 2
+    expect_kept = sum(int(oracle_facets(w, p)["keep"].sum()) for p in range(2))
+    assert abs(st["facet_echoes_kept"] - expect_kept) <= 2
+
+
+def test_everything_culled_gives_exact_zeros():
+    w = make_workload("tiny", n_pulses=2)
+    w.instrument["cull_two_way_db"] = 10.0          # nothing reaches +10 dB
+    got = _gpu(w)
+    assert np.all(got == 0)
+    assert np.all(oracle_generate(w) == 0)
+
+
+def test_zero_amplitude_and_single_facet():
+    w = make_workload("tiny", n_pulses=2)
+    w.scene["xi"][:] = 0
+    assert np.all(_gpu(w) == 0)
+    tx, rx = (10.0, -300e3, 700e3), (250e3, -300e3, 700e3)
+    r = np.linalg.norm(np.array(tx)) + np.linalg.norm(np.array(rx))
+    w1 = custom_workload(tx_pos=tx, rx_pos=rx, t0=r / 299792458.0 - 100.3 / 12e6)
+    _assert_parity(_gpu(w1), oracle_generate(w1), "single facet")
+
+
+def test_non_integer_replica_length_and_odd_sizes():
+    """T*fs = 24.6 samples: echoes cover 24 or 25 samples depending on the sub-sample delay (G2)."""
+    w = make_workload("tiny", n_pulses=2)
+    w.instrument["chirp_len_s"] = 24.6 / 12e6
+    w.instrument["chirp_rate_hz_per_s"] = 10e6 / w.instrument["chirp_len_s"]
+    w.instrument["n_samples"] = 251
+    w.scene["nx"], w.scene["ny"] = 61, 37
+    w.scene["xi"] = np.ascontiguousarray(w.scene["xi"][:37, :61])
+    _assert_parity(_gpu(w), oracle_generate(w), "non-integer L")
+
+
+def test_no_waves_and_eight_channels():
+    w = make_workload("tiny", n_pulses=2)
+    w.scene["n_waves"] = 0
+    for k in ("kx", "ky", "amp", "omega", "phase"):
+        w.scene[k] = np.zeros(0)
+    w.instrument["channel_offset_m"] = np.linspace(-7.0, 7.0, 8)
+    _assert_parity(_gpu(w), oracle_generate(w), "8 channels, flat")
+
+
+def test_speckle_from_seed_moments():
+    """xi = NULL -> library derives xi from (seed, facet index) (G14): zero mean, E|xi|^2 = 1,
+    no lag-1 correlation; pinned by moments since the values are the library's own."""
+    w = make_workload("tiny", n_pulses=1)
+    w.scene["nx"] = w.scene["ny"] = 256
+    w.scene["xi"] = None
+    w.scene["n_waves"] = 0
+    for k in ("kx", "ky", "amp", "omega", "phase"):
+        w.scene[k] = np.zeros(0)
+    w.instrument["tx_aperture_m"] = np.zeros(2)
+    w.instrument["rx_aperture_m"] = np.zeros(2)
+    w.scene["sigma0_uniform"] = 1.0
+    w.scene["spacing_m"] = 1.0
+    with _sim(w) as sim:
+        amp = sim.debug_facets(0)["amp"][0]          # |amp| = |xi| here (unit gains, sigma0 d^2 = 1)
+    mag2 = np.abs(amp) ** 2
+    assert abs(mag2.mean() - 1.0) < 0.02
+    assert abs(np.mean(mag2 ** 2) - 2.0) < 0.1        # Exp(1): second moment 2
+    # remove the deterministic carrier phase by looking at magnitudes' lag-1 correlation
+    m = np.abs(amp) - np.abs(amp).mean()
+    assert abs(np.mean(m[1:] * m[:-1]) / np.mean(m * m)) < 0.02
+    w.scene["seed"] = 99
+    with _sim(w) as sim:
+        amp2 = sim.debug_facets(0)["amp"][0]
+    assert np.mean(np.abs(np.abs(amp2) - np.abs(amp))) > 0.1
+
+
+def test_error_codes():
+    from paper_2405_09938_b200 import SimError
+    w = make_workload("tiny", n_pulses=2)
+    with _sim(w) as sim:
+        for rng in ((-1, 1), (0, 3), (2, 2), (1, 0)):
+            with pytest.raises(SimError) as e:
+                sim.generate(*rng)
+            assert e.value.code == -2
+    w.geometry["tx_frame"] = w.geometry["tx_frame"] * 1.01       # not orthonormal
+    with pytest.raises(SimError) as e:
+        _sim(w)
+    assert e.value.code == -1
+    w = make_workload("tiny", n_pulses=2)
+    w.geometry["t0_s"][1] = np.nan
+    with pytest.raises(SimError) as e:
+        _sim(w)
+    assert e.value.code == -1
+    w = make_workload("tiny", n_pulses=2)
+    w.instrument["channel_offset_m"] = np.zeros(9)
+    with pytest.raises(SimError):
+        _sim(w)
+
+
+def test_host_path_and_scene_update():
+    """sim_generate_host + sim_update_scene (the end-to-end entry points bench.py times)."""
+    import torch
+    w = _hetero_small(96, 64, 2)
+    ref = oracle_generate(w)
+    with _sim(w) as sim:
+        _assert_parity(sim.generate_host().numpy(), ref, "host path")
+        xi2 = (w.scene["xi"] * np.float32(0.5)).astype(np.float32)
+        sim.update_scene(xi=torch.from_numpy(xi2).pin_memory())
+        got = sim.generate_host().numpy()
+    _assert_parity(got, 0.5 * ref, "after update_scene")
+
+
+def test_replica_is_the_transmitted_chirp():
+    w = make_workload("ati", n_pulses=1)
+    w.scene["nx"] = w.scene["ny"] = 4
+    w.scene["xi"] = np.ascontiguousarray(w.scene["xi"][:4, :4])
+    with _sim(w) as sim:
+        rep = sim.replica()
+    m = np.arange(1200)
+    expect = np.exp(1j * np.pi * 2.5e12 * (m / 60e6 - 10e-6) ** 2)
+    assert rep.shape == (1200,) and np.max(np.abs(rep - expect)) < 1e-6
+
+
+# ----------------------------------------------------------------------------- BASELINE sizes
+
+def test_ati_seeded_pulse_subset():
+    """Config 1 (ATI, 512x512, 3 channels, L = 1200) at full size: the launch configuration bench.py
+    times (all 256 pulses in one call); the oracle checks first, last and two seeded pulses."""
+    import torch
+    w = make_workload("ati")
+    rng = np.random.Generator(np.random.PCG64(20240509))
+    pulses = sorted({0, 255, *rng.integers(1, 255, 2).tolist()})
+    with _sim(w) as sim:
+        out = sim.generate()
+        torch.cuda.synchronize()
+        got = out[:, pulses].cpu().numpy()
+        st = sim.stats()
+    assert st["facet_echoes_kept"] == st["facet_echoes_nominal"] == 512 * 512 * 256 * 3
+    ref = oracle_generate(w, pulses)
+    _assert_parity(got, ref, "ati")
+
+
+def test_hetero_full_size_sampled_outputs():
+    """Config 2 (2048x2048, 256 components, maps) at full size, two pulses through the library;
+    the oracle evaluates 24 seeded output samples of one pulse one by one."""
+    w = make_workload("hetero")
+    rng = np.random.Generator(np.random.PCG64(20240510))
+    p = 1023
+    got = _gpu(w, p, p + 1)[:, 0]
+    energy = np.abs(got[1]) ** 2
+    live = np.nonzero(energy > 1e-3 * energy.max())[0]
+    ns = np.sort(rng.choice(live, 24, replace=False))
+    ref = oracle_samples(w, p, ns)
+    scale = np.sqrt(np.mean(np.abs(got[:, live]) ** 2))
+    assert np.max(np.abs(got[:, ns] - ref)) < 2e-4 * scale
+    # interferometric phase on the sampled subset
+    def ph(s):
+        return np.angle((s[0] * np.conj(s[2])).sum())
+    assert abs(np.angle(np.exp(1j * (ph(got[:, ns]) - ph(ref))))) < ATI_BAR
+
+
+def test_large_full_size_properties():
+    """Config 3 (4096x4096, Ns = 8192) at full size, one pulse at the dwell end where the cull is
+    active: kept count against the documented 0.86-0.94 band, support inside the window, zero
+    outside the tile spans, and 12 sampled outputs against the oracle."""
+    w = make_workload("large")
+    p = 2047
+    with _sim(w) as sim:
+        got = sim.generate(p, p + 1).cpu().numpy()[:, 0]
+        st = sim.stats()
+    frac = st["facet_echoes_kept"] / st["facet_echoes_nominal"]
+    assert 0.80 < frac < 0.97
+    energy = np.abs(got[1]) ** 2
+    live = np.nonzero(energy > 0)[0]
+    assert live[0] > 0 and live[-1] < 8191 and live.size < 3400          # 2987 expected
+    rng = np.random.Generator(np.random.PCG64(20240511))
+    strong = np.nonzero(energy > 1e-3 * energy.max())[0]
+    ns = np.sort(rng.choice(strong, 12, replace=False))
+    ref = oracle_samples(w, p, ns)
+    scale = np.sqrt(np.mean(np.abs(got[:, strong]) ** 2))
+    assert np.max(np.abs(got[:, ns] - ref)) < 2e-4 * scale
+
+
+def test_sweep_point_long_chirp():
+    """Sweep axis: L = 4096 replica samples on a 2^20-facet patch, one channel, sampled check."""
+    w = make_sweep_point(log2_facets=20, replica_samples=4096, n_channels=1, n_pulses=2)
+    got = _gpu(w, 1, 2)[:, 0]
+    energy = np.abs(got[0]) ** 2
+    strong = np.nonzero(energy > 1e-3 * energy.max())[0]
+    rng = np.random.Generator(np.random.PCG64(7))
+    ns = np.sort(rng.choice(strong, 16, replace=False))
+    ref = oracle_samples(w, 1, ns)
+    scale = np.sqrt(np.mean(np.abs(got[:, strong]) ** 2))
+    assert np.max(np.abs(got[:, ns] - ref)) < 2e-4 * scale
