@@ -1,0 +1,315 @@
+#!/usr/bin/env python
+"""Benchmark of the raw-data generator hot path (BASELINE.json metric: facet-echoes/s).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload ati]
+
+One *step* is one pass of the whole hot path (K1 kinematics, K2 geometry/gains/cull, K3 echo
+accumulation, K4 finalize) over every pulse and channel of the workload: `sim_generate(0, P)`.
+At N = 1 the workload is BASELINE.json configs[1] ("ATI": 512x512 facets, 3 channels, 256 pulses,
+L = 1200, Ns = 4096).  Under torchrun each rank owns its own P-pulse slab of an N*P-pulse
+acquisition (weak scaling, no data-path collective).
+
+The JSON line carries, beside the base contract: `roofline` (dominant kernel K3 against the FP32
+pipe), `cpu_baseline` (the fp64 oracle on the host cores, bounded sample), `e2e` (through
+sim_update_scene + sim_generate_host with pinned HOST buffers), `clocks`, `gpu_launches`.
+`--impl reference` times the oracle as it stands (this tier's reference arm).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+METRIC = "facet_echoes_per_s"
+UNIT = "facet-echoes/s"
+
+# FP32-pipe roofline of K3: the inner loop spends 6 FP32-pipe operations per
+# facet-sample (2 adds into the accumulators + a 4-op complex rotation); 148 SMs x 128 FP32 lanes.
+K3_FP32_OPS_PER_FACET_SAMPLE = 6.0
+SM_COUNT, FP32_LANES_PER_SM, XU_LANES_PER_SM = 148, 128, 16
+# dram bytes per K3 launch from the committed `ncu --set full` capture (profiles/), per launch of the
+# bench configuration; None until a capture exists for the current kernel.
+K3_DRAM_TRAFFIC_BYTES = None
+
+
+def _peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        return json.loads(p.read_text()), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons during the timed region (NVML; nvidia-smi fallback)."""
+
+    def __init__(self, index: int):
+        self.index, self.samples, self.reasons = index, [], set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+
+    def _loop(self):
+        nv = self._nv
+        names = {}
+        if nv:
+            for n in dir(nv):
+                if n.startswith("nvmlClocksEventReason") or n.startswith("nvmlClocksThrottleReason"):
+                    v = getattr(nv, n)
+                    if isinstance(v, int) and v:
+                        names.setdefault(v, n.replace("nvmlClocksEventReason", "").replace("nvmlClocksThrottleReason", ""))
+        while not self._stop.is_set():
+            try:
+                if nv:
+                    self.samples.append(float(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                    try:
+                        mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self._h)
+                    except Exception:
+                        mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h)
+                    for bit, name in names.items():
+                        if mask & bit and bit & (bit - 1) == 0:
+                            self.reasons.add(name)
+                else:
+                    import subprocess
+                    out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=clocks.sm,clocks.max.sm",
+                                          "--format=csv,noheader,nounits"], capture_output=True, text=True).stdout
+                    a, b = out.strip().split(",")
+                    self.samples.append(float(a)); self.max_mhz = float(b)
+            except Exception:
+                pass
+            self._stop.wait(0.05)
+
+    def __enter__(self):
+        self._thread = threading.Thread(target=self._loop, daemon=True)
+        self._thread.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        self._thread.join(timeout=2)
+
+    def summary(self):
+        import statistics
+        s = sorted(self.samples)
+        reasons = sorted(r for r in self.reasons if r not in ("None", "GpuIdle", "ApplicationsClocksSetting"))
+        return {"sm_mhz": statistics.median(s) if s else None, "sm_max_mhz": self.max_mhz,
+                "samples": len(s), "reasons": reasons}
+
+
+def _oracle_sample(w, pulses):
+    from oracle import oracle_generate, oracle_max_threads
+    t = time.perf_counter()
+    oracle_generate(w, pulses)
+    dt = time.perf_counter() - t
+    return dt, oracle_max_threads()
+
+
+def run_reference(args):
+    """This tier's reference arm: the fp64 oracle on the host cores, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from workloads import make_workload
+    w = make_workload(args.workload)
+    F, C, P = w.n_facets, w.n_channels, w.n_pulses
+    pulses_per_step = 1
+    for _ in range(args.warmup):
+        _oracle_sample(w, [0])
+    t_total, cores = 0.0, 1
+    for k in range(args.steps):
+        dt, cores = _oracle_sample(w, [(k * 37) % P])
+        t_total += dt
+    value = F * C * pulses_per_step * args.steps / t_total
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "facets": F, "channels": C, "pulses": P,
+                   "replica_samples": w.replica_samples, "n_samples": w.n_samples},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"{pulses_per_step} pulse x {C} channels of '{args.workload}' per step "
+                                   f"({F * C} facet-echoes), {args.steps} steps"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def run_cuda(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2405_09938_b200 import Simulator
+    from workloads import make_workload
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+
+    base = make_workload(args.workload)
+    P = base.n_pulses if args.pulses is None else args.pulses
+    # weak scaling: rank r simulates pulses [r P, (r+1) P) of an N*P-pulse acquisition
+    w = make_workload(args.workload, n_pulses=P, pulse_offset=rank * P)
+    F, C, Ns, L = w.n_facets, w.n_channels, w.n_samples, w.replica_samples
+    sim = Simulator(w, local_rank)
+    out = torch.empty((C, P, Ns), dtype=torch.complex64, device=f"cuda:{local_rank}")
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing (value) ----
+    sim.set_profiling(True)
+    for _ in range(args.warmup):
+        sim.generate(0, P, out=out)
+    barrier()
+    k3_ms, k_all = [], []
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        barrier()
+        t_wall = time.perf_counter()
+        ev0.record(stream)
+        for _ in range(args.steps):
+            sim.generate(0, P, out=out)
+        ev1.record(stream)
+        barrier()
+        t_wall = time.perf_counter() - t_wall
+    elapsed_ms = ev0.elapsed_time(ev1)
+    kms = sim.kernel_ms()            # per-kernel totals of the LAST timed step (events on this stream)
+    stats = sim.stats()
+    sim.set_profiling(False)
+    t = torch.tensor([elapsed_ms], dtype=torch.float64, device=f"cuda:{local_rank}")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    elapsed_ms = float(t.item())
+    ms_per_step = elapsed_ms / args.steps
+    value = world * F * P * C / (ms_per_step * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers ----
+    xi_host = torch.from_numpy(np.ascontiguousarray(w.scene["xi"])).pin_memory()
+    maps = {"xi": xi_host}
+    h2d = xi_host.numel() * 4
+    if w.scene["sigma0_lin"] is not None:
+        maps["sigma0"] = torch.from_numpy(np.ascontiguousarray(w.scene["sigma0_lin"])).pin_memory()
+        h2d += maps["sigma0"].numel() * 4
+    if w.scene["current_mps"] is not None:
+        maps["current"] = torch.from_numpy(np.ascontiguousarray(w.scene["current_mps"])).pin_memory()
+        h2d += maps["current"].numel() * 4
+    out_host = torch.empty((C, P, Ns), dtype=torch.complex64, pin_memory=True)
+    d2h = out_host.numel() * 8
+    e2e_steps = max(1, min(args.steps, 5))
+    for _ in range(1):
+        sim.update_scene(**maps); sim.generate_host(0, P, out=out_host)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        sim.update_scene(**maps)
+        sim.generate_host(0, P, out=out_host)        # returns after the D2H copy has completed
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], dtype=torch.float64, device=f"cuda:{local_rank}")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = world * F * P * C * e2e_steps / float(te.item())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (K3, FP32 pipe) ----
+    peaks, peak_src = _peaks()
+    clk = clocks.summary()
+    n_batches = max(1, stats["kernel_launches"] // 4)
+    k3_launch_ms = kms["accumulate"] / n_batches
+    fs_per_launch = stats["facet_samples"] / n_batches
+    achieved = fs_per_launch / (k3_launch_ms * 1e-3) / 1e9            # G facet-samples/s
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    peak = SM_COUNT * FP32_LANES_PER_SM * sm_max * 1e6 / K3_FP32_OPS_PER_FACET_SAMPLE / 1e9
+    xu_model_peak = SM_COUNT * (XU_LANES_PER_SM / 2) * sm_max * 1e6 / 1e9
+    roofline = {
+        "bound": "alu", "kernel": "accumulate_kernel (K3)", "achieved": achieved, "peak": peak,
+        "unit": "Gfacet-samples/s", "frac": achieved / peak, "traffic": K3_DRAM_TRAFFIC_BYTES,
+        "peak_model": f"{SM_COUNT} SM x {FP32_LANES_PER_SM} FP32 lanes x {sm_max:.0f} MHz / "
+                      f"{K3_FP32_OPS_PER_FACET_SAMPLE:.0f} FP32 ops per facet-sample (clock: {peak_src} sm_max_mhz)",
+        "launch_ms": k3_launch_ms, "facet_samples_per_launch": fs_per_launch,
+        "frac_of_survey_xu_model": achieved / xu_model_peak,
+        "survey_xu_model_peak": xu_model_peak,
+        "kernel_ms_last_step": kms, "k3_share_of_step": kms["accumulate"] / max(sum(kms.values()), 1e-9),
+    }
+
+    # ---- the oracle on the host cores, bounded sample (reported baseline, not the target) ----
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        sample = [0, P - 1] if P > 1 else [0]
+        dt, cores = _oracle_sample(w, sample)
+        cpu = {"value": F * C * len(sample) / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"pulses {sample} x {C} channels of '{args.workload}' ({F * C * len(sample)} facet-echoes, "
+                         f"{dt:.1f} s wall)"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "ms_per_pulse": ms_per_step / P, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": args.workload, "facets": F, "channels": C, "pulses": P, "replica_samples": L,
+                   "n_samples": Ns, "wave_components": int(w.scene["n_waves"]),
+                   "parallelism": f"pulse-slab x{world}",
+                   "tile_facets": stats["tile_facets"], "pulses_per_batch": stats["pulses_per_batch"],
+                   "l2": "per-step working set (facet-echo records) is "
+                         f"{F * C * P * 32 / 1e9:.1f} GB, far larger than the 126 MB L2; no flush needed"},
+        "facet_echoes_kept_frac": stats["facet_echoes_kept"] / max(stats["facet_echoes_nominal"], 1),
+        "facet_samples_per_s": stats["facet_samples"] / (ms_per_step * 1e-3) * world,
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": e2e_steps},
+        "gpu_launches": int(stats["kernel_launches"]) * args.steps,
+        "clocks": clk,
+        "wall_s_timed_region": t_wall,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="ati")
+    ap.add_argument("--pulses", type=int, default=None, help="override the dwell length (debugging)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
