@@ -61,7 +61,28 @@ speckle_kernel(float2 *xi, int64_t n, uint64_t seed)
     xi[f] = make_float2(rad * c, rad * s);
 }
 
+__global__ void __launch_bounds__(256)
+speckle_polar_kernel(const float2 *xi, uint2 *polar, int64_t n)
+{
+    const int64_t f = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= n) return;
+    const float2 v = xi[f];
+    const double turns = atan2((double)v.y, (double)v.x) * 0.15915494309189535;     // [-0.5, 0.5]
+    const double fr = turns - floor(turns);
+    uint2 o;
+    o.x = __float_as_uint(sqrtf(v.x * v.x + v.y * v.y));
+    o.y = (uint32_t)(unsigned long long)(fr * 4294967296.0 + 0.5);
+    polar[f] = o;
+}
+
 }  // namespace
+
+cudaError_t launch_speckle_polar(const float2 *xi, uint2 *xi_polar, int64_t n_facets, cudaStream_t s)
+{
+    const int blocks = (int)((n_facets + 255) / 256);
+    speckle_polar_kernel<<<blocks, 256, 0, s>>>(xi, xi_polar, n_facets);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_finalize(const DevParams &prm, const FinalizeArgs &a, int p0, int n_pl, cudaStream_t s)
 {

@@ -92,6 +92,8 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
         float gt = 0.f, a0 = 0.f;
         double rt = 0;
         float2 xi = make_float2(0.f, 0.f);
+        float xi_mag = 0.f;
+        uint32_t xi_arg = 0u;
         size_t f = 0;
         if (valid) {
             f = (size_t)j * prm.nx + i;
@@ -119,6 +121,7 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
             }
             a0 = sqrtf(sig * area);
             xi = __ldg(a.xi + f);
+            { uint2 xp = __ldg(a.xi_polar + f); xi_mag = __uint_as_float(xp.x); xi_arg = xp.y; }
             if (kDebug) {
                 if (a.dbg_pos) { a.dbg_pos[3 * f] = pos[0]; a.dbg_pos[3 * f + 1] = pos[1]; a.dbg_pos[3 * f + 2] = pos[2]; }
                 if (a.dbg_gtx) a.dbg_gtx[f] = gt;
@@ -152,13 +155,16 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
                 const float g = a0 * gt * lr.g;
                 if (keep) {
                     Rec r;
-                    r.phi = turns_to_u32(fma(prm.kappa * cp, cp, -dR * prm.inv_lambda)) + kPhiBias;
+                    // arg(A~) = arg(xi) (+ half a turn when G_t G_r < 0): exact adds on the phase word
+                    r.phi = turns_to_u32(fma(prm.kappa * cp, cp, -dR * prm.inv_lambda)) + kPhiBias + xi_arg +
+                            ((gt * lr.g < 0.f) ? 0x80000000u : 0u);
                     r.beta = turns_to_u32(-2.0 * prm.kappa * cp);
                     double sw, cw;
                     sincospi(2.0 * ((double)(int32_t)r.beta * (1.0 / 4294967296.0)), &sw, &cw);
                     r.wr = (float)cw; r.wi = (float)sw;
-                    r.ar = g * xi.x; r.ai = g * xi.y;
-                    r.b = b; r.cnt = e - b;
+                    r.flags = (fabs(sw) < 0.1) ? 1u : 0u;          // three-term recurrence ill-conditioned
+                    r.mag = fabsf(g) * xi_mag;
+                    r.b = b; r.e = e;
                     a.recs[(((size_t)c * n_pl + pl) * prm.n_tiles + tile) * prm.tile_cap + idx] = r;
                     my_bmin[c] = min(my_bmin[c], b);
                     my_bmax[c] = max(my_bmax[c], e);

@@ -22,14 +22,15 @@ struct PulseConst {
 
 // One surviving facet-echo as the accumulation kernel consumes it (32 B, 16 B aligned).
 // Phase of sample n in turns:  phi + beta*(n - n_mid)  [+ kappa (n-n_mid)^2 applied in K4],
-// in 32-bit fixed point (2^-32 turn); valid for n in [b, b+cnt).
+// in 32-bit fixed point (2^-32 turn); valid for n in [b, e).
 struct __align__(16) Rec {
-    uint32_t phi;                // frac(-dR/lambda + kappa c'^2) * 2^32 + bias (geometry.cu kPhiBias),  c' = echo centre - n_mid [samples]
+    uint32_t phi;                // frac(-dR/lambda + kappa c'^2 + arg(A~)/2pi) * 2^32 + bias (geometry.cu kPhiBias);
+                                 // c' = echo centre - n_mid [samples], A~ = a_f G_tx G_rx,c
     uint32_t beta;               // frac(-2 kappa c') * 2^32
-    float ar, ai;                // A~ = a_f G_tx G_rx,c  (complex, without the carrier phase)
+    float mag;                   // |A~|
+    uint32_t flags;              // 0: three-term recurrence is well conditioned; 1: use the rotation
     float wr, wi;                // exp(j 2 pi beta): one-sample phase step
-    int32_t b;                   // first in-window sample n_first = ceil(nu)
-    int32_t cnt;                 // number of in-window samples (floor or ceil of T*fs)
+    int32_t b, e;                // in-window samples [b, e): b = ceil(nu), e = ceil(nu + T fs)
 };
 static_assert(sizeof(Rec) == 32, "Rec must be 32 bytes");
 

@@ -25,7 +25,8 @@ struct GeometryArgs {
     const double2 *dxy;         // or null
     const float *sigma0;        // [F] or null
     const float2 *current;      // [F] or null
-    const float2 *xi;           // [F]
+    const float2 *xi;           // [F]   complex speckle (debug outputs only)
+    const uint2 *xi_polar;      // [F]   {|xi| as float bits, arg(xi) in 2^-32 turns}
     Rec *recs;                  // [C][n_pl][n_tiles][tile_cap]
     TileInfo *tinfo;            // [n_pl][n_tiles]
     TileSpan *tspan;            // [C][n_pl][n_tiles]
@@ -44,7 +45,9 @@ struct AccumulateArgs {
     const TileSpan *tspan;
     double2 *acc;               // [C][n_pl][Ns] complex128 accumulators (zeroed by the caller)
     int block_threads;          // multiple of 32
+    int samples_per_thread;     // R in {8,10,12,14,16}
 };
+int accumulate_pick_r(double span_est_samples);
 cudaError_t launch_accumulate(const DevParams &prm, const AccumulateArgs &a, int n_pl, cudaStream_t s);
 
 // K4 -- finalize (finalize.cu): out = acc * exp(j 2 pi kappa (n-n_mid)^2) * exp(-j 2 pi f0 t0[p]) -> complex64
@@ -61,5 +64,7 @@ cudaError_t launch_finalize(const DevParams &prm, const FinalizeArgs &a, int p0,
 // Speckle from seed (G14): xi[f] = circular complex Gaussian, variance 1/2 per part, Philox4x32-10
 // keyed by seed, counter = facet index, Box-Muller.
 cudaError_t launch_speckle_from_seed(float2 *xi, int64_t n_facets, uint64_t seed, cudaStream_t s);
+// xi -> {|xi|, arg(xi)} so that K2 can fold the speckle phase into the fixed-point phase word.
+cudaError_t launch_speckle_polar(const float2 *xi, uint2 *xi_polar, int64_t n_facets, cudaStream_t s);
 
 }  // namespace heeps

@@ -16,8 +16,6 @@ using namespace heeps;
 
 namespace {
 
-constexpr int kAccumR = 8;           // samples per thread in K3 (must match accumulate.cu)
-
 struct DeviceGuard {
     int prev = -1;
     bool ok = true;
@@ -54,6 +52,7 @@ struct sim_handle {
     double chirp_rate = 0, chirp_len = 0, fs = 0;
     int pulses_per_batch = 1;
     int accum_threads = 32;
+    int accum_r = 8;                     // samples per thread in K3
     bool need_slope = false;
 
     // tables
@@ -64,6 +63,7 @@ struct sim_handle {
     // maps
     DevBuf<float> sigma0;
     DevBuf<float2> current, xi;
+    DevBuf<uint2> xi_polar;              // {|xi|, arg xi in 2^-32 turns}, derived from xi on the device
     // workspace
     DevBuf<double> z;
     DevBuf<float2> slope;
@@ -213,7 +213,7 @@ void sim_destroy(sim_handle *h)
     DeviceGuard g(h->device);
     h->xt.release(); h->yt.release(); h->tt.release(); h->chirp_n.release(); h->carrier_p.release();
     h->wk.release(); h->carrier_frac.release(); h->pulses.release();
-    h->sigma0.release(); h->current.release(); h->xi.release();
+    h->sigma0.release(); h->current.release(); h->xi.release(); h->xi_polar.release();
     h->z.release(); h->slope.release(); h->dxy.release(); h->recs.release(); h->tinfo.release();
     h->tspan.release(); h->acc.release(); h->counters.release(); h->out_staging.release();
     delete h;
@@ -281,8 +281,9 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     double wave_sum = 0;
     for (int w = 0; w < Nw; ++w) wave_sum += std::fabs(sc->amp[w]);
     const double span_est = prm.len + tile * samples_per_facet + 2.0 * 2.0 * wave_sum * prm.fs_over_c0 + 3.0;
-    int threads = 32 * (int)std::ceil(span_est / (32.0 * kAccumR));
-    h->accum_threads = std::max(32, std::min(1024, threads));
+    h->accum_r = accumulate_pick_r(span_est);
+    int threads = 32 * (int)std::ceil(span_est / (32.0 * h->accum_r));
+    h->accum_threads = std::max(32, std::min(512, threads));
 
     // ---- batch size ----
     const int64_t fcap = (int64_t)prm.n_tiles * prm.tile_cap;
@@ -382,8 +383,10 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
         CKC(cudaMemcpy(h->xi.p, sc->xi, F * sizeof(float2), cudaMemcpyHostToDevice));
     } else {
         CKC(launch_speckle_from_seed(h->xi.p, (int64_t)F, sc->seed, nullptr));
-        CKC(cudaDeviceSynchronize());
     }
+    CKC(h->xi_polar.alloc(F));
+    CKC(launch_speckle_polar(h->xi.p, h->xi_polar.p, (int64_t)F, nullptr));
+    CKC(cudaDeviceSynchronize());
     CKC(h->z.alloc(F * pb));
     if (h->need_slope) CKC(h->slope.alloc(F * pb));
     if (prm.choppy) CKC(h->dxy.alloc(F * pb));
@@ -426,12 +429,12 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         CK(h, mark());
         GeometryArgs ga{};
         ga.pulses = h->pulses.p; ga.z = h->z.p; ga.slope = h->slope.p; ga.dxy = h->dxy.p;
-        ga.sigma0 = h->sigma0.p; ga.current = h->current.p; ga.xi = h->xi.p;
+        ga.sigma0 = h->sigma0.p; ga.current = h->current.p; ga.xi = h->xi.p; ga.xi_polar = h->xi_polar.p;
         ga.recs = h->recs.p; ga.tinfo = h->tinfo.p; ga.tspan = h->tspan.p; ga.counters = h->counters.p;
         ga.carrier_frac_t0 = h->carrier_frac.p;
         CK(h, launch_geometry(prm, ga, p0, n_pl, s));
         CK(h, mark());
-        AccumulateArgs aa{h->recs.p, h->tinfo.p, h->tspan.p, h->acc.p, h->accum_threads};
+        AccumulateArgs aa{h->recs.p, h->tinfo.p, h->tspan.p, h->acc.p, h->accum_threads, h->accum_r};
         CK(h, launch_accumulate(prm, aa, n_pl, s));
         CK(h, mark());
         FinalizeArgs fa{h->acc.p, h->chirp_n.p, h->carrier_p.p, out, n_out, p0 - pb0};
@@ -481,7 +484,10 @@ int sim_update_scene(sim_handle *h, const float *sigma0_lin, const float *curren
     const size_t F = (size_t)h->n_facets;
     if (sigma0_lin) CK(h, cudaMemcpyAsync(h->sigma0.p, sigma0_lin, F * sizeof(float), cudaMemcpyHostToDevice, s));
     if (current_mps) CK(h, cudaMemcpyAsync(h->current.p, current_mps, F * sizeof(float2), cudaMemcpyHostToDevice, s));
-    if (xi) CK(h, cudaMemcpyAsync(h->xi.p, xi, F * sizeof(float2), cudaMemcpyHostToDevice, s));
+    if (xi) {
+        CK(h, cudaMemcpyAsync(h->xi.p, xi, F * sizeof(float2), cudaMemcpyHostToDevice, s));
+        CK(h, launch_speckle_polar(h->xi.p, h->xi_polar.p, (int64_t)F, s));
+    }
     return SIM_OK;
 }
 
@@ -523,7 +529,7 @@ int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, d
         CK(h, launch_kinematics(prm, ka, pulse, 1, nullptr));
         GeometryArgs ga{};
         ga.pulses = h->pulses.p; ga.z = h->z.p; ga.slope = h->need_slope ? slope_buf : nullptr; ga.dxy = h->dxy.p;
-        ga.sigma0 = h->sigma0.p; ga.current = h->current.p; ga.xi = h->xi.p;
+        ga.sigma0 = h->sigma0.p; ga.current = h->current.p; ga.xi = h->xi.p; ga.xi_polar = h->xi_polar.p;
         ga.recs = h->recs.p; ga.tinfo = h->tinfo.p; ga.tspan = h->tspan.p; ga.counters = nullptr;
         ga.dbg_pos = d_pos.p; ga.dbg_tau = d_tau.p; ga.dbg_gtx = d_gtx.p; ga.dbg_grx = d_grx.p;
         ga.dbg_amp = d_amp.p; ga.dbg_keep = d_keep.p; ga.carrier_frac_t0 = h->carrier_frac.p;
