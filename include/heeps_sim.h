@@ -155,6 +155,23 @@ int sim_get_stats(sim_handle *h, sim_stats *out);
 int sim_set_profiling(sim_handle *h, int32_t enable);
 int sim_get_kernel_ms(sim_handle *h, float ms[4]);
 
+/* Pipe-throughput microbenchmarks on `device` (the FP32 / XU / FP64 pipe peaks that
+ * bound the ALU-bound kernels are measured in the same run as the numbers quoted against them).
+ * All figures are LANE operations per second at the clock the GPU ran the probe at (an FMA = 1
+ * operation; a packed f32x2 instruction = 2).  Synchronous; takes a few tens of milliseconds. */
+typedef struct {
+    double ffma_per_s;            /* scalar FFMA                                      */
+    double fadd_per_s;            /* scalar FADD                                      */
+    double ffma2_lane_per_s;      /* packed FFMA2 (f32x2)                             */
+    double fadd2_lane_per_s;      /* packed FADD2 (f32x2)                             */
+    double mix_f32x2_lane_per_s;  /* FFMA2 and FADD2 alternating (the K3 inner loop)  */
+    double mufu_per_s;            /* MUFU.SIN / MUFU.COS                              */
+    double dfma_per_s;            /* DFMA                                             */
+    int32_t sm_count;
+    int32_t reserved[3];
+} sim_pipe_peaks;
+int sim_measure_pipe_peaks(int device, sim_pipe_peaks *out);
+
 void sim_destroy(sim_handle *h);
 const char *sim_error_string(int code);
 /* Text of the last CUDA error seen by this handle ("" if none). Valid until the next call on h. */

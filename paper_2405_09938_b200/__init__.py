@@ -21,6 +21,7 @@ from .binding import (  # noqa: F401
     sim_replica,
     sim_debug_facets,
     sim_get_stats,
+    sim_measure_pipe_peaks,
 )
 from .build import build_library  # noqa: F401
 from .sharding import pulse_slab, gather_slabs  # noqa: F401

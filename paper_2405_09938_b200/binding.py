@@ -72,6 +72,12 @@ class sim_stats(C.Structure):
     ]
 
 
+class sim_pipe_peaks(C.Structure):
+    _fields_ = [("ffma_per_s", C.c_double), ("fadd_per_s", C.c_double), ("ffma2_lane_per_s", C.c_double),
+                ("fadd2_lane_per_s", C.c_double), ("mix_f32x2_lane_per_s", C.c_double), ("mufu_per_s", C.c_double),
+                ("dfma_per_s", C.c_double), ("sm_count", C.c_int32), ("reserved", C.c_int32 * 3)]
+
+
 _lib = None
 
 
@@ -104,6 +110,8 @@ def load_library():
         lib.sim_set_profiling.argtypes = [vp, i32]
         lib.sim_get_kernel_ms.restype = C.c_int
         lib.sim_get_kernel_ms.argtypes = [vp, C.POINTER(C.c_float * 4)]
+        lib.sim_measure_pipe_peaks.restype = C.c_int
+        lib.sim_measure_pipe_peaks.argtypes = [C.c_int, C.POINTER(sim_pipe_peaks)]
         lib.sim_destroy.restype = None
         lib.sim_destroy.argtypes = [vp]
         lib.sim_error_string.restype = C.c_char_p
@@ -254,6 +262,12 @@ def sim_debug_facets(handle, pulse: int, n_facets: int, n_channels: int) -> dict
                                            ("pos", "slope", "tau", "g_tx", "g_rx", "amp", "keep"))), handle)
     res["amp"] = res["amp"][..., 0] + 1j * res["amp"][..., 1]
     return res
+
+
+def sim_measure_pipe_peaks(device: int = 0) -> dict:
+    st = sim_pipe_peaks()
+    _check(load_library().sim_measure_pipe_peaks(int(device), C.byref(st)))
+    return {k: getattr(st, k) for k, _ in sim_pipe_peaks._fields_ if k != "reserved"}
 
 
 def sim_get_stats(handle) -> dict:
