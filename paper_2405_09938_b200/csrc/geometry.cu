@@ -61,6 +61,7 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
     __shared__ int s_base;
     __shared__ int s_bmin[kMaxChannels], s_bmax[kMaxChannels];
     __shared__ unsigned long long s_samples;
+    __shared__ uint32_t s_shift[kMaxChannels];
 
     const int tile = blockIdx.x, pl = blockIdx.y, p = p0 + pl;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -75,6 +76,19 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
 
     const int C = prm.n_channels, ts = prm.tile;
     const int ti0 = (tile % prm.tiles_x) * ts, tj0 = (tile / prm.tiles_x) * ts;
+    if (tid < C) {
+        // frequency shift of this (tile, pulse, channel): a quarter cycle per sample minus the dechirped
+        // tone frequency of the tile centre (rest position, flat surface)
+        const double ic = ti0 + 0.5 * (min(ts, prm.nx - ti0) - 1), jc = tj0 + 0.5 * (min(ts, prm.ny - tj0) - 1);
+        const double x = prm.cx + (ic - 0.5 * (prm.nx - 1)) * prm.spacing;
+        const double y = prm.cy + (jc - 0.5 * (prm.ny - 1)) * prm.spacing;
+        const double ax = x - pc.tx_pos[0], ay = y - pc.tx_pos[1], az = prm.cz - pc.tx_pos[2];
+        const double bx = x - pc.rx_pos[tid][0], by = y - pc.rx_pos[tid][1], bz = prm.cz - pc.rx_pos[tid][2];
+        const double dR = sqrt(ax * ax + ay * ay + az * az) + sqrt(bx * bx + by * by + bz * bz) - pc.r0;
+        const double cpc = dR * prm.fs_over_c0 - (double)prm.n_mid;
+        s_shift[tid] = turns_to_u32(0.25 + 2.0 * prm.kappa * cpc);
+    }
+    __syncthreads();
     const size_t F = (size_t)prm.nx * prm.ny;
     const float area = (float)(prm.spacing * prm.spacing);
     unsigned long long my_samples = 0;
@@ -158,7 +172,7 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
                     // arg(A~) = arg(xi) (+ half a turn when G_t G_r < 0): exact adds on the phase word
                     r.phi = turns_to_u32(fma(prm.kappa * cp, cp, -dR * prm.inv_lambda)) + kPhiBias + xi_arg +
                             ((gt * lr.g < 0.f) ? 0x80000000u : 0u);
-                    r.beta = turns_to_u32(-2.0 * prm.kappa * cp);
+                    r.beta = turns_to_u32(-2.0 * prm.kappa * cp) + s_shift[c];
                     double sw, cw;
                     sincospi(2.0 * ((double)(int32_t)r.beta * (1.0 / 4294967296.0)), &sw, &cw);
                     r.wr = (float)cw; r.wi = (float)sw;
@@ -211,6 +225,7 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
     if (tid < C) {
         TileSpan sp;
         sp.bmin = s_bmin[tid]; sp.bmax_end = s_bmax[tid];
+        sp.shift = s_shift[tid]; sp.pad = 0u;
         a.tspan[((size_t)tid * n_pl + pl) * prm.n_tiles + tile] = sp;
     }
 }

@@ -23,13 +23,17 @@ struct PulseConst {
 // One surviving facet-echo as the accumulation kernel consumes it (32 B, 16 B aligned).
 // Phase of sample n in turns:  phi + beta*(n - n_mid)  [+ kappa (n-n_mid)^2 applied in K4],
 // in 32-bit fixed point (2^-32 turn); valid for n in [b, e).
+// K2 adds a per-(tile, pulse, channel) frequency shift beta_s to every record of a tile so that the
+// shifted tone frequency sits near a quarter cycle per sample (three-term recurrence best conditioned);
+// K3 accumulates in that rotating frame and removes exp(j 2 pi beta_s (n - n_mid)) once per tile and sample.
 struct __align__(16) Rec {
     uint32_t phi;                // frac(-dR/lambda + kappa c'^2 + arg(A~)/2pi) * 2^32 + bias (geometry.cu kPhiBias);
                                  // c' = echo centre - n_mid [samples], A~ = a_f G_tx G_rx,c
-    uint32_t beta;               // frac(-2 kappa c') * 2^32
+    uint32_t beta;               // frac(-2 kappa c' + beta_s) * 2^32
     float mag;                   // |A~|
+    float wr;                    // Re exp(j 2 pi beta): one-sample phase step (shifted frame)
+    float wi;                    // Im exp(j 2 pi beta)
     uint32_t flags;              // 0: three-term recurrence is well conditioned; 1: use the rotation
-    float wr, wi;                // exp(j 2 pi beta): one-sample phase step
     int32_t b, e;                // in-window samples [b, e): b = ceil(nu), e = ceil(nu + T fs)
 };
 static_assert(sizeof(Rec) == 32, "Rec must be 32 bytes");
@@ -37,8 +41,10 @@ static_assert(sizeof(Rec) == 32, "Rec must be 32 bytes");
 struct TileInfo {               // per (pulse-in-batch, tile)
     int32_t nrec;               // surviving facets (same for every channel)
 };
-struct TileSpan {               // per (channel, pulse-in-batch, tile)
-    int32_t bmin, bmax_end;     // min b and max (b+cnt) over the tile's records
+struct __align__(16) TileSpan {  // per (channel, pulse-in-batch, tile)
+    int32_t bmin, bmax_end;     // min b and max e over the tile's records
+    uint32_t shift;             // beta_s in 2^-32 turns
+    uint32_t pad;
 };
 
 // Scalars every kernel needs.

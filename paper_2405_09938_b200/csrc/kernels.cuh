@@ -44,10 +44,18 @@ struct AccumulateArgs {
     const TileInfo *tinfo;
     const TileSpan *tspan;
     double2 *acc;               // [C][n_pl][Ns] complex128 accumulators (zeroed by the caller)
-    int block_threads;          // multiple of 32
-    int samples_per_thread;     // R in {8,10,12,14,16}
+    int block_threads;          // (warp groups) x warps_per_span x 32
+    int samples_per_thread;     // R: a lane owns R consecutive samples of a record's window
+    int warps_per_span;         // warps that together cover one window (32 R warps_per_span >= ceil(T fs))
+    int span_cap;               // entries of each warp's shared-memory span array
+    size_t smem_bytes;          // dynamic shared memory of the launch
 };
-int accumulate_pick_r(double span_est_samples);
+struct AccumulatePlan {
+    int block_threads, samples_per_thread, warps_per_span, span_cap;
+    size_t smem_bytes;
+};
+// Launch shape from the replica length and the expected delay spread of a spatial tile [samples].
+AccumulatePlan accumulate_plan(const DevParams &prm, double tile_spread_samples);
 cudaError_t launch_accumulate(const DevParams &prm, const AccumulateArgs &a, int n_pl, cudaStream_t s);
 
 // K4 -- finalize (finalize.cu): out = acc * exp(j 2 pi kappa (n-n_mid)^2) * exp(-j 2 pi f0 t0[p]) -> complex64

@@ -51,8 +51,7 @@ struct sim_handle {
     int64_t n_facets = 0;
     double chirp_rate = 0, chirp_len = 0, fs = 0;
     int pulses_per_batch = 1;
-    int accum_threads = 32;
-    int accum_r = 8;                     // samples per thread in K3
+    AccumulatePlan accum{};              // K3 launch shape
     bool need_slope = false;
 
     // tables
@@ -280,16 +279,14 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     prm.tile_cap = tile * tile;
     double wave_sum = 0;
     for (int w = 0; w < Nw; ++w) wave_sum += std::fabs(sc->amp[w]);
-    const double span_est = prm.len + tile * samples_per_facet + 2.0 * 2.0 * wave_sum * prm.fs_over_c0 + 3.0;
-    h->accum_r = accumulate_pick_r(span_est);
-    int threads = 32 * (int)std::ceil(span_est / (32.0 * h->accum_r));
-    h->accum_threads = std::max(32, std::min(512, threads));
+    const double tile_spread = tile * samples_per_facet + 2.0 * 2.0 * wave_sum * prm.fs_over_c0 + 3.0;
+    h->accum = accumulate_plan(prm, tile_spread);
 
     // ---- batch size ----
     const int64_t fcap = (int64_t)prm.n_tiles * prm.tile_cap;
     const int64_t per_pulse = (int64_t)C * fcap * (int64_t)sizeof(Rec) + h->n_facets * 8 +
                               (h->need_slope ? h->n_facets * 8 : 0) + (prm.choppy ? h->n_facets * 16 : 0) +
-                              (int64_t)C * Ns * 16 + (int64_t)prm.n_tiles * (4 + 8 * C);
+                              (int64_t)C * Ns * 16 + (int64_t)prm.n_tiles * (4 + 16 * C);
     int64_t ws = (opts && opts->workspace_bytes > 0) ? opts->workspace_bytes : ((int64_t)4 << 30);
     int pb = (int)std::max<int64_t>(1, std::min<int64_t>(ws / std::max<int64_t>(per_pulse, 1), 256));
     if (opts && opts->pulses_per_batch > 0) pb = opts->pulses_per_batch;
@@ -398,7 +395,7 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     CKC(cudaMemset(h->counters.p, 0, 2 * sizeof(unsigned long long)));
 #undef CKC
     h->stats.tile_facets = tile; h->stats.pulses_per_batch = pb; h->stats.n_tiles = prm.n_tiles;
-    h->stats.accumulate_block_threads = h->accum_threads;
+    h->stats.accumulate_block_threads = h->accum.block_threads;
     *out = h;
     return SIM_OK;
 }
@@ -434,7 +431,8 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         ga.carrier_frac_t0 = h->carrier_frac.p;
         CK(h, launch_geometry(prm, ga, p0, n_pl, s));
         CK(h, mark());
-        AccumulateArgs aa{h->recs.p, h->tinfo.p, h->tspan.p, h->acc.p, h->accum_threads, h->accum_r};
+        AccumulateArgs aa{h->recs.p, h->tinfo.p, h->tspan.p, h->acc.p, h->accum.block_threads,
+                          h->accum.samples_per_thread, h->accum.warps_per_span, h->accum.span_cap, h->accum.smem_bytes};
         CK(h, launch_accumulate(prm, aa, n_pl, s));
         CK(h, mark());
         FinalizeArgs fa{h->acc.p, h->chirp_n.p, h->carrier_p.p, out, n_out, p0 - pb0};
