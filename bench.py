@@ -30,13 +30,14 @@ sys.path.insert(0, str(ROOT))
 METRIC = "facet_echoes_per_s"
 UNIT = "facet-echoes/s"
 
-# FP32-pipe roofline of K3: the inner loop spends 6 FP32-pipe operations per
-# facet-sample (2 adds into the accumulators + a 4-op complex rotation); 148 SMs x 128 FP32 lanes.
-K3_FP32_OPS_PER_FACET_SAMPLE = 6.0
+# FP32-pipe roofline of K3: the inner loop spends 4 FP32 lane-operations per
+# facet-sample (one packed FFMA2 of the three-term recurrence + one packed FADD2 into the accumulators);
+# 148 SMs x 128 FP32 lanes.
+K3_FP32_OPS_PER_FACET_SAMPLE = 4.0
 SM_COUNT, FP32_LANES_PER_SM, XU_LANES_PER_SM = 148, 128, 16
-# dram bytes per K3 launch from the committed `ncu --set full` capture (profiles/), per launch of the
-# bench configuration; None until a capture exists for the current kernel.
-K3_DRAM_TRAFFIC_BYTES = None
+# dram bytes per kept facet-echo of a K3 launch, from the committed `ncu --set full` capture
+# profiles/r1_v3_k3_ncu_summary.txt: (2.580977e9 read + 1.1966e7 written) / (100 pulses x 3 ch x 262144).
+K3_DRAM_BYTES_PER_FACET_ECHO = (2.580977e9 + 1.1966e7) / (100 * 3 * 262144)
 
 
 def _peaks():
@@ -249,11 +250,17 @@ def run_cuda(args):
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     peak = SM_COUNT * FP32_LANES_PER_SM * sm_max * 1e6 / K3_FP32_OPS_PER_FACET_SAMPLE / 1e9
     xu_model_peak = SM_COUNT * (XU_LANES_PER_SM / 2) * sm_max * 1e6 / 1e9
+    from paper_2405_09938_b200 import sim_measure_pipe_peaks
+    pipes = sim_measure_pipe_peaks(local_rank)      # same-run pipe microbenchmarks
+    pipe_peak = pipes["mix_f32x2_lane_per_s"] / K3_FP32_OPS_PER_FACET_SAMPLE / 1e9
     roofline = {
         "bound": "alu", "kernel": "accumulate_kernel (K3)", "achieved": achieved, "peak": peak,
-        "unit": "Gfacet-samples/s", "frac": achieved / peak, "traffic": K3_DRAM_TRAFFIC_BYTES,
+        "unit": "Gfacet-samples/s", "frac": achieved / peak,
+        "traffic": K3_DRAM_BYTES_PER_FACET_ECHO * stats["facet_echoes_kept"] / n_batches,
         "peak_model": f"{SM_COUNT} SM x {FP32_LANES_PER_SM} FP32 lanes x {sm_max:.0f} MHz / "
                       f"{K3_FP32_OPS_PER_FACET_SAMPLE:.0f} FP32 ops per facet-sample (clock: {peak_src} sm_max_mhz)",
+        "measured_pipe_peak": pipe_peak, "frac_of_measured_pipe_peak": achieved / pipe_peak,
+        "pipe_peaks_lane_ops_per_s": {k: v for k, v in pipes.items() if k.endswith("_per_s")},
         "launch_ms": k3_launch_ms, "facet_samples_per_launch": fs_per_launch,
         "frac_of_survey_xu_model": achieved / xu_model_peak,
         "survey_xu_model_peak": xu_model_peak,

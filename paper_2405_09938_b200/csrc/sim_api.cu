@@ -291,6 +291,10 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     int pb = (int)std::max<int64_t>(1, std::min<int64_t>(ws / std::max<int64_t>(per_pulse, 1), 256));
     if (opts && opts->pulses_per_batch > 0) pb = opts->pulses_per_batch;
     pb = std::min(pb, P);
+    if (!(opts && opts->pulses_per_batch > 0)) {        // balance the batches of a full-dwell call
+        const int nb = (P + pb - 1) / pb;
+        pb = (P + nb - 1) / nb;
+    }
     h->pulses_per_batch = pb;
 
     // ---- host tables (fp64) ----
