@@ -90,12 +90,24 @@ typedef struct {
     uint64_t seed;
 } sim_scene;
 
+/* Echo accumulation.  Both evaluate the same defined sum:
+ *   DIRECT   every facet-echo's chirp replica is generated and added sample by sample;
+ *   SPECTRAL facet-echoes are summed into range slices (eq. 17) as Kt = 8 Chebyshev moments of the
+ *            sub-slice position, and the slices are convolved with the waveform by FFT (the paper's
+ *            "impulse response ... subsequently convolved by the waveform", with the sub-slice term
+ *            kept to ~1e-6).  Needs T*fs integer and Ns + T*fs - 1 <= 16384.
+ *   AUTO     SPECTRAL where it applies, DIRECT otherwise. */
+#define SIM_ACCUMULATE_AUTO     0
+#define SIM_ACCUMULATE_DIRECT   1
+#define SIM_ACCUMULATE_SPECTRAL 2
+
 /* Tunables; zero-initialise for defaults. */
 typedef struct {
-    int32_t tile_facets;           /* spatial tile side in facets (8..64, power of 2); 0 = auto from L and spacing */
+    int32_t tile_facets;           /* spatial tile side in facets (4..64, power of 2; SPECTRAL clamps to 32); 0 = auto */
     int32_t pulses_per_batch;      /* 0 = auto from workspace_bytes */
     int64_t workspace_bytes;       /* cap for per-batch device workspace; 0 = 4 GiB */
-    int32_t reserved[8];
+    int32_t accumulate_mode;       /* SIM_ACCUMULATE_*; SPECTRAL where it does not apply -> SIM_EINVAL */
+    int32_t reserved[7];
 } sim_options;
 
 /*
@@ -146,12 +158,15 @@ typedef struct {
     int64_t kernel_launches;       /* kernels launched by the call                     */
     int32_t tile_facets, pulses_per_batch, n_tiles, accumulate_block_threads;
     int32_t max_span_samples;      /* largest per-tile sample span seen                */
-    int32_t reserved[3];
+    int32_t accumulate_mode;       /* SIM_ACCUMULATE_DIRECT or _SPECTRAL, as resolved at sim_create */
+    int32_t fft_size;              /* SPECTRAL: transform length; else 0              */
+    int32_t reserved[1];
 } sim_stats;
 int sim_get_stats(sim_handle *h, sim_stats *out);
 
 /* Per-kernel device time of the most recent call, measured with CUDA events on the caller's
- * stream when enabled (adds event records only): ms[0..3] = K1, K2, K3, K4 totals. */
+ * stream when enabled (adds event records only): ms[0..3] = K1, K2, K3, K4 totals (SPECTRAL: K1 kinematics,
+ * K2s geometry + moments, K3s FFT convolution + finalize, 0). */
 int sim_set_profiling(sim_handle *h, int32_t enable);
 int sim_get_kernel_ms(sim_handle *h, float ms[4]);
 

@@ -17,6 +17,8 @@ HEADER_PATH = Path(__file__).resolve().parent.parent / "include" / "heeps_sim.h"
 
 SIM_OK, SIM_EINVAL, SIM_ERANGE, SIM_ENOMEM, SIM_ECUDA = 0, -1, -2, -3, -4
 SIM_MAX_CHANNELS = 8
+SIM_ACCUMULATE_AUTO, SIM_ACCUMULATE_DIRECT, SIM_ACCUMULATE_SPECTRAL = 0, 1, 2
+_MODES = {"auto": 0, "direct": 1, "spectral": 2, 0: 0, 1: 1, 2: 2}
 
 
 class SimError(RuntimeError):
@@ -60,7 +62,7 @@ class sim_scene(C.Structure):
 
 class sim_options(C.Structure):
     _fields_ = [("tile_facets", C.c_int32), ("pulses_per_batch", C.c_int32), ("workspace_bytes", C.c_int64),
-                ("reserved", C.c_int32 * 8)]
+                ("accumulate_mode", C.c_int32), ("reserved", C.c_int32 * 7)]
 
 
 class sim_stats(C.Structure):
@@ -68,7 +70,8 @@ class sim_stats(C.Structure):
         ("facet_echoes_nominal", C.c_int64), ("facet_echoes_kept", C.c_int64), ("facet_samples", C.c_int64),
         ("kernel_launches", C.c_int64),
         ("tile_facets", C.c_int32), ("pulses_per_batch", C.c_int32), ("n_tiles", C.c_int32),
-        ("accumulate_block_threads", C.c_int32), ("max_span_samples", C.c_int32), ("reserved", C.c_int32 * 3),
+        ("accumulate_block_threads", C.c_int32), ("max_span_samples", C.c_int32),
+        ("accumulate_mode", C.c_int32), ("fft_size", C.c_int32), ("reserved", C.c_int32 * 1),
     ]
 
 
@@ -215,11 +218,12 @@ def _marshal(workload):
 # ----------------------------------------------------------------------------- C-named functions
 
 def sim_create(workload, device: int = 0, *, tile_facets: int = 0, pulses_per_batch: int = 0,
-               workspace_bytes: int = 0):
+               workspace_bytes: int = 0, accumulate_mode=0):
     lib = load_library()
     ci, cg, cs, keep = _marshal(workload)
     opts = sim_options()
     opts.tile_facets, opts.pulses_per_batch, opts.workspace_bytes = tile_facets, pulses_per_batch, workspace_bytes
+    opts.accumulate_mode = _MODES[accumulate_mode]
     h = C.c_void_p()
     rc = lib.sim_create(C.byref(ci), C.byref(cg), C.byref(cs), C.byref(opts), int(device), C.byref(h))
     del keep

@@ -75,4 +75,43 @@ cudaError_t launch_speckle_from_seed(float2 *xi, int64_t n_facets, uint64_t seed
 // xi -> {|xi|, arg(xi)} so that K2 can fold the speckle phase into the fixed-point phase word.
 cudaError_t launch_speckle_polar(const float2 *xi, uint2 *xi_polar, int64_t n_facets, cudaStream_t s);
 
+// ---- spectral path (moments.cu, fftconv.cu) ----
+constexpr int kMomentOrder = 8;   // Kt Chebyshev moments per range slice (truncation ~ J_8(pi B / 2 fs) ~ 1e-6)
+
+// K2s -- geometry, gains, amplitude, cull, range-slice moments (moments.cu).
+struct MomentArgs {
+    const PulseConst *pulses;   // [P]
+    const double *z;            // from K1
+    const float2 *slope;        // or null
+    const double2 *dxy;         // or null
+    const float *sigma0;        // [F] or null
+    const float2 *current;      // [F] or null
+    const uint2 *xi_polar;      // [F]
+    float2 *mom;                // [C][n_pl][Kt][nb_pad] complex moments, slice b at index b + L - 1 (zeroed by the caller)
+    int32_t nb_pad;             // row stride (>= Ns + L - 1)
+    int32_t span_cap;           // slices of a tile's shared-memory window
+    int32_t replica;            // L = T fs (integer on this path)
+    unsigned long long *counters;
+};
+size_t moments_smem_bytes(const DevParams &prm, int span_cap);
+cudaError_t launch_moments(const DevParams &prm, const MomentArgs &a, int p0, int n_pl, cudaStream_t s);
+
+// K3s -- convolution of the moments with the waveform kernels + finalize (fftconv.cu).
+struct FftConvArgs {
+    const float2 *mom;          // [C][n_pl][Kt][nb_pad]
+    const float2 *cspec;        // [Kt][nfft]  FFT(c_k)/nfft in the forward transform's output order
+    const float2 *tw;           // [nfft]      exp(-2 pi i k / nfft)
+    const double2 *carrier_p;   // [P]         exp(-j 2 pi f0 t0[p])
+    float2 *out;                // [C][n_out_pulses][Ns]
+    int32_t n_out_pulses, out_pulse0;
+    int32_t nfft;               // power of two, 256..16384, >= Ns + L - 1
+    int32_t nb;                 // Ns + L - 1 valid slices
+    int32_t nb_pad;
+    int32_t replica;            // L
+};
+cudaError_t launch_fftconv(const DevParams &prm, const FftConvArgs &a, int p0, int n_pl, cudaStream_t s);
+// cspec[k] = FFT(zero-padded ck[k][0..L)) / nfft for k < Kt (run once at sim_create).
+cudaError_t launch_kernel_spectra(int nfft, const float2 *ck, int replica, const float2 *tw, float2 *cspec,
+                                  cudaStream_t s);
+
 }  // namespace heeps

@@ -53,6 +53,8 @@ struct sim_handle {
     int pulses_per_batch = 1;
     AccumulatePlan accum{};              // K3 launch shape
     bool need_slope = false;
+    bool spectral = false;               // accumulate_mode resolved at sim_create
+    int nfft = 0, nb = 0, nb_pad = 0, replica = 0, span_cap_m = 0;
 
     // tables
     DevBuf<double2> xt, yt, tt, chirp_n, carrier_p;
@@ -73,6 +75,8 @@ struct sim_handle {
     DevBuf<double2> acc;
     DevBuf<unsigned long long> counters;
     DevBuf<float2> out_staging;
+    // spectral path
+    DevBuf<float2> mom, cspec, tw;
 
     // bookkeeping
     sim_stats stats{};
@@ -215,6 +219,7 @@ void sim_destroy(sim_handle *h)
     h->sigma0.release(); h->current.release(); h->xi.release(); h->xi_polar.release();
     h->z.release(); h->slope.release(); h->dxy.release(); h->recs.release(); h->tinfo.release();
     h->tspan.release(); h->acc.release(); h->counters.release(); h->out_staging.release();
+    h->mom.release(); h->cspec.release(); h->tw.release();
     delete h;
 }
 
@@ -229,6 +234,7 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
         int t = opts->tile_facets;
         if (t < 4 || t > 64 || (t & (t - 1))) return SIM_EINVAL;
     }
+    if (opts && (opts->accumulate_mode < 0 || opts->accumulate_mode > 2)) return SIM_EINVAL;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
         cudaGetLastError();
@@ -264,11 +270,29 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     prm.cur_ux = sc->current_uniform[0]; prm.cur_uy = sc->current_uniform[1];
     h->need_slope = prm.tilt != 0;
 
+    // ---- accumulation mode (SIM_ACCUMULATE_*): the spectral path needs an integer replica length
+    //      (one waveform kernel for every facet) and a transform that fits shared memory ----
+    const double len_round = std::nearbyint(prm.len);
+    const bool len_integer = std::fabs(prm.len - len_round) < 1e-9 * std::max(1.0, prm.len) && len_round >= 1.0;
+    int nfft = 256;
+    while (nfft < Ns + (int)len_round - 1 && nfft < (1 << 20)) nfft <<= 1;
+    const bool spectral_ok = len_integer && nfft <= 16384;
+    const int mode = opts ? opts->accumulate_mode : SIM_ACCUMULATE_AUTO;
+    if (mode == SIM_ACCUMULATE_SPECTRAL && !spectral_ok) { delete h; return SIM_EINVAL; }
+    h->spectral = (mode == SIM_ACCUMULATE_SPECTRAL) || (mode == SIM_ACCUMULATE_AUTO && spectral_ok);
+    h->replica = (int)len_round;
+    h->nfft = nfft;
+    h->nb = Ns + h->replica - 1;
+    h->nb_pad = (h->nb + 3) & ~3;
+
     // ---- tiling: a spatial tile must stay narrow in delay compared with the replica ----
     const double grad = std::max(0.25, path_gradient_l1(g, sc));
     const double samples_per_facet = sc->spacing_m * grad * prm.fs_over_c0;   // delay spread per facet step
     int tile = opts ? opts->tile_facets : 0;
-    if (tile == 0) {
+    if (h->spectral) {
+        if (tile == 0) tile = 32;
+        tile = std::min(tile, 32);                                // facet state lives in registers (moments.cu)
+    } else if (tile == 0) {
         tile = 64;
         const double budget = std::max(16.0, prm.len / 12.0);     // spread <= ~8 % of the replica
         while (tile > 8 && tile * samples_per_facet > budget) tile >>= 1;
@@ -281,12 +305,16 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     for (int w = 0; w < Nw; ++w) wave_sum += std::fabs(sc->amp[w]);
     const double tile_spread = tile * samples_per_facet + 2.0 * 2.0 * wave_sum * prm.fs_over_c0 + 3.0;
     h->accum = accumulate_plan(prm, tile_spread);
+    h->span_cap_m = std::min(4096, (((int)std::ceil(tile_spread) + 8) + 31) & ~31);
 
     // ---- batch size ----
     const int64_t fcap = (int64_t)prm.n_tiles * prm.tile_cap;
-    const int64_t per_pulse = (int64_t)C * fcap * (int64_t)sizeof(Rec) + h->n_facets * 8 +
-                              (h->need_slope ? h->n_facets * 8 : 0) + (prm.choppy ? h->n_facets * 16 : 0) +
-                              (int64_t)C * Ns * 16 + (int64_t)prm.n_tiles * (4 + 16 * C);
+    const int64_t per_pulse_common = h->n_facets * 8 + (h->need_slope ? h->n_facets * 8 : 0) +
+                                     (prm.choppy ? h->n_facets * 16 : 0);
+    const int64_t per_pulse = per_pulse_common +
+        (h->spectral ? (int64_t)C * kMomentOrder * h->nb_pad * 8
+                     : (int64_t)C * fcap * (int64_t)sizeof(Rec) + (int64_t)C * Ns * 16 +
+                           (int64_t)prm.n_tiles * (4 + 16 * C));
     int64_t ws = (opts && opts->workspace_bytes > 0) ? opts->workspace_bytes : ((int64_t)4 << 30);
     int pb = (int)std::max<int64_t>(1, std::min<int64_t>(ws / std::max<int64_t>(per_pulse, 1), 256));
     if (opts && opts->pulses_per_batch > 0) pb = opts->pulses_per_batch;
@@ -391,15 +419,57 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     CKC(h->z.alloc(F * pb));
     if (h->need_slope) CKC(h->slope.alloc(F * pb));
     if (prm.choppy) CKC(h->dxy.alloc(F * pb));
-    CKC(h->recs.alloc((size_t)C * pb * fcap));
-    CKC(h->tinfo.alloc((size_t)pb * prm.n_tiles));
-    CKC(h->tspan.alloc((size_t)C * pb * prm.n_tiles));
-    CKC(h->acc.alloc((size_t)C * pb * Ns));
+    if (!h->spectral) {
+        CKC(h->recs.alloc((size_t)C * pb * fcap));
+        CKC(h->tinfo.alloc((size_t)pb * prm.n_tiles));
+        CKC(h->tspan.alloc((size_t)C * pb * prm.n_tiles));
+        CKC(h->acc.alloc((size_t)C * pb * Ns));
+    } else {
+        // waveform kernels c_k[m] = exp(j 2 pi kappa ((m-L/2)^2 + (m-L/2))) e_k j^k J_k(2 pi kappa (m-L/2))
+        // (moments.cu header), their spectra, and the transform's twiddle table
+        const int L = h->replica;
+        std::vector<float2> ck((size_t)kMomentOrder * L), tw((size_t)nfft);
+        for (int m = 0; m < L; ++m) {
+            const long double mm = (long double)m - 0.5L * (long double)L;
+            long double turns = (long double)prm.kappa * (mm * mm + mm);
+            turns -= floorl(turns);
+            const double cr = std::cos(2.0 * M_PI * (double)turns), ci = std::sin(2.0 * M_PI * (double)turns);
+            const double zarg = 2.0 * M_PI * prm.kappa * (double)mm;
+            for (int k = 0; k < kMomentOrder; ++k) {
+                const double jk = (k == 0 ? 1.0 : 2.0) * jn(k, zarg);
+                double re = cr * jk, im = ci * jk, t;
+                switch (k & 3) {                                   // * j^k
+                    case 1: t = re; re = -im; im = t; break;
+                    case 2: re = -re; im = -im; break;
+                    case 3: t = re; re = im; im = -t; break;
+                    default: break;
+                }
+                ck[(size_t)k * L + m] = make_float2((float)re, (float)im);
+            }
+        }
+        for (int k = 0; k < nfft; ++k) {
+            const double a = -2.0 * M_PI * (double)k / (double)nfft;
+            tw[k] = make_float2((float)std::cos(a), (float)std::sin(a));
+        }
+        DevBuf<float2> d_ck;
+        CKC(d_ck.alloc(ck.size()));
+        CKC(h->tw.alloc(tw.size()));
+        CKC(h->cspec.alloc((size_t)kMomentOrder * nfft));
+        CKC(cudaMemcpy(d_ck.p, ck.data(), ck.size() * sizeof(float2), cudaMemcpyHostToDevice));
+        CKC(cudaMemcpy(h->tw.p, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice));
+        cudaError_t e_spec = launch_kernel_spectra(nfft, d_ck.p, L, h->tw.p, h->cspec.p, nullptr);
+        if (e_spec == cudaSuccess) e_spec = cudaDeviceSynchronize();
+        d_ck.release();
+        CKC(e_spec);
+        CKC(h->mom.alloc((size_t)C * pb * kMomentOrder * h->nb_pad));
+    }
     CKC(h->counters.alloc(2));
     CKC(cudaMemset(h->counters.p, 0, 2 * sizeof(unsigned long long)));
 #undef CKC
     h->stats.tile_facets = tile; h->stats.pulses_per_batch = pb; h->stats.n_tiles = prm.n_tiles;
     h->stats.accumulate_block_threads = h->accum.block_threads;
+    h->stats.accumulate_mode = h->spectral ? SIM_ACCUMULATE_SPECTRAL : SIM_ACCUMULATE_DIRECT;
+    h->stats.fft_size = h->spectral ? nfft : 0;
     *out = h;
     return SIM_OK;
 }
@@ -421,7 +491,30 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         }
         return cudaEventRecord(h->events[h->events_used++], s);
     };
-    for (int p0 = pb0; p0 < pb1; p0 += h->pulses_per_batch) {
+    for (int p0 = pb0; h->spectral && p0 < pb1; p0 += h->pulses_per_batch) {
+        const int n_pl = std::min(h->pulses_per_batch, pb1 - p0);
+        CK(h, cudaMemsetAsync(h->mom.p, 0, (size_t)prm.n_channels * n_pl * kMomentOrder * h->nb_pad * sizeof(float2), s));
+        CK(h, mark());
+        KinematicsArgs ka{h->xt.p, h->yt.p, h->tt.p, h->wk.p, h->n_pulses, h->z.p, h->slope.p, h->dxy.p};
+        CK(h, launch_kinematics(prm, ka, p0, n_pl, s));
+        CK(h, mark());
+        MomentArgs ma{};
+        ma.pulses = h->pulses.p; ma.z = h->z.p; ma.slope = h->slope.p; ma.dxy = h->dxy.p;
+        ma.sigma0 = h->sigma0.p; ma.current = h->current.p; ma.xi_polar = h->xi_polar.p;
+        ma.mom = h->mom.p; ma.nb_pad = h->nb_pad; ma.span_cap = h->span_cap_m; ma.replica = h->replica;
+        ma.counters = h->counters.p;
+        CK(h, launch_moments(prm, ma, p0, n_pl, s));
+        CK(h, mark());
+        FftConvArgs fa{};
+        fa.mom = h->mom.p; fa.cspec = h->cspec.p; fa.tw = h->tw.p; fa.carrier_p = h->carrier_p.p;
+        fa.out = out; fa.n_out_pulses = n_out; fa.out_pulse0 = p0 - pb0;
+        fa.nfft = h->nfft; fa.nb = h->nb; fa.nb_pad = h->nb_pad; fa.replica = h->replica;
+        CK(h, launch_fftconv(prm, fa, p0, n_pl, s));
+        CK(h, mark());
+        CK(h, mark());                                   // K4 slot: finalize is fused into K3s
+        launches += 3;
+    }
+    for (int p0 = pb0; !h->spectral && p0 < pb1; p0 += h->pulses_per_batch) {
         const int n_pl = std::min(h->pulses_per_batch, pb1 - p0);
         CK(h, cudaMemsetAsync(h->acc.p, 0, (size_t)prm.n_channels * n_pl * prm.n_samples * sizeof(double2), s));
         CK(h, mark());
@@ -521,8 +614,17 @@ int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, d
     DevBuf<double> d_pos, d_tau, d_gtx, d_grx, d_amp;
     DevBuf<int32_t> d_keep;
     DevBuf<float2> d_slope;
+    DevBuf<Rec> d_recs;                  // spectral handles own no record workspace
+    DevBuf<TileInfo> d_tinfo;
+    DevBuf<TileSpan> d_tspan;
     int rc = SIM_OK;
     auto run = [&]() -> int {
+        Rec *recs = h->recs.p; TileInfo *tinfo = h->tinfo.p; TileSpan *tspan = h->tspan.p;
+        if (!recs) {
+            CK(h, d_recs.alloc(C * (size_t)prm.n_tiles * prm.tile_cap)); CK(h, d_tinfo.alloc(prm.n_tiles));
+            CK(h, d_tspan.alloc(C * (size_t)prm.n_tiles));
+            recs = d_recs.p; tinfo = d_tinfo.p; tspan = d_tspan.p;
+        }
         CK(h, d_pos.alloc(3 * F)); CK(h, d_tau.alloc(C * F)); CK(h, d_gtx.alloc(F));
         CK(h, d_grx.alloc(C * F)); CK(h, d_amp.alloc(2 * C * F)); CK(h, d_keep.alloc(F));
         float2 *slope_buf = h->slope.p;
@@ -532,7 +634,7 @@ int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, d
         GeometryArgs ga{};
         ga.pulses = h->pulses.p; ga.z = h->z.p; ga.slope = h->need_slope ? slope_buf : nullptr; ga.dxy = h->dxy.p;
         ga.sigma0 = h->sigma0.p; ga.current = h->current.p; ga.xi = h->xi.p; ga.xi_polar = h->xi_polar.p;
-        ga.recs = h->recs.p; ga.tinfo = h->tinfo.p; ga.tspan = h->tspan.p; ga.counters = nullptr;
+        ga.recs = recs; ga.tinfo = tinfo; ga.tspan = tspan; ga.counters = nullptr;
         ga.dbg_pos = d_pos.p; ga.dbg_tau = d_tau.p; ga.dbg_gtx = d_gtx.p; ga.dbg_grx = d_grx.p;
         ga.dbg_amp = d_amp.p; ga.dbg_keep = d_keep.p; ga.carrier_frac_t0 = h->carrier_frac.p;
         CK(h, launch_geometry(prm, ga, pulse, 1, nullptr));
@@ -552,7 +654,7 @@ int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, d
     };
     rc = run();
     d_pos.release(); d_tau.release(); d_gtx.release(); d_grx.release(); d_amp.release(); d_keep.release();
-    d_slope.release();
+    d_slope.release(); d_recs.release(); d_tinfo.release(); d_tspan.release();
     return rc;
 }
 

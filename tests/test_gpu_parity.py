@@ -18,6 +18,12 @@ REL_L2_BAR = 1e-4
 ATI_BAR = 1e-3
 
 
+@pytest.fixture(params=["direct", "spectral"])
+def mode(request):
+    """Both forms of the echo accumulation (include/heeps_sim.h SIM_ACCUMULATE_*) against the same oracle."""
+    return request.param
+
+
 def _sim(w, **opts):
     from paper_2405_09938_b200 import Simulator
     return Simulator(w, 0, **opts)
@@ -42,29 +48,33 @@ def _assert_parity(got, ref, what=""):
 
 # ----------------------------------------------------------------------------- Tiny, in full
 
-def test_tiny_all_pulses():
+def test_tiny_all_pulses(mode):
     w = make_workload("tiny")
-    got = _gpu(w)
+    got = _gpu(w, accumulate_mode=mode)
     ref = oracle_generate(w)
     assert got.shape == (1, 32, 256) and got.dtype == np.complex64
     worst = _assert_parity(got, ref, "tiny")
     assert worst < 2e-5            # headroom: the budget is not being eaten by the kernel
-    # samples outside every echo window are exactly zero on both sides
-    assert np.array_equal(got == 0, ref == 0)
+    if mode == "direct":
+        # samples outside every echo window are exactly zero on both sides
+        assert np.array_equal(got == 0, ref == 0)
+    else:
+        # the transform leaves rounding-level leakage (~1e-7 of the peak) outside the support
+        assert np.max(np.abs(got[ref == 0])) < 1e-5 * np.abs(ref).max()
 
 
 @pytest.mark.parametrize("tile", [4, 8, 16, 32, 64])
-def test_tiny_tile_sizes_and_batches(tile):
+def test_tiny_tile_sizes_and_batches(tile, mode):
     w = make_workload("tiny", n_pulses=7)
     ref = oracle_generate(w)
-    got = _gpu(w, tile_facets=tile, pulses_per_batch=3)      # ragged last batch
+    got = _gpu(w, tile_facets=tile, pulses_per_batch=3, accumulate_mode=mode)      # ragged last batch
     _assert_parity(got, ref, f"tile {tile}")
 
 
-def test_pulse_ranges_are_idempotent_and_consistent():
+def test_pulse_ranges_are_idempotent_and_consistent(mode):
     import torch
     w = make_workload("tiny", n_pulses=9)
-    with _sim(w) as sim:
+    with _sim(w, accumulate_mode=mode) as sim:
         full = sim.generate().cpu().numpy()
         part = sim.generate(3, 8).cpu().numpy()
         again = sim.generate(3, 8).cpu().numpy()
@@ -116,21 +126,21 @@ def _hetero_small(nx=150, ny=90, n_pulses=3):
     return w
 
 
-def test_hetero_recipe_ragged_grid():
+def test_hetero_recipe_ragged_grid(mode):
     """sigma0 map + tilt modulation + current front + 256 components, grid not a tile multiple."""
     w = _hetero_small()
-    got = _gpu(w)
+    got = _gpu(w, accumulate_mode=mode)
     ref = oracle_generate(w)
     _assert_parity(got, ref, "hetero_small")
 
 
-def test_choppy_wave_model_flag():
+def test_choppy_wave_model_flag(mode):
     w = make_workload("tiny", n_pulses=3)
     w.scene["choppy"] = 1
-    _assert_parity(_gpu(w), oracle_generate(w), "choppy")
+    _assert_parity(_gpu(w, accumulate_mode=mode), oracle_generate(w), "choppy")
 
 
-def test_cull_active_and_window_clipping():
+def test_cull_active_and_window_clipping(mode):
     """Wide patch: part of the facets fall below -30 dB two-way (culled), and the delay spread
     exceeds the sampling window so echoes are clipped at both ends (silently)."""
     w = make_workload("tiny", n_pulses=2)
@@ -139,9 +149,9 @@ def test_cull_active_and_window_clipping():
     assert 0.1 < o["keep"].mean() < 0.95
     ref = oracle_generate(w)
     assert np.abs(ref[0, 0, 0]) > 0 and np.abs(ref[0, 0, -1]) > 0      # window is full edge to edge
-    got = _gpu(w)
+    got = _gpu(w, accumulate_mode=mode)
     _assert_parity(got, ref, "cull+clip")
-    with _sim(w) as sim:
+    with _sim(w, accumulate_mode=mode) as sim:
         sim.generate()
         st = sim.stats()
     assert st["facet_echoes_nominal"] == 4096 * 2
@@ -149,22 +159,22 @@ def test_cull_active_and_window_clipping():
     assert abs(st["facet_echoes_kept"] - expect_kept) <= 2
 
 
-def test_everything_culled_gives_exact_zeros():
+def test_everything_culled_gives_exact_zeros(mode):
     w = make_workload("tiny", n_pulses=2)
     w.instrument["cull_two_way_db"] = 10.0          # nothing reaches +10 dB
-    got = _gpu(w)
+    got = _gpu(w, accumulate_mode=mode)
     assert np.all(got == 0)
     assert np.all(oracle_generate(w) == 0)
 
 
-def test_zero_amplitude_and_single_facet():
+def test_zero_amplitude_and_single_facet(mode):
     w = make_workload("tiny", n_pulses=2)
     w.scene["xi"][:] = 0
-    assert np.all(_gpu(w) == 0)
+    assert np.all(_gpu(w, accumulate_mode=mode) == 0)
     tx, rx = (10.0, -300e3, 700e3), (250e3, -300e3, 700e3)
     r = np.linalg.norm(np.array(tx)) + np.linalg.norm(np.array(rx))
     w1 = custom_workload(tx_pos=tx, rx_pos=rx, t0=r / 299792458.0 - 100.3 / 12e6)
-    _assert_parity(_gpu(w1), oracle_generate(w1), "single facet")
+    _assert_parity(_gpu(w1, accumulate_mode=mode), oracle_generate(w1), "single facet")
 
 
 def test_non_integer_replica_length_and_odd_sizes():
@@ -175,16 +185,26 @@ def test_non_integer_replica_length_and_odd_sizes():
     w.instrument["n_samples"] = 251
     w.scene["nx"], w.scene["ny"] = 61, 37
     w.scene["xi"] = np.ascontiguousarray(w.scene["xi"][:37, :61])
-    _assert_parity(_gpu(w), oracle_generate(w), "non-integer L")
+    ref = oracle_generate(w)
+    _assert_parity(_gpu(w, accumulate_mode='direct'), ref, "non-integer L")
+    # the spectral form needs one waveform kernel for every facet: refused when forced, AUTO falls back
+    from paper_2405_09938_b200 import SimError
+    with pytest.raises(SimError) as e:
+        _sim(w, accumulate_mode='spectral')
+    assert e.value.code == -1
+    with _sim(w) as sim:
+        got = sim.generate().cpu().numpy()
+        assert sim.stats()["accumulate_mode"] == 1
+    _assert_parity(got, ref, "non-integer L, auto")
 
 
-def test_no_waves_and_eight_channels():
+def test_no_waves_and_eight_channels(mode):
     w = make_workload("tiny", n_pulses=2)
     w.scene["n_waves"] = 0
     for k in ("kx", "ky", "amp", "omega", "phase"):
         w.scene[k] = np.zeros(0)
     w.instrument["channel_offset_m"] = np.linspace(-7.0, 7.0, 8)
-    _assert_parity(_gpu(w), oracle_generate(w), "8 channels, flat")
+    _assert_parity(_gpu(w, accumulate_mode=mode), oracle_generate(w), "8 channels, flat")
 
 
 def test_speckle_from_seed_moments():
@@ -237,12 +257,12 @@ def test_error_codes():
         _sim(w)
 
 
-def test_host_path_and_scene_update():
+def test_host_path_and_scene_update(mode):
     """sim_generate_host + sim_update_scene (the end-to-end entry points bench.py times)."""
     import torch
     w = _hetero_small(96, 64, 2)
     ref = oracle_generate(w)
-    with _sim(w) as sim:
+    with _sim(w, accumulate_mode=mode) as sim:
         _assert_parity(sim.generate_host().numpy(), ref, "host path")
         xi2 = (w.scene["xi"] * np.float32(0.5)).astype(np.float32)
         sim.update_scene(xi=torch.from_numpy(xi2).pin_memory())
@@ -263,30 +283,31 @@ def test_replica_is_the_transmitted_chirp():
 
 # ----------------------------------------------------------------------------- BASELINE sizes
 
-def test_ati_seeded_pulse_subset():
+def test_ati_seeded_pulse_subset(mode):
     """Config 1 (ATI, 512x512, 3 channels, L = 1200) at full size: the launch configuration bench.py
     times (all 256 pulses in one call); the oracle checks first, last and two seeded pulses."""
     import torch
     w = make_workload("ati")
     rng = np.random.Generator(np.random.PCG64(20240509))
     pulses = sorted({0, 255, *rng.integers(1, 255, 2).tolist()})
-    with _sim(w) as sim:
+    with _sim(w, accumulate_mode=mode) as sim:
         out = sim.generate()
         torch.cuda.synchronize()
         got = out[:, pulses].cpu().numpy()
         st = sim.stats()
     assert st["facet_echoes_kept"] == st["facet_echoes_nominal"] == 512 * 512 * 256 * 3
+    assert st["accumulate_mode"] == {"direct": 1, "spectral": 2}[mode]
     ref = oracle_generate(w, pulses)
     _assert_parity(got, ref, "ati")
 
 
-def test_hetero_full_size_sampled_outputs():
+def test_hetero_full_size_sampled_outputs(mode):
     """Config 2 (2048x2048, 256 components, maps) at full size, two pulses through the library;
     the oracle evaluates 24 seeded output samples of one pulse one by one."""
     w = make_workload("hetero")
     rng = np.random.Generator(np.random.PCG64(20240510))
     p = 1023
-    got = _gpu(w, p, p + 1)[:, 0]
+    got = _gpu(w, p, p + 1, accumulate_mode=mode)[:, 0]
     energy = np.abs(got[1]) ** 2
     live = np.nonzero(energy > 1e-3 * energy.max())[0]
     ns = np.sort(rng.choice(live, 24, replace=False))
@@ -299,19 +320,19 @@ def test_hetero_full_size_sampled_outputs():
     assert abs(np.angle(np.exp(1j * (ph(got[:, ns]) - ph(ref))))) < ATI_BAR
 
 
-def test_large_full_size_properties():
+def test_large_full_size_properties(mode):
     """Config 3 (4096x4096, Ns = 8192) at full size, one pulse at the dwell end where the cull is
     active: kept count against the documented 0.86-0.94 band, support inside the window, zero
     outside the tile spans, and 12 sampled outputs against the oracle."""
     w = make_workload("large")
     p = 2047
-    with _sim(w) as sim:
+    with _sim(w, accumulate_mode=mode) as sim:
         got = sim.generate(p, p + 1).cpu().numpy()[:, 0]
         st = sim.stats()
     frac = st["facet_echoes_kept"] / st["facet_echoes_nominal"]
     assert 0.80 < frac < 0.97
     energy = np.abs(got[1]) ** 2
-    live = np.nonzero(energy > 0)[0]
+    live = np.nonzero(energy > (0 if mode == "direct" else 1e-10 * energy.max()))[0]
     assert live[0] > 0 and live[-1] < 8191 and live.size < 3400          # 2987 expected (SURVEY 8(d))
     rng = np.random.Generator(np.random.PCG64(20240511))
     strong = np.nonzero(energy > 1e-3 * energy.max())[0]
@@ -321,10 +342,10 @@ def test_large_full_size_properties():
     assert np.max(np.abs(got[:, ns] - ref)) < 2e-4 * scale
 
 
-def test_sweep_point_long_chirp():
+def test_sweep_point_long_chirp(mode):
     """Sweep axis: L = 4096 replica samples on a 2^20-facet patch, one channel, sampled check."""
     w = make_sweep_point(log2_facets=20, replica_samples=4096, n_channels=1, n_pulses=2)
-    got = _gpu(w, 1, 2)[:, 0]
+    got = _gpu(w, 1, 2, accumulate_mode=mode)[:, 0]
     energy = np.abs(got[0]) ** 2
     strong = np.nonzero(energy > 1e-3 * energy.max())[0]
     rng = np.random.Generator(np.random.PCG64(7))
