@@ -107,7 +107,10 @@ typedef struct {
     int32_t pulses_per_batch;      /* 0 = auto from workspace_bytes */
     int64_t workspace_bytes;       /* cap for per-batch device workspace; 0 = 4 GiB */
     int32_t accumulate_mode;       /* SIM_ACCUMULATE_*; SPECTRAL where it does not apply -> SIM_EINVAL */
-    int32_t reserved[7];
+    int32_t kinematics_keyframe;   /* wave sums evaluated exactly every H-th pulse (with time derivatives) and
+                                      cubic-Hermite interpolated between: 0 = auto (largest H <= 64 whose error
+                                      bound sum_w A_w (omega_w h)^4/384 <= 1e-9 m), 1 = every pulse, n = force H = n */
+    int32_t reserved[6];
 } sim_options;
 
 /*
@@ -160,7 +163,7 @@ typedef struct {
     int32_t max_span_samples;      /* largest per-tile sample span seen                */
     int32_t accumulate_mode;       /* SIM_ACCUMULATE_DIRECT or _SPECTRAL, as resolved at sim_create */
     int32_t fft_size;              /* SPECTRAL: transform length; else 0              */
-    int32_t reserved[1];
+    int32_t kinematics_keyframe;   /* H as resolved at sim_create                     */
 } sim_stats;
 int sim_get_stats(sim_handle *h, sim_stats *out);
 

@@ -62,7 +62,7 @@ class sim_scene(C.Structure):
 
 class sim_options(C.Structure):
     _fields_ = [("tile_facets", C.c_int32), ("pulses_per_batch", C.c_int32), ("workspace_bytes", C.c_int64),
-                ("accumulate_mode", C.c_int32), ("reserved", C.c_int32 * 7)]
+                ("accumulate_mode", C.c_int32), ("kinematics_keyframe", C.c_int32), ("reserved", C.c_int32 * 6)]
 
 
 class sim_stats(C.Structure):
@@ -71,7 +71,7 @@ class sim_stats(C.Structure):
         ("kernel_launches", C.c_int64),
         ("tile_facets", C.c_int32), ("pulses_per_batch", C.c_int32), ("n_tiles", C.c_int32),
         ("accumulate_block_threads", C.c_int32), ("max_span_samples", C.c_int32),
-        ("accumulate_mode", C.c_int32), ("fft_size", C.c_int32), ("reserved", C.c_int32 * 1),
+        ("accumulate_mode", C.c_int32), ("fft_size", C.c_int32), ("kinematics_keyframe", C.c_int32),
     ]
 
 
@@ -218,12 +218,13 @@ def _marshal(workload):
 # ----------------------------------------------------------------------------- C-named functions
 
 def sim_create(workload, device: int = 0, *, tile_facets: int = 0, pulses_per_batch: int = 0,
-               workspace_bytes: int = 0, accumulate_mode=0):
+               workspace_bytes: int = 0, accumulate_mode=0, kinematics_keyframe: int = 0):
     lib = load_library()
     ci, cg, cs, keep = _marshal(workload)
     opts = sim_options()
     opts.tile_facets, opts.pulses_per_batch, opts.workspace_bytes = tile_facets, pulses_per_batch, workspace_bytes
     opts.accumulate_mode = _MODES[accumulate_mode]
+    opts.kinematics_keyframe = int(kinematics_keyframe)
     h = C.c_void_p()
     rc = lib.sim_create(C.byref(ci), C.byref(cg), C.byref(cs), C.byref(opts), int(device), C.byref(h))
     del keep
@@ -277,7 +278,7 @@ def sim_measure_pipe_peaks(device: int = 0) -> dict:
 def sim_get_stats(handle) -> dict:
     st = sim_stats()
     _check(load_library().sim_get_stats(handle, C.byref(st)), handle)
-    return {k: getattr(st, k) for k, _ in sim_stats._fields_ if k != "reserved"}
+    return {k: getattr(st, k) for k, _ in sim_stats._fields_}
 
 
 # ----------------------------------------------------------------------------- convenience wrapper

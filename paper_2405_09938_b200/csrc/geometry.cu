@@ -58,6 +58,7 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
     }
     __syncthreads();
     const size_t F = (size_t)prm.nx * prm.ny;
+    const SurfaceInterp it = surface_interp(a.surf, a.pulses, p, pl);
     const float area = (float)(prm.spacing * prm.spacing);
     unsigned long long my_samples = 0;
     int my_bmin[kMaxChannels], my_bmax[kMaxChannels];
@@ -79,7 +80,6 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
         size_t f = 0;
         if (valid) {
             f = (size_t)j * prm.nx + i;
-            const size_t fp = (size_t)pl * F + f;
             // O1 rest point, O3 displaced position (current by advection, G10)
             double xb = prm.cx + ((double)i - 0.5 * (prm.nx - 1)) * prm.spacing;
             double yb = prm.cy + ((double)j - 0.5 * (prm.ny - 1)) * prm.spacing;
@@ -87,8 +87,8 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
             if (a.current) { float2 cv = __ldg(a.current + f); cux = cv.x; cuy = cv.y; }
             pos[0] = xb + cux * pc.t;
             pos[1] = yb + cuy * pc.t;
-            pos[2] = prm.cz + a.z[fp];
-            if (a.dxy) { double2 dd = a.dxy[fp]; pos[0] += dd.x; pos[1] += dd.y; }
+            pos[2] = prm.cz + surface_z(a.surf, it, F, f);
+            if (a.surf.dxy) { double2 dd = surface_dxy(a.surf, it, F, f); pos[0] += dd.x; pos[1] += dd.y; }
             // O4/O6 transmit leg and the cull reference (G6)
             Leg lt = leg(pos, pc.tx_pos, pc.tx_a, pc.tx_e, prm.ap_tx_a, prm.ap_tx_e);
             Leg lr = leg(pos, pc.rx_ref, pc.rx_a, pc.rx_e, prm.ap_rx_a, prm.ap_rx_e);
@@ -97,7 +97,7 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
             // O8 amplitude
             float sig = a.sigma0 ? __ldg(a.sigma0 + f) : (float)prm.sigma0_uniform;
             if (prm.tilt) {
-                float2 sl = a.slope[fp];
+                float2 sl = surface_slope(a.surf, it, F, f);
                 float fac = 1.f + 2.f * (sl.x * (float)prm.look_x + sl.y * (float)prm.look_y);
                 sig *= fmaxf(fac, 0.f);
             }

@@ -1,10 +1,13 @@
 // Launch wrappers of the four hot-path kernels (implemented in the .cu files beside this header).
 #pragma once
 #include "heeps_common.cuh"
+#include "surface.cuh"
 
 namespace heeps {
 
-// K1 -- facet kinematics (kinematics.cu).  One launch covers `n_pl` pulses starting at pulse p0.
+// K1 -- facet kinematics (kinematics.cu).  One launch fills `n_rows` rows: with H = 1 row r is pulse
+// first + r; with H > 1 row r is keyframe first + r, i.e. pulse min((first + r) H, P - 1), and the time
+// derivatives are written too (surface.cuh).
 struct KinematicsArgs {
     const double2 *xt;      // [Nw][nx]  A_w exp(j kx_w x_i)
     const double2 *yt;      // [Nw][ny]  exp(j (ky_w y_j + phase_w))
@@ -14,15 +17,20 @@ struct KinematicsArgs {
     double *z;              // [n_pl][F]            surface height above centre_z
     float2 *slope;          // [n_pl][F] or null    grad z
     double2 *dxy;           // [n_pl][F] or null    CWM horizontal displacement
+    int32_t H;              // keyframe spacing in pulses (1 = every pulse)
+    const double *omega;    // [Nw] (H > 1)
+    double *zt;             // time derivatives (H > 1): [n_rows][F]
+    float2 *slope_t;        // or null
+    double2 *dxy_t;         // or null
 };
-cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a, int p0, int n_pl, cudaStream_t s);
+cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a, int first, int n_rows, cudaStream_t s);
+cudaError_t launch_surface_slope(const DevParams &prm, const SurfaceArgs &sa, const PulseConst *pulses, int p,
+                                 float2 *out, cudaStream_t s);
 
 // K2 -- geometry, gains, amplitude, cull, tile bucketing (geometry.cu).
 struct GeometryArgs {
     const PulseConst *pulses;   // [P]
-    const double *z;            // from K1
-    const float2 *slope;        // or null
-    const double2 *dxy;         // or null
+    SurfaceArgs surf;           // from K1
     const float *sigma0;        // [F] or null
     const float2 *current;      // [F] or null
     const float2 *xi;           // [F]   complex speckle (debug outputs only)
@@ -81,9 +89,7 @@ constexpr int kMomentOrder = 8;   // Kt Chebyshev moments per range slice (trunc
 // K2s -- geometry, gains, amplitude, cull, range-slice moments (moments.cu).
 struct MomentArgs {
     const PulseConst *pulses;   // [P]
-    const double *z;            // from K1
-    const float2 *slope;        // or null
-    const double2 *dxy;         // or null
+    SurfaceArgs surf;           // from K1
     const float *sigma0;        // [F] or null
     const float2 *current;      // [F] or null
     const uint2 *xi_polar;      // [F]

@@ -78,6 +78,7 @@ moments_kernel(DevParams prm, MomentArgs a, int p0, int n_pl)
 
     // ---- facet state, once for all channels (O1..O3, Tx leg, cull reference, amplitude) ----
     const size_t F = (size_t)prm.nx * prm.ny;
+    const SurfaceInterp it = surface_interp(a.surf, a.pulses, p, pl);
     const float area = (float)(prm.spacing * prm.spacing);
     double pos[FPT][3], rt[FPT];
     float gt[FPT], amag[FPT];
@@ -94,22 +95,21 @@ moments_kernel(DevParams prm, MomentArgs a, int p0, int n_pl)
         pos[q][0] = pos[q][1] = pos[q][2] = 0.0;
         if (k < ts * ts && i < prm.nx && j < prm.ny) {
             const size_t f = (size_t)j * prm.nx + i;
-            const size_t fp = (size_t)pl * F + f;
             const double xb = prm.cx + ((double)i - 0.5 * (prm.nx - 1)) * prm.spacing;
             const double yb = prm.cy + ((double)j - 0.5 * (prm.ny - 1)) * prm.spacing;
             double cux = prm.cur_ux, cuy = prm.cur_uy;
             if (a.current) { const float2 cv = __ldg(a.current + f); cux = cv.x; cuy = cv.y; }
             pos[q][0] = xb + cux * pc.t;
             pos[q][1] = yb + cuy * pc.t;
-            pos[q][2] = prm.cz + a.z[fp];
-            if (a.dxy) { const double2 dd = a.dxy[fp]; pos[q][0] += dd.x; pos[q][1] += dd.y; }
+            pos[q][2] = prm.cz + surface_z(a.surf, it, F, f);
+            if (a.surf.dxy) { const double2 dd = surface_dxy(a.surf, it, F, f); pos[q][0] += dd.x; pos[q][1] += dd.y; }
             const Leg lt = leg(pos[q], pc.tx_pos, pc.tx_a, pc.tx_e, prm.ap_tx_a, prm.ap_tx_e);
             const Leg lr = leg(pos[q], pc.rx_ref, pc.rx_a, pc.rx_e, prm.ap_rx_a, prm.ap_rx_e);
             rt[q] = lt.r; gt[q] = lt.g;
             keep[q] = !(fabsf(lt.g * lr.g) < prm.cull_thr);                 // O7 (G6)
             float sig = a.sigma0 ? __ldg(a.sigma0 + f) : (float)prm.sigma0_uniform;
             if (prm.tilt) {
-                const float2 sl = a.slope[fp];
+                const float2 sl = surface_slope(a.surf, it, F, f);
                 sig *= fmaxf(1.f + 2.f * (sl.x * (float)prm.look_x + sl.y * (float)prm.look_y), 0.f);
             }
             const uint2 xp = __ldg(a.xi_polar + f);

@@ -66,9 +66,11 @@ struct sim_handle {
     DevBuf<float2> current, xi;
     DevBuf<uint2> xi_polar;              // {|xi|, arg xi in 2^-32 turns}, derived from xi on the device
     // workspace
-    DevBuf<double> z;
-    DevBuf<float2> slope;
-    DevBuf<double2> dxy;
+    DevBuf<double> z, zt, omega;
+    DevBuf<float2> slope, slope_t;
+    DevBuf<double2> dxy, dxy_t;
+    int key_H = 1;                       // keyframe spacing of the kinematics (1 = every pulse)
+    int surf_rows_cap = 0;               // rows of the surface buffers
     DevBuf<Rec> recs;
     DevBuf<TileInfo> tinfo;
     DevBuf<TileSpan> tspan;
@@ -192,6 +194,58 @@ double path_gradient_l1(const sim_geometry *g, const sim_scene *sc)
     return worst;
 }
 
+// Rows of the surface buffers a batch [p0, p0 + n_pl) needs: its pulses (H = 1) or its keyframes.
+void surface_rows(const sim_handle *h, int p0, int n_pl, int *first, int *rows)
+{
+    const int H = h->key_H, P = h->n_pulses;
+    if (H <= 1) { *first = p0; *rows = n_pl; return; }
+    const int n_keys = (P - 1 + H - 1) / H + 1;
+    const int j0 = std::min(p0 / H, n_keys - 2), j1 = std::min((p0 + n_pl - 1) / H, n_keys - 2) + 1;
+    *first = j0; *rows = j1 - j0 + 1;
+}
+
+struct SurfBufs {
+    double *z, *zt; float2 *slope, *slope_t; double2 *dxy, *dxy_t;
+};
+
+// K1 for the batch; fills `sa` for K2.
+int run_kinematics(sim_handle *h, const SurfBufs &b, int p0, int n_pl, cudaStream_t s, SurfaceArgs *sa)
+{
+    int first = 0, rows = 0;
+    surface_rows(h, p0, n_pl, &first, &rows);
+    KinematicsArgs ka{};
+    ka.xt = h->xt.p; ka.yt = h->yt.p; ka.tt = h->tt.p; ka.wk = h->wk.p; ka.n_pulses_total = h->n_pulses;
+    ka.z = b.z; ka.slope = b.slope; ka.dxy = b.dxy;
+    ka.H = h->key_H; ka.omega = h->omega.p; ka.zt = b.zt; ka.slope_t = b.slope_t; ka.dxy_t = b.dxy_t;
+    cudaError_t e = launch_kinematics(h->prm, ka, first, rows, s);
+    if (e != cudaSuccess) return fail_cuda(h, e, "launch_kinematics");
+    sa->z = b.z; sa->zt = b.zt; sa->slope = b.slope; sa->slope_t = b.slope_t; sa->dxy = b.dxy; sa->dxy_t = b.dxy_t;
+    sa->H = h->key_H; sa->key0 = first; sa->n_pulses_total = h->n_pulses;
+    return SIM_OK;
+}
+
+// Keyframe spacing (surface.cuh): largest H whose cubic-Hermite error bound sum_w A_w (omega_w h)^4 / 384
+// stays under 1e-9 m (and the same for the CWM displacement); 1 when pulse times are not increasing.
+int choose_keyframe_spacing(const sim_geometry *g, const sim_scene *sc, int requested)
+{
+    const int P = g->n_pulses;
+    if (requested == 1 || P < 4 || sc->n_waves == 0) return 1;
+    for (int p = 0; p + 1 < P; ++p) if (!(g->t_pulse_s[p + 1] > g->t_pulse_s[p])) return 1;
+    if (requested > 1) return std::min(requested, P - 1);
+    for (int H = 64; H >= 2; H >>= 1) {
+        if (H > P - 1) continue;
+        double hmax = 0;
+        for (int k = 0; k < P - 1; k += H) hmax = std::max(hmax, g->t_pulse_s[std::min(k + H, P - 1)] - g->t_pulse_s[k]);
+        double bound = 0;
+        for (int w = 0; w < sc->n_waves; ++w) {
+            const double x = sc->omega[w] * hmax;
+            bound += std::fabs(sc->amp[w]) * x * x * x * x / 384.0;
+        }
+        if (bound <= 1e-9) return H;
+    }
+    return 1;
+}
+
 }  // namespace
 
 extern "C" {
@@ -217,7 +271,8 @@ void sim_destroy(sim_handle *h)
     h->xt.release(); h->yt.release(); h->tt.release(); h->chirp_n.release(); h->carrier_p.release();
     h->wk.release(); h->carrier_frac.release(); h->pulses.release();
     h->sigma0.release(); h->current.release(); h->xi.release(); h->xi_polar.release();
-    h->z.release(); h->slope.release(); h->dxy.release(); h->recs.release(); h->tinfo.release();
+    h->z.release(); h->slope.release(); h->dxy.release();
+    h->zt.release(); h->slope_t.release(); h->dxy_t.release(); h->omega.release(); h->recs.release(); h->tinfo.release();
     h->tspan.release(); h->acc.release(); h->counters.release(); h->out_staging.release();
     h->mom.release(); h->cspec.release(); h->tw.release();
     delete h;
@@ -235,6 +290,7 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
         if (t < 4 || t > 64 || (t & (t - 1))) return SIM_EINVAL;
     }
     if (opts && (opts->accumulate_mode < 0 || opts->accumulate_mode > 2)) return SIM_EINVAL;
+    if (opts && (opts->kinematics_keyframe < 0 || opts->kinematics_keyframe > 4096)) return SIM_EINVAL;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
         cudaGetLastError();
@@ -307,10 +363,12 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     h->accum = accumulate_plan(prm, tile_spread);
     h->span_cap_m = std::min(4096, (((int)std::ceil(tile_spread) + 8) + 31) & ~31);
 
+    h->key_H = choose_keyframe_spacing(g, sc, opts ? opts->kinematics_keyframe : 0);
     // ---- batch size ----
     const int64_t fcap = (int64_t)prm.n_tiles * prm.tile_cap;
-    const int64_t per_pulse_common = h->n_facets * 8 + (h->need_slope ? h->n_facets * 8 : 0) +
-                                     (prm.choppy ? h->n_facets * 16 : 0);
+    const int64_t surf_row = h->n_facets * 8 + (h->need_slope ? h->n_facets * 8 : 0) +
+                             (prm.choppy ? h->n_facets * 16 : 0);
+    const int64_t per_pulse_common = h->key_H > 1 ? 2 * surf_row / h->key_H + 1 : surf_row;
     const int64_t per_pulse = per_pulse_common +
         (h->spectral ? (int64_t)C * kMomentOrder * h->nb_pad * 8
                      : (int64_t)C * fcap * (int64_t)sizeof(Rec) + (int64_t)C * Ns * 16 +
@@ -416,9 +474,20 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     CKC(h->xi_polar.alloc(F));
     CKC(launch_speckle_polar(h->xi.p, h->xi_polar.p, (int64_t)F, nullptr));
     CKC(cudaDeviceSynchronize());
-    CKC(h->z.alloc(F * pb));
-    if (h->need_slope) CKC(h->slope.alloc(F * pb));
-    if (prm.choppy) CKC(h->dxy.alloc(F * pb));
+    {
+        const size_t rows = h->key_H > 1 ? (size_t)(pb / h->key_H + 3) : (size_t)pb;
+        h->surf_rows_cap = (int)rows;
+        CKC(h->z.alloc(F * rows));
+        if (h->need_slope) CKC(h->slope.alloc(F * rows));
+        if (prm.choppy) CKC(h->dxy.alloc(F * rows));
+        if (h->key_H > 1) {
+            CKC(h->zt.alloc(F * rows));
+            if (h->need_slope) CKC(h->slope_t.alloc(F * rows));
+            if (prm.choppy) CKC(h->dxy_t.alloc(F * rows));
+        }
+        CKC(h->omega.alloc(std::max(Nw, 1)));
+        if (Nw) CKC(cudaMemcpy(h->omega.p, sc->omega, (size_t)Nw * sizeof(double), cudaMemcpyHostToDevice));
+    }
     if (!h->spectral) {
         CKC(h->recs.alloc((size_t)C * pb * fcap));
         CKC(h->tinfo.alloc((size_t)pb * prm.n_tiles));
@@ -470,6 +539,7 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     h->stats.accumulate_block_threads = h->accum.block_threads;
     h->stats.accumulate_mode = h->spectral ? SIM_ACCUMULATE_SPECTRAL : SIM_ACCUMULATE_DIRECT;
     h->stats.fft_size = h->spectral ? nfft : 0;
+    h->stats.kinematics_keyframe = h->key_H;
     *out = h;
     return SIM_OK;
 }
@@ -491,15 +561,15 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         }
         return cudaEventRecord(h->events[h->events_used++], s);
     };
+    const SurfBufs bufs{h->z.p, h->zt.p, h->slope.p, h->slope_t.p, h->dxy.p, h->dxy_t.p};
     for (int p0 = pb0; h->spectral && p0 < pb1; p0 += h->pulses_per_batch) {
         const int n_pl = std::min(h->pulses_per_batch, pb1 - p0);
         CK(h, cudaMemsetAsync(h->mom.p, 0, (size_t)prm.n_channels * n_pl * kMomentOrder * h->nb_pad * sizeof(float2), s));
         CK(h, mark());
-        KinematicsArgs ka{h->xt.p, h->yt.p, h->tt.p, h->wk.p, h->n_pulses, h->z.p, h->slope.p, h->dxy.p};
-        CK(h, launch_kinematics(prm, ka, p0, n_pl, s));
-        CK(h, mark());
         MomentArgs ma{};
-        ma.pulses = h->pulses.p; ma.z = h->z.p; ma.slope = h->slope.p; ma.dxy = h->dxy.p;
+        { int rc = run_kinematics(h, bufs, p0, n_pl, s, &ma.surf); if (rc != SIM_OK) return rc; }
+        CK(h, mark());
+        ma.pulses = h->pulses.p;
         ma.sigma0 = h->sigma0.p; ma.current = h->current.p; ma.xi_polar = h->xi_polar.p;
         ma.mom = h->mom.p; ma.nb_pad = h->nb_pad; ma.span_cap = h->span_cap_m; ma.replica = h->replica;
         ma.counters = h->counters.p;
@@ -518,11 +588,10 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         const int n_pl = std::min(h->pulses_per_batch, pb1 - p0);
         CK(h, cudaMemsetAsync(h->acc.p, 0, (size_t)prm.n_channels * n_pl * prm.n_samples * sizeof(double2), s));
         CK(h, mark());
-        KinematicsArgs ka{h->xt.p, h->yt.p, h->tt.p, h->wk.p, h->n_pulses, h->z.p, h->slope.p, h->dxy.p};
-        CK(h, launch_kinematics(prm, ka, p0, n_pl, s));
-        CK(h, mark());
         GeometryArgs ga{};
-        ga.pulses = h->pulses.p; ga.z = h->z.p; ga.slope = h->slope.p; ga.dxy = h->dxy.p;
+        { int rc = run_kinematics(h, bufs, p0, n_pl, s, &ga.surf); if (rc != SIM_OK) return rc; }
+        CK(h, mark());
+        ga.pulses = h->pulses.p;
         ga.sigma0 = h->sigma0.p; ga.current = h->current.p; ga.xi = h->xi.p; ga.xi_polar = h->xi_polar.p;
         ga.recs = h->recs.p; ga.tinfo = h->tinfo.p; ga.tspan = h->tspan.p; ga.counters = h->counters.p;
         ga.carrier_frac_t0 = h->carrier_frac.p;
@@ -613,7 +682,7 @@ int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, d
     const size_t F = (size_t)h->n_facets, C = prm.n_channels;
     DevBuf<double> d_pos, d_tau, d_gtx, d_grx, d_amp;
     DevBuf<int32_t> d_keep;
-    DevBuf<float2> d_slope;
+    DevBuf<float2> d_slope, d_slope_out;
     DevBuf<Rec> d_recs;                  // spectral handles own no record workspace
     DevBuf<TileInfo> d_tinfo;
     DevBuf<TileSpan> d_tspan;
@@ -627,12 +696,19 @@ int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, d
         }
         CK(h, d_pos.alloc(3 * F)); CK(h, d_tau.alloc(C * F)); CK(h, d_gtx.alloc(F));
         CK(h, d_grx.alloc(C * F)); CK(h, d_amp.alloc(2 * C * F)); CK(h, d_keep.alloc(F));
-        float2 *slope_buf = h->slope.p;
-        if (!slope_buf) { CK(h, d_slope.alloc(F)); slope_buf = d_slope.p; }
-        KinematicsArgs ka{h->xt.p, h->yt.p, h->tt.p, h->wk.p, h->n_pulses, h->z.p, slope_buf, h->dxy.p};
-        CK(h, launch_kinematics(prm, ka, pulse, 1, nullptr));
+        // the slope is reported even when the scene does not use it: temporary rows (value + rate)
+        SurfBufs bufs{h->z.p, h->zt.p, h->slope.p, h->slope_t.p, h->dxy.p, h->dxy_t.p};
+        if (!bufs.slope) {
+            CK(h, d_slope.alloc(F * 3 * 2));
+            bufs.slope = d_slope.p; bufs.slope_t = d_slope.p + F * 3;
+        }
         GeometryArgs ga{};
-        ga.pulses = h->pulses.p; ga.z = h->z.p; ga.slope = h->need_slope ? slope_buf : nullptr; ga.dxy = h->dxy.p;
+        { int rc2 = run_kinematics(h, bufs, pulse, 1, nullptr, &ga.surf); if (rc2 != SIM_OK) return rc2; }
+        ga.pulses = h->pulses.p;
+        // per-facet slope of this pulse (interpolated like K2 sees it), for the report only
+        CK(h, d_slope_out.alloc(F));
+        CK(h, launch_surface_slope(prm, ga.surf, h->pulses.p, pulse, d_slope_out.p, nullptr));
+        if (!h->need_slope) { ga.surf.slope = nullptr; ga.surf.slope_t = nullptr; }
         ga.sigma0 = h->sigma0.p; ga.current = h->current.p; ga.xi = h->xi.p; ga.xi_polar = h->xi_polar.p;
         ga.recs = recs; ga.tinfo = tinfo; ga.tspan = tspan; ga.counters = nullptr;
         ga.dbg_pos = d_pos.p; ga.dbg_tau = d_tau.p; ga.dbg_gtx = d_gtx.p; ga.dbg_grx = d_grx.p;
@@ -647,14 +723,14 @@ int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, d
         if (keep) CK(h, cudaMemcpy(keep, d_keep.p, F * sizeof(int32_t), cudaMemcpyDeviceToHost));
         if (slope) {
             std::vector<float2> tmp(F);
-            CK(h, cudaMemcpy(tmp.data(), slope_buf, F * sizeof(float2), cudaMemcpyDeviceToHost));
+            CK(h, cudaMemcpy(tmp.data(), d_slope_out.p, F * sizeof(float2), cudaMemcpyDeviceToHost));
             for (size_t f = 0; f < F; ++f) { slope[2 * f] = tmp[f].x; slope[2 * f + 1] = tmp[f].y; }
         }
         return SIM_OK;
     };
     rc = run();
     d_pos.release(); d_tau.release(); d_gtx.release(); d_grx.release(); d_amp.release(); d_keep.release();
-    d_slope.release(); d_recs.release(); d_tinfo.release(); d_tspan.release();
+    d_slope.release(); d_slope_out.release(); d_recs.release(); d_tinfo.release(); d_tspan.release();
     return rc;
 }
 

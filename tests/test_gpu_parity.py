@@ -86,6 +86,31 @@ def test_pulse_ranges_are_idempotent_and_consistent(mode):
     assert np.max(np.abs(part - full[:, 3:8])) <= 1e-5 * np.abs(full).max()
 
 
+def test_kinematics_keyframes(mode):
+    """Wave sums evaluated exactly only at keyframe pulses, cubic Hermite between (surface.cuh); the oracle
+    evaluates every pulse exactly.  Covers z, the tilt-modulation slopes, the CWM displacement, a ragged
+    last keyframe interval, batches that start inside an interval, and the auto choice of H."""
+    w = _hetero_small(96, 64, 11)
+    w.scene["choppy"] = 1
+    ref = oracle_generate(w)
+    for H, batch in ((4, 0), (4, 3), (10, 5), (1, 0)):
+        with _sim(w, accumulate_mode=mode, kinematics_keyframe=H, pulses_per_batch=batch) as sim:
+            got = sim.generate().cpu().numpy()
+            assert sim.stats()["kinematics_keyframe"] == H
+            part = sim.generate(5, 9).cpu().numpy()
+        _assert_parity(got, ref, f"keyframes H={H} batch={batch}")
+        _assert_parity(part, ref[:, 5:9], f"keyframes H={H} range")
+    # auto: the ATI dwell (PRF 1700 Hz, omega <= 3.1 rad/s) admits H > 1 within the 1e-9 m bound
+    wa = make_workload("ati")
+    wa.scene["nx"] = wa.scene["ny"] = 8
+    wa.scene["xi"] = np.ascontiguousarray(wa.scene["xi"][:8, :8])
+    with _sim(wa, accumulate_mode=mode) as sim:
+        assert sim.stats()["kinematics_keyframe"] >= 8
+        g = sim.debug_facets(137)
+    o = oracle_facets(wa, 137)
+    assert np.max(np.abs(g["pos"] - o["pos"])) < 3e-9              # interpolated height against the exact one
+
+
 # ----------------------------------------------------------------------------- per-kernel unit parity (T1)
 
 @pytest.mark.parametrize("name", ["tiny", "hetero_small"])
