@@ -5,12 +5,14 @@
 
 One *step* is one pass of the whole hot path (K1 kinematics, K2 geometry/gains/cull, K3 echo
 accumulation, K4 finalize) over every pulse and channel of the workload: `sim_generate(0, P)`.
+The timed path is the library's default (SIM_ACCUMULATE_AUTO = the spectral form where it applies);
+the direct form of the same workload is timed beside it and reported under `direct_form`.
 At N = 1 the workload is BASELINE.json configs[1] ("ATI": 512x512 facets, 3 channels, 256 pulses,
 L = 1200, Ns = 4096).  Under torchrun each rank owns its own P-pulse slab of an N*P-pulse
 acquisition (weak scaling, no data-path collective).
 
-The JSON line carries, beside the base contract: `roofline` (dominant kernel K3 against the FP32
-pipe), `cpu_baseline` (the fp64 oracle on the host cores, bounded sample), `e2e` (through
+The JSON line carries, beside the base contract: `roofline` (dominant kernel of the timed path against
+its pipe; K3 of the direct form against the FP32 pipe under `direct_form.roofline`), `cpu_baseline` (the fp64 oracle on the host cores, bounded sample), `e2e` (through
 sim_update_scene + sim_generate_host with pinned HOST buffers), `clocks`, `gpu_launches`.
 `--impl reference` times the oracle as it stands (this tier's reference arm).
 """
@@ -34,7 +36,12 @@ UNIT = "facet-echoes/s"
 # facet-sample (one packed FFMA2 of the three-term recurrence + one packed FADD2 into the accumulators);
 # 148 SMs x 128 FP32 lanes.
 K3_FP32_OPS_PER_FACET_SAMPLE = 4.0
-SM_COUNT, FP32_LANES_PER_SM, XU_LANES_PER_SM = 148, 128, 16
+SM_COUNT, FP32_LANES_PER_SM, XU_LANES_PER_SM, FP64_LANES_PER_SM = 148, 128, 16, 64
+# FP64-pipe roofline of K2s: SURVEY.md 8(d) counts ~60 DFMA per facet-antenna (range,
+# direction cosines, window and phase in fp64); a facet-pulse sees Tx + cull reference + C receive antennas.
+K2_DFMA_PER_FACET_ANTENNA = 60.0
+# dram bytes per facet-pulse of a K2s launch from the committed ncu capture (profiles/); None until captured.
+K2S_DRAM_BYTES_PER_FACET_PULSE = None
 # dram bytes per kept facet-echo of a K3 launch, from the committed `ncu --set full` capture
 # profiles/r1_v3_k3_ncu_summary.txt: (2.580977e9 read + 1.1966e7 written) / (100 pulses x 3 ch x 262144).
 K3_DRAM_BYTES_PER_FACET_ECHO = (2.580977e9 + 1.1966e7) / (100 * 3 * 262144)
@@ -92,7 +99,7 @@ class ClockSampler:
                     self.samples.append(float(a)); self.max_mhz = float(b)
             except Exception:
                 pass
-            self._stop.wait(0.05)
+            self._stop.wait(0.01)
 
     def __enter__(self):
         self._thread = threading.Thread(target=self._loop, daemon=True)
@@ -151,11 +158,78 @@ def run_reference(args):
     return 0
 
 
+def _time_steps(sim, out, P, steps, warmup, stream, barrier, torch, clocks_index=None):
+    """W warm-ups, then K steps of sim_generate(0, P) between CUDA events on the launching stream."""
+    sim.set_profiling(True)
+    for _ in range(warmup):
+        sim.generate(0, P, out=out)
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(clocks_index) if clocks_index is not None else None
+    if sampler:
+        sampler.__enter__()
+    barrier()
+    t_wall = time.perf_counter()
+    ev0.record(stream)
+    for _ in range(steps):
+        sim.generate(0, P, out=out)
+    ev1.record(stream)
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    if sampler:
+        sampler.__exit__()
+    kms = sim.kernel_ms()            # per-kernel totals of the LAST timed step (events on this stream)
+    stats = sim.stats()
+    sim.set_profiling(False)
+    return ev0.elapsed_time(ev1), t_wall, kms, stats, (sampler.summary() if sampler else None)
+
+
+def _roofline_direct(kms, stats, sm_max, pipes):
+    """K3 (accumulate_kernel) against the FP32 pipe: 4 lane-ops per facet-sample (DESIGN.md 4/K3)."""
+    n_batches = max(1, stats["kernel_launches"] // 4)
+    launch_ms = kms["accumulate"] / n_batches
+    fs_per_launch = stats["facet_samples"] / n_batches
+    achieved = fs_per_launch / (launch_ms * 1e-3) / 1e9
+    peak = SM_COUNT * FP32_LANES_PER_SM * sm_max * 1e6 / K3_FP32_OPS_PER_FACET_SAMPLE / 1e9
+    pipe_peak = pipes["mix_f32x2_lane_per_s"] / K3_FP32_OPS_PER_FACET_SAMPLE / 1e9
+    return {
+        "bound": "alu", "kernel": "accumulate_kernel (K3, direct form)", "achieved": achieved, "peak": peak,
+        "unit": "Gfacet-samples/s", "frac": achieved / peak,
+        "traffic": K3_DRAM_BYTES_PER_FACET_ECHO * stats["facet_echoes_kept"] / n_batches,
+        "peak_model": f"{SM_COUNT} SM x {FP32_LANES_PER_SM} FP32 lanes x {sm_max:.0f} MHz / "
+                      f"{K3_FP32_OPS_PER_FACET_SAMPLE:.0f} FP32 lane-ops per facet-sample",
+        "measured_pipe_peak": pipe_peak, "frac_of_measured_pipe_peak": achieved / pipe_peak,
+        "launch_ms": launch_ms, "facet_samples_per_launch": fs_per_launch,
+        "kernel_share_of_step": kms["accumulate"] / max(sum(kms.values()), 1e-9),
+    }
+
+
+def _roofline_spectral(kms, stats, sm_max, pipes, n_channels):
+    """K2s (moments_kernel) against the FP64 pipe: SURVEY.md 8(d) counts ~60 DFMA per facet-antenna;
+    antennas per facet-pulse = Tx + cull reference + C receive phase centres (DESIGN.md 5/K2s)."""
+    n_batches = max(1, stats["kernel_launches"] // 3)
+    launch_ms = kms["geometry"] / n_batches
+    facet_pulses = stats["facet_echoes_nominal"] / n_channels / n_batches
+    dfma = facet_pulses * K2_DFMA_PER_FACET_ANTENNA * (2 + n_channels)
+    achieved = dfma / (launch_ms * 1e-3) / 1e9
+    peak = SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6 / 1e9
+    return {
+        "bound": "alu", "kernel": "moments_kernel (K2s, spectral form)", "achieved": achieved, "peak": peak,
+        "unit": "GDFMA/s", "frac": achieved / peak,
+        "traffic": K2S_DRAM_BYTES_PER_FACET_PULSE * facet_pulses if K2S_DRAM_BYTES_PER_FACET_PULSE else None,
+        "peak_model": f"{SM_COUNT} SM x {FP64_LANES_PER_SM} FP64 lanes x {sm_max:.0f} MHz; algorithmic work "
+                      f"{K2_DFMA_PER_FACET_ANTENNA:.0f} DFMA x (2 + C) antennas per facet-pulse",
+        "measured_pipe_peak": pipes["dfma_per_s"] / 1e9, "frac_of_measured_pipe_peak": achieved / (pipes["dfma_per_s"] / 1e9),
+        "launch_ms": launch_ms, "facet_pulses_per_launch": facet_pulses,
+        "kernel_share_of_step": kms["geometry"] / max(sum(kms.values()), 1e-9),
+    }
+
+
 def run_cuda(args):
     import numpy as np
     import torch
     import torch.distributed as dist
-    from paper_2405_09938_b200 import Simulator
+    from paper_2405_09938_b200 import Simulator, sim_measure_pipe_peaks
     from workloads import make_workload
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -172,7 +246,7 @@ def run_cuda(args):
     # weak scaling: rank r simulates pulses [r P, (r+1) P) of an N*P-pulse acquisition
     w = make_workload(args.workload, n_pulses=P, pulse_offset=rank * P)
     F, C, Ns, L = w.n_facets, w.n_channels, w.n_samples, w.replica_samples
-    sim = Simulator(w, local_rank)
+    sim = Simulator(w, local_rank, accumulate_mode=args.mode)
     out = torch.empty((C, P, Ns), dtype=torch.complex64, device=f"cuda:{local_rank}")
     stream = torch.cuda.current_stream()
 
@@ -182,31 +256,14 @@ def run_cuda(args):
         torch.cuda.synchronize()
 
     # ---- device-resident timing (value) ----
-    sim.set_profiling(True)
-    for _ in range(args.warmup):
-        sim.generate(0, P, out=out)
-    barrier()
-    k3_ms, k_all = [], []
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local_rank) as clocks:
-        barrier()
-        t_wall = time.perf_counter()
-        ev0.record(stream)
-        for _ in range(args.steps):
-            sim.generate(0, P, out=out)
-        ev1.record(stream)
-        barrier()
-        t_wall = time.perf_counter() - t_wall
-    elapsed_ms = ev0.elapsed_time(ev1)
-    kms = sim.kernel_ms()            # per-kernel totals of the LAST timed step (events on this stream)
-    stats = sim.stats()
-    sim.set_profiling(False)
+    elapsed_ms, t_wall, kms, stats, clk = _time_steps(sim, out, P, args.steps, args.warmup, stream, barrier, torch,
+                                                      clocks_index=local_rank)
     t = torch.tensor([elapsed_ms], dtype=torch.float64, device=f"cuda:{local_rank}")
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    elapsed_ms = float(t.item())
-    ms_per_step = elapsed_ms / args.steps
+    ms_per_step = float(t.item()) / args.steps
     value = world * F * P * C / (ms_per_step * 1e-3)
+    spectral = stats["accumulate_mode"] == 2
 
     # ---- end to end through the C ABI with HOST buffers ----
     xi_host = torch.from_numpy(np.ascontiguousarray(w.scene["xi"])).pin_memory()
@@ -220,62 +277,58 @@ def run_cuda(args):
         h2d += maps["current"].numel() * 4
     out_host = torch.empty((C, P, Ns), dtype=torch.complex64, pin_memory=True)
     d2h = out_host.numel() * 8
-    e2e_steps = max(1, min(args.steps, 5))
-    for _ in range(1):
-        sim.update_scene(**maps); sim.generate_host(0, P, out=out_host)
+    e2e_steps = max(1, min(args.steps, 10))
+    sim.update_scene(**maps); sim.generate_host(0, P, out=out_host)
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         sim.update_scene(**maps)
         sim.generate_host(0, P, out=out_host)        # returns after the D2H copy has completed
     barrier()
-    e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device=f"cuda:{local_rank}")
+    te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=f"cuda:{local_rank}")
     if world > 1:
         dist.all_reduce(te, op=dist.ReduceOp.MAX)
     e2e_value = world * F * P * C * e2e_steps / float(te.item())
+    sim.close()
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
 
-    # ---- roofline of the dominant kernel (K3, FP32 pipe) ----
+    # ---- rooflines (bound "alu"): the dominant kernel of the timed path, and K3 of the direct form ----
     peaks, peak_src = _peaks()
-    clk = clocks.summary()
-    n_batches = max(1, stats["kernel_launches"] // 4)
-    k3_launch_ms = kms["accumulate"] / n_batches
-    fs_per_launch = stats["facet_samples"] / n_batches
-    achieved = fs_per_launch / (k3_launch_ms * 1e-3) / 1e9            # G facet-samples/s
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
-    peak = SM_COUNT * FP32_LANES_PER_SM * sm_max * 1e6 / K3_FP32_OPS_PER_FACET_SAMPLE / 1e9
-    xu_model_peak = SM_COUNT * (XU_LANES_PER_SM / 2) * sm_max * 1e6 / 1e9
-    from paper_2405_09938_b200 import sim_measure_pipe_peaks
-    pipes = sim_measure_pipe_peaks(local_rank)      # same-run pipe microbenchmarks
-    pipe_peak = pipes["mix_f32x2_lane_per_s"] / K3_FP32_OPS_PER_FACET_SAMPLE / 1e9
-    roofline = {
-        "bound": "alu", "kernel": "accumulate_kernel (K3)", "achieved": achieved, "peak": peak,
-        "unit": "Gfacet-samples/s", "frac": achieved / peak,
-        "traffic": K3_DRAM_BYTES_PER_FACET_ECHO * stats["facet_echoes_kept"] / n_batches,
-        "peak_model": f"{SM_COUNT} SM x {FP32_LANES_PER_SM} FP32 lanes x {sm_max:.0f} MHz / "
-                      f"{K3_FP32_OPS_PER_FACET_SAMPLE:.0f} FP32 ops per facet-sample (clock: {peak_src} sm_max_mhz)",
-        "measured_pipe_peak": pipe_peak, "frac_of_measured_pipe_peak": achieved / pipe_peak,
-        "pipe_peaks_lane_ops_per_s": {k: v for k, v in pipes.items() if k.endswith("_per_s")},
-        "launch_ms": k3_launch_ms, "facet_samples_per_launch": fs_per_launch,
-        "frac_of_survey_xu_model": achieved / xu_model_peak,
-        "survey_xu_model_peak": xu_model_peak,
-        "kernel_ms_last_step": kms, "k3_share_of_step": kms["accumulate"] / max(sum(kms.values()), 1e-9),
-    }
+    pipes = sim_measure_pipe_peaks(local_rank)          # same-run pipe microbenchmarks
+    roofline = (_roofline_spectral(kms, stats, sm_max, pipes, C) if spectral
+                else _roofline_direct(kms, stats, sm_max, pipes))
+    roofline["clock_source"] = f"{peak_src} sm_max_mhz"
+    roofline["kernel_ms_last_step"] = kms
+    roofline["pipe_peaks_lane_ops_per_s"] = {k: v for k, v in pipes.items() if k.endswith("_per_s")}
+    direct = None
+    if spectral and world == 1 and not args.no_direct:
+        # the same workload through the direct form (every chirp replica generated sample by sample)
+        with Simulator(w, local_rank, accumulate_mode="direct") as sim_d:
+            d_ms, _, d_kms, d_stats, _ = _time_steps(sim_d, out, P, max(3, args.steps // 4), 3, stream, barrier, torch)
+        d_steps = max(3, args.steps // 4)
+        direct = {"value": F * P * C / (d_ms / d_steps * 1e-3), "unit": UNIT, "ms_per_step": d_ms / d_steps,
+                  "steps": d_steps, "roofline": _roofline_direct(d_kms, d_stats, sm_max, pipes),
+                  "kernel_ms_last_step": d_kms}
 
     # ---- the oracle on the host cores, bounded sample (reported baseline, not the target) ----
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         sample = [0, P - 1] if P > 1 else [0]
-        dt, cores = _oracle_sample(w, sample)
-        cpu = {"value": F * C * len(sample) / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"pulses {sample} x {C} channels of '{args.workload}' ({F * C * len(sample)} facet-echoes, "
-                         f"{dt:.1f} s wall)"}
+        reps = 4                                           # ~10 s of CPU work on 16 cores
+        dt = 0.0
+        for _ in range(reps):
+            d, cores = _oracle_sample(w, sample)
+            dt += d
+        cpu = {"value": F * C * len(sample) * reps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"pulses {sample} x {C} channels of '{args.workload}', {reps} repeats "
+                         f"({F * C * len(sample) * reps} facet-echoes, {dt:.1f} s wall)"}
 
+    moment_bytes = C * P * 8 * (Ns + L) * 8
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "ms_per_pulse": ms_per_step / P, "higher_is_better": True, "scaling": "weak",
@@ -283,12 +336,17 @@ def run_cuda(args):
         "config": {"workload": args.workload, "facets": F, "channels": C, "pulses": P, "replica_samples": L,
                    "n_samples": Ns, "wave_components": int(w.scene["n_waves"]),
                    "parallelism": f"pulse-slab x{world}",
+                   "accumulate_mode": "spectral" if spectral else "direct", "fft_size": stats["fft_size"],
+                   "kinematics_keyframe": stats["kinematics_keyframe"],
                    "tile_facets": stats["tile_facets"], "pulses_per_batch": stats["pulses_per_batch"],
-                   "l2": "per-step working set (facet-echo records) is "
-                         f"{F * C * P * 32 / 1e9:.1f} GB, far larger than the 126 MB L2; no flush needed"},
+                   "l2": (f"per-step working set: {moment_bytes / 1e6:.0f} MB of range-slice moments (zeroed, "
+                          f"scattered into and read back every step) + {C * P * Ns * 8 / 1e6:.0f} MB of output, "
+                          "larger than the 126 MB L2; no flush" if spectral else
+                          f"per-step working set (facet-echo records) is {F * C * P * 32 / 1e9:.1f} GB, far larger "
+                          "than the 126 MB L2; no flush needed")},
         "facet_echoes_kept_frac": stats["facet_echoes_kept"] / max(stats["facet_echoes_nominal"], 1),
-        "facet_samples_per_s": stats["facet_samples"] / (ms_per_step * 1e-3) * world,
         "roofline": roofline,
+        "direct_form": direct,
         "cpu_baseline": cpu,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps},
@@ -305,12 +363,15 @@ def run_cuda(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=40)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="ati")
+    ap.add_argument("--mode", default="auto", choices=["auto", "direct", "spectral"],
+                    help="echo accumulation (include/heeps_sim.h SIM_ACCUMULATE_*)")
     ap.add_argument("--pulses", type=int, default=None, help="override the dwell length (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-direct", action="store_true", help="skip the direct-form comparison leg")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     if args.impl == "reference":

@@ -22,7 +22,64 @@ __device__ __forceinline__ uint32_t turns_to_u32(double x)
 // argument on [-pi, pi)) plus half an lsb of the truncation (round to nearest).
 constexpr uint32_t kPhiBias = 0x80000000u + 256u;
 
+// sqrt and reciprocal sqrt of a squared range in one go: rsqrt seed, one fused correction of the root
+// (|error| <= 1 ulp of r); replaces IEEE sqrt() + 1/r (about a third of their instruction count).
+__device__ __forceinline__ void root_and_inverse(double r2, double &r, double &inv)
+{
+    const double y = rsqrt(r2);
+    const double rr = r2 * y;
+    r = fma(fma(-rr, rr, r2), 0.5 * y, rr);
+    inv = y;
+}
+
+__device__ __forceinline__ float sinc_pi_fast(float x)
+{   // same function, approximate division (2 ulp)
+    if (x == 0.f) return 1.f;
+    return __fdividef(sinpif(x), 3.14159265358979323846f * x);
+}
+
+__device__ __forceinline__ uint32_t turns_to_u32_fast(double x)
+{   // frac(x) in 2^-32 turn units for |x| < 2^30: the 64-bit integer conversion wraps modulo one turn
+    return (uint32_t)(unsigned long long)__double2ll_rn(x * 4294967296.0);
+}
+
 struct Leg { double r; float g; };
+
+// One antenna leg with the pieces the receive-channel series needs: d = pos - ant, r = |d|, 1/r and
+// the un-normalised projections on the azimuth / elevation axes.
+struct LegParts { double r, inv, da, de, dx, dy, dz; };
+
+__device__ __forceinline__ LegParts leg_parts(const double pos[3], const double ant[3], const double ax_a[3],
+                                              const double ax_e[3])
+{
+    LegParts o;
+    o.dx = pos[0] - ant[0]; o.dy = pos[1] - ant[1]; o.dz = pos[2] - ant[2];
+    root_and_inverse(fma(o.dx, o.dx, fma(o.dy, o.dy, o.dz * o.dz)), o.r, o.inv);
+    o.da = fma(o.dx, ax_a[0], fma(o.dy, ax_a[1], o.dz * ax_a[2]));
+    o.de = fma(o.dx, ax_e[0], fma(o.dy, ax_e[1], o.dz * ax_e[2]));
+    return o;
+}
+
+__device__ __forceinline__ float pattern(double da, double de, double inv, double ap_a, double ap_e)
+{   // O6: sinc(La u_a / lambda) sinc(Le u_e / lambda), direction cosines u = (d . axis) / r
+    return sinc_pi_fast((float)(ap_a * (da * inv))) * sinc_pi_fast((float)(ap_e * (de * inv)));
+}
+
+// Receive phase centre c sits at rx_ref + o v^ (G8).  With d = pos - rx_ref, r = |d|:
+//   r_c^2 = r^2 + X,  X = o^2 - 2 o (d . v^),  delta = X / r^2   (|delta| <= ~2|o|/r)
+//   r_c   = r (1 + delta/2 - delta^2/8 + delta^3/16)            truncation 5/128 delta^4
+//   1/r_c = (1/r)(1 - delta/2 + 3 delta^2/8 - 5 delta^3/16)     truncation 35/128 delta^4
+// sim_create enables this only when |o| <= 1e-4 r_min (delta^4 < 3e-15: below fp64 rounding of r).
+__device__ __forceinline__ void channel_leg_series(const LegParts &ref, double dv, double o, double va, double ve,
+                                                   double &r_c, double &inv_c, double &da_c, double &de_c)
+{
+    const double X = fma(o, o, -2.0 * o * dv);
+    const double dl = X * ref.inv * ref.inv;
+    r_c = fma(ref.r, dl * fma(dl, fma(dl, 0.0625, -0.125), 0.5), ref.r);
+    inv_c = fma(ref.inv, dl * fma(dl, fma(dl, -0.3125, 0.375), -0.5), ref.inv);
+    da_c = fma(-o, va, ref.da);
+    de_c = fma(-o, ve, ref.de);
+}
 
 __device__ __forceinline__ Leg leg(const double pos[3], const double ant[3], const double ax_a[3],
                                    const double ax_e[3], double ap_a, double ap_e)

@@ -18,6 +18,9 @@ struct PulseConst {
     double rx_a[3], rx_e[3];
     double rx_ref[3];            // un-offset Rx phase centre (cull reference, G6)
     double rx_pos[kMaxChannels][3];   // P_rx + o_c * v_rx/|v_rx|   (G8)
+    double rx_vhat[3];           // v_rx/|v_rx|
+    double rx_va, rx_ve;         // v^ . azimuth axis, v^ . elevation axis (Rx frame)
+    double ch_off[kMaxChannels]; // o_c
 };
 
 // One surviving facet-echo as the accumulation kernel consumes it (32 B, 16 B aligned).
@@ -64,6 +67,7 @@ struct DevParams {
     // scene
     int32_t n_waves, choppy, tilt, has_sigma0, has_current;
     double sigma0_uniform, look_x, look_y, cur_ux, cur_uy;
+    int32_t series_channels;     // receive-channel legs by series about the un-offset phase centre (geometry_common.cuh)
 };
 
 }  // namespace heeps

@@ -37,7 +37,7 @@ constexpr int kThreads = 256;
 constexpr int kKt = kMomentOrder;      // 8
 static_assert(kKt == 8, "the reduce-scatter below is written for 8 moments / 8 threads per slice");
 
-template <int FPT>
+template <int FPT, bool kSeries>
 __global__ void __launch_bounds__(kThreads)
 moments_kernel(DevParams prm, MomentArgs a, int p0, int n_pl)
 {
@@ -80,7 +80,8 @@ moments_kernel(DevParams prm, MomentArgs a, int p0, int n_pl)
     const size_t F = (size_t)prm.nx * prm.ny;
     const SurfaceInterp it = surface_interp(a.surf, a.pulses, p, pl);
     const float area = (float)(prm.spacing * prm.spacing);
-    double pos[FPT][3], rt[FPT];
+    double pos[FPT][3], rt[FPT], dv[FPT];
+    LegParts ref[FPT];
     float gt[FPT], amag[FPT];
     uint32_t xarg[FPT];
     bool keep[FPT];
@@ -103,10 +104,12 @@ moments_kernel(DevParams prm, MomentArgs a, int p0, int n_pl)
             pos[q][1] = yb + cuy * pc.t;
             pos[q][2] = prm.cz + surface_z(a.surf, it, F, f);
             if (a.surf.dxy) { const double2 dd = surface_dxy(a.surf, it, F, f); pos[q][0] += dd.x; pos[q][1] += dd.y; }
-            const Leg lt = leg(pos[q], pc.tx_pos, pc.tx_a, pc.tx_e, prm.ap_tx_a, prm.ap_tx_e);
-            const Leg lr = leg(pos[q], pc.rx_ref, pc.rx_a, pc.rx_e, prm.ap_rx_a, prm.ap_rx_e);
-            rt[q] = lt.r; gt[q] = lt.g;
-            keep[q] = !(fabsf(lt.g * lr.g) < prm.cull_thr);                 // O7 (G6)
+            const LegParts lt = leg_parts(pos[q], pc.tx_pos, pc.tx_a, pc.tx_e);
+            ref[q] = leg_parts(pos[q], pc.rx_ref, pc.rx_a, pc.rx_e);
+            dv[q] = fma(ref[q].dx, pc.rx_vhat[0], fma(ref[q].dy, pc.rx_vhat[1], ref[q].dz * pc.rx_vhat[2]));
+            rt[q] = lt.r; gt[q] = pattern(lt.da, lt.de, lt.inv, prm.ap_tx_a, prm.ap_tx_e);
+            const float g_ref = pattern(ref[q].da, ref[q].de, ref[q].inv, prm.ap_rx_a, prm.ap_rx_e);
+            keep[q] = !(fabsf(gt[q] * g_ref) < prm.cull_thr);               // O7 (G6)
             float sig = a.sigma0 ? __ldg(a.sigma0 + f) : (float)prm.sigma0_uniform;
             if (prm.tilt) {
                 const float2 sl = surface_slope(a.surf, it, F, f);
@@ -132,15 +135,22 @@ moments_kernel(DevParams prm, MomentArgs a, int p0, int n_pl)
         for (int q = 0; q < FPT; ++q) {
             bin[q] = -1; rank[q] = 0; br[q] = bi[q] = yy[q] = 0.f;
             if (!keep[q]) continue;
-            const Leg lr = leg(pos[q], pc.rx_pos[c], pc.rx_a, pc.rx_e, prm.ap_rx_a, prm.ap_rx_e);
-            const double dR = (rt[q] + lr.r) - pc.r0;
+            double r_c, inv_c, da_c, de_c;
+            if (kSeries) {
+                channel_leg_series(ref[q], dv[q], pc.ch_off[c], pc.rx_va, pc.rx_ve, r_c, inv_c, da_c, de_c);
+            } else {
+                const LegParts lc = leg_parts(pos[q], pc.rx_pos[c], pc.rx_a, pc.rx_e);
+                r_c = lc.r; inv_c = lc.inv; da_c = lc.da; de_c = lc.de;
+            }
+            const float g_rx = pattern(da_c, de_c, inv_c, prm.ap_rx_a, prm.ap_rx_e);
+            const double dR = (rt[q] + r_c) - pc.r0;
             const double nu = dR * prm.fs_over_c0 - prm.half_len;
             const double bd = ceil(nu);
             if (!(bd > -(double)L && bd < (double)prm.n_samples)) continue;    // window misses [0, Ns)
             const int b = (int)bd;
             const double eps = bd - nu;                                    // [0, 1)
-            const float g = gt[q] * lr.g;
-            const uint32_t ph = turns_to_u32(fma(prm.kappa * eps, eps, -dR * prm.inv_lambda)) + xarg[q] +
+            const float g = gt[q] * g_rx;
+            const uint32_t ph = turns_to_u32_fast(fma(prm.kappa * eps, eps, -dR * prm.inv_lambda)) + xarg[q] +
                                 ((g < 0.f) ? 0x80000000u : 0u);
             float sn, cs;
             __sincosf((float)(int32_t)ph * 1.4629180792671596e-9f, &sn, &cs);   // 2 pi / 2^32
@@ -270,10 +280,13 @@ cudaError_t launch_moments(const DevParams &prm, const MomentArgs &a, int p0, in
 {
     dim3 grid(prm.n_tiles, n_pl);
     const size_t smem = moments_smem_bytes(prm, a.span_cap);
+    const bool series = prm.series_channels != 0;
     if (prm.tile_cap <= kThreads) {
-        moments_kernel<1><<<grid, kThreads, smem, s>>>(prm, a, p0, n_pl);
+        if (series) moments_kernel<1, true><<<grid, kThreads, smem, s>>>(prm, a, p0, n_pl);
+        else        moments_kernel<1, false><<<grid, kThreads, smem, s>>>(prm, a, p0, n_pl);
     } else if (prm.tile_cap <= 4 * kThreads) {
-        moments_kernel<4><<<grid, kThreads, smem, s>>>(prm, a, p0, n_pl);
+        if (series) moments_kernel<4, true><<<grid, kThreads, smem, s>>>(prm, a, p0, n_pl);
+        else        moments_kernel<4, false><<<grid, kThreads, smem, s>>>(prm, a, p0, n_pl);
     } else {
         return cudaErrorInvalidValue;      // the spectral path tiles at <= 32 x 32 facets
     }

@@ -363,6 +363,19 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     h->accum = accumulate_plan(prm, tile_spread);
     h->span_cap_m = std::min(4096, (((int)std::ceil(tile_spread) + 8) + 31) & ~31);
 
+    {   // receive-channel legs by series (geometry_common.cuh): offsets small against the nearest range
+        double o_max = 0, r_min = 1e300;
+        for (int c = 0; c < C; ++c) o_max = std::max(o_max, std::fabs(in->channel_offset_m[c]));
+        const double radius = 0.5 * std::hypot(nx * sc->spacing_m, ny * sc->spacing_m) + 4.0 * wave_sum + 100.0;
+        for (int p = 0; p < P; ++p) {
+            const double *r = g->rx_pos_m + 3 * p;
+            const double d = std::sqrt((r[0] - sc->centre_m[0]) * (r[0] - sc->centre_m[0]) +
+                                       (r[1] - sc->centre_m[1]) * (r[1] - sc->centre_m[1]) +
+                                       (r[2] - sc->centre_m[2]) * (r[2] - sc->centre_m[2]));
+            r_min = std::min(r_min, d - radius);
+        }
+        prm.series_channels = (r_min > 0 && o_max <= 1e-4 * r_min) ? 1 : 0;
+    }
     h->key_H = choose_keyframe_spacing(g, sc, opts ? opts->kinematics_keyframe : 0);
     // ---- batch size ----
     const int64_t fcap = (int64_t)prm.n_tiles * prm.tile_cap;
@@ -421,7 +434,11 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
             pc.rx_a[k] = g->rx_frame[9 * p + 3 + k]; pc.rx_e[k] = g->rx_frame[9 * p + 6 + k];
             pc.rx_ref[k] = g->rx_pos_m[3 * p + k];
             for (int c = 0; c < C; ++c) pc.rx_pos[c][k] = g->rx_pos_m[3 * p + k] + in->channel_offset_m[c] * v[k] / vn;
+            pc.rx_vhat[k] = v[k] / vn;
+            pc.rx_va += pc.rx_vhat[k] * pc.rx_a[k];
+            pc.rx_ve += pc.rx_vhat[k] * pc.rx_e[k];
         }
+        for (int c = 0; c < C; ++c) pc.ch_off[c] = in->channel_offset_m[c];
         // carrier phase of the reference path: f0 * (r0/c0), reduced in long double
         long double cyc = (long double)pc.r0 * ((long double)in->f0_hz / (long double)kC0);
         long double fr = cyc - floorl(cyc);
