@@ -246,7 +246,7 @@ def run_cuda(args):
     # weak scaling: rank r simulates pulses [r P, (r+1) P) of an N*P-pulse acquisition
     w = make_workload(args.workload, n_pulses=P, pulse_offset=rank * P)
     F, C, Ns, L = w.n_facets, w.n_channels, w.n_samples, w.replica_samples
-    sim = Simulator(w, local_rank, accumulate_mode=args.mode)
+    sim = Simulator(w, local_rank, accumulate_mode=args.mode, tile_facets=args.tile)
     out = torch.empty((C, P, Ns), dtype=torch.complex64, device=f"cuda:{local_rank}")
     stream = torch.cuda.current_stream()
 
@@ -369,6 +369,7 @@ def main():
     ap.add_argument("--workload", default="ati")
     ap.add_argument("--mode", default="auto", choices=["auto", "direct", "spectral"],
                     help="echo accumulation (include/heeps_sim.h SIM_ACCUMULATE_*)")
+    ap.add_argument("--tile", type=int, default=0, help="spatial tile side in facets (0 = library default)")
     ap.add_argument("--pulses", type=int, default=None, help="override the dwell length (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-direct", action="store_true", help="skip the direct-form comparison leg")

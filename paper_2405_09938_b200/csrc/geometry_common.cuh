@@ -33,9 +33,19 @@ __device__ __forceinline__ void root_and_inverse(double r2, double &r, double &i
 }
 
 __device__ __forceinline__ float sinc_pi_fast(float x)
-{   // same function, approximate division (2 ulp)
+{   // same function without sinpif/IEEE division: with n = rint(x), r = x - n in [-1/2, 1/2],
+    //   sin(pi x)/(pi x) = (-1)^n [sin(pi r)/(pi r)] r / x,
+    // the bracket by its Taylor series through (pi r)^10 (next term 3.6e-8 at r = 1/2).  |x| < 2^22.
     if (x == 0.f) return 1.f;
-    return __fdividef(sinpif(x), 3.14159265358979323846f * x);
+    const float n = rintf(x), r = x - n;
+    const float t = r * r;
+    float p = fmaf(t, -2.3460810e-3f, 2.6147848e-2f);        // -pi^10/11!, pi^8/9!
+    p = fmaf(t, p, -1.9075182e-1f);                            // -pi^6/7!
+    p = fmaf(t, p, 8.1174243e-1f);                             //  pi^4/5!
+    p = fmaf(t, p, -1.6449341f);                               // -pi^2/3!
+    p = fmaf(t, p, 1.0f);
+    const float q = __fdividef(p * r, x);
+    return ((int)n & 1) ? -q : q;
 }
 
 __device__ __forceinline__ uint32_t turns_to_u32_fast(double x)
