@@ -110,7 +110,13 @@ typedef struct {
     int32_t kinematics_keyframe;   /* wave sums evaluated exactly every H-th pulse (with time derivatives) and
                                       cubic-Hermite interpolated between: 0 = auto (largest H <= 64 whose error
                                       bound sum_w A_w (omega_w h)^4/384 <= 1e-9 m), 1 = every pulse, n = force H = n */
-    int32_t reserved[6];
+    int32_t geometry_keyframe;     /* SPECTRAL only: 0 = auto -- where kinematics keyframes are in use (H > 1), C <= 4 and
+                                      the receive offsets are small, ranges / gains are evaluated exactly at the
+                                      keyframe pulses only and interpolated between (Hermite path length, quadratic
+                                      gains), after sim_create has verified the interpolants against the exact geometry
+                                      at every pulse on a lattice of scene points (path 2e-8 m, gains 3e-6);
+                                      1 = off (exact geometry at every pulse) */
+    int32_t reserved[5];
 } sim_options;
 
 /*
@@ -164,6 +170,7 @@ typedef struct {
     int32_t accumulate_mode;       /* SIM_ACCUMULATE_DIRECT or _SPECTRAL, as resolved at sim_create */
     int32_t fft_size;              /* SPECTRAL: transform length; else 0              */
     int32_t kinematics_keyframe;   /* H as resolved at sim_create                     */
+    int32_t geometry_keyframed;    /* 1 when ranges / gains are interpolated between keyframes (sim_options) */
 } sim_stats;
 int sim_get_stats(sim_handle *h, sim_stats *out);
 

@@ -62,7 +62,8 @@ class sim_scene(C.Structure):
 
 class sim_options(C.Structure):
     _fields_ = [("tile_facets", C.c_int32), ("pulses_per_batch", C.c_int32), ("workspace_bytes", C.c_int64),
-                ("accumulate_mode", C.c_int32), ("kinematics_keyframe", C.c_int32), ("reserved", C.c_int32 * 6)]
+                ("accumulate_mode", C.c_int32), ("kinematics_keyframe", C.c_int32), ("geometry_keyframe", C.c_int32),
+                ("reserved", C.c_int32 * 5)]
 
 
 class sim_stats(C.Structure):
@@ -72,6 +73,7 @@ class sim_stats(C.Structure):
         ("tile_facets", C.c_int32), ("pulses_per_batch", C.c_int32), ("n_tiles", C.c_int32),
         ("accumulate_block_threads", C.c_int32), ("max_span_samples", C.c_int32),
         ("accumulate_mode", C.c_int32), ("fft_size", C.c_int32), ("kinematics_keyframe", C.c_int32),
+        ("geometry_keyframed", C.c_int32),
     ]
 
 
@@ -218,13 +220,15 @@ def _marshal(workload):
 # ----------------------------------------------------------------------------- C-named functions
 
 def sim_create(workload, device: int = 0, *, tile_facets: int = 0, pulses_per_batch: int = 0,
-               workspace_bytes: int = 0, accumulate_mode=0, kinematics_keyframe: int = 0):
+               workspace_bytes: int = 0, accumulate_mode=0, kinematics_keyframe: int = 0,
+               geometry_keyframe: int = 0):
     lib = load_library()
     ci, cg, cs, keep = _marshal(workload)
     opts = sim_options()
     opts.tile_facets, opts.pulses_per_batch, opts.workspace_bytes = tile_facets, pulses_per_batch, workspace_bytes
     opts.accumulate_mode = _MODES[accumulate_mode]
     opts.kinematics_keyframe = int(kinematics_keyframe)
+    opts.geometry_keyframe = int(geometry_keyframe)
     h = C.c_void_p()
     rc = lib.sim_create(C.byref(ci), C.byref(cg), C.byref(cs), C.byref(opts), int(device), C.byref(h))
     del keep

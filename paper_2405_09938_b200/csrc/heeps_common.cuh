@@ -21,6 +21,7 @@ struct PulseConst {
     double rx_vhat[3];           // v_rx/|v_rx|
     double rx_va, rx_ve;         // v^ . azimuth axis, v^ . elevation axis (Rx frame)
     double ch_off[kMaxChannels]; // o_c
+    double tx_vel[3], rx_vel[3]; // platform velocities (keyframed geometry: d/dt of the path length)
 };
 
 // One surviving facet-echo as the accumulation kernel consumes it (32 B, 16 B aligned).

@@ -1,0 +1,481 @@
+// K2k -- geometry, gains, amplitude, cull and range-slice moments with the GEOMETRY evaluated exactly only
+// at the kinematics keyframes (SURVEY.md §8(a) A2..A6 moment form).
+//
+// moments.cu evaluates the fp64 antenna legs and the sinc patterns of every facet at every pulse: 1156
+// instructions per facet-pulse, issue-bound (profiles/r1_v4).  But over one keyframe interval (H pulses, a few
+// milliseconds) everything a facet-echo needs is a smooth function of time:
+//
+//   R(t)   = r_t + r_r,ref  bistatic path to the un-offset phase centre: cubic HERMITE from the exact values and
+//            time derivatives at the two keyframes,  dR/dt = u_t.(v_f - V_tx) + u_r.(v_f - V_rx)  with the facet
+//            velocity v_f = (current + dD_h/dt, dz/dt) from K1's rate rows.  Error <= h^4 max|R''''| / 384:
+//            platform term 3 V^4/r^3 ~ 0.02 m/s^4 -> 4e-13 m at h = 9.4 ms; wave term = K1's own bound (1e-9 m).
+//   d_c(t) = r_r,c - r_r,ref  (receive phase centre c, |o_c| <= 1e-4 r): linear in t, fp32 (|d_c| < 1 m).
+//   P(t)   = G_t G_r,ref      quadratic through t0, t_mid, t1 with the sinc arguments at t_mid taken as the mean of
+//            the end values (they are linear in t to ~1e-7); G_r,c = G_r,ref + o_c dG/do with dG/do by one
+//            finite difference at t_mid.  |a_f|(t) (tilt modulation) quadratic the same way.
+//
+// sim_create verifies these three interpolants against the exact geometry on a 3 x 3 lattice of scene points
+// at EVERY pulse (host, long double) and falls back to moments.cu when any bound fails (sim_api.cu
+// geometry_keyframes_ok): non-smooth state vectors never reach this kernel.
+//
+// One CTA = one spatial tile x one keyframe interval.  A thread owns FPT facets, holds their interpolants in
+// registers (15 + 2C words per facet) and loops over the interval's pulses; per pulse and for all C channels at
+// once: slice, sub-slice position and complex weight of every facet-echo -> counting sort by slice through a
+// shared-memory histogram (integer ATOMS) and an index list -> 8 threads per slice sum the Kt Chebyshev
+// moments (packed FFMA2), reduce-scatter by shuffles, one RED.ADD.F32x2 per (slice, k).  Histogram, payload
+// and index list are double-buffered: three barriers per pulse.
+//
+// Bound: issue slots (FP32 + FP64 mix); HBM/L2: four surface rows per facet and INTERVAL, the maps once.
+#include "kernels.cuh"
+#include "geometry_common.cuh"
+
+namespace heeps {
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kKt = kMomentOrder;
+static_assert(kKt == 8, "the reduce-scatter below is written for 8 moments / 8 threads per slice");
+
+struct __align__(16) KeyPulse {          // per pulse of the interval (shared memory)
+    double w00, w10, w01, w11;           // Hermite weights (surface.cuh)
+    double r0;                           // c0 t0[p]
+    float s, pad0;                       // (t - t0) / h
+    int32_t base[kMaxKeyChannels];       // first slice of the tile's shared-memory window, per channel
+};
+
+// Exact state of one facet at one keyframe pulse.
+template <int C>
+struct KeyEval {
+    double R, Rd;                        // path to the un-offset phase centre and its time derivative
+    float xat, xet, xar, xer;            // sinc arguments: Tx azimuth / elevation, Rx (un-offset) azimuth / elevation
+    float xao, xeo;                      // Rx arguments at the finite-difference offset o_fd
+    float dl[C];                         // r_r,c - r_r,ref
+};
+
+template <int C>
+__device__ __forceinline__ KeyEval<C> key_eval(const DevParams &prm, const PulseConst &pc, const double pos[3],
+                                               const double vel[3], double o_fd)
+{
+    KeyEval<C> o;
+    const LegParts lt = leg_parts(pos, pc.tx_pos, pc.tx_a, pc.tx_e);
+    const LegParts lr = leg_parts(pos, pc.rx_ref, pc.rx_a, pc.rx_e);
+    o.R = lt.r + lr.r;
+    const double at = fma(lt.dx, vel[0] - pc.tx_vel[0], fma(lt.dy, vel[1] - pc.tx_vel[1], lt.dz * (vel[2] - pc.tx_vel[2])));
+    const double ar = fma(lr.dx, vel[0] - pc.rx_vel[0], fma(lr.dy, vel[1] - pc.rx_vel[1], lr.dz * (vel[2] - pc.rx_vel[2])));
+    o.Rd = fma(at, lt.inv, ar * lr.inv);
+    o.xat = (float)(prm.ap_tx_a * (lt.da * lt.inv)); o.xet = (float)(prm.ap_tx_e * (lt.de * lt.inv));
+    o.xar = (float)(prm.ap_rx_a * (lr.da * lr.inv)); o.xer = (float)(prm.ap_rx_e * (lr.de * lr.inv));
+    const double dv = fma(lr.dx, pc.rx_vhat[0], fma(lr.dy, pc.rx_vhat[1], lr.dz * pc.rx_vhat[2]));
+    {
+        double r_c, inv_c, da_c, de_c;
+        channel_leg_series(lr, dv, o_fd, pc.rx_va, pc.rx_ve, r_c, inv_c, da_c, de_c);
+        o.xao = (float)(prm.ap_rx_a * (da_c * inv_c)); o.xeo = (float)(prm.ap_rx_e * (de_c * inv_c));
+    }
+#pragma unroll
+    for (int c = 0; c < C; ++c) {
+        // r_c - r = r (dl/2 - dl^2/8 + dl^3/16), dl = (o^2 - 2 o d.v^)/r^2   (geometry_common.cuh)
+        const double oc = pc.ch_off[c];
+        const double dl = fma(oc, oc, -2.0 * oc * dv) * lr.inv * lr.inv;
+        o.dl[c] = (float)(lr.r * (dl * fma(dl, fma(dl, 0.0625, -0.125), 0.5)));
+    }
+    return o;
+}
+
+__device__ __forceinline__ float pattern_x(float xa, float xe) { return sinc_pi_fast(xa) * sinc_pi_fast(xe); }
+
+template <int FPT, int C, bool kTilt>
+__global__ void __launch_bounds__(kThreads, 2)
+moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_first)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ PulseConst pc2[2];
+    __shared__ KeyPulse s_kp[kMaxKeyPulses];
+    __shared__ double s_rc[2][kMaxKeyChannels];          // path length of the tile centre at the two keyframes
+    __shared__ unsigned long long s_samples;
+    __shared__ int s_kept;
+
+    const int span = a.span_cap, hstride = span + 1;
+    const int cap = prm.tile_cap;
+    // [2][C][cap] float2 weight | [2][C][cap] float y | [2][C][cap] u16 index list | [2][C][span + 1] int histogram
+    float2 *payload = reinterpret_cast<float2 *>(smem_raw);
+    float *payload_y = reinterpret_cast<float *>(smem_raw + (size_t)2 * C * cap * 8);
+    unsigned short *idx = reinterpret_cast<unsigned short *>(smem_raw + (size_t)2 * C * cap * 12);
+    int *hist = reinterpret_cast<int *>(smem_raw + (size_t)2 * C * cap * 14);
+
+    const int tile = blockIdx.x, j = j_first + blockIdx.y;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int H = a.surf.H, P = a.surf.n_pulses_total;
+    const int n_keys = (P - 1 + H - 1) / H + 1;
+    const int k0 = min(j * H, P - 1), k1 = min((j + 1) * H, P - 1);
+    // pulses of this interval inside the batch: [lo, hi)
+    const int lo = max(j * H, p0), hi = min((j == n_keys - 2) ? P : (j + 1) * H, p0 + n_pl);
+    if (lo >= hi) return;
+    {
+        const double *s0 = reinterpret_cast<const double *>(a.pulses + k0);
+        const double *s1 = reinterpret_cast<const double *>(a.pulses + k1);
+        double *d0 = reinterpret_cast<double *>(&pc2[0]), *d1 = reinterpret_cast<double *>(&pc2[1]);
+        for (int k = tid; k < (int)(sizeof(PulseConst) / sizeof(double)); k += kThreads) { d0[k] = s0[k]; d1[k] = s1[k]; }
+    }
+    if (tid == 0) { s_samples = 0ull; s_kept = 0; }
+    for (int k = tid; k < 2 * C * hstride; k += kThreads) hist[k] = 0;
+    __syncthreads();
+
+    const int ts = prm.tile, lts = 31 - __clz(ts);
+    const int ti0 = (tile % prm.tiles_x) * ts, tj0 = (tile / prm.tiles_x) * ts;
+    if (tid < 2 * C) {
+        // tile centre (rest, flat) at the two keyframes: positions the slice window of every pulse between
+        const int e = tid / C, c = tid - e * C;
+        const PulseConst &pc = pc2[e];
+        const double ic = ti0 + 0.5 * (min(ts, prm.nx - ti0) - 1), jc = tj0 + 0.5 * (min(ts, prm.ny - tj0) - 1);
+        const double x = prm.cx + (ic - 0.5 * (prm.nx - 1)) * prm.spacing;
+        const double y = prm.cy + (jc - 0.5 * (prm.ny - 1)) * prm.spacing;
+        const double ax = x - pc.tx_pos[0], ay = y - pc.tx_pos[1], az = prm.cz - pc.tx_pos[2];
+        const double bx = x - pc.rx_pos[c][0], by = y - pc.rx_pos[c][1], bz = prm.cz - pc.rx_pos[c][2];
+        s_rc[e][c] = sqrt(ax * ax + ay * ay + az * az) + sqrt(bx * bx + by * by + bz * bz);
+    }
+    __syncthreads();
+    for (int ip = tid; ip < hi - lo; ip += kThreads) {
+        const int p = lo + ip;
+        const double t0 = pc2[0].t, t1 = pc2[1].t, t = a.pulses[p].t;
+        const double h = t1 - t0;
+        const double s = (h != 0.0) ? (t - t0) / h : 0.0;
+        const double s2 = s * s, s3 = s2 * s;
+        KeyPulse kp;
+        kp.w00 = 2.0 * s3 - 3.0 * s2 + 1.0;
+        kp.w10 = (s3 - 2.0 * s2 + s) * h;
+        kp.w01 = -2.0 * s3 + 3.0 * s2;
+        kp.w11 = (s3 - s2) * h;
+        kp.r0 = a.pulses[p].r0;
+        kp.s = (float)s; kp.pad0 = 0.f;
+#pragma unroll
+        for (int c = 0; c < kMaxKeyChannels; ++c) {
+            int base = 0;
+            if (c < C) {
+                const double rc = fma(s, s_rc[1][c] - s_rc[0][c], s_rc[0][c]);
+                double bc = ceil((rc - kp.r0) * prm.fs_over_c0 - prm.half_len) - 0.5 * span;
+                bc = fmin(fmax(bc, -1.0e9), 1.0e9);
+                base = (int)bc;
+            }
+            kp.base[c] = base;
+        }
+        s_kp[ip] = kp;
+    }
+
+    // ---- interpolants of this thread's facets over the interval ----
+    const size_t F = (size_t)prm.nx * prm.ny;
+    const size_t row0 = (size_t)(j - a.surf.key0) * F, row1 = row0 + F;
+    const float area = (float)(prm.spacing * prm.spacing);
+    double o_fd = 0.0;
+#pragma unroll
+    for (int c = 0; c < C; ++c) o_fd = fmax(o_fd, fabs(pc2[0].ch_off[c]));
+    const float inv_ofd = (o_fd > 0.0) ? (float)(1.0 / o_fd) : 0.f;
+
+    double R0[FPT], R0d[FPT], R1[FPT], R1d[FPT];
+    float dl0[FPT][C], ddl[FPT][C];
+    float pq0[FPT], pqa[FPT], pqb[FPT], bq[FPT];         // P(s) = pq0 + s (pqa + s pqb); bq = G_t dG_r/do
+    float am0[FPT], ama[FPT], amb[FPT];                  // |a_f|(s), quadratic when tilt-modulated
+    uint32_t xarg[FPT];
+    bool valid[FPT];
+#pragma unroll
+    for (int q = 0; q < FPT; ++q) {
+        const int k = q * kThreads + tid;
+        const int li = k & (ts - 1), lj = k >> lts;
+        const int i = ti0 + li, jj = tj0 + lj;
+        valid[q] = (k < ts * ts && i < prm.nx && jj < prm.ny);
+        R0[q] = R0d[q] = R1[q] = R1d[q] = 0.0;
+        pq0[q] = pqa[q] = pqb[q] = bq[q] = 0.f; am0[q] = ama[q] = amb[q] = 0.f; xarg[q] = 0u;
+#pragma unroll
+        for (int c = 0; c < C; ++c) { dl0[q][c] = 0.f; ddl[q][c] = 0.f; }
+        if (!valid[q]) continue;
+        const size_t f = (size_t)jj * prm.nx + i;
+        const double xb = prm.cx + ((double)i - 0.5 * (prm.nx - 1)) * prm.spacing;
+        const double yb = prm.cy + ((double)jj - 0.5 * (prm.ny - 1)) * prm.spacing;
+        double cux = prm.cur_ux, cuy = prm.cur_uy;
+        if (a.current) { const float2 cv = __ldg(a.current + f); cux = cv.x; cuy = cv.y; }
+        KeyEval<C> ev[2];
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const PulseConst &pc = pc2[e];
+            const size_t r = (e ? row1 : row0) + f;
+            double pos[3] = {fma(cux, pc.t, xb), fma(cuy, pc.t, yb), prm.cz + a.surf.z[r]};
+            double vel[3] = {cux, cuy, a.surf.zt[r]};
+            if (a.surf.dxy) {
+                const double2 dd = a.surf.dxy[r], dt = a.surf.dxy_t[r];
+                pos[0] += dd.x; pos[1] += dd.y; vel[0] += dt.x; vel[1] += dt.y;
+            }
+            ev[e] = key_eval<C>(prm, pc, pos, vel, o_fd);
+        }
+        R0[q] = ev[0].R; R0d[q] = ev[0].Rd; R1[q] = ev[1].R; R1d[q] = ev[1].Rd;
+#pragma unroll
+        for (int c = 0; c < C; ++c) { dl0[q][c] = ev[0].dl[c]; ddl[q][c] = ev[1].dl[c] - ev[0].dl[c]; }
+        // gains at s = 0, 1/2, 1 (sinc arguments at the midpoint = mean of the end values)
+        const float gt0 = pattern_x(ev[0].xat, ev[0].xet), gr0 = pattern_x(ev[0].xar, ev[0].xer);
+        const float gt1 = pattern_x(ev[1].xat, ev[1].xet), gr1 = pattern_x(ev[1].xar, ev[1].xer);
+        const float gtm = pattern_x(0.5f * (ev[0].xat + ev[1].xat), 0.5f * (ev[0].xet + ev[1].xet));
+        const float grm = pattern_x(0.5f * (ev[0].xar + ev[1].xar), 0.5f * (ev[0].xer + ev[1].xer));
+        const float gom = pattern_x(0.5f * (ev[0].xao + ev[1].xao), 0.5f * (ev[0].xeo + ev[1].xeo));
+        const float P0 = gt0 * gr0, Pm = gtm * grm, P1 = gt1 * gr1;
+        pq0[q] = P0; pqa[q] = -3.f * P0 + 4.f * Pm - P1; pqb[q] = 2.f * P0 - 4.f * Pm + 2.f * P1;
+        bq[q] = gtm * (gom - grm) * inv_ofd;
+        // amplitude (O8): sqrt(sigma0 tilt d^2) |xi|
+        const float sig = a.sigma0 ? __ldg(a.sigma0 + f) : (float)prm.sigma0_uniform;
+        const uint2 xp = __ldg(a.xi_polar + f);
+        const float xmag = __uint_as_float(xp.x);
+        xarg[q] = xp.y;
+        if (kTilt) {
+            const float2 sl0 = a.surf.slope[row0 + f], sd0 = a.surf.slope_t[row0 + f];
+            const float2 sl1 = a.surf.slope[row1 + f], sd1 = a.surf.slope_t[row1 + f];
+            const float hh = (float)(pc2[1].t - pc2[0].t);
+            // Hermite at s = 1/2: (v0 + v1)/2 + h (d0 - d1)/8
+            const float smx = 0.5f * (sl0.x + sl1.x) + 0.125f * hh * (sd0.x - sd1.x);
+            const float smy = 0.5f * (sl0.y + sl1.y) + 0.125f * hh * (sd0.y - sd1.y);
+            const float lx = (float)prm.look_x, ly = (float)prm.look_y;
+            const float A0 = sqrtf(sig * fmaxf(1.f + 2.f * (sl0.x * lx + sl0.y * ly), 0.f) * area) * xmag;
+            const float Am = sqrtf(sig * fmaxf(1.f + 2.f * (smx * lx + smy * ly), 0.f) * area) * xmag;
+            const float A1 = sqrtf(sig * fmaxf(1.f + 2.f * (sl1.x * lx + sl1.y * ly), 0.f) * area) * xmag;
+            am0[q] = A0; ama[q] = -3.f * A0 + 4.f * Am - A1; amb[q] = 2.f * A0 - 4.f * Am + 2.f * A1;
+        } else {
+            am0[q] = sqrtf(sig * area) * xmag;
+        }
+    }
+    __syncthreads();                                     // s_kp complete
+
+    const float kappa_f = (float)prm.kappa;
+    const int L = a.replica;
+    float och[C];
+#pragma unroll
+    for (int c = 0; c < C; ++c) och[c] = (float)pc2[0].ch_off[c];
+    unsigned long long my_samples = 0;
+    int my_kept = 0;
+
+    for (int ip = 0; ip < hi - lo; ++ip) {
+        const int buf = ip & 1;
+        const int pl = lo + ip - p0;
+        const KeyPulse &kp = s_kp[ip];
+        float2 *pay = payload + (size_t)buf * C * cap;
+        float *pay_y = payload_y + (size_t)buf * C * cap;
+        unsigned short *ix = idx + (size_t)buf * C * cap;
+        int *hs = hist + buf * C * hstride;
+        const float s = kp.s;
+        unsigned pulse_samples = 0;
+
+        // ---- A: slice, sub-slice position, complex weight of every facet-echo; rank inside the slice ----
+        int pr[FPT][C];                                  // (slice << 12 | rank) or -1
+#pragma unroll
+        for (int q = 0; q < FPT; ++q) {
+#pragma unroll
+            for (int c = 0; c < C; ++c) pr[q][c] = -1;
+            if (!valid[q]) continue;
+            const float Pv = fmaf(s, fmaf(s, pqb[q], pqa[q]), pq0[q]);
+            if (fabsf(Pv) < prm.cull_thr) continue;                        // O7 (G6)
+            ++my_kept;
+            const float am = kTilt ? fmaf(s, fmaf(s, amb[q], ama[q]), am0[q]) : am0[q];
+            const double R = fma(kp.w00, R0[q], fma(kp.w10, R0d[q], fma(kp.w01, R1[q], kp.w11 * R1d[q])));
+            const double dRref = R - kp.r0;
+            const int k = q * kThreads + tid;
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+                const float dl = fmaf(s, ddl[q][c], dl0[q][c]);
+                const double dR = dRref + (double)dl;
+                const double nu = fma(dR, prm.fs_over_c0, -prm.half_len);
+                const double bd = ceil(nu);
+                if (!(bd > -(double)L && bd < (double)prm.n_samples)) continue;    // window misses [0, Ns)
+                const int b = (int)bd;
+                const float eps = (float)(bd - nu);                               // [0, 1)
+                const float g = fmaf(och[c], bq[q], Pv);
+                const uint32_t ph = turns_to_u32_fast(fma(-dR, prm.inv_lambda, (double)(kappa_f * eps * eps))) +
+                                    xarg[q] + ((g < 0.f) ? 0x80000000u : 0u);
+                float sn, cs;
+                __sincosf((float)(int32_t)ph * 1.4629180792671596e-9f, &sn, &cs);   // 2 pi / 2^32
+                const float mag = fabsf(g) * am;
+                const float yv = fmaf(2.f, eps, -1.f);
+                pulse_samples += (unsigned)(min(b + L, prm.n_samples) - max(b, 0));
+                const int rel = b - kp.base[c];
+                if (rel >= 0 && rel < span) {
+                    pay[c * cap + k] = make_float2(mag * cs, mag * sn);
+                    pay_y[c * cap + k] = yv;
+                    pr[q][c] = (rel << 12) | atomicAdd(&hs[c * hstride + rel + 1], 1);
+                } else {                                                   // outside the tile window: rare
+                    const float br = mag * cs, bi = mag * sn;
+                    float2 *row = a.mom + ((size_t)(c * n_pl + pl) * kKt) * a.nb_pad + (b + L - 1);
+                    float t0 = 1.f, t1 = yv;
+                    atomicAdd(row, make_float2(br, bi));
+                    atomicAdd(row + a.nb_pad, make_float2(br * t1, bi * t1));
+                    for (int kk = 2; kk < kKt; ++kk) {
+                        const float t2 = 2.f * yv * t1 - t0;
+                        atomicAdd(row + (size_t)kk * a.nb_pad, make_float2(br * t2, bi * t2));
+                        t0 = t1; t1 = t2;
+                    }
+                }
+            }
+        }
+        my_samples += pulse_samples;
+        __syncthreads();
+
+        // ---- B: exclusive scan of each channel's histogram (one warp per channel), then the index list ----
+        if ((tid >> 5) < C) {
+            int *hc = hs + (tid >> 5) * hstride;
+            int carry = 0;
+            for (int k0s = 1; k0s <= span; k0s += 32) {
+                const int k = k0s + lane;
+                int v = (k <= span) ? hc[k] : 0;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int t = __shfl_up_sync(0xffffffffu, v, o);
+                    if (lane >= o) v += t;
+                }
+                if (k <= span) hc[k] = v + carry;
+                carry += __shfl_sync(0xffffffffu, v, 31);
+            }
+        }
+        __syncthreads();                                 // hs[c][s] = first sorted position of slice s
+#pragma unroll
+        for (int q = 0; q < FPT; ++q)
+#pragma unroll
+            for (int c = 0; c < C; ++c)
+                if (pr[q][c] >= 0)
+                    ix[c * cap + hs[c * hstride + (pr[q][c] >> 12)] + (pr[q][c] & 4095)] =
+                        (unsigned short)(q * kThreads + tid);
+        {   // the other histogram is free since the previous pulse's stage C: zero it for the next pulse
+            int *hn = hist + (buf ^ 1) * C * hstride;
+            for (int k = tid; k < C * hstride; k += kThreads) hn[k] = 0;
+        }
+        __syncthreads();
+
+        // ---- C: 8 threads per slice: Chebyshev moments, reduce-scatter, one RED per (slice, k) ----
+        const int sub = tid & 7;
+        for (int s0 = 0; s0 < C * span; s0 += kThreads / 8) {
+            const int sl = s0 + (tid >> 3);
+            int c = 0, sidx = 0, first = 0, cnt = 0;
+            if (sl < C * span) {
+                c = sl / span; sidx = sl - c * span;
+                first = hs[c * hstride + sidx]; cnt = hs[c * hstride + sidx + 1] - first;
+            }
+            if (__ballot_sync(0xffffffffu, cnt > 0) == 0u) continue;       // warp-uniform
+            float2 m[kKt];
+#pragma unroll
+            for (int k = 0; k < kKt; ++k) m[k] = make_float2(0.f, 0.f);
+            const unsigned short *ixc = ix + c * cap + first;
+            const float2 *payc = pay + c * cap;
+            const float *payc_y = pay_y + c * cap;
+            for (int i = sub; i < cnt; i += 8) {
+                const int src = ixc[i];
+                const float2 w = payc[src];
+                const float yv = payc_y[src];
+                const float2 y2 = make_float2(yv + yv, yv + yv);
+                float2 t0 = make_float2(1.f, 1.f), t1 = make_float2(yv, yv);
+                m[0] = __fadd2_rn(m[0], w);
+                m[1] = __ffma2_rn(w, t1, m[1]);
+#pragma unroll
+                for (int k = 2; k < kKt; ++k) {
+                    const float2 t2 = __ffma2_rn(y2, t1, make_float2(-t0.x, -t0.y));
+                    m[k] = __ffma2_rn(w, t2, m[k]);
+                    t0 = t1; t1 = t2;
+                }
+            }
+            // reduce-scatter over the 8 threads of the slice: thread `sub` ends with moment k = sub
+            float2 h4[4], h2[2], h1;
+            {
+                const bool hi4 = sub & 4;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const float2 send = hi4 ? m[k] : m[k + 4], kp2 = hi4 ? m[k + 4] : m[k];
+                    h4[k].x = kp2.x + __shfl_xor_sync(0xffffffffu, send.x, 4);
+                    h4[k].y = kp2.y + __shfl_xor_sync(0xffffffffu, send.y, 4);
+                }
+            }
+            {
+                const bool hi2 = sub & 2;
+#pragma unroll
+                for (int k = 0; k < 2; ++k) {
+                    const float2 send = hi2 ? h4[k] : h4[k + 2], kp2 = hi2 ? h4[k + 2] : h4[k];
+                    h2[k].x = kp2.x + __shfl_xor_sync(0xffffffffu, send.x, 2);
+                    h2[k].y = kp2.y + __shfl_xor_sync(0xffffffffu, send.y, 2);
+                }
+            }
+            {
+                const bool hi1 = sub & 1;
+                const float2 send = hi1 ? h2[0] : h2[1], kp2 = hi1 ? h2[1] : h2[0];
+                h1.x = kp2.x + __shfl_xor_sync(0xffffffffu, send.x, 1);
+                h1.y = kp2.y + __shfl_xor_sync(0xffffffffu, send.y, 1);
+            }
+            if (cnt > 0) {
+                float2 *row = a.mom + ((size_t)(c * n_pl + pl) * kKt + sub) * a.nb_pad;
+                atomicAdd(row + (kp.base[c] + sidx + L - 1), h1);
+            }
+        }
+        // no barrier here: the next pulse writes the other payload / index / histogram buffers, and this
+        // pulse's buffers are rewritten only two barriers later
+    }
+
+    // ---- counters ----
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        my_samples += __shfl_xor_sync(0xffffffffu, my_samples, o);
+        my_kept += __shfl_xor_sync(0xffffffffu, my_kept, o);
+    }
+    if (lane == 0) {
+        if (my_samples) atomicAdd(&s_samples, my_samples);
+        if (my_kept) atomicAdd(&s_kept, my_kept);
+    }
+    __syncthreads();
+    if (tid == 0 && a.counters) {
+        if (s_kept) atomicAdd(a.counters + 0, (unsigned long long)s_kept * C);
+        if (s_samples) atomicAdd(a.counters + 1, s_samples);
+    }
+}
+
+template <int FPT, int C>
+cudaError_t launch_fc(const DevParams &prm, const MomentArgs &a, int p0, int n_pl, int j_first, int n_int,
+                      size_t smem, cudaStream_t s)
+{
+    dim3 grid(prm.n_tiles, n_int);
+    auto go = [&](auto kern) -> cudaError_t {
+        if (smem > 48 * 1024) {
+            cudaError_t rc = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (rc != cudaSuccess) return rc;
+        }
+        kern<<<grid, kThreads, smem, s>>>(prm, a, p0, n_pl, j_first);
+        return cudaGetLastError();
+    };
+    return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true>) : go(moments_keyframed_kernel<FPT, C, false>);
+}
+
+template <int FPT>
+cudaError_t launch_f(const DevParams &prm, const MomentArgs &a, int p0, int n_pl, int j_first, int n_int,
+                     size_t smem, cudaStream_t s)
+{
+    switch (prm.n_channels) {
+        case 1: return launch_fc<FPT, 1>(prm, a, p0, n_pl, j_first, n_int, smem, s);
+        case 2: return launch_fc<FPT, 2>(prm, a, p0, n_pl, j_first, n_int, smem, s);
+        case 3: return launch_fc<FPT, 3>(prm, a, p0, n_pl, j_first, n_int, smem, s);
+        case 4: return launch_fc<FPT, 4>(prm, a, p0, n_pl, j_first, n_int, smem, s);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace
+
+size_t moments_keyframed_smem_bytes(const DevParams &prm, int span_cap)
+{
+    const size_t C = prm.n_channels;
+    return (size_t)2 * C * prm.tile_cap * 14 + (size_t)2 * C * (span_cap + 1) * 4;
+}
+
+cudaError_t launch_moments_keyframed(const DevParams &prm, const MomentArgs &a, int p0, int n_pl, cudaStream_t s)
+{
+    const int H = a.surf.H, P = a.surf.n_pulses_total;
+    if (H <= 1 || H + 1 > kMaxKeyPulses || prm.n_channels > kMaxKeyChannels || !prm.series_channels ||
+        a.span_cap >= (1 << 19) || prm.tile_cap > 4096)
+        return cudaErrorInvalidValue;
+    const int n_keys = (P - 1 + H - 1) / H + 1;
+    const int j_first = min(p0 / H, n_keys - 2), j_last = min((p0 + n_pl - 1) / H, n_keys - 2);
+    const int n_int = j_last - j_first + 1;
+    const size_t smem = moments_keyframed_smem_bytes(prm, a.span_cap);
+    if (prm.tile_cap <= kThreads) return launch_f<1>(prm, a, p0, n_pl, j_first, n_int, smem, s);
+    if (prm.tile_cap <= 4 * kThreads) return launch_f<4>(prm, a, p0, n_pl, j_first, n_int, smem, s);
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace heeps

@@ -70,6 +70,7 @@ struct sim_handle {
     DevBuf<float2> slope, slope_t;
     DevBuf<double2> dxy, dxy_t;
     int key_H = 1;                       // keyframe spacing of the kinematics (1 = every pulse)
+    bool geo_keyframed = false;          // spectral path: ranges / gains interpolated between keyframes (K2k)
     int surf_rows_cap = 0;               // rows of the surface buffers
     DevBuf<Rec> recs;
     DevBuf<TileInfo> tinfo;
@@ -246,6 +247,111 @@ int choose_keyframe_spacing(const sim_geometry *g, const sim_scene *sc, int requ
     return 1;
 }
 
+// ---- guard of the keyframed geometry (moments_keyframed.cu) ----
+// Evaluates, in long double on a 3 x 3 lattice of scene points (rest height, drifting with the uniform
+// current), the three interpolants the kernel uses over every keyframe interval of spacing H -- Hermite path
+// length, linear receive-channel path difference, quadratic gain product with the finite-difference channel
+// term -- against the exact geometry at EVERY pulse.  True iff all stay inside: path 2e-8 m, gains 3e-6.
+long double sincl_pi(long double x)
+{
+    if (x == 0.0L) return 1.0L;
+    const long double a = 3.14159265358979323846264338327950288L * x;
+    return sinl(a) / a;
+}
+
+struct GuardEval {
+    long double R, Rd, xat, xet, xar, xer, xao, xeo, dl[SIM_MAX_CHANNELS], gt, gr[SIM_MAX_CHANNELS];
+};
+
+GuardEval guard_eval(const sim_instrument *in, const sim_geometry *g, int p, const long double pos[3],
+                     const long double vel[3], long double o_fd)
+{
+    GuardEval o{};
+    const long double lambda = (long double)kC0 / in->f0_hz;
+    const double *tp = g->tx_pos_m + 3 * p, *rp = g->rx_pos_m + 3 * p, *tv = g->tx_vel_mps + 3 * p,
+                 *rv = g->rx_vel_mps + 3 * p, *tf = g->tx_frame + 9 * p, *rf = g->rx_frame + 9 * p;
+    long double vn = sqrtl((long double)rv[0] * rv[0] + (long double)rv[1] * rv[1] + (long double)rv[2] * rv[2]);
+    long double dt[3], dr[3], rt = 0, rr = 0;
+    for (int k = 0; k < 3; ++k) { dt[k] = pos[k] - tp[k]; dr[k] = pos[k] - rp[k]; rt += dt[k] * dt[k]; rr += dr[k] * dr[k]; }
+    rt = sqrtl(rt); rr = sqrtl(rr);
+    o.R = rt + rr;
+    for (int k = 0; k < 3; ++k) o.Rd += dt[k] * (vel[k] - tv[k]) / rt + dr[k] * (vel[k] - rv[k]) / rr;
+    auto args = [&](const long double d[3], long double r, const double *frame, const double ap[2], long double &xa,
+                    long double &xe) {
+        long double da = 0, de = 0;
+        for (int k = 0; k < 3; ++k) { da += d[k] * frame[3 + k]; de += d[k] * frame[6 + k]; }
+        xa = ap[0] / lambda * da / r; xe = ap[1] / lambda * de / r;
+    };
+    args(dt, rt, tf, in->tx_aperture_m, o.xat, o.xet);
+    args(dr, rr, rf, in->rx_aperture_m, o.xar, o.xer);
+    o.gt = sincl_pi(o.xat) * sincl_pi(o.xet);
+    auto offset_leg = [&](long double off, long double &r_c, long double &xa, long double &xe) {
+        long double d[3]; r_c = 0;
+        for (int k = 0; k < 3; ++k) { d[k] = pos[k] - (rp[k] + off * rv[k] / vn); r_c += d[k] * d[k]; }
+        r_c = sqrtl(r_c);
+        args(d, r_c, rf, in->rx_aperture_m, xa, xe);
+    };
+    long double r_o;
+    offset_leg(o_fd, r_o, o.xao, o.xeo);
+    for (int c = 0; c < in->n_channels; ++c) {
+        long double r_c, xa, xe;
+        offset_leg(in->channel_offset_m[c], r_c, xa, xe);
+        o.dl[c] = r_c - rr;
+        o.gr[c] = sincl_pi(xa) * sincl_pi(xe);
+    }
+    return o;
+}
+
+bool geometry_keyframes_ok(const sim_instrument *in, const sim_geometry *g, const sim_scene *sc, int H)
+{
+    const int P = g->n_pulses, C = in->n_channels;
+    if (H <= 1 || H + 1 > kMaxKeyPulses || C > kMaxKeyChannels) return false;
+    const int n_keys = (P - 1 + H - 1) / H + 1;
+    long double o_fd = 0;
+    for (int c = 0; c < C; ++c) o_fd = std::max<long double>(o_fd, std::fabs(in->channel_offset_m[c]));
+    const long double vel[3] = {sc->current_uniform[0], sc->current_uniform[1], 0.0L};
+    for (int gx = -1; gx <= 1; ++gx)
+        for (int gy = -1; gy <= 1; ++gy) {
+            const long double x0 = sc->centre_m[0] + gx * 0.5L * (sc->nx - 1) * sc->spacing_m;
+            const long double y0 = sc->centre_m[1] + gy * 0.5L * (sc->ny - 1) * sc->spacing_m;
+            auto at = [&](int p, long double pos[3]) {
+                pos[0] = x0 + vel[0] * g->t_pulse_s[p]; pos[1] = y0 + vel[1] * g->t_pulse_s[p]; pos[2] = sc->centre_m[2];
+            };
+            for (int j = 0; j + 1 < n_keys; ++j) {
+                const int k0 = std::min(j * H, P - 1), k1 = std::min((j + 1) * H, P - 1);
+                if (k1 - k0 < 2) continue;
+                long double pa[3], pb[3];
+                at(k0, pa); at(k1, pb);
+                const GuardEval e0 = guard_eval(in, g, k0, pa, vel, o_fd), e1 = guard_eval(in, g, k1, pb, vel, o_fd);
+                const long double t0 = g->t_pulse_s[k0], h = (long double)g->t_pulse_s[k1] - t0;
+                if (!(h > 0)) return false;
+                auto pat = [&](long double a, long double b) { return sincl_pi(a) * sincl_pi(b); };
+                const long double P0 = e0.gt * pat(e0.xar, e0.xer), P1 = e1.gt * pat(e1.xar, e1.xer);
+                const long double gtm = pat(0.5L * (e0.xat + e1.xat), 0.5L * (e0.xet + e1.xet));
+                const long double grm = pat(0.5L * (e0.xar + e1.xar), 0.5L * (e0.xer + e1.xer));
+                const long double gom = pat(0.5L * (e0.xao + e1.xao), 0.5L * (e0.xeo + e1.xeo));
+                const long double Pm = gtm * grm, bq = o_fd > 0 ? gtm * (gom - grm) / o_fd : 0.0L;
+                for (int p = k0 + 1; p < k1; ++p) {
+                    long double pp[3];
+                    at(p, pp);
+                    const GuardEval ex = guard_eval(in, g, p, pp, vel, o_fd);
+                    const long double s = ((long double)g->t_pulse_s[p] - t0) / h, s2 = s * s, s3 = s2 * s;
+                    const long double Rh = (2 * s3 - 3 * s2 + 1) * e0.R + (s3 - 2 * s2 + s) * h * e0.Rd +
+                                           (-2 * s3 + 3 * s2) * e1.R + (s3 - s2) * h * e1.Rd;
+                    if (!(fabsl(Rh - ex.R) <= 2e-8L)) return false;
+                    const long double Pq = P0 + s * ((-3 * P0 + 4 * Pm - P1) + s * (2 * P0 - 4 * Pm + 2 * P1));
+                    for (int c = 0; c < C; ++c) {
+                        const long double dl = e0.dl[c] + s * (e1.dl[c] - e0.dl[c]);
+                        if (!(fabsl(dl - ex.dl[c]) <= 2e-8L)) return false;
+                        const long double gq = Pq + (long double)in->channel_offset_m[c] * bq;
+                        if (!(fabsl(gq - ex.gt * ex.gr[c]) <= 3e-6L)) return false;
+                    }
+                }
+            }
+        }
+    return true;
+}
+
 }  // namespace
 
 extern "C" {
@@ -291,6 +397,7 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     }
     if (opts && (opts->accumulate_mode < 0 || opts->accumulate_mode > 2)) return SIM_EINVAL;
     if (opts && (opts->kinematics_keyframe < 0 || opts->kinematics_keyframe > 4096)) return SIM_EINVAL;
+    if (opts && (opts->geometry_keyframe < 0 || opts->geometry_keyframe > 1)) return SIM_EINVAL;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
         cudaGetLastError();
@@ -377,6 +484,19 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
         prm.series_channels = (r_min > 0 && o_max <= 1e-4 * r_min) ? 1 : 0;
     }
     h->key_H = choose_keyframe_spacing(g, sc, opts ? opts->kinematics_keyframe : 0);
+    if (h->spectral && h->key_H > 1 && prm.series_channels && C <= kMaxKeyChannels &&
+        !(opts && opts->geometry_keyframe == 1)) {
+        // keyframed geometry: the spacing the wave bound admits, halved until the geometry bounds hold too
+        // (a forced spacing is tried as it is)
+        const bool forced = opts && opts->kinematics_keyframe > 1;
+        for (int H = h->key_H; H > 1; H = forced ? 1 : H / 2) {
+            if (H + 1 <= kMaxKeyPulses && moments_keyframed_smem_bytes(prm, h->span_cap_m) <= 200 * 1024 &&
+                geometry_keyframes_ok(in, g, sc, H)) {
+                h->key_H = H; h->geo_keyframed = true;
+                break;
+            }
+        }
+    }
     // ---- batch size ----
     const int64_t fcap = (int64_t)prm.n_tiles * prm.tile_cap;
     const int64_t surf_row = h->n_facets * 8 + (h->need_slope ? h->n_facets * 8 : 0) +
@@ -435,6 +555,7 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
             pc.rx_ref[k] = g->rx_pos_m[3 * p + k];
             for (int c = 0; c < C; ++c) pc.rx_pos[c][k] = g->rx_pos_m[3 * p + k] + in->channel_offset_m[c] * v[k] / vn;
             pc.rx_vhat[k] = v[k] / vn;
+            pc.tx_vel[k] = g->tx_vel_mps[3 * p + k]; pc.rx_vel[k] = v[k];
             pc.rx_va += pc.rx_vhat[k] * pc.rx_a[k];
             pc.rx_ve += pc.rx_vhat[k] * pc.rx_e[k];
         }
@@ -557,6 +678,7 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     h->stats.accumulate_mode = h->spectral ? SIM_ACCUMULATE_SPECTRAL : SIM_ACCUMULATE_DIRECT;
     h->stats.fft_size = h->spectral ? nfft : 0;
     h->stats.kinematics_keyframe = h->key_H;
+    h->stats.geometry_keyframed = h->geo_keyframed ? 1 : 0;
     *out = h;
     return SIM_OK;
 }
@@ -590,7 +712,8 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         ma.sigma0 = h->sigma0.p; ma.current = h->current.p; ma.xi_polar = h->xi_polar.p;
         ma.mom = h->mom.p; ma.nb_pad = h->nb_pad; ma.span_cap = h->span_cap_m; ma.replica = h->replica;
         ma.counters = h->counters.p;
-        CK(h, launch_moments(prm, ma, p0, n_pl, s));
+        if (h->geo_keyframed) CK(h, launch_moments_keyframed(prm, ma, p0, n_pl, s));
+        else CK(h, launch_moments(prm, ma, p0, n_pl, s));
         CK(h, mark());
         FftConvArgs fa{};
         fa.mom = h->mom.p; fa.cspec = h->cspec.p; fa.tw = h->tw.p; fa.carrier_p = h->carrier_p.p;

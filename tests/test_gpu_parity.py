@@ -111,6 +111,53 @@ def test_kinematics_keyframes(mode):
     assert np.max(np.abs(g["pos"] - o["pos"])) < 3e-9              # interpolated height against the exact one
 
 
+def test_geometry_keyframes_on_and_off():
+    """Spectral path: ranges / gains interpolated between the kinematics keyframes (moments_keyframed.cu, the
+    default where sim_create's host guard admits it) against exact geometry at every pulse (moments.cu); both
+    against the oracle.  Covers tilt modulation, the CWM displacement, a current map, 3 channels, a ragged grid,
+    batches starting inside an interval, forced and automatic spacing, and a scene that culls."""
+    w = _hetero_small(96, 64, 11)
+    w.scene["choppy"] = 1
+    ref = oracle_generate(w)
+    for H, batch, gk in ((4, 0, 0), (4, 3, 0), (10, 5, 0), (0, 0, 0), (4, 0, 1)):
+        with _sim(w, accumulate_mode="spectral", kinematics_keyframe=H, pulses_per_batch=batch,
+                  geometry_keyframe=gk) as sim:
+            got = sim.generate().cpu().numpy()
+            st = sim.stats()
+            part = sim.generate(5, 9).cpu().numpy()
+        assert st["geometry_keyframed"] == (0 if gk else 1), (H, batch, gk, st)
+        _assert_parity(got, ref, f"geometry keyframes H={H} batch={batch} off={gk}")
+        _assert_parity(part, ref[:, 5:9], f"geometry keyframes H={H} range")
+    # a culling, window-clipping scene (wide patch): kept counts of the two kernels agree, both match the oracle
+    wc = make_workload("tiny", n_pulses=12)
+    wc.scene["spacing_m"] = 220.0
+    refc = oracle_generate(wc)
+    kept = []
+    for gk in (0, 1):
+        with _sim(wc, accumulate_mode="spectral", geometry_keyframe=gk) as sim:
+            got = sim.generate().cpu().numpy()
+            st = sim.stats()
+        assert st["geometry_keyframed"] == 1 - gk
+        kept.append(st["facet_echoes_kept"])
+        _assert_parity(got, refc, f"culling scene off={gk}")
+    expect_kept = sum(int(oracle_facets(wc, p)["keep"].sum()) for p in range(12))
+    assert 0 < expect_kept < wc.n_facets * 12
+    assert abs(kept[0] - expect_kept) <= 4 and abs(kept[1] - expect_kept) <= 4
+
+
+def test_geometry_keyframes_guard_rejects_rough_state_vectors():
+    """Per-pulse platform positions that are not smooth in time (10 cm jitter): the host guard must refuse the
+    interpolated geometry, and the exact per-pulse kernel must still match the oracle."""
+    w = make_workload("tiny", n_pulses=16)
+    rng = np.random.default_rng(5)
+    w.geometry["tx_pos_m"] = w.geometry["tx_pos_m"] + 0.1 * rng.standard_normal(w.geometry["tx_pos_m"].shape)
+    ref = oracle_generate(w)
+    with _sim(w, accumulate_mode="spectral") as sim:
+        got = sim.generate().cpu().numpy()
+        assert sim.stats()["geometry_keyframed"] == 0
+    _assert_parity(got, ref, "jittered state vectors")
+
+
 # ----------------------------------------------------------------------------- per-kernel unit parity (T1)
 
 @pytest.mark.parametrize("name", ["tiny", "hetero_small"])
