@@ -106,7 +106,7 @@ cudaError_t launch_moments(const DevParams &prm, const MomentArgs &a, int p0, in
 // interpolated between (moments_keyframed.cu).  Needs surf.H in [2, kMaxKeyPulses - 1], C <= kMaxKeyChannels,
 // series_channels; sim_create verifies the interpolation bounds on the host before choosing it.
 constexpr int kMaxKeyChannels = 4;
-constexpr int kMaxKeyPulses = 130;
+constexpr int kMaxKeyPulses = 66;
 size_t moments_keyframed_smem_bytes(const DevParams &prm, int span_cap);
 cudaError_t launch_moments_keyframed(const DevParams &prm, const MomentArgs &a, int p0, int n_pl, cudaStream_t s);
 

@@ -82,6 +82,32 @@ __device__ __forceinline__ KeyEval<C> key_eval(const DevParams &prm, const Pulse
     return o;
 }
 
+constexpr int kScrRow = 9;                // float2 per thread row of the transposition scratch (8 moments + 1 pad)
+constexpr int kScrTeam = 8 * kScrRow;     // float2 per 8-thread team
+__host__ __device__ constexpr int hist_words(int C, int span) { return (2 * C * (span + 1) + 1) & ~1; }
+
+// Packed f32x2 arithmetic on 64-bit registers (FFMA2 / FADD2): the operands stay register pairs from the
+// shared-memory load to the transposition store, no pack / unpack moves in the moment loop.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk(float x, float y)
+{
+    f32x2 d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(x), "f"(y));
+    return d;
+}
+__device__ __forceinline__ f32x2 ffma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
 __device__ __forceinline__ float pattern_x(float xa, float xe) { return sinc_pi_fast(xa) * sinc_pi_fast(xe); }
 
 template <int FPT, int C, bool kTilt>
@@ -94,6 +120,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     __shared__ double s_rc[2][kMaxKeyChannels];          // path length of the tile centre at the two keyframes
     __shared__ unsigned long long s_samples;
     __shared__ int s_kept;
+    __shared__ int s_rng[kMaxKeyChannels][2];
 
     const int span = a.span_cap, hstride = span + 1;
     const int cap = prm.tile_cap;
@@ -102,6 +129,8 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     float *payload_y = reinterpret_cast<float *>(smem_raw + (size_t)2 * C * cap * 8);
     unsigned short *idx = reinterpret_cast<unsigned short *>(smem_raw + (size_t)2 * C * cap * 12);
     int *hist = reinterpret_cast<int *>(smem_raw + (size_t)2 * C * cap * 14);
+    // [kThreads / 8][kScrTeam] float2 transposition scratch of stage C (8-byte aligned: hist is padded)
+    float2 *scratch = reinterpret_cast<float2 *>(smem_raw + (size_t)2 * C * cap * 14 + (size_t)hist_words(C, span) * 4);
 
     const int tile = blockIdx.x, j = j_first + blockIdx.y;
     const int tid = threadIdx.x, lane = tid & 31;
@@ -241,13 +270,18 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     }
     __syncthreads();                                     // s_kp complete
 
-    const float kappa_f = (float)prm.kappa;
+    // phase of a facet-echo in 2^-32 turns: -dR/lambda + kappa eps^2 (+ speckle argument, + 1/2 if the gain is negative)
+    const double il32 = prm.inv_lambda * 4294967296.0;
+    const float kappa32 = (float)(prm.kappa * 4294967296.0);
     const int L = a.replica;
+    const unsigned win_hi = (unsigned)(prm.n_samples + L - 1);
     float och[C];
 #pragma unroll
     for (int c = 0; c < C; ++c) och[c] = (float)pc2[0].ch_off[c];
     unsigned long long my_samples = 0;
     int my_kept = 0;
+    const int sub = tid & 7, team = tid >> 3, warp = tid >> 5;
+    float2 *scr = scratch + team * kScrTeam;
 
     for (int ip = 0; ip < hi - lo; ++ip) {
         const int buf = ip & 1;
@@ -258,18 +292,16 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         unsigned short *ix = idx + (size_t)buf * C * cap;
         int *hs = hist + buf * C * hstride;
         const float s = kp.s;
-        unsigned pulse_samples = 0;
 
-        // ---- A: slice, sub-slice position, complex weight of every facet-echo; rank inside the slice ----
+        // ---- A: slice, sub-slice position, complex weight of every facet-echo; rank inside the slice.
+        //      Straight-line code for all FPT x C echoes of the thread (predicated stores), so that the
+        //      independent chains interleave; only the rare out-of-window echo branches.
         int pr[FPT][C];                                  // (slice << 12 | rank) or -1
 #pragma unroll
         for (int q = 0; q < FPT; ++q) {
-#pragma unroll
-            for (int c = 0; c < C; ++c) pr[q][c] = -1;
-            if (!valid[q]) continue;
             const float Pv = fmaf(s, fmaf(s, pqb[q], pqa[q]), pq0[q]);
-            if (fabsf(Pv) < prm.cull_thr) continue;                        // O7 (G6)
-            ++my_kept;
+            const bool keep = valid[q] && !(fabsf(Pv) < prm.cull_thr);     // O7 (G6)
+            my_kept += keep ? 1 : 0;
             const float am = kTilt ? fmaf(s, fmaf(s, amb[q], ama[q]), am0[q]) : am0[q];
             const double R = fma(kp.w00, R0[q], fma(kp.w10, R0d[q], fma(kp.w01, R1[q], kp.w11 * R1d[q])));
             const double dRref = R - kp.r0;
@@ -279,24 +311,26 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                 const float dl = fmaf(s, ddl[q][c], dl0[q][c]);
                 const double dR = dRref + (double)dl;
                 const double nu = fma(dR, prm.fs_over_c0, -prm.half_len);
-                const double bd = ceil(nu);
-                if (!(bd > -(double)L && bd < (double)prm.n_samples)) continue;    // window misses [0, Ns)
-                const int b = (int)bd;
-                const float eps = (float)(bd - nu);                               // [0, 1)
+                const int b = __double2int_ru(nu);                                // ceil, saturating
+                const bool inwin = keep && ((unsigned)b + (unsigned)(L - 1) < win_hi);   // window meets [0, Ns)
+                const float eps = (float)((double)b - nu);                        // [0, 1)
                 const float g = fmaf(och[c], bq[q], Pv);
-                const uint32_t ph = turns_to_u32_fast(fma(-dR, prm.inv_lambda, (double)(kappa_f * eps * eps))) +
+                const uint32_t ph = (uint32_t)(unsigned long long)__double2ll_rn(
+                                        fma(-dR, il32, (double)(kappa32 * eps * eps))) +
                                     xarg[q] + ((g < 0.f) ? 0x80000000u : 0u);
                 float sn, cs;
                 __sincosf((float)(int32_t)ph * 1.4629180792671596e-9f, &sn, &cs);   // 2 pi / 2^32
                 const float mag = fabsf(g) * am;
                 const float yv = fmaf(2.f, eps, -1.f);
-                pulse_samples += (unsigned)(min(b + L, prm.n_samples) - max(b, 0));
                 const int rel = b - kp.base[c];
-                if (rel >= 0 && rel < span) {
+                const bool inspan = (unsigned)rel < (unsigned)span;
+                pr[q][c] = -1;
+                if (inwin && inspan) {
                     pay[c * cap + k] = make_float2(mag * cs, mag * sn);
                     pay_y[c * cap + k] = yv;
                     pr[q][c] = (rel << 12) | atomicAdd(&hs[c * hstride + rel + 1], 1);
-                } else {                                                   // outside the tile window: rare
+                }
+                if (inwin && !inspan) {                                    // outside the tile window: rare
                     const float br = mag * cs, bi = mag * sn;
                     float2 *row = a.mom + ((size_t)(c * n_pl + pl) * kKt) * a.nb_pad + (b + L - 1);
                     float t0 = 1.f, t1 = yv;
@@ -307,19 +341,20 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                         atomicAdd(row + (size_t)kk * a.nb_pad, make_float2(br * t2, bi * t2));
                         t0 = t1; t1 = t2;
                     }
+                    my_samples += (unsigned)(min(b + L, prm.n_samples) - max(b, 0));
                 }
             }
         }
-        my_samples += pulse_samples;
         __syncthreads();
 
         // ---- B: exclusive scan of each channel's histogram (one warp per channel), then the index list ----
-        if ((tid >> 5) < C) {
-            int *hc = hs + (tid >> 5) * hstride;
-            int carry = 0;
+        if (warp < C) {
+            int *hc = hs + warp * hstride;
+            int carry = 0, smin = span, smax = 0;
             for (int k0s = 1; k0s <= span; k0s += 32) {
                 const int k = k0s + lane;
                 int v = (k <= span) ? hc[k] : 0;
+                if (v > 0) { smin = min(smin, k - 1); smax = max(smax, k); }
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
                     const int t = __shfl_up_sync(0xffffffffu, v, o);
@@ -328,6 +363,9 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                 if (k <= span) hc[k] = v + carry;
                 carry += __shfl_sync(0xffffffffu, v, 31);
             }
+            smin = __reduce_min_sync(0xffffffffu, smin);
+            smax = __reduce_max_sync(0xffffffffu, smax);
+            if (lane == 0) { s_rng[warp][0] = smin; s_rng[warp][1] = smax; }     // occupied slices [smin, smax)
         }
         __syncthreads();                                 // hs[c][s] = first sorted position of slice s
 #pragma unroll
@@ -343,66 +381,62 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         }
         __syncthreads();
 
-        // ---- C: 8 threads per slice: Chebyshev moments, reduce-scatter, one RED per (slice, k) ----
-        const int sub = tid & 7;
-        for (int s0 = 0; s0 < C * span; s0 += kThreads / 8) {
-            const int sl = s0 + (tid >> 3);
-            int c = 0, sidx = 0, first = 0, cnt = 0;
-            if (sl < C * span) {
-                c = sl / span; sidx = sl - c * span;
-                first = hs[c * hstride + sidx]; cnt = hs[c * hstride + sidx + 1] - first;
-            }
-            if (__ballot_sync(0xffffffffu, cnt > 0) == 0u) continue;       // warp-uniform
-            float2 m[kKt];
-#pragma unroll
-            for (int k = 0; k < kKt; ++k) m[k] = make_float2(0.f, 0.f);
-            const unsigned short *ixc = ix + c * cap + first;
+        // ---- C: 8 threads per slice: Chebyshev moments, transpose through shared memory, one RED per (slice, k).
+        //      The recurrence runs on a_k = sigma_k T_k, sigma = + + - - + + - -, which needs no negation:
+        //      a_{k+1} = -+ 2y a_k + a_{k-1} (minus for odd k); sigma_k is applied to the slice sum.
+#pragma unroll 1
+        for (int c = 0; c < C; ++c) {
+            const int smin = s_rng[c][0], smax = s_rng[c][1];
+            const int *hc = hs + c * hstride;
+            const unsigned short *ixc0 = ix + c * cap;
             const float2 *payc = pay + c * cap;
             const float *payc_y = pay_y + c * cap;
-            for (int i = sub; i < cnt; i += 8) {
-                const int src = ixc[i];
-                const float2 w = payc[src];
-                const float yv = payc_y[src];
-                const float2 y2 = make_float2(yv + yv, yv + yv);
-                float2 t0 = make_float2(1.f, 1.f), t1 = make_float2(yv, yv);
-                m[0] = __fadd2_rn(m[0], w);
-                m[1] = __ffma2_rn(w, t1, m[1]);
+            for (int s0 = smin; s0 < smax; s0 += kThreads / 8) {
+                if (s0 + warp * 4 >= smax) continue;                       // warp-uniform
+                const int sidx = s0 + team;
+                int first = 0, cnt = 0;
+                if (sidx < smax) { first = hc[sidx]; cnt = hc[sidx + 1] - first; }
+                f32x2 m[kKt];
 #pragma unroll
-                for (int k = 2; k < kKt; ++k) {
-                    const float2 t2 = __ffma2_rn(y2, t1, make_float2(-t0.x, -t0.y));
-                    m[k] = __ffma2_rn(w, t2, m[k]);
-                    t0 = t1; t1 = t2;
-                }
-            }
-            // reduce-scatter over the 8 threads of the slice: thread `sub` ends with moment k = sub
-            float2 h4[4], h2[2], h1;
-            {
-                const bool hi4 = sub & 4;
+                for (int k = 0; k < kKt; ++k) m[k] = 0ull;
+                const unsigned short *ixc = ixc0 + first;
+                auto add = [&](int src) {
+                    const f32x2 w = *reinterpret_cast<const f32x2 *>(payc + src);
+                    const float yv = payc_y[src];
+                    const f32x2 y2 = pk(yv + yv, yv + yv), ny2 = pk(-(yv + yv), -(yv + yv));
+                    f32x2 t0 = pk(1.f, 1.f), t1 = pk(yv, yv);
+                    m[0] = fadd2(m[0], w);
+                    m[1] = ffma2(w, t1, m[1]);
 #pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const float2 send = hi4 ? m[k] : m[k + 4], kp2 = hi4 ? m[k + 4] : m[k];
-                    h4[k].x = kp2.x + __shfl_xor_sync(0xffffffffu, send.x, 4);
-                    h4[k].y = kp2.y + __shfl_xor_sync(0xffffffffu, send.y, 4);
+                    for (int k = 2; k < kKt; ++k) {
+                        const f32x2 t2 = ffma2((k & 1) ? y2 : ny2, t1, t0);
+                        m[k] = ffma2(w, t2, m[k]);
+                        t0 = t1; t1 = t2;
+                    }
+                };
+                int i = sub;
+                for (; i + 8 < cnt; i += 16) {
+                    const int sa = ixc[i], sb = ixc[i + 8];
+                    add(sa); add(sb);
                 }
-            }
-            {
-                const bool hi2 = sub & 2;
+                if (i < cnt) add(ixc[i]);
+                // transpose: thread `sub` of the team ends with the team's sum of moment k = sub
+                f32x2 *scr64 = reinterpret_cast<f32x2 *>(scr);
 #pragma unroll
-                for (int k = 0; k < 2; ++k) {
-                    const float2 send = hi2 ? h4[k] : h4[k + 2], kp2 = hi2 ? h4[k + 2] : h4[k];
-                    h2[k].x = kp2.x + __shfl_xor_sync(0xffffffffu, send.x, 2);
-                    h2[k].y = kp2.y + __shfl_xor_sync(0xffffffffu, send.y, 2);
+                for (int k = 0; k < kKt; ++k) scr64[sub * kScrRow + k] = m[k];
+                __syncwarp();
+                f32x2 hsum = scr64[sub];
+#pragma unroll
+                for (int r = 1; r < 8; ++r) hsum = fadd2(hsum, scr64[r * kScrRow + sub]);
+                __syncwarp();
+                float2 h1 = *reinterpret_cast<float2 *>(&hsum);
+                if (cnt > 0) {
+                    if (sub & 2) { h1.x = -h1.x; h1.y = -h1.y; }
+                    const int b = kp.base[c] + sidx;
+                    float2 *row = a.mom + ((size_t)(c * n_pl + pl) * kKt + sub) * a.nb_pad;
+                    atomicAdd(row + (b + L - 1), h1);
+                    if (sub == 0) my_samples += (unsigned long long)cnt * (unsigned)(min(b + L, prm.n_samples) - max(b, 0));
                 }
-            }
-            {
-                const bool hi1 = sub & 1;
-                const float2 send = hi1 ? h2[0] : h2[1], kp2 = hi1 ? h2[1] : h2[0];
-                h1.x = kp2.x + __shfl_xor_sync(0xffffffffu, send.x, 1);
-                h1.y = kp2.y + __shfl_xor_sync(0xffffffffu, send.y, 1);
-            }
-            if (cnt > 0) {
-                float2 *row = a.mom + ((size_t)(c * n_pl + pl) * kKt + sub) * a.nb_pad;
-                atomicAdd(row + (kp.base[c] + sidx + L - 1), h1);
             }
         }
         // no barrier here: the next pulse writes the other payload / index / histogram buffers, and this
@@ -432,10 +466,9 @@ cudaError_t launch_fc(const DevParams &prm, const MomentArgs &a, int p0, int n_p
 {
     dim3 grid(prm.n_tiles, n_int);
     auto go = [&](auto kern) -> cudaError_t {
-        if (smem > 48 * 1024) {
-            cudaError_t rc = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (rc != cudaSuccess) return rc;
-        }
+        // always opt in: static + dynamic shared memory together may pass 48 KB even when the dynamic part does not
+        cudaError_t rc = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (rc != cudaSuccess) return rc;
         kern<<<grid, kThreads, smem, s>>>(prm, a, p0, n_pl, j_first);
         return cudaGetLastError();
     };
@@ -460,7 +493,8 @@ cudaError_t launch_f(const DevParams &prm, const MomentArgs &a, int p0, int n_pl
 size_t moments_keyframed_smem_bytes(const DevParams &prm, int span_cap)
 {
     const size_t C = prm.n_channels;
-    return (size_t)2 * C * prm.tile_cap * 14 + (size_t)2 * C * (span_cap + 1) * 4;
+    return (size_t)2 * C * prm.tile_cap * 14 + (size_t)hist_words((int)C, span_cap) * 4 +
+           (size_t)(kThreads / 8) * kScrTeam * sizeof(float2);
 }
 
 cudaError_t launch_moments_keyframed(const DevParams &prm, const MomentArgs &a, int p0, int n_pl, cudaStream_t s)
