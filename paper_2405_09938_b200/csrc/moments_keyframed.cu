@@ -9,7 +9,8 @@
 //            time derivatives at the two keyframes,  dR/dt = u_t.(v_f - V_tx) + u_r.(v_f - V_rx)  with the facet
 //            velocity v_f = (current + dD_h/dt, dz/dt) from K1's rate rows.  Error <= h^4 max|R''''| / 384:
 //            platform term 3 V^4/r^3 ~ 0.02 m/s^4 -> 4e-13 m at h = 9.4 ms; wave term = K1's own bound (1e-9 m).
-//   d_c(t) = r_r,c - r_r,ref  (receive phase centre c, |o_c| <= 1e-4 r): linear in t, fp32 (|d_c| < 1 m).
+//   d_c(t) = r_r,c - r_r,ref  (receive phase centre c, |o_c| <= 1e-4 r) = o_c a(t) + o_c^2 b, a = -(d.v^)/r linear
+//            in t, b = (1 - a^2)/(2 r); fp32 (|d_c| < 1 m).
 //   P(t)   = G_t G_r,ref      quadratic through t0, t_mid, t1 with the sinc arguments at t_mid taken as the mean of
 //            the end values (they are linear in t to ~1e-7); G_r,c = G_r,ref + o_c dG/do with dG/do by one
 //            finite difference at t_mid.  |a_f|(t) (tilt modulation) quadratic the same way.
@@ -19,11 +20,11 @@
 // geometry_keyframes_ok): non-smooth state vectors never reach this kernel.
 //
 // One CTA = one spatial tile x one keyframe interval.  A thread owns FPT facets, holds their interpolants in
-// registers (15 + 2C words per facet) and loops over the interval's pulses; per pulse and for all C channels at
+// registers (18 words per facet) and loops over the interval's pulses; per pulse and for all C channels at
 // once: slice, sub-slice position and complex weight of every facet-echo -> counting sort by slice through a
 // shared-memory histogram (integer ATOMS) and an index list -> 8 threads per slice sum the Kt Chebyshev
 // moments (packed FFMA2), reduce-scatter by shuffles, one RED.ADD.F32x2 per (slice, k).  Histogram, payload
-// and index list are double-buffered: three barriers per pulse.
+// are double-buffered: three barriers per pulse.
 //
 // Bound: issue slots (FP32 + FP64 mix); HBM/L2: four surface rows per facet and INTERVAL, the maps once.
 #include "kernels.cuh"
@@ -38,7 +39,8 @@ constexpr int kKt = kMomentOrder;
 static_assert(kKt == 8, "the reduce-scatter below is written for 8 moments / 8 threads per slice");
 
 struct __align__(16) KeyPulse {          // per pulse of the interval (shared memory)
-    double w00, w10, w01, w11;           // Hermite weights (surface.cuh)
+    double sd;                           // (t - t0) / h
+    float u0, u1;                        // s (1-s)^2, -s^2 (1-s): weights of the Hermite cubic's bend (see R below)
     double r0;                           // c0 t0[p]
     float s, pad0;                       // (t - t0) / h
     int32_t base[kMaxKeyChannels];       // first slice of the tile's shared-memory window, per channel
@@ -50,7 +52,7 @@ struct KeyEval {
     double R, Rd;                        // path to the un-offset phase centre and its time derivative
     float xat, xet, xar, xer;            // sinc arguments: Tx azimuth / elevation, Rx (un-offset) azimuth / elevation
     float xao, xeo;                      // Rx arguments at the finite-difference offset o_fd
-    float dl[C];                         // r_r,c - r_r,ref
+    float la, lb;                        // r_r,c - r_r,ref = o_c la + o_c^2 lb  (series in o_c / r)
 };
 
 template <int C>
@@ -72,13 +74,11 @@ __device__ __forceinline__ KeyEval<C> key_eval(const DevParams &prm, const Pulse
         channel_leg_series(lr, dv, o_fd, pc.rx_va, pc.rx_ve, r_c, inv_c, da_c, de_c);
         o.xao = (float)(prm.ap_rx_a * (da_c * inv_c)); o.xeo = (float)(prm.ap_rx_e * (de_c * inv_c));
     }
-#pragma unroll
-    for (int c = 0; c < C; ++c) {
-        // r_c - r = r (dl/2 - dl^2/8 + dl^3/16), dl = (o^2 - 2 o d.v^)/r^2   (geometry_common.cuh)
-        const double oc = pc.ch_off[c];
-        const double dl = fma(oc, oc, -2.0 * oc * dv) * lr.inv * lr.inv;
-        o.dl[c] = (float)(lr.r * (dl * fma(dl, fma(dl, 0.0625, -0.125), 0.5)));
-    }
+    // r_c - r = r (dl/2 - dl^2/8 + ...), dl = (o^2 - 2 o d.v^)/r^2  (geometry_common.cuh)
+    //         = -o (d.v^)/r + o^2 (1 - (d.v^/r)^2)/(2 r) + O(o^3/r^2)
+    const double cv = dv * lr.inv;
+    o.la = (float)(-cv);
+    o.lb = (float)(0.5 * lr.inv * fma(-cv, cv, 1.0));
     return o;
 }
 
@@ -124,12 +124,12 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
 
     const int span = a.span_cap, hstride = span + 1;
     const int cap = prm.tile_cap;
-    // [2][C][cap] float2 weight | [2][C][cap] float y | [2][C][cap] u16 index list | [2][C][span + 1] int histogram
+    // [2][C][cap] float2 weight | [2][C][cap] float y | [2][C][cap] u16 index list | [2][C][span + 1] int histogram |
+    // [kThreads / 8][kScrTeam] float2 transposition scratch of stage C (8-byte aligned: hist is padded)
     float2 *payload = reinterpret_cast<float2 *>(smem_raw);
     float *payload_y = reinterpret_cast<float *>(smem_raw + (size_t)2 * C * cap * 8);
     unsigned short *idx = reinterpret_cast<unsigned short *>(smem_raw + (size_t)2 * C * cap * 12);
     int *hist = reinterpret_cast<int *>(smem_raw + (size_t)2 * C * cap * 14);
-    // [kThreads / 8][kScrTeam] float2 transposition scratch of stage C (8-byte aligned: hist is padded)
     float2 *scratch = reinterpret_cast<float2 *>(smem_raw + (size_t)2 * C * cap * 14 + (size_t)hist_words(C, span) * 4);
 
     const int tile = blockIdx.x, j = j_first + blockIdx.y;
@@ -171,10 +171,9 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         const double s = (h != 0.0) ? (t - t0) / h : 0.0;
         const double s2 = s * s, s3 = s2 * s;
         KeyPulse kp;
-        kp.w00 = 2.0 * s3 - 3.0 * s2 + 1.0;
-        kp.w10 = (s3 - 2.0 * s2 + s) * h;
-        kp.w01 = -2.0 * s3 + 3.0 * s2;
-        kp.w11 = (s3 - s2) * h;
+        kp.sd = s;
+        kp.u0 = (float)(s3 - 2.0 * s2 + s);
+        kp.u1 = (float)(s3 - s2);
         kp.r0 = a.pulses[p].r0;
         kp.s = (float)s; kp.pad0 = 0.f;
 #pragma unroll
@@ -200,8 +199,13 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     for (int c = 0; c < C; ++c) o_fd = fmax(o_fd, fabs(pc2[0].ch_off[c]));
     const float inv_ofd = (o_fd > 0.0) ? (float)(1.0 / o_fd) : 0.f;
 
-    double R0[FPT], R0d[FPT], R1[FPT], R1d[FPT];
-    float dl0[FPT][C], ddl[FPT][C];
+    // Hermite cubic of the path length as chord + bend:  R(s) = R0 + s D + u0(s) ra + u1(s) rb,  D = R1 - R0,
+    // ra = h R0' - D, rb = h R1' - D.  The bend is millimetres (h^2 R''/8), so ra, rb are fp32.
+    double R0[FPT], RD[FPT];
+    float ra[FPT], rb[FPT];
+    float la0[FPT], dla[FPT];                            // r_r,c - r_r,ref = o_c (la0 + s dla) + o_c^2 lb
+    float lb_sum = 0.f;                                  // lb varies by 1e-4 relative over a tile: one value per thread
+    int lb_n = 0;
     float pq0[FPT], pqa[FPT], pqb[FPT], bq[FPT];         // P(s) = pq0 + s (pqa + s pqb); bq = G_t dG_r/do
     float am0[FPT], ama[FPT], amb[FPT];                  // |a_f|(s), quadratic when tilt-modulated
     uint32_t xarg[FPT];
@@ -212,10 +216,9 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         const int li = k & (ts - 1), lj = k >> lts;
         const int i = ti0 + li, jj = tj0 + lj;
         valid[q] = (k < ts * ts && i < prm.nx && jj < prm.ny);
-        R0[q] = R0d[q] = R1[q] = R1d[q] = 0.0;
+        R0[q] = RD[q] = 0.0; ra[q] = rb[q] = 0.f;
         pq0[q] = pqa[q] = pqb[q] = bq[q] = 0.f; am0[q] = ama[q] = amb[q] = 0.f; xarg[q] = 0u;
-#pragma unroll
-        for (int c = 0; c < C; ++c) { dl0[q][c] = 0.f; ddl[q][c] = 0.f; }
+        la0[q] = dla[q] = 0.f;
         if (!valid[q]) continue;
         const size_t f = (size_t)jj * prm.nx + i;
         const double xb = prm.cx + ((double)i - 0.5 * (prm.nx - 1)) * prm.spacing;
@@ -235,9 +238,13 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
             }
             ev[e] = key_eval<C>(prm, pc, pos, vel, o_fd);
         }
-        R0[q] = ev[0].R; R0d[q] = ev[0].Rd; R1[q] = ev[1].R; R1d[q] = ev[1].Rd;
-#pragma unroll
-        for (int c = 0; c < C; ++c) { dl0[q][c] = ev[0].dl[c]; ddl[q][c] = ev[1].dl[c] - ev[0].dl[c]; }
+        {
+            const double hh = pc2[1].t - pc2[0].t, D = ev[1].R - ev[0].R;
+            R0[q] = ev[0].R; RD[q] = D;
+            ra[q] = (float)fma(hh, ev[0].Rd, -D); rb[q] = (float)fma(hh, ev[1].Rd, -D);
+        }
+        la0[q] = ev[0].la; dla[q] = ev[1].la - ev[0].la;
+        lb_sum += 0.5f * (ev[0].lb + ev[1].lb); ++lb_n;
         // gains at s = 0, 1/2, 1 (sinc arguments at the midpoint = mean of the end values)
         const float gt0 = pattern_x(ev[0].xat, ev[0].xet), gr0 = pattern_x(ev[0].xar, ev[0].xer);
         const float gt1 = pattern_x(ev[1].xat, ev[1].xet), gr1 = pattern_x(ev[1].xar, ev[1].xer);
@@ -278,6 +285,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     float och[C];
 #pragma unroll
     for (int c = 0; c < C; ++c) och[c] = (float)pc2[0].ch_off[c];
+    const float lbt = lb_n ? lb_sum / (float)lb_n : 0.f;
     unsigned long long my_samples = 0;
     int my_kept = 0;
     const int sub = tid & 7, team = tid >> 3, warp = tid >> 5;
@@ -303,12 +311,13 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
             const bool keep = valid[q] && !(fabsf(Pv) < prm.cull_thr);     // O7 (G6)
             my_kept += keep ? 1 : 0;
             const float am = kTilt ? fmaf(s, fmaf(s, amb[q], ama[q]), am0[q]) : am0[q];
-            const double R = fma(kp.w00, R0[q], fma(kp.w10, R0d[q], fma(kp.w01, R1[q], kp.w11 * R1d[q])));
+            const double R = fma(kp.sd, RD[q], R0[q]) + (double)fmaf(kp.u0, ra[q], kp.u1 * rb[q]);
             const double dRref = R - kp.r0;
+            const float la = fmaf(s, dla[q], la0[q]);
             const int k = q * kThreads + tid;
 #pragma unroll
             for (int c = 0; c < C; ++c) {
-                const float dl = fmaf(s, ddl[q][c], dl0[q][c]);
+                const float dl = och[c] * fmaf(och[c], lbt, la);
                 const double dR = dRref + (double)dl;
                 const double nu = fma(dR, prm.fs_over_c0, -prm.half_len);
                 const int b = __double2int_ru(nu);                                // ceil, saturating
