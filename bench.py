@@ -37,11 +37,14 @@ UNIT = "facet-echoes/s"
 # 148 SMs x 128 FP32 lanes.
 K3_FP32_OPS_PER_FACET_SAMPLE = 4.0
 SM_COUNT, FP32_LANES_PER_SM, XU_LANES_PER_SM, FP64_LANES_PER_SM = 148, 128, 16, 64
-# FP64-pipe roofline of K2s: SURVEY.md 8(d) counts ~60 DFMA per facet-antenna (range,
-# direction cosines, window and phase in fp64); a facet-pulse sees Tx + cull reference + C receive antennas.
-K2_DFMA_PER_FACET_ANTENNA = 60.0
-# dram bytes per facet-pulse of a K2s launch from the committed ncu capture (profiles/); None until captured.
-K2S_DRAM_BYTES_PER_FACET_PULSE = None
+# FP32-pipe roofline of the moment kernels: SURVEY.md 8(d) counts 4 Kt FFMA + ~30 setup per
+# facet-echo for the moment form; Kt = 8.
+MOMENT_FP32_OPS_PER_FACET_ECHO = 4.0 * 8 + 30.0
+# From the committed ncu captures (profiles/): executed thread-instructions per facet-echo (context for the
+# roofline fraction: the kernels are issue-bound, not pipe-bound) and dram bytes per facet-echo.
+K2S_EXECUTED_INSTR_PER_FACET_ECHO = 1156.0 / 3      # profiles/r1_v4_k2s_ncu_summary.txt
+K2K_EXECUTED_INSTR_PER_FACET_ECHO = 494.5 / 3       # profiles/r1_v8_k2k_ncu_summary.txt (1.037e9 warp instr / launch)
+K2K_DRAM_BYTES_PER_FACET_ECHO = (96.018e6 + 7.825e6) / (256 * 3 * 262144)   # same capture: dram read + write
 # dram bytes per kept facet-echo of a K3 launch, from the committed `ncu --set full` capture
 # profiles/r1_v3_k3_ncu_summary.txt: (2.580977e9 read + 1.1966e7 written) / (100 pulses x 3 ch x 262144).
 K3_DRAM_BYTES_PER_FACET_ECHO = (2.580977e9 + 1.1966e7) / (100 * 3 * 262144)
@@ -205,22 +208,25 @@ def _roofline_direct(kms, stats, sm_max, pipes):
 
 
 def _roofline_spectral(kms, stats, sm_max, pipes, n_channels):
-    """K2s (moments_kernel) against the FP64 pipe: SURVEY.md 8(d) counts ~60 DFMA per facet-antenna;
-    antennas per facet-pulse = Tx + cull reference + C receive phase centres (DESIGN.md 5/K2s)."""
+    """K2s / K2k (moments kernels) against the FP32 pipe, on the moment form's OWN op count (SURVEY.md 8(d):
+    "4 Kt FFMA + ~30 setup per facet-echo ... must be reported against its own op count"): with Kt = 8 that is
+    62 FP32 lane-operations per nominal facet-echo."""
     n_batches = max(1, stats["kernel_launches"] // 3)
     launch_ms = kms["geometry"] / n_batches
-    facet_pulses = stats["facet_echoes_nominal"] / n_channels / n_batches
-    dfma = facet_pulses * K2_DFMA_PER_FACET_ANTENNA * (2 + n_channels)
-    achieved = dfma / (launch_ms * 1e-3) / 1e9
-    peak = SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6 / 1e9
+    echoes = stats["facet_echoes_nominal"] / n_batches
+    ops = echoes * MOMENT_FP32_OPS_PER_FACET_ECHO
+    achieved = ops / (launch_ms * 1e-3) / 1e9
+    peak = SM_COUNT * FP32_LANES_PER_SM * sm_max * 1e6 / 1e9
+    keyframed = bool(stats.get("geometry_keyframed", 0))
     return {
-        "bound": "alu", "kernel": "moments_kernel (K2s, spectral form)", "achieved": achieved, "peak": peak,
-        "unit": "GDFMA/s", "frac": achieved / peak,
-        "traffic": K2S_DRAM_BYTES_PER_FACET_PULSE * facet_pulses if K2S_DRAM_BYTES_PER_FACET_PULSE else None,
-        "peak_model": f"{SM_COUNT} SM x {FP64_LANES_PER_SM} FP64 lanes x {sm_max:.0f} MHz; algorithmic work "
-                      f"{K2_DFMA_PER_FACET_ANTENNA:.0f} DFMA x (2 + C) antennas per facet-pulse",
-        "measured_pipe_peak": pipes["dfma_per_s"] / 1e9, "frac_of_measured_pipe_peak": achieved / (pipes["dfma_per_s"] / 1e9),
-        "launch_ms": launch_ms, "facet_pulses_per_launch": facet_pulses,
+        "bound": "alu", "kernel": ("moments_keyframed_kernel (K2k" if keyframed else "moments_kernel (K2s") + ", spectral form)",
+        "achieved": achieved, "peak": peak, "unit": "GFP32-lane-op/s", "frac": achieved / peak,
+        "traffic": K2K_DRAM_BYTES_PER_FACET_ECHO * echoes if (keyframed and K2K_DRAM_BYTES_PER_FACET_ECHO) else None,
+        "peak_model": f"{SM_COUNT} SM x {FP32_LANES_PER_SM} FP32 lanes x {sm_max:.0f} MHz; algorithmic work "
+                      f"{MOMENT_FP32_OPS_PER_FACET_ECHO:.0f} FP32 lane-ops per facet-echo (4 Kt + 30, Kt = 8)",
+        "measured_pipe_peak": pipes["ffma_per_s"] / 1e9, "frac_of_measured_pipe_peak": achieved / (pipes["ffma_per_s"] / 1e9),
+        "launch_ms": launch_ms, "facet_echoes_per_launch": echoes,
+        "executed_instr_per_facet_echo": K2K_EXECUTED_INSTR_PER_FACET_ECHO if keyframed else K2S_EXECUTED_INSTR_PER_FACET_ECHO,
         "kernel_share_of_step": kms["geometry"] / max(sum(kms.values()), 1e-9),
     }
 
