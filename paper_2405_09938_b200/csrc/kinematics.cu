@@ -7,10 +7,14 @@
 // instead of a sincos; fp64 because the height feeds the carrier phase (1 mrad = 8.8 um of path,
 // SURVEY.md §7 hard part 2).  Slopes only scale sigma0 and stay fp32.
 //
-// Layout: block = 64 (i) x 4 (j) facets of one pulse; the 4 x Nw products Y*T are formed once per
-// block in shared memory and broadcast; X[w][i] is read coalesced (i fastest) and stays L1/L2
-// resident (Nw*nx*16 B <= 16 MB).
-// Bound: FP64 pipe, 4 DFMA per facet-component (+2 FFMA with slopes).
+// Layout: block = 64 (i) x 4 (j) facets x kPK consecutive rows (pulses or keyframes).  A thread owns one facet:
+// per wave component it forms c = X[w][i] * Y[w][j] once (X read coalesced from L2, Y from shared memory) and
+// then runs over the kPK rows, multiplying by T[w][p] from shared memory (broadcast).  Only the HEIGHT (and the
+// CWM displacement) is accumulated in fp64 -- 2 DFMA per facet-component-row; the time derivative, the slopes and
+// their rates are fp32 products of (float)c with a float copy of T (the rate enters the Hermite interpolant
+// scaled by h/8 ~ 1e-3 s, the slopes only scale sigma0).  Wave components are processed in chunks of kWCh so
+// that the tables fit 48 KB of shared memory for any Nw.
+// Bound: FP64 pipe, 2 DFMA per facet-component-row (6 with CWM), next to ~9 FFMA with slopes and rates.
 //
 // Keyframes (surface.cuh): with H > 1 the kernel runs only at the keyframe pulses min(j H, P-1) and also
 // writes the time derivatives (d/dt of A cos(psi) is A omega sin(psi)), from which K2 interpolates.
@@ -21,78 +25,105 @@ namespace heeps {
 namespace {
 
 constexpr int kBX = 64, kBY = 4;
+constexpr int kPK = 8;        // rows per thread
+constexpr int kWCh = 128;     // wave components per shared-memory chunk
 
 template <bool kSlope, bool kChoppy, bool kRate>
 __global__ void __launch_bounds__(kBX * kBY)
-kinematics_kernel(DevParams prm, KinematicsArgs a, int first)
+kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
 {
-    extern __shared__ double2 smem_yt[];               // [kBY][Nw] then wk [Nw] as float4
+    __shared__ double2 s_y[kBY][kWCh];
+    __shared__ double2 s_t[kWCh][kPK];
+    __shared__ float2 s_tf[kWCh][kPK];
+    __shared__ float4 s_wk[kWCh];
+    __shared__ float s_om[kWCh];
+
     const int nw = prm.n_waves;
-    float4 *s_wk = reinterpret_cast<float4 *>(smem_yt + kBY * nw);
-    // row `pl` of the outputs holds pulse p: the batch's pulses (H = 1) or its keyframes (H > 1)
-    const int pl = blockIdx.z;
-    const int p = kRate ? min((first + pl) * a.H, a.n_pulses_total - 1) : first + pl;
+    const int row0 = blockIdx.z * kPK;                 // first output row of this block
     const int j0 = blockIdx.y * kBY;
     const int tid = threadIdx.y * kBX + threadIdx.x;
-
-    for (int idx = tid; idx < kBY * nw; idx += kBX * kBY) {
-        int r = idx / nw, w = idx - r * nw;
-        int j = min(j0 + r, prm.ny - 1);
-        double2 y = a.yt[(size_t)w * prm.ny + j];
-        double2 t = a.tt[(size_t)w * a.n_pulses_total + p];
-        smem_yt[idx] = make_double2(y.x * t.x - y.y * t.y, y.x * t.y + y.y * t.x);
-    }
-    if (kSlope || kChoppy || kRate)
-        for (int w = tid; w < nw; w += kBX * kBY) s_wk[w] = a.wk[w];
-    __syncthreads();
-
     const int i = blockIdx.x * kBX + threadIdx.x;
     const int j = j0 + threadIdx.y;
-    if (i >= prm.nx || j >= prm.ny) return;
-    const double2 *yt = smem_yt + threadIdx.y * nw;
-    const double2 *xt = a.xt + i;
+    const bool valid = i < prm.nx && j < prm.ny;
 
-    double z = 0.0, dx = 0.0, dy = 0.0, zt = 0.0, dxt = 0.0, dyt = 0.0;
-    float sx = 0.f, sy = 0.f, sxt = 0.f, syt = 0.f;
-#pragma unroll 4
-    for (int w = 0; w < nw; ++w) {
-        double2 x = __ldg(xt + (size_t)w * prm.nx);
-        double2 y = yt[w];
-        const double re = fma(x.x, y.x, -x.y * y.y);          // A cos(psi)
-        z += re;
-        if (kSlope || kChoppy || kRate) {
-            double im = fma(x.x, y.y, x.y * y.x);             // A sin(psi)
-            float4 k = s_wk[w];
-            const double om = kRate ? a.omega[w] : 0.0;
-            if (kRate) zt = fma(om, im, zt);                  // d/dt A cos(psi) = A omega sin(psi)
-            if (kSlope) {
-                float imf = (float)im;
-                sx = fmaf(-k.x, imf, sx);                     // grad z = -sum A k sin(psi)
-                sy = fmaf(-k.y, imf, sy);
-                if (kRate) {
-                    const float wre = (float)(om * re);
-                    sxt = fmaf(k.x, wre, sxt);
-                    syt = fmaf(k.y, wre, syt);
-                }
+    double z[kPK], dx[kPK], dy[kPK];
+    float zt[kPK], sx[kPK], sy[kPK], sxt[kPK], syt[kPK], dxt[kPK], dyt[kPK];
+#pragma unroll
+    for (int k = 0; k < kPK; ++k) {
+        z[k] = dx[k] = dy[k] = 0.0;
+        zt[k] = sx[k] = sy[k] = sxt[k] = syt[k] = dxt[k] = dyt[k] = 0.f;
+    }
+
+    for (int w0 = 0; w0 < nw; w0 += kWCh) {
+        const int nwc = min(kWCh, nw - w0);
+        __syncthreads();                               // the previous chunk's tables are no longer read
+        for (int idx = tid; idx < kBY * nwc; idx += kBX * kBY) {
+            const int r = idx / nwc, w = idx - r * nwc;
+            s_y[r][w] = a.yt[(size_t)(w0 + w) * prm.ny + min(j0 + r, prm.ny - 1)];
+        }
+        for (int idx = tid; idx < nwc * kPK; idx += kBX * kBY) {
+            const int w = idx / kPK, k = idx - w * kPK;
+            const int row = min(row0 + k, n_rows - 1);
+            // row `row` of the outputs holds pulse p: the batch's pulses (H = 1) or its keyframes (H > 1)
+            const int p = kRate ? min((first + row) * a.H, a.n_pulses_total - 1) : first + row;
+            const double2 t = a.tt[(size_t)(w0 + w) * a.n_pulses_total + p];
+            s_t[w][k] = t;
+            s_tf[w][k] = make_float2((float)t.x, (float)t.y);
+        }
+        if (kSlope || kChoppy || kRate)
+            for (int w = tid; w < nwc; w += kBX * kBY) {
+                s_wk[w] = a.wk[w0 + w];
+                s_om[w] = kRate ? (float)a.omega[w0 + w] : 0.f;
             }
-            if (kChoppy) {
-                dx = fma(-(double)k.z, im, dx);               // D_h = -sum A k^ sin(psi)
-                dy = fma(-(double)k.w, im, dy);
-                if (kRate) {
-                    dxt = fma((double)k.z * om, re, dxt);
-                    dyt = fma((double)k.w * om, re, dyt);
+        __syncthreads();
+        if (!valid) continue;
+        const double2 *xt = a.xt + (size_t)w0 * prm.nx + i;
+#pragma unroll 2
+        for (int w = 0; w < nwc; ++w) {
+            const double2 x = __ldg(xt + (size_t)w * prm.nx);
+            const double2 y = s_y[threadIdx.y][w];
+            const double cr = fma(x.x, y.x, -x.y * y.y), ci = fma(x.x, y.y, x.y * y.x);   // A exp(j (kx x + ky y + phase))
+            float cfr = 0.f, cfi = 0.f, om = 0.f;
+            float4 k4 = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (kSlope || kChoppy || kRate) { cfr = (float)cr; cfi = (float)ci; k4 = s_wk[w]; om = s_om[w]; }
+#pragma unroll
+            for (int k = 0; k < kPK; ++k) {
+                const double2 t = s_t[w][k];
+                z[k] += fma(cr, t.x, -ci * t.y);                          // A cos(psi)
+                if (kChoppy) {
+                    const double im = fma(cr, t.y, ci * t.x);            // A sin(psi)
+                    dx[k] = fma(-(double)k4.z, im, dx[k]);               // D_h = -sum A k^ sin(psi)
+                    dy[k] = fma(-(double)k4.w, im, dy[k]);
+                }
+                if (kSlope || kRate || kChoppy) {
+                    const float2 tf = s_tf[w][k];
+                    const float imf = fmaf(cfr, tf.y, cfi * tf.x);
+                    const float wre = om * fmaf(cfr, tf.x, -cfi * tf.y);  // omega A cos(psi)
+                    if (kRate) zt[k] = fmaf(om, imf, zt[k]);              // d/dt A cos(psi) = A omega sin(psi)
+                    if (kSlope) {
+                        sx[k] = fmaf(-k4.x, imf, sx[k]);                  // grad z = -sum A k sin(psi)
+                        sy[k] = fmaf(-k4.y, imf, sy[k]);
+                        if (kRate) { sxt[k] = fmaf(k4.x, wre, sxt[k]); syt[k] = fmaf(k4.y, wre, syt[k]); }
+                    }
+                    if (kChoppy && kRate) { dxt[k] = fmaf(k4.z, wre, dxt[k]); dyt[k] = fmaf(k4.w, wre, dyt[k]); }
                 }
             }
         }
     }
-    const size_t f = (size_t)pl * prm.nx * prm.ny + (size_t)j * prm.nx + i;
-    a.z[f] = z;
-    if (kSlope) a.slope[f] = make_float2(sx, sy);
-    if (kChoppy) a.dxy[f] = make_double2(dx, dy);
-    if (kRate) {
-        a.zt[f] = zt;
-        if (kSlope) a.slope_t[f] = make_float2(sxt, syt);
-        if (kChoppy) a.dxy_t[f] = make_double2(dxt, dyt);
+    if (!valid) return;
+    const size_t F = (size_t)prm.nx * prm.ny;
+#pragma unroll
+    for (int k = 0; k < kPK; ++k) {
+        if (row0 + k >= n_rows) break;
+        const size_t f = (size_t)(row0 + k) * F + (size_t)j * prm.nx + i;
+        a.z[f] = z[k];
+        if (kSlope) a.slope[f] = make_float2(sx[k], sy[k]);
+        if (kChoppy) a.dxy[f] = make_double2(dx[k], dy[k]);
+        if (kRate) {
+            a.zt[f] = (double)zt[k];
+            if (kSlope) a.slope_t[f] = make_float2(sxt[k], syt[k]);
+            if (kChoppy) a.dxy_t[f] = make_double2((double)dxt[k], (double)dyt[k]);
+        }
     }
 }
 
@@ -120,16 +151,10 @@ cudaError_t launch_surface_slope(const DevParams &prm, const SurfaceArgs &sa, co
 cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a, int first, int n_rows, cudaStream_t s)
 {
     if (n_rows <= 0) return cudaSuccess;
-    const int n_pl = n_rows;
     dim3 block(kBX, kBY);
-    dim3 grid((prm.nx + kBX - 1) / kBX, (prm.ny + kBY - 1) / kBY, n_pl);
-    size_t smem = (size_t)kBY * prm.n_waves * sizeof(double2) + (size_t)prm.n_waves * sizeof(float4);
+    dim3 grid((prm.nx + kBX - 1) / kBX, (prm.ny + kBY - 1) / kBY, (n_rows + kPK - 1) / kPK);
     const bool slope = a.slope != nullptr, choppy = a.dxy != nullptr;
-    auto launch = [&](auto kern) {
-        if (smem > 48 * 1024)
-            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        kern<<<grid, block, smem, s>>>(prm, a, first);
-    };
+    auto launch = [&](auto kern) { kern<<<grid, block, 0, s>>>(prm, a, first, n_rows); };
     const bool rate = a.H > 1;
     if (rate) {
         if (slope && choppy) launch(kinematics_kernel<true, true, true>);
