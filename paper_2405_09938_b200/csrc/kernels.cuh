@@ -20,7 +20,6 @@ struct KinematicsArgs {
     int32_t H;              // keyframe spacing in pulses (1 = every pulse)
     const double *omega;    // [Nw] (H > 1)
     double *zt;             // time derivatives (H > 1): [n_rows][F]
-    float2 *slope_t;        // or null
     double2 *dxy_t;         // or null
 };
 cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a, int first, int n_rows, cudaStream_t s);

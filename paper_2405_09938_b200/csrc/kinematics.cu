@@ -10,11 +10,11 @@
 // Layout: block = 64 (i) x 4 (j) facets x kPK consecutive rows (pulses or keyframes).  A thread owns one facet:
 // per wave component it forms c = X[w][i] * Y[w][j] once (X read coalesced from L2, Y from shared memory) and
 // then runs over the kPK rows, multiplying by T[w][p] from shared memory (broadcast).  Only the HEIGHT (and the
-// CWM displacement) is accumulated in fp64 -- 2 DFMA per facet-component-row; the time derivative, the slopes and
-// their rates are fp32 products of (float)c with a float copy of T (the rate enters the Hermite interpolant
+// CWM displacement) is accumulated in fp64 -- 2 DFMA per facet-component-row; the time derivative and the slopes
+// (linear between keyframes: no slope rates) are fp32 products of (float)c with a float copy of T (the rate enters the Hermite interpolant
 // scaled by h/8 ~ 1e-3 s, the slopes only scale sigma0).  Wave components are processed in chunks of kWCh so
 // that the tables fit 48 KB of shared memory for any Nw.
-// Bound: FP64 pipe, 2 DFMA per facet-component-row (6 with CWM), next to ~9 FFMA with slopes and rates.
+// Bound: FP64 pipe, 2 DFMA per facet-component-row (6 with CWM), next to 4 FP32 instructions with slopes and rates.
 //
 // Keyframes (surface.cuh): with H > 1 the kernel runs only at the keyframe pulses min(j H, P-1) and also
 // writes the time derivatives (d/dt of A cos(psi) is A omega sin(psi)), from which K2 interpolates.
@@ -30,7 +30,7 @@ constexpr int kWCh = 128;     // wave components per shared-memory chunk
 
 template <bool kSlope, bool kChoppy, bool kRate>
 __global__ void __launch_bounds__(kBX * kBY)
-kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
+kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows, int rows_per_block)
 {
     __shared__ double2 s_y[kBY][kWCh];
     __shared__ double2 s_t[kWCh][kPK];
@@ -39,7 +39,8 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
     __shared__ float s_om[kWCh];
 
     const int nw = prm.n_waves;
-    const int row0 = blockIdx.z * kPK;                 // first output row of this block
+    const int row0 = blockIdx.z * rows_per_block;      // first output row of this block
+    const int nk = min(rows_per_block, n_rows - row0); // rows of this block (<= kPK, block-uniform)
     const int j0 = blockIdx.y * kBY;
     const int tid = threadIdx.y * kBX + threadIdx.x;
     const int i = blockIdx.x * kBX + threadIdx.x;
@@ -47,11 +48,12 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
     const bool valid = i < prm.nx && j < prm.ny;
 
     double z[kPK], dx[kPK], dy[kPK];
-    float zt[kPK], sx[kPK], sy[kPK], sxt[kPK], syt[kPK], dxt[kPK], dyt[kPK];
+    float zt[kPK], dxt[kPK], dyt[kPK];
+    float2 sxy[kPK];
 #pragma unroll
     for (int k = 0; k < kPK; ++k) {
         z[k] = dx[k] = dy[k] = 0.0;
-        zt[k] = sx[k] = sy[k] = sxt[k] = syt[k] = dxt[k] = dyt[k] = 0.f;
+        zt[k] = dxt[k] = dyt[k] = 0.f; sxy[k] = make_float2(0.f, 0.f);
     }
 
     for (int w0 = 0; w0 < nw; w0 += kWCh) {
@@ -63,7 +65,7 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
         }
         for (int idx = tid; idx < nwc * kPK; idx += kBX * kBY) {
             const int w = idx / kPK, k = idx - w * kPK;
-            const int row = min(row0 + k, n_rows - 1);
+            const int row = min(row0 + min(k, nk - 1), n_rows - 1);
             // row `row` of the outputs holds pulse p: the batch's pulses (H = 1) or its keyframes (H > 1)
             const int p = kRate ? min((first + row) * a.H, a.n_pulses_total - 1) : first + row;
             const double2 t = a.tt[(size_t)(w0 + w) * a.n_pulses_total + p];
@@ -86,26 +88,27 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
             float cfr = 0.f, cfi = 0.f, om = 0.f;
             float4 k4 = make_float4(0.f, 0.f, 0.f, 0.f);
             if (kSlope || kChoppy || kRate) { cfr = (float)cr; cfi = (float)ci; k4 = s_wk[w]; om = s_om[w]; }
+            const float2 nk2 = make_float2(-k4.x, -k4.y);
 #pragma unroll
             for (int k = 0; k < kPK; ++k) {
+                if (k >= nk) break;                                       // block-uniform
                 const double2 t = s_t[w][k];
-                z[k] += fma(cr, t.x, -ci * t.y);                          // A cos(psi)
+                z[k] = fma(cr, t.x, z[k]);                                // A cos(psi)
+                z[k] = fma(-ci, t.y, z[k]);
                 if (kChoppy) {
                     const double im = fma(cr, t.y, ci * t.x);            // A sin(psi)
                     dx[k] = fma(-(double)k4.z, im, dx[k]);               // D_h = -sum A k^ sin(psi)
                     dy[k] = fma(-(double)k4.w, im, dy[k]);
                 }
-                if (kSlope || kRate || kChoppy) {
+                if (kSlope || kRate) {
                     const float2 tf = s_tf[w][k];
                     const float imf = fmaf(cfr, tf.y, cfi * tf.x);
-                    const float wre = om * fmaf(cfr, tf.x, -cfi * tf.y);  // omega A cos(psi)
                     if (kRate) zt[k] = fmaf(om, imf, zt[k]);              // d/dt A cos(psi) = A omega sin(psi)
-                    if (kSlope) {
-                        sx[k] = fmaf(-k4.x, imf, sx[k]);                  // grad z = -sum A k sin(psi)
-                        sy[k] = fmaf(-k4.y, imf, sy[k]);
-                        if (kRate) { sxt[k] = fmaf(k4.x, wre, sxt[k]); syt[k] = fmaf(k4.y, wre, syt[k]); }
+                    if (kSlope) sxy[k] = __ffma2_rn(nk2, make_float2(imf, imf), sxy[k]);   // grad z = -sum A k sin(psi)
+                    if (kChoppy && kRate) {
+                        const float wre = om * fmaf(cfr, tf.x, -cfi * tf.y);          // omega A cos(psi)
+                        dxt[k] = fmaf(k4.z, wre, dxt[k]); dyt[k] = fmaf(k4.w, wre, dyt[k]);
                     }
-                    if (kChoppy && kRate) { dxt[k] = fmaf(k4.z, wre, dxt[k]); dyt[k] = fmaf(k4.w, wre, dyt[k]); }
                 }
             }
         }
@@ -114,14 +117,13 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
     const size_t F = (size_t)prm.nx * prm.ny;
 #pragma unroll
     for (int k = 0; k < kPK; ++k) {
-        if (row0 + k >= n_rows) break;
+        if (k >= nk) break;
         const size_t f = (size_t)(row0 + k) * F + (size_t)j * prm.nx + i;
         a.z[f] = z[k];
-        if (kSlope) a.slope[f] = make_float2(sx[k], sy[k]);
+        if (kSlope) a.slope[f] = sxy[k];
         if (kChoppy) a.dxy[f] = make_double2(dx[k], dy[k]);
         if (kRate) {
             a.zt[f] = (double)zt[k];
-            if (kSlope) a.slope_t[f] = make_float2(sxt[k], syt[k]);
             if (kChoppy) a.dxy_t[f] = make_double2((double)dxt[k], (double)dyt[k]);
         }
     }
@@ -152,9 +154,11 @@ cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a, int
 {
     if (n_rows <= 0) return cudaSuccess;
     dim3 block(kBX, kBY);
-    dim3 grid((prm.nx + kBX - 1) / kBX, (prm.ny + kBY - 1) / kBY, (n_rows + kPK - 1) / kPK);
+    // rows split evenly over the fewest blocks of <= kPK rows (17 rows -> 6 + 6 + 5, not 8 + 8 + 1)
+    const int n_chunks = (n_rows + kPK - 1) / kPK, rows_per_block = (n_rows + n_chunks - 1) / n_chunks;
+    dim3 grid((prm.nx + kBX - 1) / kBX, (prm.ny + kBY - 1) / kBY, (n_rows + rows_per_block - 1) / rows_per_block);
     const bool slope = a.slope != nullptr, choppy = a.dxy != nullptr;
-    auto launch = [&](auto kern) { kern<<<grid, block, 0, s>>>(prm, a, first, n_rows); };
+    auto launch = [&](auto kern) { kern<<<grid, block, 0, s>>>(prm, a, first, n_rows, rows_per_block); };
     const bool rate = a.H > 1;
     if (rate) {
         if (slope && choppy) launch(kinematics_kernel<true, true, true>);

@@ -8,7 +8,7 @@
 //   R(t)   = r_t + r_r,ref  bistatic path to the un-offset phase centre: cubic HERMITE from the exact values and
 //            time derivatives at the two keyframes,  dR/dt = u_t.(v_f - V_tx) + u_r.(v_f - V_rx)  with the facet
 //            velocity v_f = (current + dD_h/dt, dz/dt) from K1's rate rows.  Error <= h^4 max|R''''| / 384:
-//            platform term 3 V^4/r^3 ~ 0.02 m/s^4 -> 4e-13 m at h = 9.4 ms; wave term = K1's own bound (1e-9 m).
+//            platform term 3 V^4/r^3 ~ 0.02 m/s^4 -> 4e-13 m at h = 9.4 ms; wave term = K1's own bound (2e-9 m).
 //   d_c(t) = r_r,c - r_r,ref  (receive phase centre c, |o_c| <= 1e-4 r) = o_c a(t) + o_c^2 b, a = -(d.v^)/r linear
 //            in t, b = (1 - a^2)/(2 r); fp32 (|d_c| < 1 m).
 //   P(t)   = G_t G_r,ref      quadratic through t0, t_mid, t1 with the sinc arguments at t_mid taken as the mean of
@@ -260,12 +260,8 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         const float xmag = __uint_as_float(xp.x);
         xarg[q] = xp.y;
         if (kTilt) {
-            const float2 sl0 = a.surf.slope[row0 + f], sd0 = a.surf.slope_t[row0 + f];
-            const float2 sl1 = a.surf.slope[row1 + f], sd1 = a.surf.slope_t[row1 + f];
-            const float hh = (float)(pc2[1].t - pc2[0].t);
-            // Hermite at s = 1/2: (v0 + v1)/2 + h (d0 - d1)/8
-            const float smx = 0.5f * (sl0.x + sl1.x) + 0.125f * hh * (sd0.x - sd1.x);
-            const float smy = 0.5f * (sl0.y + sl1.y) + 0.125f * hh * (sd0.y - sd1.y);
+            const float2 sl0 = a.surf.slope[row0 + f], sl1 = a.surf.slope[row1 + f];
+            const float smx = 0.5f * (sl0.x + sl1.x), smy = 0.5f * (sl0.y + sl1.y);   // slopes are linear between keyframes
             const float lx = (float)prm.look_x, ly = (float)prm.look_y;
             const float A0 = sqrtf(sig * fmaxf(1.f + 2.f * (sl0.x * lx + sl0.y * ly), 0.f) * area) * xmag;
             const float Am = sqrtf(sig * fmaxf(1.f + 2.f * (smx * lx + smy * ly), 0.f) * area) * xmag;

@@ -67,7 +67,7 @@ struct sim_handle {
     DevBuf<uint2> xi_polar;              // {|xi|, arg xi in 2^-32 turns}, derived from xi on the device
     // workspace
     DevBuf<double> z, zt, omega;
-    DevBuf<float2> slope, slope_t;
+    DevBuf<float2> slope;
     DevBuf<double2> dxy, dxy_t;
     int key_H = 1;                       // keyframe spacing of the kinematics (1 = every pulse)
     bool geo_keyframed = false;          // spectral path: ranges / gains interpolated between keyframes (K2k)
@@ -206,7 +206,7 @@ void surface_rows(const sim_handle *h, int p0, int n_pl, int *first, int *rows)
 }
 
 struct SurfBufs {
-    double *z, *zt; float2 *slope, *slope_t; double2 *dxy, *dxy_t;
+    double *z, *zt; float2 *slope; double2 *dxy, *dxy_t;
 };
 
 // K1 for the batch; fills `sa` for K2.
@@ -217,16 +217,18 @@ int run_kinematics(sim_handle *h, const SurfBufs &b, int p0, int n_pl, cudaStrea
     KinematicsArgs ka{};
     ka.xt = h->xt.p; ka.yt = h->yt.p; ka.tt = h->tt.p; ka.wk = h->wk.p; ka.n_pulses_total = h->n_pulses;
     ka.z = b.z; ka.slope = b.slope; ka.dxy = b.dxy;
-    ka.H = h->key_H; ka.omega = h->omega.p; ka.zt = b.zt; ka.slope_t = b.slope_t; ka.dxy_t = b.dxy_t;
+    ka.H = h->key_H; ka.omega = h->omega.p; ka.zt = b.zt; ka.dxy_t = b.dxy_t;
     cudaError_t e = launch_kinematics(h->prm, ka, first, rows, s);
     if (e != cudaSuccess) return fail_cuda(h, e, "launch_kinematics");
-    sa->z = b.z; sa->zt = b.zt; sa->slope = b.slope; sa->slope_t = b.slope_t; sa->dxy = b.dxy; sa->dxy_t = b.dxy_t;
+    sa->z = b.z; sa->zt = b.zt; sa->slope = b.slope; sa->dxy = b.dxy; sa->dxy_t = b.dxy_t;
     sa->H = h->key_H; sa->key0 = first; sa->n_pulses_total = h->n_pulses;
     return SIM_OK;
 }
 
 // Keyframe spacing (surface.cuh): largest H whose cubic-Hermite error bound sum_w A_w (omega_w h)^4 / 384
-// stays under 1e-9 m (and the same for the CWM displacement); 1 when pulse times are not increasing.
+// stays under 2e-9 m (2.3e-7 rad of carrier phase; the same for the CWM displacement) and, with tilt modulation,
+// whose linear-interpolation error of the slopes, 4 x the root-sum-square of A_w |k_w| (omega_w h)^2 / 8 over the
+// components (random phases), stays under 4e-5 (the slopes only scale sigma0); 1 when pulse times are not increasing.
 int choose_keyframe_spacing(const sim_geometry *g, const sim_scene *sc, int requested)
 {
     const int P = g->n_pulses;
@@ -237,12 +239,14 @@ int choose_keyframe_spacing(const sim_geometry *g, const sim_scene *sc, int requ
         if (H > P - 1) continue;
         double hmax = 0;
         for (int k = 0; k < P - 1; k += H) hmax = std::max(hmax, g->t_pulse_s[std::min(k + H, P - 1)] - g->t_pulse_s[k]);
-        double bound = 0;
+        double bound = 0, slope2 = 0;
         for (int w = 0; w < sc->n_waves; ++w) {
             const double x = sc->omega[w] * hmax;
             bound += std::fabs(sc->amp[w]) * x * x * x * x / 384.0;
+            const double sl = std::fabs(sc->amp[w]) * std::hypot(sc->kx[w], sc->ky[w]) * x * x / 8.0;
+            slope2 += sl * sl;
         }
-        if (bound <= 1e-9) return H;
+        if (bound <= 2e-9 && (!sc->tilt_modulation || 4.0 * std::sqrt(slope2) <= 4e-5)) return H;
     }
     return 1;
 }
@@ -378,7 +382,7 @@ void sim_destroy(sim_handle *h)
     h->wk.release(); h->carrier_frac.release(); h->pulses.release();
     h->sigma0.release(); h->current.release(); h->xi.release(); h->xi_polar.release();
     h->z.release(); h->slope.release(); h->dxy.release();
-    h->zt.release(); h->slope_t.release(); h->dxy_t.release(); h->omega.release(); h->recs.release(); h->tinfo.release();
+    h->zt.release(); h->dxy_t.release(); h->omega.release(); h->recs.release(); h->tinfo.release();
     h->tspan.release(); h->acc.release(); h->counters.release(); h->out_staging.release();
     h->mom.release(); h->cspec.release(); h->tw.release();
     delete h;
@@ -620,7 +624,6 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
         if (prm.choppy) CKC(h->dxy.alloc(F * rows));
         if (h->key_H > 1) {
             CKC(h->zt.alloc(F * rows));
-            if (h->need_slope) CKC(h->slope_t.alloc(F * rows));
             if (prm.choppy) CKC(h->dxy_t.alloc(F * rows));
         }
         CKC(h->omega.alloc(std::max(Nw, 1)));
@@ -700,7 +703,7 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         }
         return cudaEventRecord(h->events[h->events_used++], s);
     };
-    const SurfBufs bufs{h->z.p, h->zt.p, h->slope.p, h->slope_t.p, h->dxy.p, h->dxy_t.p};
+    const SurfBufs bufs{h->z.p, h->zt.p, h->slope.p, h->dxy.p, h->dxy_t.p};
     for (int p0 = pb0; h->spectral && p0 < pb1; p0 += h->pulses_per_batch) {
         const int n_pl = std::min(h->pulses_per_batch, pb1 - p0);
         CK(h, cudaMemsetAsync(h->mom.p, 0, (size_t)prm.n_channels * n_pl * kMomentOrder * h->nb_pad * sizeof(float2), s));
@@ -836,11 +839,11 @@ int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, d
         }
         CK(h, d_pos.alloc(3 * F)); CK(h, d_tau.alloc(C * F)); CK(h, d_gtx.alloc(F));
         CK(h, d_grx.alloc(C * F)); CK(h, d_amp.alloc(2 * C * F)); CK(h, d_keep.alloc(F));
-        // the slope is reported even when the scene does not use it: temporary rows (value + rate)
-        SurfBufs bufs{h->z.p, h->zt.p, h->slope.p, h->slope_t.p, h->dxy.p, h->dxy_t.p};
+        // the slope is reported even when the scene does not use it: temporary rows
+        SurfBufs bufs{h->z.p, h->zt.p, h->slope.p, h->dxy.p, h->dxy_t.p};
         if (!bufs.slope) {
             CK(h, d_slope.alloc(F * 3 * 2));
-            bufs.slope = d_slope.p; bufs.slope_t = d_slope.p + F * 3;
+            bufs.slope = d_slope.p;
         }
         GeometryArgs ga{};
         { int rc2 = run_kinematics(h, bufs, pulse, 1, nullptr, &ga.surf); if (rc2 != SIM_OK) return rc2; }
@@ -848,7 +851,7 @@ int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, d
         // per-facet slope of this pulse (interpolated like K2 sees it), for the report only
         CK(h, d_slope_out.alloc(F));
         CK(h, launch_surface_slope(prm, ga.surf, h->pulses.p, pulse, d_slope_out.p, nullptr));
-        if (!h->need_slope) { ga.surf.slope = nullptr; ga.surf.slope_t = nullptr; }
+        if (!h->need_slope) ga.surf.slope = nullptr;
         ga.sigma0 = h->sigma0.p; ga.current = h->current.p; ga.xi = h->xi.p; ga.xi_polar = h->xi_polar.p;
         ga.recs = recs; ga.tinfo = tinfo; ga.tspan = tspan; ga.counters = nullptr;
         ga.dbg_pos = d_pos.p; ga.dbg_tau = d_tau.p; ga.dbg_gtx = d_gtx.p; ga.dbg_grx = d_grx.p;

@@ -4,7 +4,9 @@
 // pulses kf_j = min(j H, P-1), where it also stores the time derivatives; between keyframes the state is
 // the cubic Hermite interpolant in t.  Waves are slow against the PRF (omega <= ~3 rad/s): the interpolation
 // error of one component is <= A (omega h)^4 / 384 (h = keyframe spacing in seconds), and sim_create picks H
-// so that the sum of these bounds stays under 1e-9 m (hard part 3).  The oracle always
+// so that the sum of these bounds stays under 2e-9 m (hard part 3).  The slopes only scale sigma0
+// (tilt modulation): they are interpolated LINEARLY, per-component error <= A_w |k_w| (omega_w h)^2 / 8 (4 x their root-sum-square kept
+// under 4e-5 by sim_create).  The oracle always
 // evaluates exactly per pulse.
 #pragma once
 #include "heeps_common.cuh"
@@ -13,7 +15,7 @@ namespace heeps {
 
 struct SurfaceArgs {
     const double *z, *zt;               // [n][F] height above centre_z and its time derivative (zt: H > 1 only)
-    const float2 *slope, *slope_t;      // [n][F] or null (tilt modulation only)
+    const float2 *slope;                // [n][F] or null (tilt modulation only; LINEAR between keyframes)
     const double2 *dxy, *dxy_t;         // [n][F] or null (Choppy Wave Model only)
     int32_t H;                          // 1: n = pulses of the batch; > 1: n = keyframes of the batch
     int32_t key0;                       // H > 1: index j of the first keyframe held
@@ -23,6 +25,7 @@ struct SurfaceArgs {
 struct SurfaceInterp {                  // per (CTA, pulse)
     size_t row0, row1;                  // rows of the two bracketing keyframes (H = 1: row0 = pulse row)
     double w00, w10, w01, w11;          // Hermite weights of z0, zt0, z1, zt1 (w10, w11 include h)
+    float s;                            // (t - t0) / h
 };
 
 __device__ __forceinline__ SurfaceInterp surface_interp(const SurfaceArgs &sa, const PulseConst *pulses, int p, int pl)
@@ -30,7 +33,7 @@ __device__ __forceinline__ SurfaceInterp surface_interp(const SurfaceArgs &sa, c
     SurfaceInterp it;
     if (sa.H <= 1) {
         it.row0 = it.row1 = (size_t)pl;
-        it.w00 = 1.0; it.w10 = it.w01 = it.w11 = 0.0;
+        it.w00 = 1.0; it.w10 = it.w01 = it.w11 = 0.0; it.s = 0.f;
         return it;
     }
     const int P = sa.n_pulses_total;
@@ -48,6 +51,7 @@ __device__ __forceinline__ SurfaceInterp surface_interp(const SurfaceArgs &sa, c
     it.w10 = (s3 - 2.0 * s2 + s) * h;
     it.w01 = -2.0 * s3 + 3.0 * s2;
     it.w11 = (s3 - s2) * h;
+    it.s = (float)s;
     return it;
 }
 
@@ -62,10 +66,8 @@ __device__ __forceinline__ float2 surface_slope(const SurfaceArgs &sa, const Sur
 {
     if (sa.H <= 1) return sa.slope[it.row0 * F + f];
     const size_t a = it.row0 * F + f, b = it.row1 * F + f;
-    const float2 s0 = sa.slope[a], d0 = sa.slope_t[a], s1 = sa.slope[b], d1 = sa.slope_t[b];
-    const float w00 = (float)it.w00, w10 = (float)it.w10, w01 = (float)it.w01, w11 = (float)it.w11;
-    return make_float2(w00 * s0.x + w10 * d0.x + w01 * s1.x + w11 * d1.x,
-                       w00 * s0.y + w10 * d0.y + w01 * s1.y + w11 * d1.y);
+    const float2 s0 = sa.slope[a], s1 = sa.slope[b];
+    return make_float2(fmaf(it.s, s1.x - s0.x, s0.x), fmaf(it.s, s1.y - s0.y, s0.y));
 }
 
 __device__ __forceinline__ double2 surface_dxy(const SurfaceArgs &sa, const SurfaceInterp &it, size_t F, size_t f)
