@@ -87,10 +87,15 @@ struct sim_handle {
     std::vector<cudaEvent_t> events;     // 5 per batch when profiling
     size_t events_used = 0;
     std::string cuda_err;
+    // sim_generate_host: device->host copies of finished batches overlap the next batch's kernels
+    cudaStream_t copy_stream = nullptr;
+    std::vector<cudaEvent_t> copy_events;
 
     ~sim_handle()
     {
         for (auto e : events) cudaEventDestroy(e);
+        for (auto e : copy_events) cudaEventDestroy(e);
+        if (copy_stream) cudaStreamDestroy(copy_stream);
     }
 };
 
@@ -686,11 +691,34 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     return SIM_OK;
 }
 
-static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cudaStream_t s)
+// `host_dst` non-null: `out` is the device staging buffer and every finished batch is copied to
+// host_dst (same [C][n_out][Ns] layout) on the handle's copy stream while the next batch computes.
+static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cudaStream_t s,
+                       int batch_pulses = 0, float2 *host_dst = nullptr)
 {
     const DevParams &prm = h->prm;
     const int n_out = pb1 - pb0;
+    const int batch = batch_pulses > 0 ? std::min(batch_pulses, h->pulses_per_batch) : h->pulses_per_batch;
     int64_t launches = 0;
+    size_t copies = 0;
+    auto ship = [&](int p0, int n_pl) -> cudaError_t {
+        if (!host_dst) return cudaSuccess;
+        if (copies == h->copy_events.size()) {
+            cudaEvent_t e;
+            cudaError_t rc = cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+            if (rc != cudaSuccess) return rc;
+            h->copy_events.push_back(e);
+        }
+        cudaEvent_t e = h->copy_events[copies++];
+        cudaError_t rc = cudaEventRecord(e, s);
+        if (rc == cudaSuccess) rc = cudaStreamWaitEvent(h->copy_stream, e, 0);
+        const size_t row = (size_t)prm.n_samples * sizeof(float2);
+        const size_t off = (size_t)(p0 - pb0) * prm.n_samples;
+        if (rc == cudaSuccess)
+            rc = cudaMemcpy2DAsync(host_dst + off, (size_t)n_out * row, out + off, (size_t)n_out * row,
+                                   (size_t)n_pl * row, prm.n_channels, cudaMemcpyDeviceToHost, h->copy_stream);
+        return rc;
+    };
     CK(h, cudaMemsetAsync(h->counters.p, 0, 2 * sizeof(unsigned long long), s));
     h->events_used = 0;
     auto mark = [&]() -> cudaError_t {
@@ -704,8 +732,8 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         return cudaEventRecord(h->events[h->events_used++], s);
     };
     const SurfBufs bufs{h->z.p, h->zt.p, h->slope.p, h->dxy.p, h->dxy_t.p};
-    for (int p0 = pb0; h->spectral && p0 < pb1; p0 += h->pulses_per_batch) {
-        const int n_pl = std::min(h->pulses_per_batch, pb1 - p0);
+    for (int p0 = pb0; h->spectral && p0 < pb1; p0 += batch) {
+        const int n_pl = std::min(batch, pb1 - p0);
         CK(h, cudaMemsetAsync(h->mom.p, 0, (size_t)prm.n_channels * n_pl * kMomentOrder * h->nb_pad * sizeof(float2), s));
         CK(h, mark());
         MomentArgs ma{};
@@ -725,10 +753,11 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         CK(h, launch_fftconv(prm, fa, p0, n_pl, s));
         CK(h, mark());
         CK(h, mark());                                   // K4 slot: finalize is fused into K3s
+        CK(h, ship(p0, n_pl));
         launches += 3;
     }
-    for (int p0 = pb0; !h->spectral && p0 < pb1; p0 += h->pulses_per_batch) {
-        const int n_pl = std::min(h->pulses_per_batch, pb1 - p0);
+    for (int p0 = pb0; !h->spectral && p0 < pb1; p0 += batch) {
+        const int n_pl = std::min(batch, pb1 - p0);
         CK(h, cudaMemsetAsync(h->acc.p, 0, (size_t)prm.n_channels * n_pl * prm.n_samples * sizeof(double2), s));
         CK(h, mark());
         GeometryArgs ga{};
@@ -747,6 +776,7 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         FinalizeArgs fa{h->acc.p, h->chirp_n.p, h->carrier_p.p, out, n_out, p0 - pb0};
         CK(h, launch_finalize(prm, fa, p0, n_pl, s));
         CK(h, mark());
+        CK(h, ship(p0, n_pl));
         launches += 4;
     }
     h->stats.kernel_launches = launches;
@@ -774,9 +804,14 @@ int sim_generate_host(sim_handle *h, int32_t pulse_begin, int32_t pulse_end, voi
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     const size_t n = (size_t)h->prm.n_channels * (pulse_end - pulse_begin) * h->prm.n_samples;
     if (h->out_staging.n < n) CK(h, h->out_staging.alloc(n));
-    int rc = run_batches(h, pulse_begin, pulse_end, h->out_staging.p, s);
+    if (!h->copy_stream) CK(h, cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+    // about four batches per call (whole keyframe intervals), so that the copy of one overlaps the kernels of the next
+    const int n = pulse_end - pulse_begin, H = std::max(1, h->key_H);
+    int batch = std::max((n + 3) / 4, std::min(n, 32));
+    batch = ((batch + H - 1) / H) * H;
+    int rc = run_batches(h, pulse_begin, pulse_end, h->out_staging.p, s, batch, static_cast<float2 *>(iq_host));
     if (rc != SIM_OK) return rc;
-    CK(h, cudaMemcpyAsync(iq_host, h->out_staging.p, n * sizeof(float2), cudaMemcpyDeviceToHost, s));
+    CK(h, cudaStreamSynchronize(h->copy_stream));
     CK(h, cudaStreamSynchronize(s));
     return SIM_OK;
 }
