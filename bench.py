@@ -121,6 +121,17 @@ class ClockSampler:
                 "samples": len(s), "reasons": reasons}
 
 
+def _workload(name, n_pulses=None, pulse_offset=0):
+    """BASELINE.json configs by name, or one point of the stress sweep (configs[4], reading G23) as
+    `sweep:f<log2 facets>:l<replica samples>:c<channels>`, e.g. sweep:f24:l1200:c3 (64 pulses by default)."""
+    from workloads import make_workload, make_sweep_point
+    if name.startswith("sweep:"):
+        kv = {t[0]: int(t[1:]) for t in name.split(":")[1:]}
+        return make_sweep_point(log2_facets=kv.get("f", 24), replica_samples=kv.get("l", 1200),
+                                n_channels=kv.get("c", 3), n_pulses=n_pulses or 64)
+    return make_workload(name, n_pulses=n_pulses, pulse_offset=pulse_offset)
+
+
 def _oracle_sample(w, pulses):
     from oracle import oracle_generate, oracle_max_threads
     t = time.perf_counter()
@@ -134,8 +145,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    from workloads import make_workload
-    w = make_workload(args.workload)
+    w = _workload(args.workload, args.pulses)
     F, C, P = w.n_facets, w.n_channels, w.n_pulses
     pulses_per_step = 1
     for _ in range(args.warmup):
@@ -236,7 +246,6 @@ def run_cuda(args):
     import torch
     import torch.distributed as dist
     from paper_2405_09938_b200 import Simulator, sim_measure_pipe_peaks
-    from workloads import make_workload
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -247,10 +256,11 @@ def run_cuda(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
 
-    base = make_workload(args.workload)
-    P = base.n_pulses if args.pulses is None else args.pulses
     # weak scaling: rank r simulates pulses [r P, (r+1) P) of an N*P-pulse acquisition
-    w = make_workload(args.workload, n_pulses=P, pulse_offset=rank * P)
+    w = _workload(args.workload, args.pulses, 0)
+    P = w.n_pulses
+    if rank > 0:
+        w = _workload(args.workload, P, rank * P)
     F, C, Ns, L = w.n_facets, w.n_channels, w.n_samples, w.replica_samples
     sim = Simulator(w, local_rank, accumulate_mode=args.mode, tile_facets=args.tile)
     out = torch.empty((C, P, Ns), dtype=torch.complex64, device=f"cuda:{local_rank}")
@@ -324,8 +334,14 @@ def run_cuda(args):
     # ---- the oracle on the host cores, bounded sample (reported baseline, not the target) ----
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        sample = [0, P - 1] if P > 1 else [0]
-        reps = 4                                           # ~10 s of CPU work on 16 cores
+        # bounded sample: about 2.5e7 facet-echoes of oracle work (~10-40 s on 16 cores)
+        per_pulse = F * C
+        if per_pulse * 2 * 4 <= 3e7:
+            sample, reps = ([0, P - 1] if P > 1 else [0]), 4
+        elif per_pulse * 2 <= 3e7:
+            sample, reps = ([0, P - 1] if P > 1 else [0]), 1
+        else:
+            sample, reps = [P // 2], 1                     # one pulse of a large scene (minutes beyond 5e7 facets)
         dt = 0.0
         for _ in range(reps):
             d, cores = _oracle_sample(w, sample)
@@ -372,7 +388,8 @@ def main():
     ap.add_argument("--steps", type=int, default=40)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="ati")
+    ap.add_argument("--workload", default="ati",
+                    help="tiny | ati | hetero | large | sweep:f<log2 facets>:l<replica samples>:c<channels>")
     ap.add_argument("--mode", default="auto", choices=["auto", "direct", "spectral"],
                     help="echo accumulation (include/heeps_sim.h SIM_ACCUMULATE_*)")
     ap.add_argument("--tile", type=int, default=0, help="spatial tile side in facets (0 = library default)")
