@@ -14,10 +14,15 @@
 // (linear between keyframes: no slope rates) are fp32 products of (float)c with a float copy of T (the rate enters the Hermite interpolant
 // scaled by h/8 ~ 1e-3 s, the slopes only scale sigma0).  Wave components are processed in chunks of kWCh so
 // that the tables fit 48 KB of shared memory for any Nw.
-// Bound: FP64 pipe, 2 DFMA per facet-component-row (6 with CWM), next to 4 FP32 instructions with slopes and rates.
+// Bound: 2 DFMA per facet-component-row (6 with CWM) next to 4 FP32 instructions with slopes and rates; measured
+// (profiles/r1_v10): FP64 pipe 20 %, shared-memory data path 68 % -- the broadcast T-table loads (one LDS.128 +
+// one LDS.64 per component-row and warp) are what binds; next step: two facets per thread or fp64 MMA fragments.
 //
 // Keyframes (surface.cuh): with H > 1 the kernel runs only at the keyframe pulses min(j H, P-1) and also
 // writes the time derivatives (d/dt of A cos(psi) is A omega sin(psi)), from which K2 interpolates.
+#include <algorithm>
+#include <type_traits>
+
 #include "kernels.cuh"
 
 namespace heeps {
@@ -25,33 +30,33 @@ namespace heeps {
 namespace {
 
 constexpr int kBX = 64, kBY = 4;
-constexpr int kPK = 8;        // rows per thread
+constexpr int kPK = 8;        // most rows per thread (the kernel is instantiated for 4..8)
 constexpr int kWCh = 128;     // wave components per shared-memory chunk
 
-template <bool kSlope, bool kChoppy, bool kRate>
+template <int NK, bool kSlope, bool kChoppy, bool kRate>
 __global__ void __launch_bounds__(kBX * kBY)
-kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows, int rows_per_block)
+kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
 {
     __shared__ double2 s_y[kBY][kWCh];
-    __shared__ double2 s_t[kWCh][kPK];
-    __shared__ float2 s_tf[kWCh][kPK];
+    __shared__ double2 s_t[kWCh][NK];
+    __shared__ float2 s_tf[kWCh][NK];
     __shared__ float4 s_wk[kWCh];
     __shared__ float s_om[kWCh];
 
     const int nw = prm.n_waves;
-    const int row0 = blockIdx.z * rows_per_block;      // first output row of this block
-    const int nk = min(rows_per_block, n_rows - row0); // rows of this block (<= kPK, block-uniform)
+    const int row0 = blockIdx.z * NK;                  // first output row of this block
+    const int nk = min(NK, n_rows - row0);             // rows this block stores (the last block recomputes its last row)
     const int j0 = blockIdx.y * kBY;
     const int tid = threadIdx.y * kBX + threadIdx.x;
     const int i = blockIdx.x * kBX + threadIdx.x;
     const int j = j0 + threadIdx.y;
     const bool valid = i < prm.nx && j < prm.ny;
 
-    double z[kPK], dx[kPK], dy[kPK];
-    float zt[kPK], dxt[kPK], dyt[kPK];
-    float2 sxy[kPK];
+    double z[NK], dx[NK], dy[NK];
+    float zt[NK], dxt[NK], dyt[NK];
+    float2 sxy[NK];
 #pragma unroll
-    for (int k = 0; k < kPK; ++k) {
+    for (int k = 0; k < NK; ++k) {
         z[k] = dx[k] = dy[k] = 0.0;
         zt[k] = dxt[k] = dyt[k] = 0.f; sxy[k] = make_float2(0.f, 0.f);
     }
@@ -63,8 +68,8 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows, int ro
             const int r = idx / nwc, w = idx - r * nwc;
             s_y[r][w] = a.yt[(size_t)(w0 + w) * prm.ny + min(j0 + r, prm.ny - 1)];
         }
-        for (int idx = tid; idx < nwc * kPK; idx += kBX * kBY) {
-            const int w = idx / kPK, k = idx - w * kPK;
+        for (int idx = tid; idx < nwc * NK; idx += kBX * kBY) {
+            const int w = idx / NK, k = idx - w * NK;
             const int row = min(row0 + min(k, nk - 1), n_rows - 1);
             // row `row` of the outputs holds pulse p: the batch's pulses (H = 1) or its keyframes (H > 1)
             const int p = kRate ? min((first + row) * a.H, a.n_pulses_total - 1) : first + row;
@@ -90,8 +95,7 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows, int ro
             if (kSlope || kChoppy || kRate) { cfr = (float)cr; cfi = (float)ci; k4 = s_wk[w]; om = s_om[w]; }
             const float2 nk2 = make_float2(-k4.x, -k4.y);
 #pragma unroll
-            for (int k = 0; k < kPK; ++k) {
-                if (k >= nk) break;                                       // block-uniform
+            for (int k = 0; k < NK; ++k) {
                 const double2 t = s_t[w][k];
                 z[k] = fma(cr, t.x, z[k]);                                // A cos(psi)
                 z[k] = fma(-ci, t.y, z[k]);
@@ -116,7 +120,7 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows, int ro
     if (!valid) return;
     const size_t F = (size_t)prm.nx * prm.ny;
 #pragma unroll
-    for (int k = 0; k < kPK; ++k) {
+    for (int k = 0; k < NK; ++k) {
         if (k >= nk) break;
         const size_t f = (size_t)(row0 + k) * F + (size_t)j * prm.nx + i;
         a.z[f] = z[k];
@@ -154,22 +158,32 @@ cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a, int
 {
     if (n_rows <= 0) return cudaSuccess;
     dim3 block(kBX, kBY);
-    // rows split evenly over the fewest blocks of <= kPK rows (17 rows -> 6 + 6 + 5, not 8 + 8 + 1)
-    const int n_chunks = (n_rows + kPK - 1) / kPK, rows_per_block = (n_rows + n_chunks - 1) / n_chunks;
-    dim3 grid((prm.nx + kBX - 1) / kBX, (prm.ny + kBY - 1) / kBY, (n_rows + rows_per_block - 1) / rows_per_block);
-    const bool slope = a.slope != nullptr, choppy = a.dxy != nullptr;
-    auto launch = [&](auto kern) { kern<<<grid, block, 0, s>>>(prm, a, first, n_rows, rows_per_block); };
-    const bool rate = a.H > 1;
-    if (rate) {
-        if (slope && choppy) launch(kinematics_kernel<true, true, true>);
-        else if (slope)      launch(kinematics_kernel<true, false, true>);
-        else if (choppy)     launch(kinematics_kernel<false, true, true>);
-        else                 launch(kinematics_kernel<false, false, true>);
-    } else {
-        if (slope && choppy) launch(kinematics_kernel<true, true, false>);
-        else if (slope)      launch(kinematics_kernel<true, false, false>);
-        else if (choppy)     launch(kinematics_kernel<false, true, false>);
-        else                 launch(kinematics_kernel<false, false, false>);
+    // rows split evenly over the fewest blocks of <= kPK rows (17 rows -> 6 + 6 + 5, not 8 + 8 + 1); at least 4 rows
+    // per block (a shorter launch recomputes its last row)
+    const int n_chunks = (n_rows + kPK - 1) / kPK, nk = std::max(4, (n_rows + n_chunks - 1) / n_chunks);
+    dim3 grid((prm.nx + kBX - 1) / kBX, (prm.ny + kBY - 1) / kBY, (n_rows + nk - 1) / nk);
+    const bool slope = a.slope != nullptr, choppy = a.dxy != nullptr, rate = a.H > 1;
+    auto launch = [&](auto kern) { kern<<<grid, block, 0, s>>>(prm, a, first, n_rows); };
+    auto pick = [&](auto nk_tag) {
+        constexpr int NK = decltype(nk_tag)::value;
+        if (rate) {
+            if (slope && choppy) launch(kinematics_kernel<NK, true, true, true>);
+            else if (slope)      launch(kinematics_kernel<NK, true, false, true>);
+            else if (choppy)     launch(kinematics_kernel<NK, false, true, true>);
+            else                 launch(kinematics_kernel<NK, false, false, true>);
+        } else {
+            if (slope && choppy) launch(kinematics_kernel<NK, true, true, false>);
+            else if (slope)      launch(kinematics_kernel<NK, true, false, false>);
+            else if (choppy)     launch(kinematics_kernel<NK, false, true, false>);
+            else                 launch(kinematics_kernel<NK, false, false, false>);
+        }
+    };
+    switch (nk) {
+        case 4: pick(std::integral_constant<int, 4>{}); break;
+        case 5: pick(std::integral_constant<int, 5>{}); break;
+        case 6: pick(std::integral_constant<int, 6>{}); break;
+        case 7: pick(std::integral_constant<int, 7>{}); break;
+        default: pick(std::integral_constant<int, 8>{}); break;
     }
     return cudaGetLastError();
 }
