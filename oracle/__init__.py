@@ -11,6 +11,8 @@ from .binding import (  # noqa: F401
     oracle_generate,
     oracle_facets,
     oracle_samples,
+    oracle_speckle,
+    oracle_philox,
     oracle_max_threads,
     rel_l2_per_vector,
     ati_phase,

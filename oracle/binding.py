@@ -50,6 +50,7 @@ class _Desc(C.Structure):
         ("tilt_modulation", C.c_int32), ("look_dir", C.c_double * 2),
         ("current_mps", C.c_void_p), ("current_uniform", C.c_double * 2),
         ("xi", C.c_void_p),
+        ("speckle_tau_s", C.c_double), ("speckle_doppler_hz", C.c_double), ("seed", C.c_uint64),
     ]
 
 
@@ -69,6 +70,10 @@ def _load():
         _lib.heeps_oracle_max_threads.restype = C.c_int
         _lib.heeps_oracle_samples.restype = C.c_int
         _lib.heeps_oracle_samples.argtypes = [C.POINTER(_Desc), C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32]
+        _lib.heeps_oracle_speckle.restype = C.c_int
+        _lib.heeps_oracle_speckle.argtypes = [C.POINTER(_Desc), C.c_int32, C.c_void_p]
+        _lib.heeps_oracle_philox.restype = None
+        _lib.heeps_oracle_philox.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     return _lib
 
 
@@ -128,6 +133,9 @@ def _marshal(w):
     xi = np.ascontiguousarray(sc["xi"], dtype=np.float32)
     assert xi.shape == (ny, nx, 2)
     d.xi = ptr(xi)
+    d.speckle_tau_s = float(sc.get("speckle_tau_s", 0.0))
+    d.speckle_doppler_hz = float(sc.get("speckle_doppler_hz", 0.0))
+    d.seed = int(sc.get("seed", 0))
     return d, keep
 
 
@@ -181,6 +189,27 @@ def oracle_facets(w, pulse: int) -> dict:
     del keep
     res["amp"] = res["amp"][..., 0] + 1j * res["amp"][..., 1]
     return res
+
+
+def oracle_speckle(w, pulse: int) -> np.ndarray:
+    """complex128 [ny][nx]: the intra-facet speckle s_f(t_p) (eq. (7), (10)) of every facet at one pulse."""
+    lib = _load()
+    d, keep = _marshal(w)
+    out = np.zeros((d.ny, d.nx, 2), dtype=np.float64)
+    rc = lib.heeps_oracle_speckle(C.byref(d), int(pulse), out.ctypes.data)
+    if rc != 0:
+        raise ValueError(f"heeps_oracle_speckle failed ({rc})")
+    del keep
+    return out[..., 0] + 1j * out[..., 1]
+
+
+def oracle_philox(counter, key) -> np.ndarray:
+    """uint32[4]: one Philox4x32-10 block of the oracle's own generator (known-answer pins)."""
+    lib = _load()
+    c = np.ascontiguousarray(np.asarray(counter, dtype=np.uint32)); k = np.ascontiguousarray(np.asarray(key, dtype=np.uint32))
+    out = np.zeros(4, dtype=np.uint32)
+    lib.heeps_oracle_philox(c.ctypes.data, k.ctypes.data, out.ctypes.data)
+    return out
 
 
 # ---------------------------------------------------------------- parity metrics

@@ -24,7 +24,8 @@
  * G4 no 1/(r_t r_r), G5 signed field pattern sinc*sinc, G6 cull on |G_t G_r,ref| from the
  * un-offset phase centre, G8 offsets along the Rx unit velocity, G9 stop-and-go,
  * G10 current by advection, G11 linear waves (CWM by flag), G12 tilt factor clamped at 0,
- * G15 A = d^2, G24 displaced point feeds the antenna direction.
+ * G15 A = d^2, G24 displaced point feeds the antenna direction, G27 the generator of the AR(1) speckle innovations
+ * (NEXT-1, off unless speckle_tau_s > 0).
  *
  * Pins: tests/test_oracle_pins.py (closed forms with mpmath, invariants, brute force by an
  * independent numpy script).  No function here is "parity unpinned".
@@ -62,6 +63,10 @@ typedef struct {
     int32_t tilt_modulation;  double look_dir[2];
     const float *current_mps; double current_uniform[2]; /* [ny][nx][2] or NULL */
     const float *xi;                            /* [ny][nx][2], required */
+    /* NEXT-1: time-dependent intra-facet speckle, eq. (7), (10) */
+    double speckle_tau_s;                       /* tau_s; <= 0: speckle constant over the dwell (xi)  */
+    double speckle_doppler_hz;                  /* f_s of eq. (7)                                      */
+    uint64_t seed;                              /* key of the innovation generator (reading G27)       */
 } oracle_desc;
 
 /* per-facet intermediates of one pulse (O2..O8), exposed for unit parity */
@@ -97,6 +102,65 @@ typedef struct {
     double tau[8], g_tx, g_rx[8], amp_re[8], amp_im[8];
     int keep;
 } facet_eval;
+
+/*
+ * Time-dependent intra-facet speckle.  Eq. (7): s(t) = [R(t) + i I(t)] exp(2 i pi f_s t);
+ * eq. (10), the order-1 autoregressive model the paper adopts:
+ *     R(t + dt) = beta R(t) + (1 - beta^2)^(1/2) R',   beta = exp(-dt / tau_s),   R' ~ N(0, variance 1/2)
+ * (the same for I; "sigma = 1/2" of eq. (10) read as the variance, reading G13), started from R(0) + i I(0) = xi_f
+ * at pulse 0 and stepped pulse by pulse with dt = t_pulse[q] - t_pulse[q-1].
+ * Reading G27 (the paper names no generator): the innovation R' + i I' of facet f at pulse q is drawn from the
+ * counter-based generator Philox4x32-10 (Salmon et al., SC'11) with key = the two halves of `seed` and counter
+ * (f mod 2^32, f div 2^32, q, 1): with the first two output words w0, w1,
+ *     u1 = ((w0 >> 8) + 1) / 2^24 in (0, 1],  u2 = (w1 >> 8) / 2^24 in [0, 1),
+ *     R' + i I' = sqrt(-ln u1) (cos 2 pi u2 + i sin 2 pi u2)        (Box-Muller; each part has variance 1/2).
+ */
+static void philox4x32_10(const uint32_t ctr_in[4], const uint32_t key_in[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr_in[0], c1 = ctr_in[1], c2 = ctr_in[2], c3 = ctr_in[3], k0 = key_in[0], k1 = key_in[1];
+    for (int r = 0; r < 10; ++r) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+static void speckle_innovation(uint64_t seed, uint64_t facet, uint32_t pulse, double *re, double *im)
+{
+    const uint32_t ctr[4] = { (uint32_t)facet, (uint32_t)(facet >> 32), pulse, 1u };
+    const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    uint32_t w[4];
+    philox4x32_10(ctr, key, w);
+    const double u1 = ((double)(w[0] >> 8) + 1.0) / 16777216.0, u2 = (double)(w[1] >> 8) / 16777216.0;
+    const double rad = sqrt(-log(u1));
+    *re = rad * cos(2.0 * M_PI * u2);
+    *im = rad * sin(2.0 * M_PI * u2);
+}
+
+/* s_f(t_p) of eq. (7): the AR(1) state after p steps times the intra-facet Doppler factor. */
+static void speckle_at(const oracle_desc *d, size_t f, int p, double *re, double *im)
+{
+    double R = d->xi[2 * f], I = d->xi[2 * f + 1];
+    if (d->speckle_tau_s > 0.0) {
+        for (int q = 1; q <= p; ++q) {
+            const double beta = exp(-(d->t_pulse_s[q] - d->t_pulse_s[q - 1]) / d->speckle_tau_s);
+            const double g = sqrt(1.0 - beta * beta);
+            double nr, ni;
+            speckle_innovation(d->seed, (uint64_t)f, (uint32_t)q, &nr, &ni);
+            R = beta * R + g * nr;
+            I = beta * I + g * ni;
+        }
+        const double ph = 2.0 * M_PI * d->speckle_doppler_hz * d->t_pulse_s[p];
+        const double c = cos(ph), sn = sin(ph);
+        *re = R * c - I * sn;
+        *im = R * sn + I * c;
+        return;
+    }
+    *re = R; *im = I;
+}
 
 /* O1..O8 for facet (i,j) at pulse p.  Channels limited to 8. */
 static void eval_facet(const oracle_desc *d, int p, int i, int j, facet_eval *o)
@@ -157,7 +221,8 @@ static void eval_facet(const oracle_desc *d, int p, int i, int j, facet_eval *o)
         sigma *= (f > 0.0 ? f : 0.0);
     }
     double a0 = sqrt(sigma * d->spacing_m * d->spacing_m);
-    double xr = d->xi[((size_t)j * d->nx + i) * 2 + 0], xim = d->xi[((size_t)j * d->nx + i) * 2 + 1];
+    double xr, xim;
+    speckle_at(d, (size_t)j * d->nx + i, p, &xr, &xim);
     double vn = sqrt(dot3(vrx, vrx));
     for (int c = 0; c < d->n_channels; ++c) {
         /* O4 receive leg: phase centre offset along the Rx unit velocity (G8) */
@@ -311,6 +376,19 @@ int heeps_oracle_facets(const oracle_desc *d, int32_t p, oracle_facets *o)
                 if (o->amp) { o->amp[2 * (c * F + f)] = fe.amp_re[c]; o->amp[2 * (c * F + f) + 1] = fe.amp_im[c]; }
             }
         }
+    return 0;
+}
+
+/* heeps_oracle_philox: the raw generator (for its known-answer pins). */
+void heeps_oracle_philox(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) { philox4x32_10(ctr, key, out); }
+
+/* heeps_oracle_speckle: s_f(t_p) of every facet at pulse p, out[F][2]. */
+int heeps_oracle_speckle(const oracle_desc *d, int32_t p, double *out)
+{
+    if (!d || !out || p < 0 || p >= d->n_pulses || !d->xi) return -1;
+    const size_t F = (size_t)d->nx * d->ny;
+#pragma omp parallel for schedule(static)
+    for (long f = 0; f < (long)F; ++f) speckle_at(d, (size_t)f, p, out + 2 * f, out + 2 * f + 1);
     return 0;
 }
 
