@@ -88,6 +88,13 @@ typedef struct {
     double current_uniform[2];
     const float *xi;               /* [ny][nx][2] host complex speckle, or NULL -> derived from seed (G14) */
     uint64_t seed;
+    /* Time-dependent intra-facet speckle.  speckle_tau_s > 0: the speckle of
+     * facet f at pulse p is s_f(t_p) = [R + i I](t_p) exp(2 i pi f_s t_p) (eq. 7) with the order-1 autoregressive model of
+     * eq. (10), R(t + dt) = beta R(t) + sqrt(1 - beta^2) R', beta = exp(-dt/tau_s), stepped pulse by pulse from xi_f at
+     * pulse 0; the innovations R' + i I' (variance 1/2 per part) come from Philox4x32-10 keyed by `seed`, counter
+     * (f lo, f hi, pulse, 1), Box-Muller (reading G27).  speckle_tau_s <= 0 (default): xi_f constant over the dwell. */
+    double speckle_tau_s;
+    double speckle_doppler_hz;     /* f_s of eq. (7) */
 } sim_scene;
 
 /* Echo accumulation.  Both evaluate the same defined sum:

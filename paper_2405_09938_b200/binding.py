@@ -57,6 +57,7 @@ class sim_scene(C.Structure):
         ("tilt_modulation", C.c_int32), ("look_dir", C.c_double * 2),
         ("current_mps", C.c_void_p), ("current_uniform", C.c_double * 2),
         ("xi", C.c_void_p), ("seed", C.c_uint64),
+        ("speckle_tau_s", C.c_double), ("speckle_doppler_hz", C.c_double),
     ]
 
 
@@ -214,6 +215,8 @@ def _marshal(workload):
             raise ValueError("xi must be [ny][nx][2]")
         cs.xi = ptr(a)
     cs.seed = int(sc.get("seed", 0))
+    cs.speckle_tau_s = float(sc.get("speckle_tau_s", 0.0))
+    cs.speckle_doppler_hz = float(sc.get("speckle_doppler_hz", 0.0))
     return ci, cg, cs, keep
 
 

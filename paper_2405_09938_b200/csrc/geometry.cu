@@ -102,8 +102,13 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
                 sig *= fmaxf(fac, 0.f);
             }
             a0 = sqrtf(sig * area);
-            xi = __ldg(a.xi + f);
-            { uint2 xp = __ldg(a.xi_polar + f); xi_mag = __uint_as_float(xp.x); xi_arg = xp.y; }
+            { uint2 xp = __ldg(a.xi_polar + (size_t)pl * a.xi_pulse_stride + f); xi_mag = __uint_as_float(xp.x); xi_arg = xp.y; }
+            if (!a.xi_pulse_stride) xi = __ldg(a.xi + f);
+            else if (a.dbg_amp) {                            // time-dependent speckle: the complex value for the report
+                double sn, cs;
+                sincospi(2.0 * (double)xi_arg * 2.3283064365386963e-10, &sn, &cs);
+                xi = make_float2((float)(xi_mag * cs), (float)(xi_mag * sn));
+            }
             if (kDebug) {
                 if (a.dbg_pos) { a.dbg_pos[3 * f] = pos[0]; a.dbg_pos[3 * f + 1] = pos[1]; a.dbg_pos[3 * f + 2] = pos[2]; }
                 if (a.dbg_gtx) a.dbg_gtx[f] = gt;

@@ -33,7 +33,8 @@ struct GeometryArgs {
     const float *sigma0;        // [F] or null
     const float2 *current;      // [F] or null
     const float2 *xi;           // [F]   complex speckle (debug outputs only)
-    const uint2 *xi_polar;      // [F]   {|xi| as float bits, arg(xi) in 2^-32 turns}
+    const uint2 *xi_polar;      // [F]   {|xi| as float bits, arg(xi) in 2^-32 turns}; [n_pl][F] with xi_pulse_stride = F
+    int64_t xi_pulse_stride;    // 0: static speckle; F: time-dependent speckle, one row per pulse of the batch
     Rec *recs;                  // [C][n_pl][n_tiles][tile_cap]
     TileInfo *tinfo;            // [n_pl][n_tiles]
     TileSpan *tspan;            // [C][n_pl][n_tiles]
@@ -82,6 +83,20 @@ cudaError_t launch_speckle_from_seed(float2 *xi, int64_t n_facets, uint64_t seed
 // xi -> {|xi|, arg(xi)} so that K2 can fold the speckle phase into the fixed-point phase word.
 cudaError_t launch_speckle_polar(const float2 *xi, uint2 *xi_polar, int64_t n_facets, cudaStream_t s);
 
+// Time-dependent speckle (speckle.cu; eq. (7), (10)): polar speckle of every facet at
+// every pulse of a batch.
+struct SpeckleAr1Args {
+    const float2 *xi;              // [F]  R(0) + i I(0)
+    float2 *state;                 // [F]  AR(1) state: read when `resume` (state after pulse p0 - 1), written on exit
+    uint2 *polar;                  // [n_pl][F]  {|s|, arg s in 2^-32 turns} (Doppler factor included)
+    const float2 *beta_g;          // [P]  {beta_q, sqrt(1 - beta_q^2)}, beta_q = exp(-(t_q - t_{q-1}) / tau_s); [0] unused
+    const uint32_t *doppler_turns; // [P]  frac(f_s t_p) in 2^-32 turns
+    int64_t n_facets;
+    uint64_t seed;
+    int32_t p0, n_pl, resume;
+};
+cudaError_t launch_speckle_ar1(const SpeckleAr1Args &a, cudaStream_t s);
+
 // ---- spectral path (moments.cu, fftconv.cu) ----
 constexpr int kMomentOrder = 8;   // Kt Chebyshev moments per range slice (truncation ~ J_8(pi B / 2 fs) ~ 1e-6)
 
@@ -91,7 +106,8 @@ struct MomentArgs {
     SurfaceArgs surf;           // from K1
     const float *sigma0;        // [F] or null
     const float2 *current;      // [F] or null
-    const uint2 *xi_polar;      // [F]
+    const uint2 *xi_polar;      // [F], or [n_pl][F] with xi_pulse_stride = F (time-dependent speckle)
+    int64_t xi_pulse_stride;
     float2 *mom;                // [C][n_pl][Kt][nb_pad] complex moments, slice b at index b + L - 1 (zeroed by the caller)
     int32_t nb_pad;             // row stride (>= Ns + L - 1)
     int32_t span_cap;           // slices of a tile's shared-memory window

@@ -115,7 +115,7 @@ moments_kernel(DevParams prm, MomentArgs a, int p0, int n_pl)
                 const float2 sl = surface_slope(a.surf, it, F, f);
                 sig *= fmaxf(1.f + 2.f * (sl.x * (float)prm.look_x + sl.y * (float)prm.look_y), 0.f);
             }
-            const uint2 xp = __ldg(a.xi_polar + f);
+            const uint2 xp = __ldg(a.xi_polar + (size_t)pl * a.xi_pulse_stride + f);
             amag[q] = sqrtf(sig * area) * __uint_as_float(xp.x);           // |a_f| (O8)
             xarg[q] = xp.y;
             if (keep[q]) ++my_kept;

@@ -110,7 +110,7 @@ __device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b)
 
 __device__ __forceinline__ float pattern_x(float xa, float xe) { return sinc_pi_fast(xa) * sinc_pi_fast(xe); }
 
-template <int FPT, int C, bool kTilt>
+template <int FPT, int C, bool kTilt, bool kSpeckleT>
 __global__ void __launch_bounds__(kThreads, 2)
 moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_first)
 {
@@ -256,9 +256,9 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         bq[q] = gtm * (gom - grm) * inv_ofd;
         // amplitude (O8): sqrt(sigma0 tilt d^2) |xi|
         const float sig = a.sigma0 ? __ldg(a.sigma0 + f) : (float)prm.sigma0_uniform;
-        const uint2 xp = __ldg(a.xi_polar + f);
-        const float xmag = __uint_as_float(xp.x);
-        xarg[q] = xp.y;
+        // static speckle: |xi| and arg xi are constants of the facet; time-dependent speckle (speckle.cu): per pulse
+        float xmag = 1.f;
+        if (!kSpeckleT) { const uint2 xp = __ldg(a.xi_polar + f); xmag = __uint_as_float(xp.x); xarg[q] = xp.y; }
         if (kTilt) {
             const float2 sl0 = a.surf.slope[row0 + f], sl1 = a.surf.slope[row1 + f];
             const float smx = 0.5f * (sl0.x + sl1.x), smy = 0.5f * (sl0.y + sl1.y);   // slopes are linear between keyframes
@@ -306,7 +306,14 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
             const float Pv = fmaf(s, fmaf(s, pqb[q], pqa[q]), pq0[q]);
             const bool keep = valid[q] && !(fabsf(Pv) < prm.cull_thr);     // O7 (G6)
             my_kept += keep ? 1 : 0;
-            const float am = kTilt ? fmaf(s, fmaf(s, amb[q], ama[q]), am0[q]) : am0[q];
+            float am = kTilt ? fmaf(s, fmaf(s, amb[q], ama[q]), am0[q]) : am0[q];
+            uint32_t xa = xarg[q];
+            if (kSpeckleT && valid[q]) {                  // time-dependent speckle: s_f(t_p) of this pulse (eq. (7), (10))
+                const int kk = q * kThreads + tid;
+                const uint2 xp = __ldg(a.xi_polar + (size_t)pl * a.xi_pulse_stride +
+                                       (size_t)(tj0 + (kk >> lts)) * prm.nx + (ti0 + (kk & (ts - 1))));
+                am *= __uint_as_float(xp.x); xa = xp.y;
+            }
             const double R = fma(kp.sd, RD[q], R0[q]) + (double)fmaf(kp.u0, ra[q], kp.u1 * rb[q]);
             const double dRref = R - kp.r0;
             const float la = fmaf(s, dla[q], la0[q]);
@@ -322,7 +329,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                 const float g = fmaf(och[c], bq[q], Pv);
                 const uint32_t ph = (uint32_t)(unsigned long long)__double2ll_rn(
                                         fma(-dR, il32, (double)(kappa32 * eps * eps))) +
-                                    xarg[q] + ((g < 0.f) ? 0x80000000u : 0u);
+                                    xa + ((g < 0.f) ? 0x80000000u : 0u);
                 float sn, cs;
                 __sincosf((float)(int32_t)ph * 1.4629180792671596e-9f, &sn, &cs);   // 2 pi / 2^32
                 const float mag = fabsf(g) * am;
@@ -477,7 +484,9 @@ cudaError_t launch_fc(const DevParams &prm, const MomentArgs &a, int p0, int n_p
         kern<<<grid, kThreads, smem, s>>>(prm, a, p0, n_pl, j_first);
         return cudaGetLastError();
     };
-    return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true>) : go(moments_keyframed_kernel<FPT, C, false>);
+    if (a.xi_pulse_stride)
+        return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, true>) : go(moments_keyframed_kernel<FPT, C, false, true>);
+    return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, false>) : go(moments_keyframed_kernel<FPT, C, false, false>);
 }
 
 template <int FPT>

@@ -65,6 +65,13 @@ struct sim_handle {
     DevBuf<float> sigma0;
     DevBuf<float2> current, xi;
     DevBuf<uint2> xi_polar;              // {|xi|, arg xi in 2^-32 turns}, derived from xi on the device
+    // time-dependent speckle (speckle.cu; sim_scene.speckle_tau_s > 0)
+    bool speckle_ar1 = false;
+    uint64_t seed = 0;
+    DevBuf<float2> xi_state, beta_g;     // AR(1) state after pulse xi_state_pulse; per-pulse {beta, sqrt(1 - beta^2)}
+    DevBuf<uint32_t> doppler_turns;      // frac(f_s t_p) in 2^-32 turns
+    DevBuf<uint2> xi_t;                  // [pulses_per_batch][F] polar speckle of the batch
+    int xi_state_pulse = -1;
     // workspace
     DevBuf<double> z, zt, omega;
     DevBuf<float2> slope;
@@ -172,6 +179,9 @@ int validate(const sim_instrument *in, const sim_geometry *g, const sim_scene *s
     }
     if (!sc->sigma0_lin && !(sc->sigma0_uniform >= 0 && std::isfinite(sc->sigma0_uniform))) return SIM_EINVAL;
     if (!finite_all(sc->look_dir, 2) || !finite_all(sc->current_uniform, 2)) return SIM_EINVAL;
+    if (!std::isfinite(sc->speckle_tau_s) || !std::isfinite(sc->speckle_doppler_hz)) return SIM_EINVAL;
+    if (sc->speckle_tau_s > 0)
+        for (int p = 0; p + 1 < g->n_pulses; ++p) if (!(g->t_pulse_s[p + 1] >= g->t_pulse_s[p])) return SIM_EINVAL;
     return SIM_OK;
 }
 
@@ -213,6 +223,23 @@ void surface_rows(const sim_handle *h, int p0, int n_pl, int *first, int *rows)
 struct SurfBufs {
     double *z, *zt; float2 *slope; double2 *dxy, *dxy_t;
 };
+
+// Time-dependent speckle of the batch (speckle.cu): fills h->xi_t and returns the pointer / row stride the K2 kernels use.
+int run_speckle(sim_handle *h, int p0, int n_pl, cudaStream_t s, const uint2 **polar, int64_t *stride)
+{
+    *polar = h->xi_polar.p; *stride = 0;
+    if (!h->speckle_ar1) return SIM_OK;
+    SpeckleAr1Args a{};
+    a.xi = h->xi.p; a.state = h->xi_state.p; a.polar = h->xi_t.p; a.beta_g = h->beta_g.p;
+    a.doppler_turns = h->doppler_turns.p; a.n_facets = h->n_facets; a.seed = h->seed;
+    a.p0 = p0; a.n_pl = n_pl;
+    a.resume = (p0 > 0 && h->xi_state_pulse == p0 - 1) ? 1 : 0;
+    cudaError_t e = launch_speckle_ar1(a, s);
+    if (e != cudaSuccess) return fail_cuda(h, e, "launch_speckle_ar1");
+    h->xi_state_pulse = p0 + n_pl - 1;
+    *polar = h->xi_t.p; *stride = h->n_facets;
+    return SIM_OK;
+}
 
 // K1 for the batch; fills `sa` for K2.
 int run_kinematics(sim_handle *h, const SurfBufs &b, int p0, int n_pl, cudaStream_t s, SurfaceArgs *sa)
@@ -386,6 +413,7 @@ void sim_destroy(sim_handle *h)
     h->xt.release(); h->yt.release(); h->tt.release(); h->chirp_n.release(); h->carrier_p.release();
     h->wk.release(); h->carrier_frac.release(); h->pulses.release();
     h->sigma0.release(); h->current.release(); h->xi.release(); h->xi_polar.release();
+    h->xi_state.release(); h->beta_g.release(); h->doppler_turns.release(); h->xi_t.release();
     h->z.release(); h->slope.release(); h->dxy.release();
     h->zt.release(); h->dxy_t.release(); h->omega.release(); h->recs.release(); h->tinfo.release();
     h->tspan.release(); h->acc.release(); h->counters.release(); h->out_staging.release();
@@ -511,7 +539,9 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     const int64_t surf_row = h->n_facets * 8 + (h->need_slope ? h->n_facets * 8 : 0) +
                              (prm.choppy ? h->n_facets * 16 : 0);
     const int64_t per_pulse_common = h->key_H > 1 ? 2 * surf_row / h->key_H + 1 : surf_row;
-    const int64_t per_pulse = per_pulse_common +
+    h->speckle_ar1 = sc->speckle_tau_s > 0;
+    h->seed = sc->seed;
+    const int64_t per_pulse = per_pulse_common + (h->speckle_ar1 ? h->n_facets * 8 : 0) +
         (h->spectral ? (int64_t)C * kMomentOrder * h->nb_pad * 8
                      : (int64_t)C * fcap * (int64_t)sizeof(Rec) + (int64_t)C * Ns * 16 +
                            (int64_t)prm.n_tiles * (4 + 16 * C));
@@ -620,6 +650,21 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     }
     CKC(h->xi_polar.alloc(F));
     CKC(launch_speckle_polar(h->xi.p, h->xi_polar.p, (int64_t)F, nullptr));
+    if (h->speckle_ar1) {
+        std::vector<float2> bg(P);
+        std::vector<uint32_t> dop(P);
+        for (int p = 0; p < P; ++p) {
+            const double beta = p ? std::exp(-(g->t_pulse_s[p] - g->t_pulse_s[p - 1]) / sc->speckle_tau_s) : 1.0;
+            bg[p] = make_float2((float)beta, (float)std::sqrt(std::max(0.0, 1.0 - beta * beta)));
+            const long double turns = (long double)sc->speckle_doppler_hz * (long double)g->t_pulse_s[p];
+            const long double fr = turns - floorl(turns);
+            dop[p] = (uint32_t)(unsigned long long)(fr * 4294967296.0L + 0.5L);
+        }
+        CKC(h->beta_g.alloc(P)); CKC(h->doppler_turns.alloc(P)); CKC(h->xi_state.alloc(F));
+        CKC(h->xi_t.alloc(F * (size_t)pb));
+        CKC(cudaMemcpy(h->beta_g.p, bg.data(), (size_t)P * sizeof(float2), cudaMemcpyHostToDevice));
+        CKC(cudaMemcpy(h->doppler_turns.p, dop.data(), (size_t)P * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    }
     CKC(cudaDeviceSynchronize());
     {
         const size_t rows = h->key_H > 1 ? (size_t)(pb / h->key_H + 3) : (size_t)pb;
@@ -740,7 +785,8 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         { int rc = run_kinematics(h, bufs, p0, n_pl, s, &ma.surf); if (rc != SIM_OK) return rc; }
         CK(h, mark());
         ma.pulses = h->pulses.p;
-        ma.sigma0 = h->sigma0.p; ma.current = h->current.p; ma.xi_polar = h->xi_polar.p;
+        ma.sigma0 = h->sigma0.p; ma.current = h->current.p;
+        { int rc = run_speckle(h, p0, n_pl, s, &ma.xi_polar, &ma.xi_pulse_stride); if (rc != SIM_OK) return rc; }
         ma.mom = h->mom.p; ma.nb_pad = h->nb_pad; ma.span_cap = h->span_cap_m; ma.replica = h->replica;
         ma.counters = h->counters.p;
         if (h->geo_keyframed) CK(h, launch_moments_keyframed(prm, ma, p0, n_pl, s));
@@ -764,7 +810,8 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         { int rc = run_kinematics(h, bufs, p0, n_pl, s, &ga.surf); if (rc != SIM_OK) return rc; }
         CK(h, mark());
         ga.pulses = h->pulses.p;
-        ga.sigma0 = h->sigma0.p; ga.current = h->current.p; ga.xi = h->xi.p; ga.xi_polar = h->xi_polar.p;
+        ga.sigma0 = h->sigma0.p; ga.current = h->current.p; ga.xi = h->xi.p;
+        { int rc = run_speckle(h, p0, n_pl, s, &ga.xi_polar, &ga.xi_pulse_stride); if (rc != SIM_OK) return rc; }
         ga.recs = h->recs.p; ga.tinfo = h->tinfo.p; ga.tspan = h->tspan.p; ga.counters = h->counters.p;
         ga.carrier_frac_t0 = h->carrier_frac.p;
         CK(h, launch_geometry(prm, ga, p0, n_pl, s));
@@ -805,11 +852,9 @@ int sim_generate_host(sim_handle *h, int32_t pulse_begin, int32_t pulse_end, voi
     const size_t n = (size_t)h->prm.n_channels * (pulse_end - pulse_begin) * h->prm.n_samples;
     if (h->out_staging.n < n) CK(h, h->out_staging.alloc(n));
     if (!h->copy_stream) CK(h, cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
-    // about four batches per call (whole keyframe intervals), so that the copy of one overlaps the kernels of the next
-    const int n = pulse_end - pulse_begin, H = std::max(1, h->key_H);
-    int batch = std::max((n + 3) / 4, std::min(n, 32));
-    batch = ((batch + H - 1) / H) * H;
-    int rc = run_batches(h, pulse_begin, pulse_end, h->out_staging.p, s, batch, static_cast<float2 *>(iq_host));
+    // the workspace-sized batches of the call are shipped as they finish (splitting a dwell that fits one batch
+    // costs more in K1 / K2k efficiency than the overlapped copy returns: measured on ATI)
+    int rc = run_batches(h, pulse_begin, pulse_end, h->out_staging.p, s, 0, static_cast<float2 *>(iq_host));
     if (rc != SIM_OK) return rc;
     CK(h, cudaStreamSynchronize(h->copy_stream));
     CK(h, cudaStreamSynchronize(s));
@@ -829,6 +874,7 @@ int sim_update_scene(sim_handle *h, const float *sigma0_lin, const float *curren
     if (xi) {
         CK(h, cudaMemcpyAsync(h->xi.p, xi, F * sizeof(float2), cudaMemcpyHostToDevice, s));
         CK(h, launch_speckle_polar(h->xi.p, h->xi_polar.p, (int64_t)F, s));
+        h->xi_state_pulse = -1;                          // the cached AR(1) state started from the old xi
     }
     return SIM_OK;
 }
@@ -887,7 +933,8 @@ int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, d
         CK(h, d_slope_out.alloc(F));
         CK(h, launch_surface_slope(prm, ga.surf, h->pulses.p, pulse, d_slope_out.p, nullptr));
         if (!h->need_slope) ga.surf.slope = nullptr;
-        ga.sigma0 = h->sigma0.p; ga.current = h->current.p; ga.xi = h->xi.p; ga.xi_polar = h->xi_polar.p;
+        ga.sigma0 = h->sigma0.p; ga.current = h->current.p; ga.xi = h->xi.p;
+        { int rc2 = run_speckle(h, pulse, 1, nullptr, &ga.xi_polar, &ga.xi_pulse_stride); if (rc2 != SIM_OK) return rc2; }
         ga.recs = recs; ga.tinfo = tinfo; ga.tspan = tspan; ga.counters = nullptr;
         ga.dbg_pos = d_pos.p; ga.dbg_tau = d_tau.p; ga.dbg_gtx = d_gtx.p; ga.dbg_grx = d_grx.p;
         ga.dbg_amp = d_amp.p; ga.dbg_keep = d_keep.p; ga.carrier_frac_t0 = h->carrier_frac.p;

@@ -158,6 +158,41 @@ def test_geometry_keyframes_guard_rejects_rough_state_vectors():
     _assert_parity(got, ref, "jittered state vectors")
 
 
+# ----------------------------------------------------------------------------- NEXT-1: time-dependent speckle
+
+def _with_ar1_speckle(w, tau=4e-3, doppler=35.0, seed=0x1234567_89ABCDEF):
+    w.scene["speckle_tau_s"], w.scene["speckle_doppler_hz"], w.scene["seed"] = tau, doppler, seed
+    return w
+
+
+def test_time_dependent_speckle(mode):
+    """AR(1) intra-facet speckle with Doppler factor (eq. (7), (10); speckle.cu) against the oracle's own
+    implementation of the same recursion and generator: Tiny in full; pulse sub-ranges (replay from pulse 0 and
+    resume from the cached state give the same samples); batches; a 3-channel scene with tilt and current map."""
+    w = _with_ar1_speckle(make_workload("tiny"))
+    ref = oracle_generate(w)
+    assert rel_l2_per_vector(ref[:, 8:], oracle_generate(make_workload("tiny"))[:, 8:]).min() > 0.5   # it does decorrelate
+    for opts in ({}, {"pulses_per_batch": 5}, {"kinematics_keyframe": 1}, {"geometry_keyframe": 1}):
+        with _sim(w, accumulate_mode=mode, **opts) as sim:
+            got = sim.generate().cpu().numpy()
+            late = sim.generate(20, 27).cpu().numpy()          # not consecutive with the previous call: replay
+            cont = sim.generate(27, 32).cpu().numpy()          # consecutive: resumes from the cached state
+        _assert_parity(got, ref, f"ar1 speckle {opts}")
+        _assert_parity(late, ref[:, 20:27], "ar1 speckle replay")
+        _assert_parity(cont, ref[:, 27:32], "ar1 speckle resume")
+    wh = _with_ar1_speckle(_hetero_small(96, 64, 11), tau=2e-3, doppler=-60.0, seed=99)
+    _assert_parity(_gpu(wh, accumulate_mode=mode), oracle_generate(wh), "ar1 speckle hetero_small")
+
+
+def test_time_dependent_speckle_facet_amplitudes():
+    """sim_debug_facets reports the complex amplitude with the speckle of that pulse."""
+    w = _with_ar1_speckle(make_workload("tiny", n_pulses=9))
+    with _sim(w) as sim:
+        g = sim.debug_facets(7)
+    o = oracle_facets(w, 7)
+    assert np.max(np.abs(g["amp"] - o["amp"])) < 1e-5 * np.abs(o["amp"]).max()
+
+
 # ----------------------------------------------------------------------------- per-kernel unit parity (T1)
 
 @pytest.mark.parametrize("name", ["tiny", "hetero_small"])
