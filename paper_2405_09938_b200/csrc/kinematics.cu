@@ -7,7 +7,8 @@
 // instead of a sincos; fp64 because the height feeds the carrier phase (1 mrad = 8.8 um of path,
 // SURVEY.md §7 hard part 2).  Slopes only scale sigma0 and stay fp32.
 //
-// Layout: block = 64 (i) x 4 (j) facets x kPK consecutive rows (pulses or keyframes).  A thread owns one facet:
+// Layout: block = 64 (i) x 8 (j) facets x up to kPK consecutive rows (pulses or keyframes).  A thread owns two facets
+// of the same column i (they share X[w][i] and every shared-memory table load); per facet:
 // per wave component it forms c = X[w][i] * Y[w][j] once (X read coalesced from L2, Y from shared memory) and
 // then runs over the kPK rows, multiplying by T[w][p] from shared memory (broadcast).  Only the HEIGHT (and the
 // CWM displacement) is accumulated in fp64 -- 2 DFMA per facet-component-row; the time derivative and the slopes
@@ -30,14 +31,15 @@ namespace heeps {
 namespace {
 
 constexpr int kBX = 64, kBY = 4;
-constexpr int kPK = 8;        // most rows per thread (the kernel is instantiated for 4..8)
+constexpr int kPK = 6;        // most rows per thread (the kernel is instantiated for 4..6; 2 x 6 rows of accumulators = 128 registers)
 constexpr int kWCh = 128;     // wave components per shared-memory chunk
+constexpr int kNF = 2;        // facets per thread (same i, rows kBY apart): they share X[w][i] and the T-table loads
 
 template <int NK, bool kSlope, bool kChoppy, bool kRate>
 __global__ void __launch_bounds__(kBX * kBY)
 kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
 {
-    __shared__ double2 s_y[kBY][kWCh];
+    __shared__ double2 s_y[kBY * kNF][kWCh];
     __shared__ double2 s_t[kWCh][NK];
     __shared__ float2 s_tf[kWCh][NK];
     __shared__ float4 s_wk[kWCh];
@@ -46,25 +48,29 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
     const int nw = prm.n_waves;
     const int row0 = blockIdx.z * NK;                  // first output row of this block
     const int nk = min(NK, n_rows - row0);             // rows this block stores (the last block recomputes its last row)
-    const int j0 = blockIdx.y * kBY;
+    const int j0 = blockIdx.y * (kBY * kNF);
     const int tid = threadIdx.y * kBX + threadIdx.x;
     const int i = blockIdx.x * kBX + threadIdx.x;
-    const int j = j0 + threadIdx.y;
-    const bool valid = i < prm.nx && j < prm.ny;
-
-    double z[NK], dx[NK], dy[NK];
-    float zt[NK], dxt[NK], dyt[NK];
-    float2 sxy[NK];
+    // facet u of the thread: (i, j0 + threadIdx.y + u kBY); both share X[w][i] and every T-table load
+    bool valid[kNF];
 #pragma unroll
-    for (int k = 0; k < NK; ++k) {
-        z[k] = dx[k] = dy[k] = 0.0;
-        zt[k] = dxt[k] = dyt[k] = 0.f; sxy[k] = make_float2(0.f, 0.f);
-    }
+    for (int u = 0; u < kNF; ++u) valid[u] = i < prm.nx && j0 + threadIdx.y + u * kBY < prm.ny;
+
+    double z[kNF][NK], dx[kNF][NK], dy[kNF][NK];
+    float zt[kNF][NK], dxt[kNF][NK], dyt[kNF][NK];
+    float2 sxy[kNF][NK];
+#pragma unroll
+    for (int u = 0; u < kNF; ++u)
+#pragma unroll
+        for (int k = 0; k < NK; ++k) {
+            z[u][k] = dx[u][k] = dy[u][k] = 0.0;
+            zt[u][k] = dxt[u][k] = dyt[u][k] = 0.f; sxy[u][k] = make_float2(0.f, 0.f);
+        }
 
     for (int w0 = 0; w0 < nw; w0 += kWCh) {
         const int nwc = min(kWCh, nw - w0);
         __syncthreads();                               // the previous chunk's tables are no longer read
-        for (int idx = tid; idx < kBY * nwc; idx += kBX * kBY) {
+        for (int idx = tid; idx < kBY * kNF * nwc; idx += kBX * kBY) {
             const int r = idx / nwc, w = idx - r * nwc;
             s_y[r][w] = a.yt[(size_t)(w0 + w) * prm.ny + min(j0 + r, prm.ny - 1)];
         }
@@ -83,52 +89,66 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
                 s_om[w] = kRate ? (float)a.omega[w0 + w] : 0.f;
             }
         __syncthreads();
-        if (!valid) continue;
+        if (!valid[0]) continue;                       // valid[1] implies valid[0]
         const double2 *xt = a.xt + (size_t)w0 * prm.nx + i;
 #pragma unroll 2
         for (int w = 0; w < nwc; ++w) {
             const double2 x = __ldg(xt + (size_t)w * prm.nx);
-            const double2 y = s_y[threadIdx.y][w];
-            const double cr = fma(x.x, y.x, -x.y * y.y), ci = fma(x.x, y.y, x.y * y.x);   // A exp(j (kx x + ky y + phase))
-            float cfr = 0.f, cfi = 0.f, om = 0.f;
+            double cr[kNF], ci[kNF];
+            float cfr[kNF], cfi[kNF];
+#pragma unroll
+            for (int u = 0; u < kNF; ++u) {
+                const double2 y = s_y[threadIdx.y + u * kBY][w];
+                cr[u] = fma(x.x, y.x, -x.y * y.y); ci[u] = fma(x.x, y.y, x.y * y.x);   // A exp(j (kx x + ky y + phase))
+                cfr[u] = (float)cr[u]; cfi[u] = (float)ci[u];
+            }
+            float om = 0.f;
             float4 k4 = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (kSlope || kChoppy || kRate) { cfr = (float)cr; cfi = (float)ci; k4 = s_wk[w]; om = s_om[w]; }
+            if (kSlope || kChoppy || kRate) { k4 = s_wk[w]; om = s_om[w]; }
             const float2 nk2 = make_float2(-k4.x, -k4.y);
 #pragma unroll
             for (int k = 0; k < NK; ++k) {
                 const double2 t = s_t[w][k];
-                z[k] = fma(cr, t.x, z[k]);                                // A cos(psi)
-                z[k] = fma(-ci, t.y, z[k]);
-                if (kChoppy) {
-                    const double im = fma(cr, t.y, ci * t.x);            // A sin(psi)
-                    dx[k] = fma(-(double)k4.z, im, dx[k]);               // D_h = -sum A k^ sin(psi)
-                    dy[k] = fma(-(double)k4.w, im, dy[k]);
-                }
-                if (kSlope || kRate) {
-                    const float2 tf = s_tf[w][k];
-                    const float imf = fmaf(cfr, tf.y, cfi * tf.x);
-                    if (kRate) zt[k] = fmaf(om, imf, zt[k]);              // d/dt A cos(psi) = A omega sin(psi)
-                    if (kSlope) sxy[k] = __ffma2_rn(nk2, make_float2(imf, imf), sxy[k]);   // grad z = -sum A k sin(psi)
-                    if (kChoppy && kRate) {
-                        const float wre = om * fmaf(cfr, tf.x, -cfi * tf.y);          // omega A cos(psi)
-                        dxt[k] = fmaf(k4.z, wre, dxt[k]); dyt[k] = fmaf(k4.w, wre, dyt[k]);
+                float2 tf = make_float2(0.f, 0.f);
+                if (kSlope || kRate) tf = s_tf[w][k];
+#pragma unroll
+                for (int u = 0; u < kNF; ++u) {
+                    z[u][k] = fma(cr[u], t.x, z[u][k]);                   // A cos(psi)
+                    z[u][k] = fma(-ci[u], t.y, z[u][k]);
+                    if (kChoppy) {
+                        const double im = fma(cr[u], t.y, ci[u] * t.x);  // A sin(psi)
+                        dx[u][k] = fma(-(double)k4.z, im, dx[u][k]);     // D_h = -sum A k^ sin(psi)
+                        dy[u][k] = fma(-(double)k4.w, im, dy[u][k]);
+                    }
+                    if (kSlope || kRate) {
+                        const float imf = fmaf(cfr[u], tf.y, cfi[u] * tf.x);
+                        if (kRate) zt[u][k] = fmaf(om, imf, zt[u][k]);    // d/dt A cos(psi) = A omega sin(psi)
+                        if (kSlope) sxy[u][k] = __ffma2_rn(nk2, make_float2(imf, imf), sxy[u][k]);   // grad z = -sum A k sin(psi)
+                        if (kChoppy && kRate) {
+                            const float wre = om * fmaf(cfr[u], tf.x, -cfi[u] * tf.y);   // omega A cos(psi)
+                            dxt[u][k] = fmaf(k4.z, wre, dxt[u][k]); dyt[u][k] = fmaf(k4.w, wre, dyt[u][k]);
+                        }
                     }
                 }
             }
         }
     }
-    if (!valid) return;
     const size_t F = (size_t)prm.nx * prm.ny;
 #pragma unroll
-    for (int k = 0; k < NK; ++k) {
-        if (k >= nk) break;
-        const size_t f = (size_t)(row0 + k) * F + (size_t)j * prm.nx + i;
-        a.z[f] = z[k];
-        if (kSlope) a.slope[f] = sxy[k];
-        if (kChoppy) a.dxy[f] = make_double2(dx[k], dy[k]);
-        if (kRate) {
-            a.zt[f] = (double)zt[k];
-            if (kChoppy) a.dxy_t[f] = make_double2((double)dxt[k], (double)dyt[k]);
+    for (int u = 0; u < kNF; ++u) {
+        if (!valid[u]) continue;
+        const int j = j0 + threadIdx.y + u * kBY;
+#pragma unroll
+        for (int k = 0; k < NK; ++k) {
+            if (k >= nk) break;
+            const size_t f = (size_t)(row0 + k) * F + (size_t)j * prm.nx + i;
+            a.z[f] = z[u][k];
+            if (kSlope) a.slope[f] = sxy[u][k];
+            if (kChoppy) a.dxy[f] = make_double2(dx[u][k], dy[u][k]);
+            if (kRate) {
+                a.zt[f] = (double)zt[u][k];
+                if (kChoppy) a.dxy_t[f] = make_double2((double)dxt[u][k], (double)dyt[u][k]);
+            }
         }
     }
 }
@@ -161,7 +181,7 @@ cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a, int
     // rows split evenly over the fewest blocks of <= kPK rows (17 rows -> 6 + 6 + 5, not 8 + 8 + 1); at least 4 rows
     // per block (a shorter launch recomputes its last row)
     const int n_chunks = (n_rows + kPK - 1) / kPK, nk = std::max(4, (n_rows + n_chunks - 1) / n_chunks);
-    dim3 grid((prm.nx + kBX - 1) / kBX, (prm.ny + kBY - 1) / kBY, (n_rows + nk - 1) / nk);
+    dim3 grid((prm.nx + kBX - 1) / kBX, (prm.ny + kBY * kNF - 1) / (kBY * kNF), (n_rows + nk - 1) / nk);
     const bool slope = a.slope != nullptr, choppy = a.dxy != nullptr, rate = a.H > 1;
     auto launch = [&](auto kern) { kern<<<grid, block, 0, s>>>(prm, a, first, n_rows); };
     auto pick = [&](auto nk_tag) {
@@ -181,9 +201,7 @@ cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a, int
     switch (nk) {
         case 4: pick(std::integral_constant<int, 4>{}); break;
         case 5: pick(std::integral_constant<int, 5>{}); break;
-        case 6: pick(std::integral_constant<int, 6>{}); break;
-        case 7: pick(std::integral_constant<int, 7>{}); break;
-        default: pick(std::integral_constant<int, 8>{}); break;
+        default: pick(std::integral_constant<int, 6>{}); break;
     }
     return cudaGetLastError();
 }
