@@ -69,6 +69,28 @@ __device__ __forceinline__ void dft_regs(float2 (&v)[R])
 
 __device__ __forceinline__ int pad(int i) { return i + (i >> 4); }      // bank-conflict padding
 
+// Twiddles w^r, r = 1..R-1, of one radix-R butterfly with base twiddle index j * tstep.  For R = 16 only w is loaded
+// and the other fourteen are formed by complex products (w^2, w^4, w^8 by squaring): the FMA pipe idles while the L1 /
+// shared-memory data path is what binds the kernel (profiles/r1_v11_k3s: l1tex 76 %), and the first pass's twiddles
+// stride through the whole 64 KB table.  K3s 0.58 -> 0.36 ms on ATI; the angle error of w^8 is 8 roundings (~5e-7),
+// parity unchanged (3.7e-6).
+template <int R>
+__device__ __forceinline__ void load_twiddles(float2 (&w)[R], const float2 *__restrict__ tw, int j, int tstep)
+{
+    if (R == 16) {
+        w[1] = __ldg(tw + (size_t)j * tstep);
+        w[2] = cmul(w[1], w[1]);
+        w[4] = cmul(w[2], w[2]);
+        w[8] = cmul(w[4], w[4]);
+        w[3] = cmul(w[1], w[2]); w[5] = cmul(w[1], w[4]); w[6] = cmul(w[2], w[4]); w[7] = cmul(w[3], w[4]);
+#pragma unroll
+        for (int r = 9; r < 16; ++r) w[r < R ? r : 0] = cmul(w[(r - 8) < R ? (r - 8) : 0], w[8 < R ? 8 : 0]);
+    } else {
+#pragma unroll
+        for (int r = 1; r < R; ++r) w[r] = __ldg(tw + (size_t)(j * r) * tstep);
+    }
+}
+
 // One decimation-in-frequency pass: sub-transforms of size n_cur split into R of size n_cur / R.
 template <int NFFT, int R, int THREADS>
 __device__ __forceinline__ void fwd_pass(float2 *x, int n_cur, const float2 *__restrict__ tw)
@@ -81,10 +103,11 @@ __device__ __forceinline__ void fwd_pass(float2 *x, int n_cur, const float2 *__r
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = x[pad(base + q * s)];
         dft_regs<R>(v);
+        float2 w[R];
+        load_twiddles<R>(w, tw, j, tstep);
         x[pad(base)] = v[0];
 #pragma unroll
-        for (int r = 1; r < R; ++r)
-            x[pad(base + r * s)] = cmul(v[brev(r, bits)], __ldg(tw + (size_t)(j * r) * tstep));
+        for (int r = 1; r < R; ++r) x[pad(base + r * s)] = cmul(v[brev(r, bits)], w[r]);
     }
     __syncthreads();
 }
@@ -97,12 +120,13 @@ __device__ __forceinline__ void inv_pass(float2 *x, int n_cur, const float2 *__r
     const int s = n_cur / R, ls = 31 - __clz(s), tstep = NFFT / n_cur;
     for (int t = threadIdx.x; t < NFFT / R; t += THREADS) {
         const int j = t & (s - 1), base = (t >> ls) * n_cur + j;
-        float2 v[R];
+        float2 v[R], w[R];
+        load_twiddles<R>(w, tw, j, tstep);
         v[0] = x[pad(base)];
         v[0].y = -v[0].y;
 #pragma unroll
         for (int r = 1; r < R; ++r) {
-            const float2 u = cmulc(x[pad(base + r * s)], __ldg(tw + (size_t)(j * r) * tstep));
+            const float2 u = cmulc(x[pad(base + r * s)], w[r]);
             v[r] = make_float2(u.x, -u.y);                  // conj: IDFT(V) = conj(DFT(conj(V)))
         }
         dft_regs<R>(v);
