@@ -51,6 +51,9 @@ class _Desc(C.Structure):
         ("current_mps", C.c_void_p), ("current_uniform", C.c_double * 2),
         ("xi", C.c_void_p),
         ("speckle_tau_s", C.c_double), ("speckle_doppler_hz", C.c_double), ("seed", C.c_uint64),
+        ("wave_nodes_x", C.c_int32), ("wave_nodes_y", C.c_int32), ("wave_node_spacing_m", C.c_double),
+        ("node_kx", C.c_void_p), ("node_ky", C.c_void_p), ("node_amp", C.c_void_p), ("node_omega", C.c_void_p),
+        ("node_phase", C.c_void_p),
     ]
 
 
@@ -136,6 +139,13 @@ def _marshal(w):
     d.speckle_tau_s = float(sc.get("speckle_tau_s", 0.0))
     d.speckle_doppler_hz = float(sc.get("speckle_doppler_hz", 0.0))
     d.seed = int(sc.get("seed", 0))
+    if sc.get("wave_nodes") is not None:                      # heterogeneous surface
+        wn = sc["wave_nodes"]                                 # dict: spacing_m, kx/ky/amp/omega/phase [ny_n][nx_n][Nw]
+        shape = np.asarray(wn["kx"]).shape
+        d.wave_nodes_y, d.wave_nodes_x, d.n_waves = int(shape[0]), int(shape[1]), int(shape[2])
+        d.wave_node_spacing_m = float(wn["spacing_m"])
+        for k in ("kx", "ky", "amp", "omega", "phase"):
+            setattr(d, "node_" + k, ptr(_f64(wn[k], shape)))
     return d, keep
 
 

@@ -25,7 +25,8 @@
  * un-offset phase centre, G8 offsets along the Rx unit velocity, G9 stop-and-go,
  * G10 current by advection, G11 linear waves (CWM by flag), G12 tilt factor clamped at 0,
  * G15 A = d^2, G24 displaced point feeds the antenna direction, G27 the generator of the AR(1) speckle innovations
- * (NEXT-1, off unless speckle_tau_s > 0).
+ * (NEXT-1, off unless speckle_tau_s > 0), G28 blending of slopes and velocities on the heterogeneous surface (NEXT-2, off
+ * unless wave_nodes_x > 0).
  *
  * Pins: tests/test_oracle_pins.py (closed forms with mpmath, invariants, brute force by an
  * independent numpy script).  No function here is "parity unpinned".
@@ -67,6 +68,12 @@ typedef struct {
     double speckle_tau_s;                       /* tau_s; <= 0: speckle constant over the dwell (xi)  */
     double speckle_doppler_hz;                  /* f_s of eq. (7)                                      */
     uint64_t seed;                              /* key of the innovation generator (reading G27)       */
+    /* NEXT-2: heterogeneous surface, eq. (1), (2).  wave_nodes_x > 0: the wave tables
+     * above are ignored; node (a, b) of a lattice of step L whose node (0, 0) sits at the rest position of facet (0, 0)
+     * carries its own table of n_waves components -- the homogeneous tile T2L centred on that node. */
+    int32_t wave_nodes_x, wave_nodes_y;
+    double wave_node_spacing_m;                 /* L */
+    const double *node_kx, *node_ky, *node_amp, *node_omega, *node_phase;   /* [nodes_y][nodes_x][n_waves] */
 } oracle_desc;
 
 /* per-facet intermediates of one pulse (O2..O8), exposed for unit parity */
@@ -170,21 +177,50 @@ static void eval_facet(const oracle_desc *d, int p, int i, int j, facet_eval *o)
     /* O1 rest point */
     double xb = d->centre_m[0] + (i - (d->nx - 1) / 2.0) * d->spacing_m;
     double yb = d->centre_m[1] + (j - (d->ny - 1) / 2.0) * d->spacing_m;
-    /* O2 wave sums (linear surface, CWM horizontal displacement by flag) */
+    /* O2 wave sums (linear surface, CWM horizontal displacement by flag).
+     * Heterogeneous surface: the displacement at a rest point of the heterogeneous tile TL is the
+     * weighted sum of the displacements of the four homogeneous tiles T2L_i centred on TL's corners, eq. (1),
+     *     D_TL(x, t) = sum_{i=1..4} W^i(x) D^i_T2L(x, t),
+     * with the constant weights of eq. (2),  W^i = (1 - w_x - w_y + w_x w_y)^(1/2),  w_x = |x^i - x|/L, w_y = |y^i - y|/L
+     * (their squares add to one).  Reading G28: the same weights blend the facet slope and velocity (the gradient of
+     * W itself is not part of the facet orientation). */
     double z = 0, sx = 0, sy = 0, dx = 0, dy = 0, vx = 0, vy = 0, vz = 0;
-    for (int w = 0; w < d->n_waves; ++w) {
-        double k = hypot(d->kx[w], d->ky[w]);
-        double psi = d->kx[w] * xb + d->ky[w] * yb - d->omega[w] * t + d->phase[w];
-        double c = cos(psi), s = sin(psi), a = d->amp[w];
-        z  += a * c;
-        sx -= a * d->kx[w] * s;
-        sy -= a * d->ky[w] * s;
-        vz += a * d->omega[w] * s;
-        if (d->choppy && k > 0) {
-            dx -= a * d->kx[w] / k * s;
-            dy -= a * d->ky[w] / k * s;
-            vx += a * d->omega[w] * d->kx[w] / k * c;
-            vy += a * d->omega[w] * d->ky[w] / k * c;
+    const int hetero = d->wave_nodes_x > 0;
+    int na = 0, nb = 0;
+    double fx = 0, fy = 0;
+    if (hetero) {
+        const double L = d->wave_node_spacing_m;
+        const double ux = i * d->spacing_m / L, uy = j * d->spacing_m / L;     /* lattice coordinates of the rest point */
+        na = (int)floor(ux); nb = (int)floor(uy);
+        if (na > d->wave_nodes_x - 2) na = d->wave_nodes_x - 2;
+        if (nb > d->wave_nodes_y - 2) nb = d->wave_nodes_y - 2;
+        fx = ux - na; fy = uy - nb;
+    }
+    for (int corner = 0; corner < (hetero ? 4 : 1); ++corner) {
+        const double *kxs = d->kx, *kys = d->ky, *amps = d->amp, *oms = d->omega, *phs = d->phase;
+        double W = 1.0;
+        if (hetero) {
+            const int ca = corner & 1, cb = corner >> 1;
+            const double wx = ca ? 1.0 - fx : fx, wy = cb ? 1.0 - fy : fy;      /* |x^i - x|/L, |y^i - y|/L */
+            W = sqrt(1.0 - wx - wy + wx * wy);
+            const size_t node = ((size_t)(nb + cb) * d->wave_nodes_x + (na + ca)) * d->n_waves;
+            kxs = d->node_kx + node; kys = d->node_ky + node; amps = d->node_amp + node;
+            oms = d->node_omega + node; phs = d->node_phase + node;
+        }
+        for (int w = 0; w < d->n_waves; ++w) {
+            double k = hypot(kxs[w], kys[w]);
+            double psi = kxs[w] * xb + kys[w] * yb - oms[w] * t + phs[w];
+            double c = cos(psi), s = sin(psi), a = W * amps[w];
+            z  += a * c;
+            sx -= a * kxs[w] * s;
+            sy -= a * kys[w] * s;
+            vz += a * oms[w] * s;
+            if (d->choppy && k > 0) {
+                dx -= a * kxs[w] / k * s;
+                dy -= a * kys[w] / k * s;
+                vx += a * oms[w] * kxs[w] / k * c;
+                vy += a * oms[w] * kys[w] / k * c;
+            }
         }
     }
     double cx = d->current_uniform[0], cy = d->current_uniform[1];
