@@ -95,6 +95,15 @@ typedef struct {
      * (f lo, f hi, pulse, 1), Box-Muller (reading G27).  speckle_tau_s <= 0 (default): xi_f constant over the dwell. */
     double speckle_tau_s;
     double speckle_doppler_hz;     /* f_s of eq. (7) */
+    /* Heterogeneous surface.  wave_nodes_x > 0: kx..phase above are ignored; node
+     * (a, b) of a lattice of step wave_node_spacing_m (the tile size L), node (0, 0) at the rest position of facet (0, 0),
+     * carries its own table of n_waves components -- the homogeneous tile T2L centred on it.  The surface displacement,
+     * slope and velocity at a rest point are those of the four corner tiles of its lattice cell blended with the
+     * weights of eq. (2), W^i = sqrt((1 - |x^i - x|/L)(1 - |y^i - y|/L)) (eq. (1); reading G28).  The lattice must cover
+     * the grid: (nx-1) d <= (wave_nodes_x-1) L, likewise in y; at least 2 x 2 nodes. */
+    int32_t wave_nodes_x, wave_nodes_y;
+    double wave_node_spacing_m;
+    const double *node_kx, *node_ky, *node_amp, *node_omega, *node_phase;   /* [nodes_y][nodes_x][n_waves] host */
 } sim_scene;
 
 /* Echo accumulation.  Both evaluate the same defined sum:

@@ -202,7 +202,8 @@ static void eval_facet(const oracle_desc *d, int p, int i, int j, facet_eval *o)
         if (hetero) {
             const int ca = corner & 1, cb = corner >> 1;
             const double wx = ca ? 1.0 - fx : fx, wy = cb ? 1.0 - fy : fy;      /* |x^i - x|/L, |y^i - y|/L */
-            W = sqrt(1.0 - wx - wy + wx * wy);
+            const double W2 = 1.0 - wx - wy + wx * wy;                            /* eq. (2); = (1 - wx)(1 - wy) >= 0 */
+            W = W2 > 0.0 ? sqrt(W2) : 0.0;                                        /* rounding can leave -1e-17 at a far edge */
             const size_t node = ((size_t)(nb + cb) * d->wave_nodes_x + (na + ca)) * d->n_waves;
             kxs = d->node_kx + node; kys = d->node_ky + node; amps = d->node_amp + node;
             oms = d->node_omega + node; phs = d->node_phase + node;

@@ -58,6 +58,9 @@ class sim_scene(C.Structure):
         ("current_mps", C.c_void_p), ("current_uniform", C.c_double * 2),
         ("xi", C.c_void_p), ("seed", C.c_uint64),
         ("speckle_tau_s", C.c_double), ("speckle_doppler_hz", C.c_double),
+        ("wave_nodes_x", C.c_int32), ("wave_nodes_y", C.c_int32), ("wave_node_spacing_m", C.c_double),
+        ("node_kx", C.c_void_p), ("node_ky", C.c_void_p), ("node_amp", C.c_void_p), ("node_omega", C.c_void_p),
+        ("node_phase", C.c_void_p),
     ]
 
 
@@ -217,6 +220,13 @@ def _marshal(workload):
     cs.seed = int(sc.get("seed", 0))
     cs.speckle_tau_s = float(sc.get("speckle_tau_s", 0.0))
     cs.speckle_doppler_hz = float(sc.get("speckle_doppler_hz", 0.0))
+    if sc.get("wave_nodes") is not None:          # heterogeneous surface: dict(spacing_m, kx/ky/amp/omega/phase [ny_n][nx_n][Nw])
+        wn = sc["wave_nodes"]
+        shape = np.asarray(wn["kx"]).shape
+        cs.wave_nodes_y, cs.wave_nodes_x, cs.n_waves = int(shape[0]), int(shape[1]), int(shape[2])
+        cs.wave_node_spacing_m = float(wn["spacing_m"])
+        for k in ("kx", "ky", "amp", "omega", "phase"):
+            setattr(cs, "node_" + k, ptr(_f64(wn[k], shape)))
     return ci, cg, cs, keep
 
 

@@ -13,6 +13,12 @@ struct KinematicsArgs {
     const double2 *yt;      // [Nw][ny]  exp(j (ky_w y_j + phase_w))
     const double2 *tt;      // [Nw][P]   exp(-j omega_w t_p)
     const float4 *wk;       // [Nw]      {kx, ky, kx/|k|, ky/|k|}
+    // Heterogeneous surface (eq. (1), (2)): nodes_x > 0 -- every table above (and omega) carries a leading
+    // [nodes_y * nodes_x] dimension, one homogeneous tile T2L per node of a lattice of step node_spacing anchored at
+    // the rest position of facet (0, 0); a facet blends the four corner tiles of its cell with the weights of eq. (2).
+    int32_t nodes_x, nodes_y;
+    double node_spacing;
+    int32_t chunks_x, chunks_y;   // set by launch_kinematics: blocks per cell
     int32_t n_pulses_total; // P (row stride of tt)
     double *z;              // [n_pl][F]            surface height above centre_z
     float2 *slope;          // [n_pl][F] or null    grad z

@@ -35,7 +35,10 @@ constexpr int kPK = 6;        // most rows per thread (the kernel is instantiate
 constexpr int kWCh = 128;     // wave components per shared-memory chunk
 constexpr int kNF = 2;        // facets per thread (same i, rows kBY apart): they share X[w][i] and the T-table loads
 
-template <int NK, bool kSlope, bool kChoppy, bool kRate>
+// square of the weight of eq. (2), in the paper's expanded form: w_x = |x^i - x|/L, w_y = |y^i - y|/L
+__device__ __forceinline__ double weight2(double wx, double wy) { return __dadd_rn(__dadd_rn(1.0 - wx, -wy), __dmul_rn(wx, wy)); }
+
+template <int NK, bool kSlope, bool kChoppy, bool kRate, bool kHetero>
 __global__ void __launch_bounds__(kBX * kBY)
 kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
 {
@@ -48,13 +51,46 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
     const int nw = prm.n_waves;
     const int row0 = blockIdx.z * NK;                  // first output row of this block
     const int nk = min(NK, n_rows - row0);             // rows this block stores (the last block recomputes its last row)
-    const int j0 = blockIdx.y * (kBY * kNF);
     const int tid = threadIdx.y * kBX + threadIdx.x;
-    const int i = blockIdx.x * kBX + threadIdx.x;
+    // Heterogeneous surface: a block stays inside one cell TL of the node lattice, so that its four
+    // corner tiles T2L are the same for all its facets.  Homogeneous surface: one cell, one "corner" of weight 1.
+    constexpr bool hetero = kHetero;
+    int cell_a = 0, cell_b = 0, i_lo = 0, i_hi = prm.nx, j_lo = 0, j_hi = prm.ny;
+    int bx = blockIdx.x, by = blockIdx.y;
+    if (hetero) {
+        cell_a = blockIdx.x / a.chunks_x; bx = blockIdx.x - cell_a * a.chunks_x;
+        cell_b = blockIdx.y / a.chunks_y; by = blockIdx.y - cell_b * a.chunks_y;
+        // facet i belongs to cell floor((i d) / L), in exactly this arithmetic (the weights of eq. (2) have an infinite
+        // slope at the far edge of a cell: a facet that rounding puts on the other side of a node line would see a
+        // weight of 1e-8 instead of 0).  first(a) = the smallest index whose cell is >= a.
+        const double d = prm.spacing, L = a.node_spacing;
+        auto first = [&](int cell, int n) {
+            int k = min(n, max(0, (int)ceil(cell * (L / d))));
+            while (k > 0 && floor(((k - 1) * d) / L) >= (double)cell) --k;
+            while (k < n && floor((k * d) / L) < (double)cell) ++k;
+            return k;
+        };
+        i_lo = first(cell_a, prm.nx); j_lo = first(cell_b, prm.ny);
+        if (cell_a < a.nodes_x - 2) i_hi = first(cell_a + 1, prm.nx);
+        if (cell_b < a.nodes_y - 2) j_hi = first(cell_b + 1, prm.ny);
+    }
+    const int j0 = j_lo + by * (kBY * kNF);
+    const int i = i_lo + bx * kBX + threadIdx.x;
+    if (i_lo + bx * kBX >= i_hi || j0 >= j_hi) return;     // block-uniform: this chunk of the cell holds no facet
     // facet u of the thread: (i, j0 + threadIdx.y + u kBY); both share X[w][i] and every T-table load
     bool valid[kNF];
 #pragma unroll
-    for (int u = 0; u < kNF; ++u) valid[u] = i < prm.nx && j0 + threadIdx.y + u * kBY < prm.ny;
+    for (int u = 0; u < kNF; ++u) valid[u] = i < i_hi && j0 + threadIdx.y + u * kBY < j_hi;
+    // position inside the cell, in lattice steps (weights of eq. (2))
+    double fx = 0.0, fy[kNF];
+#pragma unroll
+    for (int u = 0; u < kNF; ++u) fy[u] = 0.0;
+    if (hetero) {
+        fx = fmin(fmax((i * prm.spacing) / a.node_spacing - cell_a, 0.0), 1.0);
+#pragma unroll
+        for (int u = 0; u < kNF; ++u)
+            fy[u] = fmin(fmax(((j0 + threadIdx.y + u * kBY) * prm.spacing) / a.node_spacing - cell_b, 0.0), 1.0);
+    }
 
     double z[kNF][NK], dx[kNF][NK], dy[kNF][NK];
     float zt[kNF][NK], dxt[kNF][NK], dyt[kNF][NK];
@@ -67,30 +103,42 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
             zt[u][k] = dxt[u][k] = dyt[u][k] = 0.f; sxy[u][k] = make_float2(0.f, 0.f);
         }
 
+    for (int corner = 0; corner < (hetero ? 4 : 1); ++corner) {
+    // tables of this corner's node (the homogeneous tile T2L_i) and the facets' weights W^i of eq. (2)
+    const int ca = corner & 1, cb = corner >> 1;
+    const size_t node = hetero ? (size_t)(cell_b + cb) * a.nodes_x + (cell_a + ca) : 0;
+    const double2 *n_xt = a.xt + node * nw * prm.nx, *n_yt = a.yt + node * nw * prm.ny;
+    const double2 *n_tt = a.tt + node * nw * a.n_pulses_total;
+    const float4 *n_wk = a.wk + node * nw;
+    const double *n_om = a.omega + node * nw;
+    double wgt[kNF];
+#pragma unroll
+    for (int u = 0; u < kNF; ++u)
+        wgt[u] = hetero ? sqrt(fmax(0.0, weight2(ca ? 1.0 - fx : fx, cb ? 1.0 - fy[u] : fy[u]))) : 1.0;
     for (int w0 = 0; w0 < nw; w0 += kWCh) {
         const int nwc = min(kWCh, nw - w0);
         __syncthreads();                               // the previous chunk's tables are no longer read
         for (int idx = tid; idx < kBY * kNF * nwc; idx += kBX * kBY) {
             const int r = idx / nwc, w = idx - r * nwc;
-            s_y[r][w] = a.yt[(size_t)(w0 + w) * prm.ny + min(j0 + r, prm.ny - 1)];
+            s_y[r][w] = n_yt[(size_t)(w0 + w) * prm.ny + min(j0 + r, prm.ny - 1)];
         }
         for (int idx = tid; idx < nwc * NK; idx += kBX * kBY) {
             const int w = idx / NK, k = idx - w * NK;
             const int row = min(row0 + min(k, nk - 1), n_rows - 1);
             // row `row` of the outputs holds pulse p: the batch's pulses (H = 1) or its keyframes (H > 1)
             const int p = kRate ? min((first + row) * a.H, a.n_pulses_total - 1) : first + row;
-            const double2 t = a.tt[(size_t)(w0 + w) * a.n_pulses_total + p];
+            const double2 t = n_tt[(size_t)(w0 + w) * a.n_pulses_total + p];
             s_t[w][k] = t;
             s_tf[w][k] = make_float2((float)t.x, (float)t.y);
         }
         if (kSlope || kChoppy || kRate)
             for (int w = tid; w < nwc; w += kBX * kBY) {
-                s_wk[w] = a.wk[w0 + w];
-                s_om[w] = kRate ? (float)a.omega[w0 + w] : 0.f;
+                s_wk[w] = n_wk[w0 + w];
+                s_om[w] = kRate ? (float)n_om[w0 + w] : 0.f;
             }
         __syncthreads();
-        if (!valid[0]) continue;                       // valid[1] implies valid[0]
-        const double2 *xt = a.xt + (size_t)w0 * prm.nx + i;
+        if (!valid[0]) continue;                       // valid[1] implies valid[0]; no barrier is skipped: `continue` is after both
+        const double2 *xt = n_xt + (size_t)w0 * prm.nx + i;
 #pragma unroll 2
         for (int w = 0; w < nwc; ++w) {
             const double2 x = __ldg(xt + (size_t)w * prm.nx);
@@ -99,7 +147,8 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
 #pragma unroll
             for (int u = 0; u < kNF; ++u) {
                 const double2 y = s_y[threadIdx.y + u * kBY][w];
-                cr[u] = fma(x.x, y.x, -x.y * y.y); ci[u] = fma(x.x, y.y, x.y * y.x);   // A exp(j (kx x + ky y + phase))
+                cr[u] = wgt[u] * fma(x.x, y.x, -x.y * y.y);                            // W A exp(j (kx x + ky y + phase))
+                ci[u] = wgt[u] * fma(x.x, y.y, x.y * y.x);
                 cfr[u] = (float)cr[u]; cfi[u] = (float)ci[u];
             }
             float om = 0.f;
@@ -132,6 +181,7 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
                 }
             }
         }
+    }
     }
     const size_t F = (size_t)prm.nx * prm.ny;
 #pragma unroll
@@ -174,7 +224,7 @@ cudaError_t launch_surface_slope(const DevParams &prm, const SurfaceArgs &sa, co
     return cudaGetLastError();
 }
 
-cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a, int first, int n_rows, cudaStream_t s)
+cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a_in, int first, int n_rows, cudaStream_t s)
 {
     if (n_rows <= 0) return cudaSuccess;
     dim3 block(kBX, kBY);
@@ -182,21 +232,32 @@ cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a, int
     // per block (a shorter launch recomputes its last row)
     const int n_chunks = (n_rows + kPK - 1) / kPK, nk = std::max(4, (n_rows + n_chunks - 1) / n_chunks);
     dim3 grid((prm.nx + kBX - 1) / kBX, (prm.ny + kBY * kNF - 1) / (kBY * kNF), (n_rows + nk - 1) / nk);
+    KinematicsArgs a = a_in;
+    if (a.nodes_x > 0) {                               // one group of blocks per cell of the node lattice
+        const int cell_facets = (int)std::ceil(a.node_spacing / prm.spacing) + 1;
+        a.chunks_x = (cell_facets + kBX - 1) / kBX; a.chunks_y = (cell_facets + kBY * kNF - 1) / (kBY * kNF);
+        grid.x = (a.nodes_x - 1) * a.chunks_x; grid.y = (a.nodes_y - 1) * a.chunks_y;
+    }
     const bool slope = a.slope != nullptr, choppy = a.dxy != nullptr, rate = a.H > 1;
     auto launch = [&](auto kern) { kern<<<grid, block, 0, s>>>(prm, a, first, n_rows); };
-    auto pick = [&](auto nk_tag) {
+    auto pick2 = [&](auto nk_tag, auto het_tag) {
         constexpr int NK = decltype(nk_tag)::value;
+        constexpr bool HET = decltype(het_tag)::value;
         if (rate) {
-            if (slope && choppy) launch(kinematics_kernel<NK, true, true, true>);
-            else if (slope)      launch(kinematics_kernel<NK, true, false, true>);
-            else if (choppy)     launch(kinematics_kernel<NK, false, true, true>);
-            else                 launch(kinematics_kernel<NK, false, false, true>);
+            if (slope && choppy) launch(kinematics_kernel<NK, true, true, true, HET>);
+            else if (slope)      launch(kinematics_kernel<NK, true, false, true, HET>);
+            else if (choppy)     launch(kinematics_kernel<NK, false, true, true, HET>);
+            else                 launch(kinematics_kernel<NK, false, false, true, HET>);
         } else {
-            if (slope && choppy) launch(kinematics_kernel<NK, true, true, false>);
-            else if (slope)      launch(kinematics_kernel<NK, true, false, false>);
-            else if (choppy)     launch(kinematics_kernel<NK, false, true, false>);
-            else                 launch(kinematics_kernel<NK, false, false, false>);
+            if (slope && choppy) launch(kinematics_kernel<NK, true, true, false, HET>);
+            else if (slope)      launch(kinematics_kernel<NK, true, false, false, HET>);
+            else if (choppy)     launch(kinematics_kernel<NK, false, true, false, HET>);
+            else                 launch(kinematics_kernel<NK, false, false, false, HET>);
         }
+    };
+    auto pick = [&](auto nk_tag) {
+        if (a.nodes_x > 0) pick2(nk_tag, std::true_type{});
+        else pick2(nk_tag, std::false_type{});
     };
     switch (nk) {
         case 4: pick(std::integral_constant<int, 4>{}); break;

@@ -77,6 +77,8 @@ struct sim_handle {
     DevBuf<float2> slope;
     DevBuf<double2> dxy, dxy_t;
     int key_H = 1;                       // keyframe spacing of the kinematics (1 = every pulse)
+    int nodes_x = 0, nodes_y = 0;        // heterogeneous surface: node lattice of the wave tables (0 = homogeneous)
+    double node_spacing = 0;
     bool geo_keyframed = false;          // spectral path: ranges / gains interpolated between keyframes (K2k)
     int surf_rows_cap = 0;               // rows of the surface buffers
     DevBuf<Rec> recs;
@@ -122,6 +124,21 @@ int fail_cuda(sim_handle *h, cudaError_t e, const char *what)
         cudaError_t e__ = (call);                                     \
         if (e__ != cudaSuccess) return fail_cuda((h), e__, #call);    \
     } while (0)
+
+// The wave tables of the scene: one homogeneous table, or one table per node of the heterogeneous lattice
+// (sim_scene.wave_nodes_x > 0).  Entry (node, w) sits at index node * n_waves + w.
+struct WaveView {
+    int n_nodes, n_waves;
+    const double *kx, *ky, *amp, *omega, *phase;
+    bool hetero;
+};
+WaveView wave_view(const sim_scene *sc)
+{
+    if (sc->wave_nodes_x > 0)
+        return {sc->wave_nodes_x * sc->wave_nodes_y, sc->n_waves, sc->node_kx, sc->node_ky, sc->node_amp, sc->node_omega,
+                sc->node_phase, true};
+    return {1, sc->n_waves, sc->kx, sc->ky, sc->amp, sc->omega, sc->phase, false};
+}
 
 bool finite_all(const double *p, size_t n)
 {
@@ -171,7 +188,21 @@ int validate(const sim_instrument *in, const sim_geometry *g, const sim_scene *s
     if (sc->nx < 1 || sc->ny < 1 || (int64_t)sc->nx * sc->ny > ((int64_t)1 << 31)) return SIM_EINVAL;
     if (!(sc->spacing_m > 0) || !std::isfinite(sc->spacing_m) || !finite_all(sc->centre_m, 3)) return SIM_EINVAL;
     if (sc->n_waves < 0 || sc->n_waves > 4096) return SIM_EINVAL;
-    if (sc->n_waves > 0) {
+    if (sc->wave_nodes_x < 0 || sc->wave_nodes_y < 0) return SIM_EINVAL;
+    if (sc->wave_nodes_x > 0) {
+        // heterogeneous surface: a lattice of >= 2 x 2 nodes of step L anchored at facet (0, 0) that covers the grid
+        if (sc->wave_nodes_x < 2 || sc->wave_nodes_y < 2 || sc->n_waves < 1) return SIM_EINVAL;
+        if ((int64_t)sc->wave_nodes_x * sc->wave_nodes_y > (1 << 20)) return SIM_EINVAL;
+        if (!(sc->wave_node_spacing_m > 0) || !std::isfinite(sc->wave_node_spacing_m)) return SIM_EINVAL;
+        if (!sc->node_kx || !sc->node_ky || !sc->node_amp || !sc->node_omega || !sc->node_phase) return SIM_EINVAL;
+        const double L = sc->wave_node_spacing_m * (1.0 + 1e-12);
+        if ((sc->nx - 1) * sc->spacing_m > (sc->wave_nodes_x - 1) * L || (sc->ny - 1) * sc->spacing_m > (sc->wave_nodes_y - 1) * L)
+            return SIM_EINVAL;
+        const size_t n = (size_t)sc->wave_nodes_x * sc->wave_nodes_y * sc->n_waves;
+        if (!finite_all(sc->node_kx, n) || !finite_all(sc->node_ky, n) || !finite_all(sc->node_amp, n) ||
+            !finite_all(sc->node_omega, n) || !finite_all(sc->node_phase, n))
+            return SIM_EINVAL;
+    } else if (sc->n_waves > 0) {
         if (!sc->kx || !sc->ky || !sc->amp || !sc->omega || !sc->phase) return SIM_EINVAL;
         if (!finite_all(sc->kx, sc->n_waves) || !finite_all(sc->ky, sc->n_waves) || !finite_all(sc->amp, sc->n_waves) ||
             !finite_all(sc->omega, sc->n_waves) || !finite_all(sc->phase, sc->n_waves))
@@ -248,6 +279,7 @@ int run_kinematics(sim_handle *h, const SurfBufs &b, int p0, int n_pl, cudaStrea
     surface_rows(h, p0, n_pl, &first, &rows);
     KinematicsArgs ka{};
     ka.xt = h->xt.p; ka.yt = h->yt.p; ka.tt = h->tt.p; ka.wk = h->wk.p; ka.n_pulses_total = h->n_pulses;
+    ka.nodes_x = h->nodes_x; ka.nodes_y = h->nodes_y; ka.node_spacing = h->node_spacing;
     ka.z = b.z; ka.slope = b.slope; ka.dxy = b.dxy;
     ka.H = h->key_H; ka.omega = h->omega.p; ka.zt = b.zt; ka.dxy_t = b.dxy_t;
     cudaError_t e = launch_kinematics(h->prm, ka, first, rows, s);
@@ -271,13 +303,21 @@ int choose_keyframe_spacing(const sim_geometry *g, const sim_scene *sc, int requ
         if (H > P - 1) continue;
         double hmax = 0;
         for (int k = 0; k < P - 1; k += H) hmax = std::max(hmax, g->t_pulse_s[std::min(k + H, P - 1)] - g->t_pulse_s[k]);
+        // heterogeneous surface: four tiles with weights that add to at most 2 (squares to 1): worst node, doubled
+        const WaveView wv = wave_view(sc);
         double bound = 0, slope2 = 0;
-        for (int w = 0; w < sc->n_waves; ++w) {
-            const double x = sc->omega[w] * hmax;
-            bound += std::fabs(sc->amp[w]) * x * x * x * x / 384.0;
-            const double sl = std::fabs(sc->amp[w]) * std::hypot(sc->kx[w], sc->ky[w]) * x * x / 8.0;
-            slope2 += sl * sl;
+        for (int n = 0; n < wv.n_nodes; ++n) {
+            double b1 = 0, s2 = 0;
+            for (int w = 0; w < wv.n_waves; ++w) {
+                const size_t k = (size_t)n * wv.n_waves + w;
+                const double x = wv.omega[k] * hmax;
+                b1 += std::fabs(wv.amp[k]) * x * x * x * x / 384.0;
+                const double sl = std::fabs(wv.amp[k]) * std::hypot(wv.kx[k], wv.ky[k]) * x * x / 8.0;
+                s2 += sl * sl;
+            }
+            bound = std::max(bound, b1); slope2 = std::max(slope2, s2);
         }
+        if (wv.hetero) bound *= 2.0;
         if (bound <= 2e-9 && (!sc->tilt_modulation || 4.0 * std::sqrt(slope2) <= 4e-5)) return H;
     }
     return 1;
@@ -502,7 +542,12 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     prm.n_tiles = prm.tiles_x * prm.tiles_y;
     prm.tile_cap = tile * tile;
     double wave_sum = 0;
-    for (int w = 0; w < Nw; ++w) wave_sum += std::fabs(sc->amp[w]);
+    const WaveView wv = wave_view(sc);
+    for (int n = 0; n < wv.n_nodes; ++n) {
+        double a1 = 0;
+        for (int w = 0; w < Nw; ++w) a1 += std::fabs(wv.amp[(size_t)n * Nw + w]);
+        wave_sum = std::max(wave_sum, wv.hetero ? 2.0 * a1 : a1);
+    }
     const double tile_spread = tile * samples_per_facet + 2.0 * 2.0 * wave_sum * prm.fs_over_c0 + 3.0;
     h->accum = accumulate_plan(prm, tile_spread);
     h->span_cap_m = std::min(4096, (((int)std::ceil(tile_spread) + 8) + 31) & ~31);
@@ -540,6 +585,8 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
                              (prm.choppy ? h->n_facets * 16 : 0);
     const int64_t per_pulse_common = h->key_H > 1 ? 2 * surf_row / h->key_H + 1 : surf_row;
     h->speckle_ar1 = sc->speckle_tau_s > 0;
+    h->nodes_x = sc->wave_nodes_x > 0 ? sc->wave_nodes_x : 0; h->nodes_y = h->nodes_x ? sc->wave_nodes_y : 0;
+    h->node_spacing = sc->wave_node_spacing_m;
     h->seed = sc->seed;
     const int64_t per_pulse = per_pulse_common + (h->speckle_ar1 ? h->n_facets * 8 : 0) +
         (h->spectral ? (int64_t)C * kMomentOrder * h->nb_pad * 8
@@ -556,26 +603,28 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     h->pulses_per_batch = pb;
 
     // ---- host tables (fp64) ----
-    std::vector<double2> xt((size_t)Nw * nx), yt((size_t)Nw * ny), tt((size_t)Nw * P);
-    std::vector<float4> wk(Nw);
-    for (int w = 0; w < Nw; ++w) {
+    // one set per node of the heterogeneous lattice (a single set on the homogeneous surface); row q = node * Nw + w
+    const size_t NQ = (size_t)wv.n_nodes * Nw;
+    std::vector<double2> xt(NQ * nx), yt(NQ * ny), tt(NQ * P);
+    std::vector<float4> wk(NQ);
+    for (size_t q = 0; q < NQ; ++q) {
+        const double kx = wv.kx[q], ky = wv.ky[q], amp = wv.amp[q], om = wv.omega[q], ph = wv.phase[q];
         for (int i = 0; i < nx; ++i) {
             double x = sc->centre_m[0] + (i - 0.5 * (nx - 1)) * sc->spacing_m;
-            double a = sc->kx[w] * x;
-            xt[(size_t)w * nx + i] = make_double2(sc->amp[w] * std::cos(a), sc->amp[w] * std::sin(a));
+            double a = kx * x;
+            xt[q * nx + i] = make_double2(amp * std::cos(a), amp * std::sin(a));
         }
         for (int j = 0; j < ny; ++j) {
             double y = sc->centre_m[1] + (j - 0.5 * (ny - 1)) * sc->spacing_m;
-            double a = sc->ky[w] * y + sc->phase[w];
-            yt[(size_t)w * ny + j] = make_double2(std::cos(a), std::sin(a));
+            double a = ky * y + ph;
+            yt[q * ny + j] = make_double2(std::cos(a), std::sin(a));
         }
         for (int p = 0; p < P; ++p) {
-            double a = -sc->omega[w] * g->t_pulse_s[p];
-            tt[(size_t)w * P + p] = make_double2(std::cos(a), std::sin(a));
+            double a = -om * g->t_pulse_s[p];
+            tt[q * P + p] = make_double2(std::cos(a), std::sin(a));
         }
-        double k = std::hypot(sc->kx[w], sc->ky[w]);
-        wk[w] = make_float4((float)sc->kx[w], (float)sc->ky[w], k > 0 ? (float)(sc->kx[w] / k) : 0.f,
-                            k > 0 ? (float)(sc->ky[w] / k) : 0.f);
+        double k = std::hypot(kx, ky);
+        wk[q] = make_float4((float)kx, (float)ky, k > 0 ? (float)(kx / k) : 0.f, k > 0 ? (float)(ky / k) : 0.f);
     }
     std::vector<PulseConst> pcs(P);
     std::vector<double2> carrier(P);
@@ -676,8 +725,8 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
             CKC(h->zt.alloc(F * rows));
             if (prm.choppy) CKC(h->dxy_t.alloc(F * rows));
         }
-        CKC(h->omega.alloc(std::max(Nw, 1)));
-        if (Nw) CKC(cudaMemcpy(h->omega.p, sc->omega, (size_t)Nw * sizeof(double), cudaMemcpyHostToDevice));
+        CKC(h->omega.alloc(std::max<size_t>(NQ, 1)));
+        if (NQ) CKC(cudaMemcpy(h->omega.p, wv.omega, NQ * sizeof(double), cudaMemcpyHostToDevice));
     }
     if (!h->spectral) {
         CKC(h->recs.alloc((size_t)C * pb * fcap));

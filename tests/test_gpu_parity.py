@@ -193,6 +193,39 @@ def test_time_dependent_speckle_facet_amplitudes():
     assert np.max(np.abs(g["amp"] - o["amp"])) < 1e-5 * np.abs(o["amp"]).max()
 
 
+# ----------------------------------------------------------------------------- NEXT-2: heterogeneous surface
+
+def _wave_nodes(w, L, nw=12, seed=3):
+    """One wave table per node of a lattice of step L covering the grid."""
+    sc = w.scene
+    rng = np.random.default_rng(seed)
+    shape = (max(int(np.ceil((sc["ny"] - 1) * sc["spacing_m"] / L)) + 1, 2),
+             max(int(np.ceil((sc["nx"] - 1) * sc["spacing_m"] / L)) + 1, 2), nw)
+    k, th = rng.uniform(0.05, 0.6, shape), rng.uniform(-1.0, 1.0, shape)
+    sc["wave_nodes"] = dict(spacing_m=L, kx=k * np.cos(th), ky=k * np.sin(th), amp=rng.uniform(0.01, 0.08, shape),
+                            omega=np.sqrt(9.81 * k), phase=rng.uniform(0, 2 * np.pi, shape))
+    return w
+
+
+def test_heterogeneous_surface(mode):
+    """Four homogeneous tiles blended with the weights of eq. (2) (kinematics.cu node lattice) against the oracle:
+    facet positions and slopes, then the raw data; cells smaller and larger than a K1 block, a lattice step that is
+    not a multiple of the facet spacing, CWM + tilt, keyframes on and off."""
+    w = _wave_nodes(make_workload("tiny", n_pulses=12), L=37.0)
+    w.scene["choppy"], w.scene["tilt_modulation"] = 1, 1
+    with _sim(w, accumulate_mode=mode) as sim:
+        g = sim.debug_facets(7)
+        got = sim.generate().cpu().numpy()
+    o = oracle_facets(w, 7)
+    assert np.max(np.abs(g["pos"] - o["pos"])) < 2e-8                  # pulse 7 sits between keyframes (bound 4e-9 per term)
+    assert np.max(np.abs(g["slope"] - o["slope"])) < 2e-5              # slopes are linear between keyframes
+    ref = oracle_generate(w)
+    _assert_parity(got, ref, "hetero surface tiny")
+    _assert_parity(_gpu(w, accumulate_mode=mode, kinematics_keyframe=1), ref, "hetero surface, exact every pulse")
+    wh = _wave_nodes(_hetero_small(150, 90, 5), L=200.0, nw=40, seed=9)      # 67-facet cells, 3 channels, sigma0 map
+    _assert_parity(_gpu(wh, accumulate_mode=mode), oracle_generate(wh), "hetero surface hetero_small")
+
+
 # ----------------------------------------------------------------------------- per-kernel unit parity (T1)
 
 @pytest.mark.parametrize("name", ["tiny", "hetero_small"])

@@ -65,17 +65,21 @@ def _numpy_surface(w, p):
 def test_blend_against_numpy_and_weight_squares_add_to_one():
     """Eq. (1) with the weights of eq. (2) by an independent numpy script, with and without the CWM displacement;
     "the squares of the weighting coefficients must add to unity" (PAPER.md:76)."""
-    for choppy in (0, 1):
-        w = _workload(choppy=choppy)
+    for choppy, L in ((0, 40.0), (1, 40.0), (1, 37.0)):        # L = 37 m: node lines fall between facets, and rounding
+        w = _workload(choppy=choppy, L=L)                       # leaves 1 - wx - wy + wx wy = -1e-17 at some far edges
         for p in (0, 2):
             o = oracle_facets(w, p)
             xb, yb, z, sx, sy, dx, dy, w2 = _numpy_surface(w, p)
             assert np.max(np.abs(w2 - 1.0)) < 1e-14
-            assert np.max(np.abs(o["pos"][:, 2] - (w.scene["centre_m"][2] + z).reshape(-1))) < 1e-12
-            assert np.max(np.abs(o["slope"][:, 0] - sx.reshape(-1))) < 1e-12
-            assert np.max(np.abs(o["slope"][:, 1] - sy.reshape(-1))) < 1e-12
+            assert np.all(np.isfinite(o["pos"]))
+            # the weight has an infinite slope at the far edge of a cell: where i d / L rounds across a node line the
+            # two evaluations differ by sqrt(1e-16) times a displacement
+            tol = 1e-12 if L == 40.0 else 2e-8
+            assert np.max(np.abs(o["pos"][:, 2] - (w.scene["centre_m"][2] + z).reshape(-1))) < tol
+            assert np.max(np.abs(o["slope"][:, 0] - sx.reshape(-1))) < tol
+            assert np.max(np.abs(o["slope"][:, 1] - sy.reshape(-1))) < tol
             ex = xb + (dx if choppy else 0.0)
-            assert np.max(np.abs(o["pos"][:, 0] - ex.reshape(-1))) < 1e-10
+            assert np.max(np.abs(o["pos"][:, 0] - ex.reshape(-1))) < max(tol, 1e-10)
 
 
 def test_unit_weight_at_the_corners():
