@@ -121,7 +121,20 @@ class ClockSampler:
                 "samples": len(s), "reasons": reasons}
 
 
+_VARIANT = {"wave_node_spacing": 0.0, "speckle_tau": 0.0}     # set from the command line (NEXT-1 / NEXT-2 modes)
+
+
 def _workload(name, n_pulses=None, pulse_offset=0):
+    w = _base_workload(name, n_pulses, pulse_offset)
+    if _VARIANT["wave_node_spacing"] > 0:          # heterogeneous surface, uncorrelated phases per node
+        from workloads import add_wave_nodes
+        add_wave_nodes(w, _VARIANT["wave_node_spacing"])
+    if _VARIANT["speckle_tau"] > 0:                # AR(1) intra-facet speckle (eq. (7), (10))
+        w.scene["speckle_tau_s"], w.scene["speckle_doppler_hz"] = _VARIANT["speckle_tau"], 20.0
+    return w
+
+
+def _base_workload(name, n_pulses=None, pulse_offset=0):
     """BASELINE.json configs by name, or one point of the stress sweep (configs[4], reading G23) as
     `sweep:f<log2 facets>:l<replica samples>:c<channels>`, e.g. sweep:f24:l1200:c3 (64 pulses by default)."""
     from workloads import make_workload, make_sweep_point
@@ -193,13 +206,14 @@ def _time_steps(sim, out, P, steps, warmup, stream, barrier, torch, clocks_index
         sampler.__exit__()
     kms = sim.kernel_ms()            # per-kernel totals of the LAST timed step (events on this stream)
     stats = sim.stats()
+    stats["n_facets_x_channels"] = sim.n_facets * sim.n_channels      # pulses of the call = nominal / this
     sim.set_profiling(False)
     return ev0.elapsed_time(ev1), t_wall, kms, stats, (sampler.summary() if sampler else None)
 
 
 def _roofline_direct(kms, stats, sm_max, pipes):
     """K3 (accumulate_kernel) against the FP32 pipe: 4 lane-ops per facet-sample (DESIGN.md 4/K3)."""
-    n_batches = max(1, stats["kernel_launches"] // 4)
+    n_batches = max(1, -(-int(stats["facet_echoes_nominal"] // max(1, stats["n_facets_x_channels"])) // max(1, stats["pulses_per_batch"])))
     launch_ms = kms["accumulate"] / n_batches
     fs_per_launch = stats["facet_samples"] / n_batches
     achieved = fs_per_launch / (launch_ms * 1e-3) / 1e9
@@ -221,7 +235,7 @@ def _roofline_spectral(kms, stats, sm_max, pipes, n_channels):
     """K2s / K2k (moments kernels) against the FP32 pipe, on the moment form's OWN op count (SURVEY.md 8(d):
     "4 Kt FFMA + ~30 setup per facet-echo ... must be reported against its own op count"): with Kt = 8 that is
     62 FP32 lane-operations per nominal facet-echo."""
-    n_batches = max(1, stats["kernel_launches"] // 3)
+    n_batches = max(1, -(-int(stats["facet_echoes_nominal"] // max(1, stats["n_facets_x_channels"])) // max(1, stats["pulses_per_batch"])))
     launch_ms = kms["geometry"] / n_batches
     echoes = stats["facet_echoes_nominal"] / n_batches
     ops = echoes * MOMENT_FP32_OPS_PER_FACET_ECHO
@@ -358,6 +372,7 @@ def run_cuda(args):
         "config": {"workload": args.workload, "facets": F, "channels": C, "pulses": P, "replica_samples": L,
                    "n_samples": Ns, "wave_components": int(w.scene["n_waves"]),
                    "parallelism": f"pulse-slab x{world}",
+                   "wave_node_spacing_m": _VARIANT["wave_node_spacing"], "speckle_tau_s": _VARIANT["speckle_tau"],
                    "accumulate_mode": "spectral" if spectral else "direct", "fft_size": stats["fft_size"],
                    "kinematics_keyframe": stats["kinematics_keyframe"],
                    "tile_facets": stats["tile_facets"], "pulses_per_batch": stats["pulses_per_batch"],
@@ -394,10 +409,15 @@ def main():
                     help="echo accumulation (include/heeps_sim.h SIM_ACCUMULATE_*)")
     ap.add_argument("--tile", type=int, default=0, help="spatial tile side in facets (0 = library default)")
     ap.add_argument("--pulses", type=int, default=None, help="override the dwell length (debugging)")
+    ap.add_argument("--wave-node-spacing", type=float, default=0.0,
+                    help="heterogeneous surface: lattice step L [m] of per-node wave tables (0 = homogeneous, the configs)")
+    ap.add_argument("--speckle-tau", type=float, default=0.0,
+                    help="time-dependent AR(1) speckle: correlation time tau_s [s] (0 = constant speckle, the configs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-direct", action="store_true", help="skip the direct-form comparison leg")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
+    _VARIANT["wave_node_spacing"], _VARIANT["speckle_tau"] = args.wave_node_spacing, args.speckle_tau
     if args.impl == "reference":
         return run_reference(args)
     return run_cuda(args)

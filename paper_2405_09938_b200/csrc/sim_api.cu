@@ -849,7 +849,7 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         CK(h, mark());
         CK(h, mark());                                   // K4 slot: finalize is fused into K3s
         CK(h, ship(p0, n_pl));
-        launches += 3;
+        launches += 3 + (h->speckle_ar1 ? 1 : 0);
     }
     for (int p0 = pb0; !h->spectral && p0 < pb1; p0 += batch) {
         const int n_pl = std::min(batch, pb1 - p0);
@@ -873,7 +873,7 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         CK(h, launch_finalize(prm, fa, p0, n_pl, s));
         CK(h, mark());
         CK(h, ship(p0, n_pl));
-        launches += 4;
+        launches += 4 + (h->speckle_ar1 ? 1 : 0);
     }
     h->stats.kernel_launches = launches;
     h->stats.facet_echoes_nominal = h->n_facets * (int64_t)n_out * prm.n_channels;

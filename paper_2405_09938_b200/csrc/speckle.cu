@@ -56,6 +56,16 @@ __device__ __forceinline__ uint2 to_polar(float2 v, uint32_t extra_turns)
     return o;
 }
 
+// the same in fp32 for the per-pulse walk (atan2f: ~1e-7 rad, 2e-8 turns)
+__device__ __forceinline__ uint2 to_polar_fast(float2 v, uint32_t extra_turns)
+{
+    const float turns = atan2f(v.y, v.x) * 0.15915494309189535f;                    // [-0.5, 0.5]
+    uint2 o;
+    o.x = __float_as_uint(sqrtf(v.x * v.x + v.y * v.y));
+    o.y = (uint32_t)__float2int_rn(turns * 2147483648.0f) * 2u + extra_turns;       // 2^-32 turns, wrapping
+    return o;
+}
+
 __global__ void __launch_bounds__(256)
 speckle_kernel(float2 *xi, int64_t n, uint64_t seed)
 {
@@ -95,7 +105,7 @@ speckle_ar1_kernel(SpeckleAr1Args a)
             st.x = fmaf(bg.x, st.x, bg.y * nn.x);
             st.y = fmaf(bg.x, st.y, bg.y * nn.y);
         }
-        a.polar[(size_t)pl * a.n_facets + f] = to_polar(st, __ldg(a.doppler_turns + p));
+        a.polar[(size_t)pl * a.n_facets + f] = to_polar_fast(st, __ldg(a.doppler_turns + p));
     }
     a.state[f] = st;                                         // state after pulse p0 + n_pl - 1
 }

@@ -14,6 +14,7 @@ from .generator import (  # noqa: F401
     Workload,
     make_workload,
     make_sweep_point,
+    add_wave_nodes,
     pm_spectrum,
     workload_digest,
 )

@@ -282,6 +282,23 @@ def make_sweep_point(*, log2_facets: int = 24, spacing_m: float | None = None,
     return w
 
 
+def add_wave_nodes(w: Workload, spacing_m: float, seed: int = MASTER_SEED + 4) -> Workload:
+    """Heterogeneous-surface variant of a workload: a lattice of wave tables of step `spacing_m`
+    covering the grid, one homogeneous tile T2L per node.  Uniform sea state as the paper describes it:
+    every node keeps the workload's spectrum (kx, ky, amp, omega) but draws its own phases, uncorrelated between nodes."""
+    sc = w.scene
+    nw = int(sc["n_waves"])
+    ny_n = max(int(np.ceil((sc["ny"] - 1) * sc["spacing_m"] / spacing_m)) + 1, 2)
+    nx_n = max(int(np.ceil((sc["nx"] - 1) * sc["spacing_m"] / spacing_m)) + 1, 2)
+    shape = (ny_n, nx_n, nw)
+    rng = np.random.Generator(np.random.PCG64(seed))
+    nodes = {k: np.ascontiguousarray(np.broadcast_to(np.asarray(sc[k], dtype=np.float64), shape)) for k in ("kx", "ky", "amp", "omega")}
+    nodes["phase"] = rng.uniform(0.0, 2.0 * np.pi, shape)
+    nodes["spacing_m"] = float(spacing_m)
+    sc["wave_nodes"] = nodes
+    return w
+
+
 def workload_digest(w: Workload) -> str:
     """SHA-256 over every generated array (G22: the workload must not drift between runs)."""
     h = hashlib.sha256()
