@@ -54,6 +54,8 @@ class _Desc(C.Structure):
         ("wave_nodes_x", C.c_int32), ("wave_nodes_y", C.c_int32), ("wave_node_spacing_m", C.c_double),
         ("node_kx", C.c_void_p), ("node_ky", C.c_void_p), ("node_amp", C.c_void_p), ("node_omega", C.c_void_p),
         ("node_phase", C.c_void_p),
+        ("pattern", C.c_void_p * 2), ("pattern_nu", C.c_int32 * 2), ("pattern_nv", C.c_int32 * 2),
+        ("pattern_u", (C.c_double * 2) * 2), ("pattern_v", (C.c_double * 2) * 2),
     ]
 
 
@@ -146,6 +148,15 @@ def _marshal(w):
         d.wave_node_spacing_m = float(wn["spacing_m"])
         for k in ("kx", "ky", "amp", "omega", "phase"):
             setattr(d, "node_" + k, ptr(_f64(wn[k], shape)))
+    for k, name in enumerate(("tx_pattern", "rx_pattern")):      # antenna patterns as complex u-v grids
+        pat = inst.get(name)
+        if pat is not None:                                      # dict: table complex [nv][nu], u=(u0,u1), v=(v0,v1)
+            tab = np.asarray(pat["table"])
+            t2 = np.ascontiguousarray(np.stack([tab.real, tab.imag], axis=-1), dtype=np.float32)
+            d.pattern[k] = ptr(t2)
+            d.pattern_nv[k], d.pattern_nu[k] = int(tab.shape[0]), int(tab.shape[1])
+            d.pattern_u[k][0], d.pattern_u[k][1] = float(pat["u"][0]), float(pat["u"][1])
+            d.pattern_v[k][0], d.pattern_v[k][1] = float(pat["v"][0]), float(pat["v"][1])
     return d, keep
 
 

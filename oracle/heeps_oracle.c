@@ -26,7 +26,7 @@
  * G10 current by advection, G11 linear waves (CWM by flag), G12 tilt factor clamped at 0,
  * G15 A = d^2, G24 displaced point feeds the antenna direction, G27 the generator of the AR(1) speckle innovations
  * (NEXT-1, off unless speckle_tau_s > 0), G28 blending of slopes and velocities on the heterogeneous surface (NEXT-2, off
- * unless wave_nodes_x > 0).
+ * unless wave_nodes_x > 0), G29 bilinear complex antenna patterns on u-v grids (NEXT-3, off unless pattern[k] is given).
  *
  * Pins: tests/test_oracle_pins.py (closed forms with mpmath, invariants, brute force by an
  * independent numpy script).  No function here is "parity unpinned".
@@ -74,6 +74,12 @@ typedef struct {
     int32_t wave_nodes_x, wave_nodes_y;
     double wave_node_spacing_m;                 /* L */
     const double *node_kx, *node_ky, *node_amp, *node_omega, *node_phase;   /* [nodes_y][nodes_x][n_waves] */
+    /* NEXT-3: antenna patterns as complex u-v grids.  pattern[k] non-NULL (k = 0 Tx,
+     * 1 Rx) replaces that antenna's analytic sinc pattern: complex field gain on a regular grid of nu x nv nodes
+     * over the direction cosines u = r^ . azimuth axis in [u0, u1], v = r^ . elevation axis in [v0, v1]. */
+    const float *pattern[2];                    /* [nv][nu][2] (re, im) */
+    int32_t pattern_nu[2], pattern_nv[2];
+    double pattern_u[2][2], pattern_v[2][2];    /* {first node, last node} */
 } oracle_desc;
 
 /* per-facet intermediates of one pulse (O2..O8), exposed for unit parity */
@@ -104,9 +110,38 @@ static double gain(const double *u, const double *frame, const double *aperture,
     return sinc_pi(aperture[0] * ua / lambda) * sinc_pi(aperture[1] * ue / lambda);
 }
 
+/*
+ * O6 with tabulated patterns ("antenna patterns are converted into u-v grids at the appropriate
+ * resolution"; the gains are complex).  Reading G29: the value between nodes is the bilinear
+ * interpolant of the four surrounding nodes, real and imaginary parts separately; a direction outside the grid has
+ * zero gain.  Antenna k = 0 is Tx, 1 is Rx; with no table the analytic aperture pattern of `gain` (imaginary part 0).
+ */
+static void gain_complex(const oracle_desc *d, int k, const double *u, const double *frame, const double *aperture,
+                         double lambda, double *re, double *im)
+{
+    if (!d->pattern[k]) { *re = gain(u, frame, aperture, lambda); *im = 0.0; return; }
+    const int nu = d->pattern_nu[k], nv = d->pattern_nv[k];
+    const double ua = dot3(u, frame + 3), ue = dot3(u, frame + 6);
+    const double gu = (ua - d->pattern_u[k][0]) / (d->pattern_u[k][1] - d->pattern_u[k][0]) * (nu - 1);   /* grid coordinates */
+    const double gv = (ue - d->pattern_v[k][0]) / (d->pattern_v[k][1] - d->pattern_v[k][0]) * (nv - 1);
+    *re = 0.0; *im = 0.0;
+    if (!(gu >= 0.0 && gu <= nu - 1 && gv >= 0.0 && gv <= nv - 1)) return;
+    int iu = (int)floor(gu), iv = (int)floor(gv);
+    if (iu > nu - 2) iu = nu - 2;
+    if (iv > nv - 2) iv = nv - 2;
+    const double fu = gu - iu, fv = gv - iv;
+    for (int b = 0; b < 2; ++b)
+        for (int a = 0; a < 2; ++a) {
+            const double wgt = (a ? fu : 1.0 - fu) * (b ? fv : 1.0 - fv);
+            const float *t = d->pattern[k] + 2 * ((size_t)(iv + b) * nu + (iu + a));
+            *re += wgt * (double)t[0];
+            *im += wgt * (double)t[1];
+        }
+}
+
 typedef struct {
     double pos[3], slope[2], vel[3];
-    double tau[8], g_tx, g_rx[8], amp_re[8], amp_im[8];
+    double tau[8], g_tx, g_rx[8], amp_re[8], amp_im[8];    /* g_tx, g_rx: real parts of the gains */
     int keep;
 } facet_eval;
 
@@ -240,16 +275,19 @@ static void eval_facet(const oracle_desc *d, int p, int i, int j, facet_eval *o)
     double dt[3] = { o->pos[0] - ptx[0], o->pos[1] - ptx[1], o->pos[2] - ptx[2] };
     double rt = sqrt(dot3(dt, dt));
     double ut[3] = { dt[0] / rt, dt[1] / rt, dt[2] / rt };
-    o->g_tx = gain(ut, d->tx_frame + 9 * p, d->tx_aperture, lambda);
+    double gt_re, gt_im;
+    gain_complex(d, 0, ut, d->tx_frame + 9 * p, d->tx_aperture, lambda, &gt_re, &gt_im);
+    o->g_tx = gt_re;
     /* O7 cull on the un-offset receive phase centre (G6) */
     double dr0[3] = { o->pos[0] - prx[0], o->pos[1] - prx[1], o->pos[2] - prx[2] };
     double rr0 = sqrt(dot3(dr0, dr0));
     double ur0[3] = { dr0[0] / rr0, dr0[1] / rr0, dr0[2] / rr0 };
-    double g_ref = gain(ur0, d->rx_frame + 9 * p, d->rx_aperture, lambda);
+    double gref_re, gref_im;
+    gain_complex(d, 1, ur0, d->rx_frame + 9 * p, d->rx_aperture, lambda, &gref_re, &gref_im);
     o->keep = 1;
     if (d->cull_two_way_db > -300.0) {
         double thr = pow(10.0, d->cull_two_way_db / 20.0);
-        if (fabs(o->g_tx * g_ref) < thr) o->keep = 0;
+        if (hypot(gt_re, gt_im) * hypot(gref_re, gref_im) < thr) o->keep = 0;       /* |G_t G_r,ref| */
     }
     /* O8 amplitude a = sqrt(sigma d^2) xi   (G15, G12) */
     double sigma = d->sigma0_lin ? (double)d->sigma0_lin[(size_t)j * d->nx + i] : d->sigma0_uniform;
@@ -269,17 +307,19 @@ static void eval_facet(const oracle_desc *d, int p, int i, int j, facet_eval *o)
         double dr[3] = { o->pos[0] - pc[0], o->pos[1] - pc[1], o->pos[2] - pc[2] };
         double rr = sqrt(dot3(dr, dr));
         double ur[3] = { dr[0] / rr, dr[1] / rr, dr[2] / rr };
-        double gr = gain(ur, d->rx_frame + 9 * p, d->rx_aperture, lambda);
+        double gr_re, gr_im;
+        gain_complex(d, 1, ur, d->rx_frame + 9 * p, d->rx_aperture, lambda, &gr_re, &gr_im);
         /* O5 */
         double tau = (rt + rr) / ORACLE_C0;
         /* carrier phase -2 pi frac(f0 tau), long double for the 2.8e7-cycle product (G3) */
         long double cyc = (long double)d->f0_hz * (long double)tau;
         double fr = (double)(cyc - floorl(cyc));
         double ph = -2.0 * M_PI * fr;
-        double g = a0 * o->g_tx * gr;
-        double ar = g * xr, ai = g * xim;
+        /* a G_t G_r: complex product of the two gains, then of the speckle */
+        double g_re = a0 * (gt_re * gr_re - gt_im * gr_im), g_im = a0 * (gt_re * gr_im + gt_im * gr_re);
+        double ar = g_re * xr - g_im * xim, ai = g_re * xim + g_im * xr;
         o->tau[c] = tau;
-        o->g_rx[c] = gr;
+        o->g_rx[c] = gr_re;
         o->amp_re[c] = ar * cos(ph) - ai * sin(ph);
         o->amp_im[c] = ar * sin(ph) + ai * cos(ph);
     }
