@@ -121,7 +121,7 @@ class ClockSampler:
                 "samples": len(s), "reasons": reasons}
 
 
-_VARIANT = {"wave_node_spacing": 0.0, "speckle_tau": 0.0}     # set from the command line (NEXT-1 / NEXT-2 modes)
+_VARIANT = {"wave_node_spacing": 0.0, "speckle_tau": 0.0, "patterns": False}     # set from the command line (NEXT-1..3 modes)
 
 
 def _workload(name, n_pulses=None, pulse_offset=0):
@@ -131,6 +131,9 @@ def _workload(name, n_pulses=None, pulse_offset=0):
         add_wave_nodes(w, _VARIANT["wave_node_spacing"])
     if _VARIANT["speckle_tau"] > 0:                # AR(1) intra-facet speckle (eq. (7), (10))
         w.scene["speckle_tau_s"], w.scene["speckle_doppler_hz"] = _VARIANT["speckle_tau"], 20.0
+    if _VARIANT["patterns"]:                       # antenna patterns as complex u-v grids, azimuth steering
+        from workloads import add_antenna_patterns
+        add_antenna_patterns(w, nu=513, nv=129, steer_rate_deg_s=1.5)
     return w
 
 
@@ -373,6 +376,7 @@ def run_cuda(args):
                    "n_samples": Ns, "wave_components": int(w.scene["n_waves"]),
                    "parallelism": f"pulse-slab x{world}",
                    "wave_node_spacing_m": _VARIANT["wave_node_spacing"], "speckle_tau_s": _VARIANT["speckle_tau"],
+                   "tabulated_patterns": _VARIANT["patterns"],
                    "accumulate_mode": "spectral" if spectral else "direct", "fft_size": stats["fft_size"],
                    "kinematics_keyframe": stats["kinematics_keyframe"],
                    "tile_facets": stats["tile_facets"], "pulses_per_batch": stats["pulses_per_batch"],
@@ -413,11 +417,14 @@ def main():
                     help="heterogeneous surface: lattice step L [m] of per-node wave tables (0 = homogeneous, the configs)")
     ap.add_argument("--speckle-tau", type=float, default=0.0,
                     help="time-dependent AR(1) speckle: correlation time tau_s [s] (0 = constant speckle, the configs)")
+    ap.add_argument("--patterns", action="store_true",
+                    help="antenna patterns as 513 x 129 complex u-v tables with 1.5 deg/s azimuth steering (default: analytic apertures)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-direct", action="store_true", help="skip the direct-form comparison leg")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     _VARIANT["wave_node_spacing"], _VARIANT["speckle_tau"] = args.wave_node_spacing, args.speckle_tau
+    _VARIANT["patterns"] = args.patterns
     if args.impl == "reference":
         return run_reference(args)
     return run_cuda(args)

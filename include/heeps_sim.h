@@ -61,6 +61,15 @@ typedef struct {
     int32_t n_channels;            /* C, 1..SIM_MAX_CHANNELS */
     const double *channel_offset_m;/* [C] host; along-track offsets about the Rx state vector (G8) */
     double cull_two_way_db;        /* facet dropped for all channels iff 20log10|G_t G_r,ref| < this; <= -300 disables (G6) */
+    /* Antenna patterns as complex u-v grids.  A non-NULL table replaces that
+     * antenna's analytic aperture pattern: complex field gain (re, im interleaved) on pattern_nv x pattern_nu nodes,
+     * u = direction cosine along the azimuth axis over [pattern_u[0], pattern_u[1]] (first and last node), v likewise
+     * along the elevation axis; bilinear between nodes, zero outside the grid (reading G29).  Time dependence (TOPSAR
+     * steering) enters through the per-pulse frames of sim_geometry.  With a table the geometry is evaluated at every
+     * pulse (sim_options.geometry_keyframe does not apply). */
+    const float *tx_pattern, *rx_pattern;              /* host [nv][nu][2] or NULL */
+    int32_t tx_pattern_nu, tx_pattern_nv, rx_pattern_nu, rx_pattern_nv;
+    double tx_pattern_u[2], tx_pattern_v[2], rx_pattern_u[2], rx_pattern_v[2];
 } sim_instrument;
 
 /* Geometry: per-pulse Tx/Rx state vectors (stop-and-go, reading G9) */

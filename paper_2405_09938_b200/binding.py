@@ -36,6 +36,11 @@ class sim_instrument(C.Structure):
         ("fs_hz", C.c_double), ("prf_hz", C.c_double), ("n_samples", C.c_int32),
         ("tx_aperture_m", C.c_double * 2), ("rx_aperture_m", C.c_double * 2),
         ("n_channels", C.c_int32), ("channel_offset_m", C.c_void_p), ("cull_two_way_db", C.c_double),
+        ("tx_pattern", C.c_void_p), ("rx_pattern", C.c_void_p),
+        ("tx_pattern_nu", C.c_int32), ("tx_pattern_nv", C.c_int32),
+        ("rx_pattern_nu", C.c_int32), ("rx_pattern_nv", C.c_int32),
+        ("tx_pattern_u", C.c_double * 2), ("tx_pattern_v", C.c_double * 2),
+        ("rx_pattern_u", C.c_double * 2), ("rx_pattern_v", C.c_double * 2),
     ]
 
 
@@ -179,6 +184,15 @@ def _marshal(workload):
     ci.n_channels = off.size
     ci.channel_offset_m = ptr(off)
     ci.cull_two_way_db = inst["cull_two_way_db"]
+    for name in ("tx_pattern", "rx_pattern"):        # dict: table complex [nv][nu], u = (first, last node), v likewise
+        pat = inst.get(name)
+        if pat is not None:
+            tab = np.asarray(pat["table"])
+            t2 = np.ascontiguousarray(np.stack([tab.real, tab.imag], axis=-1), dtype=np.float32)
+            setattr(ci, name, ptr(t2))
+            setattr(ci, name + "_nv", int(tab.shape[0])); setattr(ci, name + "_nu", int(tab.shape[1]))
+            getattr(ci, name + "_u")[:] = [float(pat["u"][0]), float(pat["u"][1])]
+            getattr(ci, name + "_v")[:] = [float(pat["v"][0]), float(pat["v"][1])]
 
     cg = sim_geometry()
     P = int(geo["n_pulses"]); cg.n_pulses = P

@@ -73,6 +73,7 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
         bool keep = false;
         double pos[3] = {0, 0, 0};
         float gt = 0.f, a0 = 0.f;
+        float2 gtc = make_float2(0.f, 0.f);                  // complex Tx gain (tabulated patterns only)
         double rt = 0;
         float2 xi = make_float2(0.f, 0.f);
         float xi_mag = 0.f;
@@ -94,6 +95,12 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
             Leg lr = leg(pos, pc.rx_ref, pc.rx_a, pc.rx_e, prm.ap_rx_a, prm.ap_rx_e);
             rt = lt.r; gt = lt.g;
             keep = !(fabsf(gt * lr.g) < prm.cull_thr);
+            if (prm.lut_any) {                               // tabulated patterns: complex gains, cull on |G_t| |G_r,ref|
+                gtc = gain_of(prm, 0, lt.g, lt.ua, lt.ue);
+                const float2 grc = gain_of(prm, 1, lr.g, lr.ua, lr.ue);
+                gt = gtc.x;
+                keep = !(hypotf(gtc.x, gtc.y) * hypotf(grc.x, grc.y) < prm.cull_thr);
+            }
             // O8 amplitude
             float sig = a.sigma0 ? __ldg(a.sigma0 + f) : (float)prm.sigma0_uniform;
             if (prm.tilt) {
@@ -139,12 +146,22 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
                 const double nu = cs - prm.half_len;
                 const int b = (int)ceil(nu);
                 const int e = (int)ceil(nu + prm.len);
-                const float g = a0 * gt * lr.g;
+                float g = a0 * gt * lr.g;
+                float2 cg = make_float2(g, 0.f);                   // a G_t G_r,c
+                uint32_t garg = (gt * lr.g < 0.f) ? 0x80000000u : 0u;
+                float grx_re = lr.g;
+                if (prm.lut_any) {
+                    const float2 grc = gain_of(prm, 1, lr.g, lr.ua, lr.ue);
+                    const float2 pr = cmulf(gtc, grc);
+                    cg = make_float2(a0 * pr.x, a0 * pr.y);
+                    g = hypotf(cg.x, cg.y);
+                    garg = arg_u32(cg);
+                    grx_re = grc.x;
+                }
                 if (keep) {
                     Rec r;
                     // arg(A~) = arg(xi) (+ half a turn when G_t G_r < 0): exact adds on the phase word
-                    r.phi = turns_to_u32(fma(prm.kappa * cp, cp, -dR * prm.inv_lambda)) + kPhiBias + xi_arg +
-                            ((gt * lr.g < 0.f) ? 0x80000000u : 0u);
+                    r.phi = turns_to_u32(fma(prm.kappa * cp, cp, -dR * prm.inv_lambda)) + kPhiBias + xi_arg + garg;
                     r.beta = turns_to_u32(-2.0 * prm.kappa * cp) + s_shift[c];
                     double sw, cw;
                     sincospi(2.0 * ((double)(int32_t)r.beta * (1.0 / 4294967296.0)), &sw, &cw);
@@ -160,13 +177,13 @@ geometry_kernel(DevParams prm, GeometryArgs a, int p0, int n_pl)
                 }
                 if (kDebug) {
                     if (a.dbg_tau) a.dbg_tau[(size_t)c * F + f] = (rt + lr.r) / kC0;
-                    if (a.dbg_grx) a.dbg_grx[(size_t)c * F + f] = lr.g;
+                    if (a.dbg_grx) a.dbg_grx[(size_t)c * F + f] = grx_re;
                     if (a.dbg_amp) {
                         double turns = dR * prm.inv_lambda;
                         turns = (turns - floor(turns)) + a.carrier_frac_t0[p];
                         double sn, cn;
                         sincospi(-2.0 * turns, &sn, &cn);
-                        double ar = (double)(g * xi.x), ai = (double)(g * xi.y);
+                        double ar = (double)cg.x * xi.x - (double)cg.y * xi.y, ai = (double)cg.x * xi.y + (double)cg.y * xi.x;
                         a.dbg_amp[2 * ((size_t)c * F + f)] = ar * cn - ai * sn;
                         a.dbg_amp[2 * ((size_t)c * F + f) + 1] = ar * sn + ai * cn;
                     }

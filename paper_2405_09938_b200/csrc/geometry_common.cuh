@@ -53,7 +53,40 @@ __device__ __forceinline__ uint32_t turns_to_u32_fast(double x)
     return (uint32_t)(unsigned long long)__double2ll_rn(x * 4294967296.0);
 }
 
-struct Leg { double r; float g; };
+struct Leg { double r; float g; double ua, ue; };    // range, analytic gain, direction cosines along azimuth / elevation
+
+// Tabulated pattern (reading G29): bilinear interpolant of the four surrounding nodes, real and imaginary parts
+// separately; zero outside the grid.  Grid coordinates in fp64 (a float direction cosine resolves only ~1e-3 of a
+// fine grid's step), weights and values in fp32.
+__device__ __forceinline__ float2 lut_gain(const PatternLut &L, double ua, double ue)
+{
+    const double gu = (ua - L.u0) * L.su, gv = (ue - L.v0) * L.sv;
+    if (!(gu >= 0.0 && gu <= (double)(L.nu - 1) && gv >= 0.0 && gv <= (double)(L.nv - 1))) return make_float2(0.f, 0.f);
+    const int iu = min((int)gu, L.nu - 2), iv = min((int)gv, L.nv - 2);
+    const float fu = (float)(gu - iu), fv = (float)(gv - iv);
+    const float2 *t = L.tab + (size_t)iv * L.nu + iu;
+    const float2 t00 = __ldg(t), t01 = __ldg(t + 1), t10 = __ldg(t + L.nu), t11 = __ldg(t + L.nu + 1);
+    const float w00 = (1.f - fu) * (1.f - fv), w01 = fu * (1.f - fv), w10 = (1.f - fu) * fv, w11 = fu * fv;
+    return make_float2(w00 * t00.x + w01 * t01.x + w10 * t10.x + w11 * t11.x,
+                       w00 * t00.y + w01 * t01.y + w10 * t10.y + w11 * t11.y);
+}
+
+// Complex gain of antenna k (0 Tx, 1 Rx): the table if there is one, else (analytic, 0).
+__device__ __forceinline__ float2 gain_of(const DevParams &prm, int k, float analytic, double ua, double ue)
+{
+    return prm.lut[k].tab ? lut_gain(prm.lut[k], ua, ue) : make_float2(analytic, 0.f);
+}
+
+__device__ __forceinline__ float2 cmulf(float2 a, float2 b)
+{
+    return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+}
+
+// arg z in 2^-32 turns (wrapping)
+__device__ __forceinline__ uint32_t arg_u32(float2 z)
+{
+    return (uint32_t)__float2int_rn(atan2f(z.y, z.x) * 0.15915494309189535f * 2147483648.0f) * 2u;
+}
 
 // One antenna leg with the pieces the receive-channel series needs: d = pos - ant, r = |d|, 1/r and
 // the un-normalised projections on the azimuth / elevation axes.
@@ -102,6 +135,7 @@ __device__ __forceinline__ Leg leg(const double pos[3], const double ant[3], con
     Leg o;
     o.r = r;
     o.g = sinc_pi((float)(ap_a * ua)) * sinc_pi((float)(ap_e * ue));
+    o.ua = ua; o.ue = ue;
     return o;
 }
 

@@ -51,6 +51,14 @@ struct __align__(16) TileSpan {  // per (channel, pulse-in-batch, tile)
     uint32_t pad;
 };
 
+// Antenna pattern as a complex u-v grid: tab[nv][nu] over the direction cosines
+// u = r^ . azimuth axis, v = r^ . elevation axis; node k of u sits at u0 + k / su.  tab == nullptr: analytic sinc aperture.
+struct PatternLut {
+    const float2 *tab;
+    int32_t nu, nv;
+    double u0, su, v0, sv;
+};
+
 // Scalars every kernel needs.
 struct DevParams {
     // grid / tiling
@@ -69,6 +77,8 @@ struct DevParams {
     int32_t n_waves, choppy, tilt, has_sigma0, has_current;
     double sigma0_uniform, look_x, look_y, cur_ux, cur_uy;
     int32_t series_channels;     // receive-channel legs by series about the un-offset phase centre (geometry_common.cuh)
+    int32_t lut_any;             // some antenna pattern is tabulated: gains are complex (geometry_common.cuh)
+    PatternLut lut[2];           // [0] Tx, [1] Rx
 };
 
 }  // namespace heeps

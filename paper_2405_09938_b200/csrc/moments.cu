@@ -83,6 +83,7 @@ moments_kernel(DevParams prm, MomentArgs a, int p0, int n_pl)
     double pos[FPT][3], rt[FPT], dv[FPT];
     LegParts ref[FPT];
     float gt[FPT], amag[FPT];
+    float gti[FPT];                                      // Im G_t (tabulated patterns only)
     uint32_t xarg[FPT];
     bool keep[FPT];
     int my_kept = 0;
@@ -92,7 +93,7 @@ moments_kernel(DevParams prm, MomentArgs a, int p0, int n_pl)
         const int li = k % ts, lj = k / ts;
         const int i = ti0 + li, j = tj0 + lj;
         keep[q] = false;
-        rt[q] = 0.0; gt[q] = 0.f; amag[q] = 0.f; xarg[q] = 0u;
+        rt[q] = 0.0; gt[q] = 0.f; gti[q] = 0.f; amag[q] = 0.f; xarg[q] = 0u;
         pos[q][0] = pos[q][1] = pos[q][2] = 0.0;
         if (k < ts * ts && i < prm.nx && j < prm.ny) {
             const size_t f = (size_t)j * prm.nx + i;
@@ -110,6 +111,12 @@ moments_kernel(DevParams prm, MomentArgs a, int p0, int n_pl)
             rt[q] = lt.r; gt[q] = pattern(lt.da, lt.de, lt.inv, prm.ap_tx_a, prm.ap_tx_e);
             const float g_ref = pattern(ref[q].da, ref[q].de, ref[q].inv, prm.ap_rx_a, prm.ap_rx_e);
             keep[q] = !(fabsf(gt[q] * g_ref) < prm.cull_thr);               // O7 (G6)
+            if (prm.lut_any) {                                              // tabulated patterns: complex gains
+                const float2 gtc = gain_of(prm, 0, gt[q], lt.da * lt.inv, lt.de * lt.inv);
+                const float2 grc = gain_of(prm, 1, g_ref, ref[q].da * ref[q].inv, ref[q].de * ref[q].inv);
+                gt[q] = gtc.x; gti[q] = gtc.y;
+                keep[q] = !(hypotf(gtc.x, gtc.y) * hypotf(grc.x, grc.y) < prm.cull_thr);
+            }
             float sig = a.sigma0 ? __ldg(a.sigma0 + f) : (float)prm.sigma0_uniform;
             if (prm.tilt) {
                 const float2 sl = surface_slope(a.surf, it, F, f);
@@ -149,9 +156,14 @@ moments_kernel(DevParams prm, MomentArgs a, int p0, int n_pl)
             if (!(bd > -(double)L && bd < (double)prm.n_samples)) continue;    // window misses [0, Ns)
             const int b = (int)bd;
             const double eps = bd - nu;                                    // [0, 1)
-            const float g = gt[q] * g_rx;
-            const uint32_t ph = turns_to_u32_fast(fma(prm.kappa * eps, eps, -dR * prm.inv_lambda)) + xarg[q] +
-                                ((g < 0.f) ? 0x80000000u : 0u);
+            float g = gt[q] * g_rx;
+            uint32_t garg = (g < 0.f) ? 0x80000000u : 0u;
+            if (prm.lut_any) {
+                const float2 cg = cmulf(make_float2(gt[q], gti[q]), gain_of(prm, 1, g_rx, da_c * inv_c, de_c * inv_c));
+                g = hypotf(cg.x, cg.y);
+                garg = arg_u32(cg);
+            }
+            const uint32_t ph = turns_to_u32_fast(fma(prm.kappa * eps, eps, -dR * prm.inv_lambda)) + xarg[q] + garg;
             float sn, cs;
             __sincosf((float)(int32_t)ph * 1.4629180792671596e-9f, &sn, &cs);   // 2 pi / 2^32
             const float mag = fabsf(g) * amag[q];

@@ -65,6 +65,7 @@ struct sim_handle {
     DevBuf<float> sigma0;
     DevBuf<float2> current, xi;
     DevBuf<uint2> xi_polar;              // {|xi|, arg xi in 2^-32 turns}, derived from xi on the device
+    DevBuf<float2> pattern[2];           // tabulated antenna patterns [nv][nu] (Tx, Rx), empty = analytic aperture
     // time-dependent speckle (speckle.cu; sim_scene.speckle_tau_s > 0)
     bool speckle_ar1 = false;
     uint64_t seed = 0;
@@ -171,6 +172,19 @@ int validate(const sim_instrument *in, const sim_geometry *g, const sim_scene *s
         return SIM_EINVAL;
     if (!(in->chirp_len_s * in->fs_hz < (double)(1 << 22))) return SIM_EINVAL;
     if (!finite_all(in->channel_offset_m, in->n_channels)) return SIM_EINVAL;
+    {   // tabulated antenna patterns: >= 2 x 2 nodes over an increasing, finite u-v range, finite values
+        const float *tab[2] = {in->tx_pattern, in->rx_pattern};
+        const int32_t nu[2] = {in->tx_pattern_nu, in->rx_pattern_nu}, nv[2] = {in->tx_pattern_nv, in->rx_pattern_nv};
+        const double *ur[2] = {in->tx_pattern_u, in->rx_pattern_u}, *vr[2] = {in->tx_pattern_v, in->rx_pattern_v};
+        for (int k = 0; k < 2; ++k) {
+            if (!tab[k]) continue;
+            if (nu[k] < 2 || nv[k] < 2 || (int64_t)nu[k] * nv[k] > ((int64_t)1 << 28)) return SIM_EINVAL;
+            if (!finite_all(ur[k], 2) || !finite_all(vr[k], 2) || !(ur[k][1] > ur[k][0]) || !(vr[k][1] > vr[k][0]))
+                return SIM_EINVAL;
+            const size_t n = (size_t)nu[k] * nv[k] * 2;
+            for (size_t i = 0; i < n; ++i) if (!std::isfinite(tab[k][i])) return SIM_EINVAL;
+        }
+    }
     if (g->n_pulses < 1) return SIM_EINVAL;
     if (!g->t_pulse_s || !g->tx_pos_m || !g->tx_vel_mps || !g->rx_pos_m || !g->rx_vel_mps || !g->tx_frame ||
         !g->rx_frame || !g->t0_s)
@@ -453,6 +467,7 @@ void sim_destroy(sim_handle *h)
     h->xt.release(); h->yt.release(); h->tt.release(); h->chirp_n.release(); h->carrier_p.release();
     h->wk.release(); h->carrier_frac.release(); h->pulses.release();
     h->sigma0.release(); h->current.release(); h->xi.release(); h->xi_polar.release();
+    h->pattern[0].release(); h->pattern[1].release();
     h->xi_state.release(); h->beta_g.release(); h->doppler_turns.release(); h->xi_t.release();
     h->z.release(); h->slope.release(); h->dxy.release();
     h->zt.release(); h->dxy_t.release(); h->omega.release(); h->recs.release(); h->tinfo.release();
@@ -566,7 +581,9 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
         prm.series_channels = (r_min > 0 && o_max <= 1e-4 * r_min) ? 1 : 0;
     }
     h->key_H = choose_keyframe_spacing(g, sc, opts ? opts->kinematics_keyframe : 0);
-    if (h->spectral && h->key_H > 1 && prm.series_channels && C <= kMaxKeyChannels &&
+    prm.lut_any = (in->tx_pattern || in->rx_pattern) ? 1 : 0;
+    // tabulated patterns: no keyframed geometry (its gain interpolant and guard are derived for the analytic aperture)
+    if (h->spectral && h->key_H > 1 && prm.series_channels && C <= kMaxKeyChannels && !prm.lut_any &&
         !(opts && opts->geometry_keyframe == 1)) {
         // keyframed geometry: the spacing the wave bound admits, halved until the geometry bounds hold too
         // (a forced spacing is tried as it is)
@@ -690,6 +707,22 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     if (sc->current_mps) {
         CKC(h->current.alloc(F));
         CKC(cudaMemcpy(h->current.p, sc->current_mps, F * sizeof(float2), cudaMemcpyHostToDevice));
+    }
+    {
+        const float *tab[2] = {in->tx_pattern, in->rx_pattern};
+        const int32_t nu[2] = {in->tx_pattern_nu, in->rx_pattern_nu}, nv[2] = {in->tx_pattern_nv, in->rx_pattern_nv};
+        const double *ur[2] = {in->tx_pattern_u, in->rx_pattern_u}, *vr[2] = {in->tx_pattern_v, in->rx_pattern_v};
+        for (int k = 0; k < 2; ++k) {
+            PatternLut &L = prm.lut[k];
+            L = PatternLut{};
+            if (!tab[k]) continue;
+            const size_t n = (size_t)nu[k] * nv[k];
+            CKC(h->pattern[k].alloc(n));
+            CKC(cudaMemcpy(h->pattern[k].p, tab[k], n * sizeof(float2), cudaMemcpyHostToDevice));
+            L.tab = h->pattern[k].p; L.nu = nu[k]; L.nv = nv[k];
+            L.u0 = ur[k][0]; L.su = (nu[k] - 1) / (ur[k][1] - ur[k][0]);
+            L.v0 = vr[k][0]; L.sv = (nv[k] - 1) / (vr[k][1] - vr[k][0]);
+        }
     }
     CKC(h->xi.alloc(F));
     if (sc->xi) {

@@ -9,7 +9,7 @@ import pytest
 
 from oracle import (ati_phase_rms_error, oracle_facets, oracle_generate, oracle_samples,
                     rel_l2_per_vector)
-from workloads import make_workload, make_sweep_point
+from workloads import add_antenna_patterns, make_workload, make_sweep_point
 from helpers import custom_workload
 
 pytestmark = pytest.mark.gpu
@@ -250,6 +250,98 @@ def test_facet_intermediates(name):
     kept = o["keep"].astype(bool) & ~margin
     scale = np.abs(o["amp"][:, kept]).max()
     assert np.max(np.abs(g["amp"][:, kept] - o["amp"][:, kept])) < 5e-6 * scale
+
+
+# ----------------------------------------------------------------------------- NEXT-3: tabulated antenna patterns
+
+def _wide_tiny(n_pulses=6, d=60.0, **kw):
+    """Tiny with 60 m facets (a 3.8 km patch: the Tx main lobe is visibly curved across it), complex u-v pattern
+    tables on both antennas and TOPSAR-like azimuth steering through the per-pulse frames."""
+    w = make_workload("tiny", n_pulses=n_pulses)
+    w.scene["spacing_m"] = d
+    return add_antenna_patterns(w, **kw)
+
+
+def test_tabulated_patterns(mode):
+    w = _wide_tiny(nu=129, nv=33, steer_rate_deg_s=40.0)            # 0.2 deg over the 5 ms dwell ~ the beam width
+    ref = oracle_generate(w)
+    _assert_parity(_gpu(w, accumulate_mode=mode), ref, "u-v tables, steered")
+    # the tables matter: the analytic apertures give something else
+    for k in ("tx_pattern", "rx_pattern"):
+        del w.instrument[k]
+    assert rel_l2_per_vector(oracle_generate(w).astype(np.complex64), ref).min() > 1e-2
+
+
+def test_tabulated_pattern_facet_intermediates():
+    """Complex gains, cull on |G_t| |G_r,ref| and amplitudes per facet; a 5 x 3 table (coarse: the weights matter)
+    and a fine one."""
+    for nu, nv in ((5, 3), (257, 65)):
+        w = _wide_tiny(n_pulses=3, nu=nu, nv=nv, steer_rate_deg_s=60.0)
+        w.instrument["cull_two_way_db"] = -6.0
+        p = 2
+        with _sim(w) as sim:
+            g = sim.debug_facets(p)
+        o = oracle_facets(w, p)
+        assert np.max(np.abs(g["g_tx"] - o["g_tx"])) < 2e-6 and np.max(np.abs(g["g_rx"] - o["g_rx"])) < 2e-6
+        w_iso = _wide_tiny(n_pulses=3, nu=nu, nv=nv, steer_rate_deg_s=60.0)
+        for k in ("tx_pattern", "rx_pattern"):
+            del w_iso.instrument[k]
+        w_iso.instrument["tx_aperture_m"] = w_iso.instrument["rx_aperture_m"] = np.zeros(2)
+        two_way = np.abs(o["amp"][0] / oracle_facets(w_iso, p)["amp"][0])       # |G_t G_r,ref|, one channel
+        margin = np.abs(two_way - 10 ** (-6.0 / 20)) < 1e-5
+        assert 0.05 < o["keep"].mean() < 0.95                                    # the cull is active
+        assert np.array_equal(g["keep"][~margin], o["keep"][~margin])
+        kept = o["keep"].astype(bool) & ~margin
+        assert np.max(np.abs(g["amp"][:, kept] - o["amp"][:, kept])) < 5e-6 * np.abs(o["amp"][:, kept]).max()
+
+
+@pytest.mark.parametrize("which", ["tx_pattern", "rx_pattern"])
+def test_one_tabulated_antenna_and_partial_coverage(which, mode):
+    """One antenna tabulated, the other analytic (its side-lobe signs fold into the complex product); the table
+    covers only part of the scene: directions outside it contribute nothing."""
+    w = _wide_tiny(n_pulses=4, d=150.0, nu=33, nv=17)
+    other = "rx_pattern" if which == "tx_pattern" else "tx_pattern"
+    del w.instrument[other]
+    pat = w.instrument[which]
+    u0, u1 = pat["u"]
+    pat["u"] = (u0 + 0.3 * (u1 - u0), u1)                       # the table now starts 30 % into the scene
+    ref = oracle_generate(w)
+    with _sim(w, accumulate_mode=mode) as sim:
+        got = sim.generate().cpu().numpy()
+        st = sim.stats()
+    _assert_parity(got, ref, which)
+    kept = sum(int(oracle_facets(w, p)["keep"].sum()) for p in range(4))
+    assert 0.3 * 4 * 4096 < kept < 0.9 * 4 * 4096
+    assert abs(st["facet_echoes_kept"] - kept) <= 8             # facets within rounding of the grid edge / threshold
+
+
+def test_tabulated_pattern_error_codes():
+    from paper_2405_09938_b200 import SimError
+    def bad(mut):
+        w = _wide_tiny(n_pulses=2, nu=9, nv=5)
+        mut(w.instrument["tx_pattern"])
+        with pytest.raises(SimError) as e:
+            _sim(w)
+        assert e.value.code == -1
+    bad(lambda p: p.update(u=(p["u"][1], p["u"][0])))                       # decreasing range
+    bad(lambda p: p.update(v=(0.0, np.nan)))
+    bad(lambda p: p.update(table=p["table"][:, :1]))                        # a single column
+    def nan_node(p):
+        p["table"][2, 3] = np.nan
+    bad(nan_node)
+
+
+def test_ati_full_size_tabulated_patterns(mode):
+    """Config 1 at full size with 513 x 129 complex tables on both antennas and 1.5 deg/s azimuth steering, all 256
+    pulses in one call (the configuration bench.py --patterns times); the oracle checks three pulses."""
+    import torch
+    w = add_antenna_patterns(make_workload("ati"), nu=513, nv=129, steer_rate_deg_s=1.5)
+    pulses = [0, 101, 255]
+    with _sim(w, accumulate_mode=mode) as sim:
+        out = sim.generate()
+        torch.cuda.synchronize()
+        got = out[:, pulses].cpu().numpy()
+    _assert_parity(got, oracle_generate(w, pulses), "ati, tables")
 
 
 # ----------------------------------------------------------------------------- edge cases

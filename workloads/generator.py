@@ -299,18 +299,63 @@ def add_wave_nodes(w: Workload, spacing_m: float, seed: int = MASTER_SEED + 4) -
     return w
 
 
+def add_antenna_patterns(w: Workload, nu: int = 257, nv: int = 65, steer_rate_deg_s: float = 0.0,
+                         margin: float = 2.5e-4) -> Workload:
+    """Tabulated-antenna variant of a workload (complex Tx / Rx gains "converted into u-v grids").
+
+    The paper's antenna-model files are not available; these synthetic tables stand in for them: on `nv` x `nu` nodes
+    over the direction cosines (u along the azimuth axis, v along elevation) the scene spans during the dwell (plus
+    `margin`), a uniformly illuminated aperture's field pattern with a quadratic phase error across the beam (complex,
+    as a measured pattern is), stored as complex64.  `steer_rate_deg_s` != 0 adds TOPSAR-like azimuth beam steering: the
+    antenna frames rotate about their elevation axis at that rate about mid-dwell (the time dependence of the gain
+    enters through the per-pulse frames).  Table values are inputs; their use (lookup, interpolation) is the method's.
+    """
+    inst, geo, sc = w.instrument, w.geometry, w.scene
+    lam = C0 / inst["f0_hz"]
+    t = geo["t_pulse_s"]
+    if steer_rate_deg_s:
+        th = np.deg2rad(steer_rate_deg_s) * (t - 0.5 * (t[0] + t[-1]))
+        c, s = np.cos(th)[:, None], np.sin(th)[:, None]
+        for key in ("tx_frame", "rx_frame"):
+            fr = geo[key]
+            b, a = fr[:, 0].copy(), fr[:, 1].copy()
+            fr[:, 0] = c * b + s * a
+            fr[:, 1] = c * a - s * b
+    # extent of the scene's direction cosines: the corners of the grid at the first, middle and last pulse
+    hx, hy = 0.5 * (sc["nx"] - 1) * sc["spacing_m"], 0.5 * (sc["ny"] - 1) * sc["spacing_m"]
+    corners = np.asarray(sc["centre_m"])[None, :] + np.array([[sx * hx, sy * hy, 0.0] for sx in (-1, 1) for sy in (-1, 1)])
+    for key, ap in (("tx", inst["tx_aperture_m"]), ("rx", inst["rx_aperture_m"])):
+        lo, hi = np.full(2, np.inf), np.full(2, -np.inf)
+        for p in (0, len(t) // 2, len(t) - 1):
+            dvec = corners - geo[key + "_pos_m"][p][None, :]
+            uhat = dvec / np.linalg.norm(dvec, axis=1, keepdims=True)
+            uv = np.stack([uhat @ geo[key + "_frame"][p, 1], uhat @ geo[key + "_frame"][p, 2]], axis=1)
+            lo, hi = np.minimum(lo, uv.min(0)), np.maximum(hi, uv.max(0))
+        ur, vr = (lo[0] - margin, hi[0] + margin), (lo[1] - margin, hi[1] + margin)
+        un, vn = np.meshgrid(np.linspace(*ur, nu), np.linspace(*vr, nv))
+        xa, xe = ap[0] * un / lam, ap[1] * vn / lam
+        tab = np.sinc(xa) * np.sinc(xe) * np.exp(1j * (0.35 * xa**2 - 0.2 * xe))
+        inst[key + "_pattern"] = dict(table=np.ascontiguousarray(tab.astype(np.complex64)), u=ur, v=vr)
+    return w
+
+
+def _digest_update(h, v):
+    if v is None:
+        h.update(b"none")
+    elif isinstance(v, np.ndarray):
+        h.update(str(v.dtype).encode() + str(v.shape).encode())
+        h.update(np.ascontiguousarray(v).tobytes())
+    elif isinstance(v, dict):
+        for key in sorted(v):
+            h.update(key.encode())
+            _digest_update(h, v[key])
+    else:
+        h.update(repr(v).encode())
+
+
 def workload_digest(w: Workload) -> str:
     """SHA-256 over every generated array (G22: the workload must not drift between runs)."""
     h = hashlib.sha256()
     for group in (w.instrument, w.geometry, w.scene):
-        for key in sorted(group):
-            v = group[key]
-            h.update(key.encode())
-            if v is None:
-                h.update(b"none")
-            elif isinstance(v, np.ndarray):
-                h.update(str(v.dtype).encode() + str(v.shape).encode())
-                h.update(np.ascontiguousarray(v).tobytes())
-            else:
-                h.update(repr(v).encode())
+        _digest_update(h, group)
     return h.hexdigest()
