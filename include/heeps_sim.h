@@ -65,8 +65,9 @@ typedef struct {
      * antenna's analytic aperture pattern: complex field gain (re, im interleaved) on pattern_nv x pattern_nu nodes,
      * u = direction cosine along the azimuth axis over [pattern_u[0], pattern_u[1]] (first and last node), v likewise
      * along the elevation axis; bilinear between nodes, zero outside the grid (reading G29).  Time dependence (TOPSAR
-     * steering) enters through the per-pulse frames of sim_geometry.  With a table the geometry is evaluated at every
-     * pulse (sim_options.geometry_keyframe does not apply). */
+     * steering) enters through the per-pulse frames of sim_geometry.  The keyframed geometry (sim_options.geometry_keyframe)
+     * accepts a table only when it is fine enough for its three-point gain interpolant (node-to-node second differences
+     * <= ~1e-4, checked at sim_create); a coarser table is looked up at every pulse. */
     const float *tx_pattern, *rx_pattern;              /* host [nv][nu][2] or NULL */
     int32_t tx_pattern_nu, tx_pattern_nv, rx_pattern_nu, rx_pattern_nv;
     double tx_pattern_u[2], tx_pattern_v[2], rx_pattern_u[2], rx_pattern_v[2];

@@ -156,18 +156,19 @@ moments_kernel(DevParams prm, MomentArgs a, int p0, int n_pl)
             if (!(bd > -(double)L && bd < (double)prm.n_samples)) continue;    // window misses [0, Ns)
             const int b = (int)bd;
             const double eps = bd - nu;                                    // [0, 1)
-            float g = gt[q] * g_rx;
-            uint32_t garg = (g < 0.f) ? 0x80000000u : 0u;
-            if (prm.lut_any) {
-                const float2 cg = cmulf(make_float2(gt[q], gti[q]), gain_of(prm, 1, g_rx, da_c * inv_c, de_c * inv_c));
-                g = hypotf(cg.x, cg.y);
-                garg = arg_u32(cg);
-            }
+            const float g = gt[q] * g_rx;
+            const uint32_t garg = (g < 0.f && !prm.lut_any) ? 0x80000000u : 0u;
             const uint32_t ph = turns_to_u32_fast(fma(prm.kappa * eps, eps, -dR * prm.inv_lambda)) + xarg[q] + garg;
             float sn, cs;
             __sincosf((float)(int32_t)ph * 1.4629180792671596e-9f, &sn, &cs);   // 2 pi / 2^32
-            const float mag = fabsf(g) * amag[q];
-            br[q] = mag * cs; bi[q] = mag * sn;
+            if (prm.lut_any) {                                             // complex gain product times the phasor
+                const float2 cg = cmulf(make_float2(gt[q], gti[q]), gain_of(prm, 1, g_rx, da_c * inv_c, de_c * inv_c));
+                const float2 w = cmulf(cg, make_float2(cs, sn));
+                br[q] = amag[q] * w.x; bi[q] = amag[q] * w.y;
+            } else {
+                const float mag = fabsf(g) * amag[q];
+                br[q] = mag * cs; bi[q] = mag * sn;
+            }
             yy[q] = (float)(2.0 * eps - 1.0);
             my_samples += (unsigned)(min(b + L, prm.n_samples) - max(b, 0));
             const int rel = b - base;

@@ -53,6 +53,7 @@ struct KeyEval {
     float xat, xet, xar, xer;            // sinc arguments: Tx azimuth / elevation, Rx (un-offset) azimuth / elevation
     float xao, xeo;                      // Rx arguments at the finite-difference offset o_fd
     float la, lb;                        // r_r,c - r_r,ref = o_c la + o_c^2 lb  (series in o_c / r)
+    double uat, uet, uar, uer, uao, ueo; // the same six as direction cosines (tabulated patterns: grid coordinates in fp64)
 };
 
 template <int C>
@@ -68,11 +69,13 @@ __device__ __forceinline__ KeyEval<C> key_eval(const DevParams &prm, const Pulse
     o.Rd = fma(at, lt.inv, ar * lr.inv);
     o.xat = (float)(prm.ap_tx_a * (lt.da * lt.inv)); o.xet = (float)(prm.ap_tx_e * (lt.de * lt.inv));
     o.xar = (float)(prm.ap_rx_a * (lr.da * lr.inv)); o.xer = (float)(prm.ap_rx_e * (lr.de * lr.inv));
+    o.uat = lt.da * lt.inv; o.uet = lt.de * lt.inv; o.uar = lr.da * lr.inv; o.uer = lr.de * lr.inv;
     const double dv = fma(lr.dx, pc.rx_vhat[0], fma(lr.dy, pc.rx_vhat[1], lr.dz * pc.rx_vhat[2]));
     {
         double r_c, inv_c, da_c, de_c;
         channel_leg_series(lr, dv, o_fd, pc.rx_va, pc.rx_ve, r_c, inv_c, da_c, de_c);
         o.xao = (float)(prm.ap_rx_a * (da_c * inv_c)); o.xeo = (float)(prm.ap_rx_e * (de_c * inv_c));
+        o.uao = da_c * inv_c; o.ueo = de_c * inv_c;
     }
     // r_c - r = r (dl/2 - dl^2/8 + ...), dl = (o^2 - 2 o d.v^)/r^2  (geometry_common.cuh)
     //         = -o (d.v^)/r + o^2 (1 - (d.v^/r)^2)/(2 r) + O(o^3/r^2)
@@ -110,7 +113,15 @@ __device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b)
 
 __device__ __forceinline__ float pattern_x(float xa, float xe) { return sinc_pi_fast(xa) * sinc_pi_fast(xe); }
 
-template <int FPT, int C, bool kTilt, bool kSpeckleT>
+// Complex gain of antenna k at direction cosines (ua, ue): the table if there is one, else the analytic aperture.
+__device__ __forceinline__ float2 gain_at(const DevParams &prm, int k, double ua, double ue)
+{
+    if (prm.lut[k].tab) return lut_gain(prm.lut[k], ua, ue);
+    const double apa = k ? prm.ap_rx_a : prm.ap_tx_a, ape = k ? prm.ap_rx_e : prm.ap_tx_e;
+    return make_float2(pattern_x((float)(apa * ua), (float)(ape * ue)), 0.f);
+}
+
+template <int FPT, int C, bool kTilt, bool kSpeckleT, bool kLut>
 __global__ void __launch_bounds__(kThreads, 2)
 moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_first)
 {
@@ -207,6 +218,8 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     float lb_sum = 0.f;                                  // lb varies by 1e-4 relative over a tile: one value per thread
     int lb_n = 0;
     float pq0[FPT], pqa[FPT], pqb[FPT], bq[FPT];         // P(s) = pq0 + s (pqa + s pqb); bq = G_t dG_r/do
+    constexpr int FL = kLut ? FPT : 1;                   // tabulated patterns: P and bq are complex, these are the imaginary parts
+    float qi0[FL], qia[FL], qib[FL], bqi[FL];
     float am0[FPT], ama[FPT], amb[FPT];                  // |a_f|(s), quadratic when tilt-modulated
     uint32_t xarg[FPT];
     bool valid[FPT];
@@ -219,6 +232,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         R0[q] = RD[q] = 0.0; ra[q] = rb[q] = 0.f;
         pq0[q] = pqa[q] = pqb[q] = bq[q] = 0.f; am0[q] = ama[q] = amb[q] = 0.f; xarg[q] = 0u;
         la0[q] = dla[q] = 0.f;
+        if (kLut) qi0[q] = qia[q] = qib[q] = bqi[q] = 0.f;
         if (!valid[q]) continue;
         const size_t f = (size_t)jj * prm.nx + i;
         const double xb = prm.cx + ((double)i - 0.5 * (prm.nx - 1)) * prm.spacing;
@@ -246,6 +260,18 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         la0[q] = ev[0].la; dla[q] = ev[1].la - ev[0].la;
         lb_sum += 0.5f * (ev[0].lb + ev[1].lb); ++lb_n;
         // gains at s = 0, 1/2, 1 (sinc arguments at the midpoint = mean of the end values)
+        if (kLut) {
+            const float2 P0 = cmulf(gain_at(prm, 0, ev[0].uat, ev[0].uet), gain_at(prm, 1, ev[0].uar, ev[0].uer));
+            const float2 P1 = cmulf(gain_at(prm, 0, ev[1].uat, ev[1].uet), gain_at(prm, 1, ev[1].uar, ev[1].uer));
+            const float2 gtm = gain_at(prm, 0, 0.5 * (ev[0].uat + ev[1].uat), 0.5 * (ev[0].uet + ev[1].uet));
+            const float2 grm = gain_at(prm, 1, 0.5 * (ev[0].uar + ev[1].uar), 0.5 * (ev[0].uer + ev[1].uer));
+            const float2 gom = gain_at(prm, 1, 0.5 * (ev[0].uao + ev[1].uao), 0.5 * (ev[0].ueo + ev[1].ueo));
+            const float2 Pm = cmulf(gtm, grm);
+            const float2 dq = cmulf(gtm, make_float2((gom.x - grm.x) * inv_ofd, (gom.y - grm.y) * inv_ofd));
+            pq0[q] = P0.x; pqa[q] = -3.f * P0.x + 4.f * Pm.x - P1.x; pqb[q] = 2.f * P0.x - 4.f * Pm.x + 2.f * P1.x;
+            qi0[q] = P0.y; qia[q] = -3.f * P0.y + 4.f * Pm.y - P1.y; qib[q] = 2.f * P0.y - 4.f * Pm.y + 2.f * P1.y;
+            bq[q] = dq.x; bqi[q] = dq.y;
+        } else {
         const float gt0 = pattern_x(ev[0].xat, ev[0].xet), gr0 = pattern_x(ev[0].xar, ev[0].xer);
         const float gt1 = pattern_x(ev[1].xat, ev[1].xet), gr1 = pattern_x(ev[1].xar, ev[1].xer);
         const float gtm = pattern_x(0.5f * (ev[0].xat + ev[1].xat), 0.5f * (ev[0].xet + ev[1].xet));
@@ -254,6 +280,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         const float P0 = gt0 * gr0, Pm = gtm * grm, P1 = gt1 * gr1;
         pq0[q] = P0; pqa[q] = -3.f * P0 + 4.f * Pm - P1; pqb[q] = 2.f * P0 - 4.f * Pm + 2.f * P1;
         bq[q] = gtm * (gom - grm) * inv_ofd;
+        }
         // amplitude (O8): sqrt(sigma0 tilt d^2) |xi|
         const float sig = a.sigma0 ? __ldg(a.sigma0 + f) : (float)prm.sigma0_uniform;
         // static speckle: |xi| and arg xi are constants of the facet; time-dependent speckle (speckle.cu): per pulse
@@ -304,7 +331,9 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
 #pragma unroll
         for (int q = 0; q < FPT; ++q) {
             const float Pv = fmaf(s, fmaf(s, pqb[q], pqa[q]), pq0[q]);
-            const bool keep = valid[q] && !(fabsf(Pv) < prm.cull_thr);     // O7 (G6)
+            const float Pi = kLut ? fmaf(s, fmaf(s, qib[kLut ? q : 0], qia[kLut ? q : 0]), qi0[kLut ? q : 0]) : 0.f;
+            const bool keep = valid[q] && !(kLut ? (fmaf(Pv, Pv, Pi * Pi) < prm.cull_thr * prm.cull_thr)
+                                                 : (fabsf(Pv) < prm.cull_thr));     // O7 (G6)
             my_kept += keep ? 1 : 0;
             float am = kTilt ? fmaf(s, fmaf(s, amb[q], ama[q]), am0[q]) : am0[q];
             uint32_t xa = xarg[q];
@@ -329,21 +358,26 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                 const float g = fmaf(och[c], bq[q], Pv);
                 const uint32_t ph = (uint32_t)(unsigned long long)__double2ll_rn(
                                         fma(-dR, il32, (double)(kappa32 * eps * eps))) +
-                                    xa + ((g < 0.f) ? 0x80000000u : 0u);
+                                    xa + ((g < 0.f && !kLut) ? 0x80000000u : 0u);
                 float sn, cs;
                 __sincosf((float)(int32_t)ph * 1.4629180792671596e-9f, &sn, &cs);   // 2 pi / 2^32
                 const float mag = fabsf(g) * am;
+                float wr = mag * cs, wi = mag * sn;                        // complex weight of the facet-echo
+                if (kLut) {                                                // complex gain times the phasor
+                    const float gi = fmaf(och[c], bqi[kLut ? q : 0], Pi);
+                    wr = am * fmaf(g, cs, -gi * sn); wi = am * fmaf(g, sn, gi * cs);
+                }
                 const float yv = fmaf(2.f, eps, -1.f);
                 const int rel = b - kp.base[c];
                 const bool inspan = (unsigned)rel < (unsigned)span;
                 pr[q][c] = -1;
                 if (inwin && inspan) {
-                    pay[c * cap + k] = make_float2(mag * cs, mag * sn);
+                    pay[c * cap + k] = make_float2(wr, wi);
                     pay_y[c * cap + k] = yv;
                     pr[q][c] = (rel << 12) | atomicAdd(&hs[c * hstride + rel + 1], 1);
                 }
                 if (inwin && !inspan) {                                    // outside the tile window: rare
-                    const float br = mag * cs, bi = mag * sn;
+                    const float br = wr, bi = wi;
                     float2 *row = a.mom + ((size_t)(c * n_pl + pl) * kKt) * a.nb_pad + (b + L - 1);
                     float t0 = 1.f, t1 = yv;
                     atomicAdd(row, make_float2(br, bi));
@@ -484,9 +518,14 @@ cudaError_t launch_fc(const DevParams &prm, const MomentArgs &a, int p0, int n_p
         kern<<<grid, kThreads, smem, s>>>(prm, a, p0, n_pl, j_first);
         return cudaGetLastError();
     };
+    if (prm.lut_any) {
+        if (a.xi_pulse_stride)
+            return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, true, true>) : go(moments_keyframed_kernel<FPT, C, false, true, true>);
+        return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, false, true>) : go(moments_keyframed_kernel<FPT, C, false, false, true>);
+    }
     if (a.xi_pulse_stride)
-        return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, true>) : go(moments_keyframed_kernel<FPT, C, false, true>);
-    return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, false>) : go(moments_keyframed_kernel<FPT, C, false, false>);
+        return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, true, false>) : go(moments_keyframed_kernel<FPT, C, false, true, false>);
+    return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, false, false>) : go(moments_keyframed_kernel<FPT, C, false, false, false>);
 }
 
 template <int FPT>

@@ -3,6 +3,7 @@
 // the caller's stream with no host synchronisation inside sim_generate.
 #include <algorithm>
 #include <cmath>
+#include <complex>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -349,9 +350,53 @@ long double sincl_pi(long double x)
     return sinl(a) / a;
 }
 
+typedef std::complex<long double> cld;
+
 struct GuardEval {
     long double R, Rd, xat, xet, xar, xer, xao, xeo, dl[SIM_MAX_CHANNELS], gt, gr[SIM_MAX_CHANNELS];
+    long double uat, uet, uar, uer, uao, ueo;          // the six sinc arguments as direction cosines
+    cld gtc, grc[SIM_MAX_CHANNELS];                    // complex gains (tabulated patterns, reading G29; else (analytic, 0))
 };
+
+// Complex gain of antenna k (0 Tx, 1 Rx) at direction cosines (ua, ue): bilinear in the u-v table when there is one
+// (zero outside the grid), else the analytic aperture pattern.
+cld host_gain(const sim_instrument *in, int k, long double ua, long double ue)
+{
+    const float *tab = k ? in->rx_pattern : in->tx_pattern;
+    if (!tab) {
+        const long double lambda = (long double)kC0 / in->f0_hz;
+        const double *ap = k ? in->rx_aperture_m : in->tx_aperture_m;
+        return cld(sincl_pi(ap[0] / lambda * ua) * sincl_pi(ap[1] / lambda * ue), 0.0L);
+    }
+    const int nu = k ? in->rx_pattern_nu : in->tx_pattern_nu, nv = k ? in->rx_pattern_nv : in->tx_pattern_nv;
+    const double *ur = k ? in->rx_pattern_u : in->tx_pattern_u, *vr = k ? in->rx_pattern_v : in->tx_pattern_v;
+    const long double gu = (ua - ur[0]) * (nu - 1) / ((long double)ur[1] - ur[0]);
+    const long double gv = (ue - vr[0]) * (nv - 1) / ((long double)vr[1] - vr[0]);
+    if (!(gu >= 0 && gu <= nu - 1 && gv >= 0 && gv <= nv - 1)) return cld(0, 0);
+    const int iu = std::min((int)gu, nu - 2), iv = std::min((int)gv, nv - 2);
+    const long double fu = gu - iu, fv = gv - iv;
+    auto node = [&](int a, int b) { const float *t = tab + 2 * ((size_t)(iv + b) * nu + iu + a); return cld(t[0], t[1]); };
+    return (1 - fv) * ((1 - fu) * node(0, 0) + fu * node(1, 0)) + fv * ((1 - fu) * node(0, 1) + fu * node(1, 1));
+}
+
+// Largest |second difference| / 8 of a table along u plus along v: the distance between the bilinear interpolant and
+// any smooth function through the nodes (h^2 |G''| / 8 per axis); and the largest |node|.  (0, 1) for an analytic antenna.
+void table_roughness(const sim_instrument *in, int k, long double &delta, long double &gmax)
+{
+    const float *tab = k ? in->rx_pattern : in->tx_pattern;
+    delta = 0; gmax = 1;
+    if (!tab) return;
+    const int nu = k ? in->rx_pattern_nu : in->tx_pattern_nu, nv = k ? in->rx_pattern_nv : in->tx_pattern_nv;
+    auto node = [&](int a, int b) { const float *t = tab + 2 * ((size_t)b * nu + a); return std::complex<double>(t[0], t[1]); };
+    double du = 0, dv = 0, gm = 0;
+    for (int b = 0; b < nv; ++b)
+        for (int a = 0; a < nu; ++a) {
+            gm = std::max(gm, std::abs(node(a, b)));
+            if (a > 0 && a + 1 < nu) du = std::max(du, std::abs(node(a - 1, b) - 2.0 * node(a, b) + node(a + 1, b)));
+            if (b > 0 && b + 1 < nv) dv = std::max(dv, std::abs(node(a, b - 1) - 2.0 * node(a, b) + node(a, b + 1)));
+        }
+    delta = (du + dv) / 8; gmax = gm;
+}
 
 GuardEval guard_eval(const sim_instrument *in, const sim_geometry *g, int p, const long double pos[3],
                      const long double vel[3], long double o_fd)
@@ -375,19 +420,30 @@ GuardEval guard_eval(const sim_instrument *in, const sim_geometry *g, int p, con
     args(dt, rt, tf, in->tx_aperture_m, o.xat, o.xet);
     args(dr, rr, rf, in->rx_aperture_m, o.xar, o.xer);
     o.gt = sincl_pi(o.xat) * sincl_pi(o.xet);
-    auto offset_leg = [&](long double off, long double &r_c, long double &xa, long double &xe) {
+    auto cosines = [&](const long double d[3], long double r, const double *frame, long double &ua, long double &ue) {
+        ua = ue = 0;
+        for (int k = 0; k < 3; ++k) { ua += d[k] * frame[3 + k]; ue += d[k] * frame[6 + k]; }
+        ua /= r; ue /= r;
+    };
+    cosines(dt, rt, tf, o.uat, o.uet);
+    cosines(dr, rr, rf, o.uar, o.uer);
+    o.gtc = host_gain(in, 0, o.uat, o.uet);
+    auto offset_leg = [&](long double off, long double &r_c, long double &xa, long double &xe, long double &ua,
+                          long double &ue) {
         long double d[3]; r_c = 0;
         for (int k = 0; k < 3; ++k) { d[k] = pos[k] - (rp[k] + off * rv[k] / vn); r_c += d[k] * d[k]; }
         r_c = sqrtl(r_c);
         args(d, r_c, rf, in->rx_aperture_m, xa, xe);
+        cosines(d, r_c, rf, ua, ue);
     };
     long double r_o;
-    offset_leg(o_fd, r_o, o.xao, o.xeo);
+    offset_leg(o_fd, r_o, o.xao, o.xeo, o.uao, o.ueo);
     for (int c = 0; c < in->n_channels; ++c) {
-        long double r_c, xa, xe;
-        offset_leg(in->channel_offset_m[c], r_c, xa, xe);
+        long double r_c, xa, xe, ua, ue;
+        offset_leg(in->channel_offset_m[c], r_c, xa, xe, ua, ue);
         o.dl[c] = r_c - rr;
         o.gr[c] = sincl_pi(xa) * sincl_pi(xe);
+        o.grc[c] = host_gain(in, 1, ua, ue);
     }
     return o;
 }
@@ -400,6 +456,19 @@ bool geometry_keyframes_ok(const sim_instrument *in, const sim_geometry *g, cons
     long double o_fd = 0;
     for (int c = 0; c < C; ++c) o_fd = std::max<long double>(o_fd, std::fabs(in->channel_offset_m[c]));
     const long double vel[3] = {sc->current_uniform[0], sc->current_uniform[1], 0.0L};
+    // Tabulated patterns: the kernel's quadratic through three lookups follows a bilinear table only as closely as the
+    // table follows a smooth function; 2.25 = 1 + the Lebesgue constant 5/4 of the three-point quadratic.  The lattice
+    // check below samples the rest; together they must stay inside 3e-5 (the analytic apertures: 3e-6).
+    const bool lut = in->tx_pattern || in->rx_pattern;
+    long double kink = 0, gain_tol = 3e-6L;
+    if (lut) {
+        long double dt_, gt_, dr_, gr_;
+        table_roughness(in, 0, dt_, gt_);
+        table_roughness(in, 1, dr_, gr_);
+        kink = 2.25L * (dt_ * gr_ + dr_ * gt_);
+        gain_tol = 3e-5L;
+        if (!(kink <= gain_tol)) return false;
+    }
     for (int gx = -1; gx <= 1; ++gx)
         for (int gy = -1; gy <= 1; ++gy) {
             const long double x0 = sc->centre_m[0] + gx * 0.5L * (sc->nx - 1) * sc->spacing_m;
@@ -421,6 +490,16 @@ bool geometry_keyframes_ok(const sim_instrument *in, const sim_geometry *g, cons
                 const long double grm = pat(0.5L * (e0.xar + e1.xar), 0.5L * (e0.xer + e1.xer));
                 const long double gom = pat(0.5L * (e0.xao + e1.xao), 0.5L * (e0.xeo + e1.xeo));
                 const long double Pm = gtm * grm, bq = o_fd > 0 ? gtm * (gom - grm) / o_fd : 0.0L;
+                // the same three-point interpolant with complex (tabulated) gains
+                cld P0c, P1c, Pmc, bqc;
+                if (lut) {
+                    P0c = e0.gtc * host_gain(in, 1, e0.uar, e0.uer); P1c = e1.gtc * host_gain(in, 1, e1.uar, e1.uer);
+                    const cld gtmc = host_gain(in, 0, 0.5L * (e0.uat + e1.uat), 0.5L * (e0.uet + e1.uet));
+                    const cld grmc = host_gain(in, 1, 0.5L * (e0.uar + e1.uar), 0.5L * (e0.uer + e1.uer));
+                    const cld gomc = host_gain(in, 1, 0.5L * (e0.uao + e1.uao), 0.5L * (e0.ueo + e1.ueo));
+                    Pmc = gtmc * grmc;
+                    bqc = o_fd > 0 ? gtmc * (gomc - grmc) / o_fd : cld(0, 0);
+                }
                 for (int p = k0 + 1; p < k1; ++p) {
                     long double pp[3];
                     at(p, pp);
@@ -433,6 +512,12 @@ bool geometry_keyframes_ok(const sim_instrument *in, const sim_geometry *g, cons
                     for (int c = 0; c < C; ++c) {
                         const long double dl = e0.dl[c] + s * (e1.dl[c] - e0.dl[c]);
                         if (!(fabsl(dl - ex.dl[c]) <= 2e-8L)) return false;
+                        if (lut) {
+                            const cld gqc = P0c + s * ((-3.0L * P0c + 4.0L * Pmc - P1c) + s * (2.0L * P0c - 4.0L * Pmc + 2.0L * P1c)) +
+                                            (long double)in->channel_offset_m[c] * bqc;
+                            if (!(std::abs(gqc - ex.gtc * ex.grc[c]) + kink <= gain_tol)) return false;
+                            continue;
+                        }
                         const long double gq = Pq + (long double)in->channel_offset_m[c] * bq;
                         if (!(fabsl(gq - ex.gt * ex.gr[c]) <= 3e-6L)) return false;
                     }
@@ -582,8 +667,7 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     }
     h->key_H = choose_keyframe_spacing(g, sc, opts ? opts->kinematics_keyframe : 0);
     prm.lut_any = (in->tx_pattern || in->rx_pattern) ? 1 : 0;
-    // tabulated patterns: no keyframed geometry (its gain interpolant and guard are derived for the analytic aperture)
-    if (h->spectral && h->key_H > 1 && prm.series_channels && C <= kMaxKeyChannels && !prm.lut_any &&
+    if (h->spectral && h->key_H > 1 && prm.series_channels && C <= kMaxKeyChannels &&
         !(opts && opts->geometry_keyframe == 1)) {
         // keyframed geometry: the spacing the wave bound admits, halved until the geometry bounds hold too
         // (a forced spacing is tried as it is)

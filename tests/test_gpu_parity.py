@@ -341,7 +341,39 @@ def test_ati_full_size_tabulated_patterns(mode):
         out = sim.generate()
         torch.cuda.synchronize()
         got = out[:, pulses].cpu().numpy()
+        if mode == "spectral":
+            assert sim.stats()["geometry_keyframed"] == 1       # fine tables: the keyframed geometry kernel takes them
     _assert_parity(got, oracle_generate(w, pulses), "ati, tables")
+
+
+def test_tabulated_patterns_keyframed_geometry_and_its_guard():
+    """Spectral path with tables: a fine table goes through the keyframed geometry kernel (complex three-point gain
+    interpolant), a coarse one fails sim_create's roughness bound and is looked up at every pulse; forcing the
+    per-pulse kernel gives the same result; all against the oracle.  Steered frames, 3 channels, active cull."""
+    def wide(nu, nv):
+        w = make_workload("tiny", n_pulses=13)
+        w.scene["spacing_m"] = 120.0                               # a 7.7 km patch: wider than the Tx main lobe
+        w.instrument["channel_offset_m"] = np.array([-1.5, 0.0, 1.5])
+        w = add_antenna_patterns(w, nu=nu, nv=nv, steer_rate_deg_s=3.0)
+        w.instrument["cull_two_way_db"] = -10.0
+        return w
+    w = wide(2049, 257)
+    ref = oracle_generate(w)
+    kept = sum(int(oracle_facets(w, p)["keep"].sum()) for p in range(13))
+    assert 0.05 * 13 * w.n_facets < kept < 0.95 * 13 * w.n_facets
+    for gk, batch in ((0, 0), (0, 4), (1, 0)):
+        with _sim(w, accumulate_mode="spectral", geometry_keyframe=gk, kinematics_keyframe=4,
+                  pulses_per_batch=batch) as sim:
+            got = sim.generate().cpu().numpy()
+            st = sim.stats()
+        assert st["geometry_keyframed"] == 1 - gk, (gk, st)
+        assert abs(st["facet_echoes_kept"] - 3 * kept) <= 24
+        _assert_parity(got, ref, f"fine tables, geometry keyframes off={gk}")
+    wc = wide(9, 5)
+    with _sim(wc, accumulate_mode="spectral", kinematics_keyframe=4) as sim:
+        got = sim.generate().cpu().numpy()
+        assert sim.stats()["geometry_keyframed"] == 0
+    _assert_parity(got, oracle_generate(wc), "coarse tables")
 
 
 # ----------------------------------------------------------------------------- edge cases
