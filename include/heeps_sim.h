@@ -161,9 +161,12 @@ int sim_create(const sim_instrument *inst, const sim_geometry *geo, const sim_sc
 int sim_generate(sim_handle *h, int32_t pulse_begin, int32_t pulse_end, void *iq_dev, void *cuda_stream);
 
 /*
- * sim_generate_host: same, but iq_host is HOST memory (pinned memory gives an asynchronous
- * copy); the device->host copy is issued on cuda_stream and the call returns after the
- * stream has been synchronised.  Used for the end-to-end measurement.
+ * sim_generate_host: same, but iq_host is HOST memory, and the call returns after the samples
+ * are there (cuda_stream synchronised).  Page-locked memory the device can address
+ * (cudaHostAlloc, cudaHostRegister, a pinned torch tensor) is written directly by the last
+ * kernel of every batch: the PCIe transfer runs inside that kernel, nothing is staged or
+ * copied.  Pageable memory goes through a device staging buffer, finished batches copied on
+ * a second stream while the next batch computes.  Used for the end-to-end measurement.
  */
 int sim_generate_host(sim_handle *h, int32_t pulse_begin, int32_t pulse_end, void *iq_host, void *cuda_stream);
 

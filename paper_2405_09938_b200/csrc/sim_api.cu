@@ -1016,6 +1016,18 @@ int sim_generate_host(sim_handle *h, int32_t pulse_begin, int32_t pulse_end, voi
     if (!g.ok) return SIM_ECUDA;
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     const size_t n = (size_t)h->prm.n_channels * (pulse_end - pulse_begin) * h->prm.n_samples;
+    {   // page-locked, device-accessible host memory (cudaHostAlloc / cudaHostRegister under unified addressing): the
+        // last kernel of every batch stores the IQ samples straight into it -- the transfer over PCIe runs inside
+        // that kernel instead of after it, no staging buffer, no copy
+        cudaPointerAttributes at{};
+        if (cudaPointerGetAttributes(&at, iq_host) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer) {
+            int rc = run_batches(h, pulse_begin, pulse_end, static_cast<float2 *>(at.devicePointer), s);
+            if (rc != SIM_OK) return rc;
+            CK(h, cudaStreamSynchronize(s));
+            return SIM_OK;
+        }
+        (void)cudaGetLastError();                        // pageable memory: not an error, staged below
+    }
     if (h->out_staging.n < n) CK(h, h->out_staging.alloc(n));
     if (!h->copy_stream) CK(h, cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
     // the workspace-sized batches of the call are shipped as they finish (splitting a dwell that fits one batch

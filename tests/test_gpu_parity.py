@@ -527,7 +527,12 @@ def test_host_path_and_scene_update(mode):
     w = _hetero_small(96, 64, 2)
     ref = oracle_generate(w)
     with _sim(w, accumulate_mode=mode) as sim:
-        _assert_parity(sim.generate_host().numpy(), ref, "host path")
+        _assert_parity(sim.generate_host().numpy(), ref, "host path")       # pinned: written by the last kernel
+        pageable = torch.empty(ref.shape, dtype=torch.complex64)            # pageable: staged and copied
+        assert not pageable.is_pinned()
+        _assert_parity(sim.generate_host(out=pageable).numpy(), ref, "host path, pageable memory")
+        part = torch.zeros((ref.shape[0], 1, ref.shape[2]), dtype=torch.complex64, pin_memory=True)
+        _assert_parity(sim.generate_host(1, 2, out=part).numpy(), ref[:, 1:2], "host path, pulse range")
         xi2 = (w.scene["xi"] * np.float32(0.5)).astype(np.float32)
         sim.update_scene(xi=torch.from_numpy(xi2).pin_memory())
         got = sim.generate_host().numpy()
