@@ -430,22 +430,33 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         // ---- C: 8 threads per slice: Chebyshev moments, transpose through shared memory, one RED per (slice, k).
         //      The recurrence runs on a_k = sigma_k T_k, sigma = + + - - + + - -, which needs no negation:
         //      a_{k+1} = -+ 2y a_k + a_{k-1} (minus for odd k); sigma_k is applied to the slice sum.
-#pragma unroll 1
-        for (int c = 0; c < C; ++c) {
-            const int smin = s_rng[c][0], smax = s_rng[c][1];
-            const int *hc = hs + c * hstride;
-            const unsigned short *ixc0 = ix + c * cap;
-            const float2 *payc = pay + c * cap;
-            const float *payc_y = pay_y + c * cap;
-            for (int s0 = smin; s0 < smax; s0 += kThreads / 8) {
-                if (s0 + warp * 4 >= smax) continue;                       // warp-uniform
-                const int sidx = s0 + team;
+        //      Work items = the occupied slices of all C channels laid end to end (a narrow tile occupies fewer than
+        //      the 32 slices one pass of the CTA's teams takes: per channel, half the teams would idle).
+        {
+            int pre[C + 1];                                                // first item of channel c
+            pre[0] = 0;
+#pragma unroll
+            for (int c = 0; c < C; ++c) pre[c + 1] = pre[c] + max(s_rng[c][1] - s_rng[c][0], 0);
+            const int total = pre[C];
+            for (int it0 = 0; it0 < total; it0 += kThreads / 8) {
+                if (it0 + warp * 4 >= total) break;                        // warp-uniform
+                const int it = it0 + team;
+                int c = 0;
+#pragma unroll
+                for (int cc = 1; cc < C; ++cc) c = (it >= pre[cc]) ? cc : c;
+                int pc0 = 0;
+#pragma unroll
+                for (int cc = 1; cc < C; ++cc) pc0 = (c == cc) ? pre[cc] : pc0;
+                const int sidx = s_rng[c][0] + (it - pc0);
+                const int *hc = hs + c * hstride;
                 int first = 0, cnt = 0;
-                if (sidx < smax) { first = hc[sidx]; cnt = hc[sidx + 1] - first; }
+                if (it < total) { first = hc[sidx]; cnt = hc[sidx + 1] - first; }
+                const float2 *payc = pay + c * cap;
+                const float *payc_y = pay_y + c * cap;
                 f32x2 m[kKt];
 #pragma unroll
                 for (int k = 0; k < kKt; ++k) m[k] = 0ull;
-                const unsigned short *ixc = ixc0 + first;
+                const unsigned short *ixc = ix + c * cap + first;
                 auto add = [&](int src) {
                     const f32x2 w = *reinterpret_cast<const f32x2 *>(payc + src);
                     const float yv = payc_y[src];
