@@ -396,18 +396,35 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         // ---- B: exclusive scan of each channel's histogram (one warp per channel), then the index list ----
         if (warp < C) {
             int *hc = hs + warp * hstride;
-            int carry = 0, smin = span, smax = 0;
-            for (int k0s = 1; k0s <= span; k0s += 32) {
-                const int k = k0s + lane;
-                int v = (k <= span) ? hc[k] : 0;
-                if (v > 0) { smin = min(smin, k - 1); smax = max(smax, k); }
+            int smin = span, smax = 0;
+            if (span <= 64) {
+                // one pass, two adjacent entries per lane: hc[1 + 2 lane], hc[2 + 2 lane]
+                const int k = 1 + 2 * lane;
+                const int v0 = (k <= span) ? hc[k] : 0, v1 = (k + 1 <= span) ? hc[k + 1] : 0;
+                if (v0 > 0) { smin = k - 1; smax = k; }
+                if (v1 > 0) { smin = min(smin, k); smax = k + 1; }
+                int v = v0 + v1;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
                     const int t = __shfl_up_sync(0xffffffffu, v, o);
                     if (lane >= o) v += t;
                 }
-                if (k <= span) hc[k] = v + carry;
-                carry += __shfl_sync(0xffffffffu, v, 31);
+                if (k <= span) hc[k] = v - v1;
+                if (k + 1 <= span) hc[k + 1] = v;
+            } else {
+                int carry = 0;
+                for (int k0s = 1; k0s <= span; k0s += 32) {
+                    const int k = k0s + lane;
+                    int v = (k <= span) ? hc[k] : 0;
+                    if (v > 0) { smin = min(smin, k - 1); smax = max(smax, k); }
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int t = __shfl_up_sync(0xffffffffu, v, o);
+                        if (lane >= o) v += t;
+                    }
+                    if (k <= span) hc[k] = v + carry;
+                    carry += __shfl_sync(0xffffffffu, v, 31);
+                }
             }
             smin = __reduce_min_sync(0xffffffffu, smin);
             smax = __reduce_max_sync(0xffffffffu, smax);
@@ -418,9 +435,10 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         for (int q = 0; q < FPT; ++q)
 #pragma unroll
             for (int c = 0; c < C; ++c)
-                if (pr[q][c] >= 0)
-                    ix[c * cap + hs[c * hstride + (pr[q][c] >> 12)] + (pr[q][c] & 4095)] =
-                        (unsigned short)(q * kThreads + tid);
+            {   // branch-free: the histogram load is unconditional (slice 0 for an echo that is not in the list)
+                const int v = pr[q][c], first = hs[c * hstride + (max(v, 0) >> 12)];
+                if (v >= 0) ix[c * cap + first + (v & 4095)] = (unsigned short)(q * kThreads + tid);
+            }
         {   // the other histogram is free since the previous pulse's stage C: zero it for the next pulse
             int *hn = hist + (buf ^ 1) * C * hstride;
             for (int k = tid; k < C * hstride; k += kThreads) hn[k] = 0;
