@@ -142,7 +142,11 @@ typedef struct {
                                       gains), after sim_create has verified the interpolants against the exact geometry
                                       at every pulse on a lattice of scene points (path 2e-8 m, gains 3e-6);
                                       1 = off (exact geometry at every pulse) */
-    int32_t reserved[5];
+    int32_t fft_band;              /* SPECTRAL with keyframed geometry: a vector whose echoes occupy a narrow band of range
+                                      slices is convolved by a transform of that band alone: 0 = auto (size from the scene's
+                                      slice extent), 1 = off (always the full Ns + L - 1 transform), n >= 256 (power of 2,
+                                      < the full size) = that band transform; wider vectors always take the full one */
+    int32_t reserved[4];
 } sim_options;
 
 /*
@@ -200,6 +204,7 @@ typedef struct {
     int32_t fft_size;              /* SPECTRAL: transform length; else 0              */
     int32_t kinematics_keyframe;   /* H as resolved at sim_create                     */
     int32_t geometry_keyframed;    /* 1 when ranges / gains are interpolated between keyframes (sim_options) */
+    int32_t fft_band_size;         /* SPECTRAL: band transform length (sim_options.fft_band), 0 = not in use */
 } sim_stats;
 int sim_get_stats(sim_handle *h, sim_stats *out);
 

@@ -72,7 +72,7 @@ class sim_scene(C.Structure):
 class sim_options(C.Structure):
     _fields_ = [("tile_facets", C.c_int32), ("pulses_per_batch", C.c_int32), ("workspace_bytes", C.c_int64),
                 ("accumulate_mode", C.c_int32), ("kinematics_keyframe", C.c_int32), ("geometry_keyframe", C.c_int32),
-                ("reserved", C.c_int32 * 5)]
+                ("fft_band", C.c_int32), ("reserved", C.c_int32 * 4)]
 
 
 class sim_stats(C.Structure):
@@ -82,7 +82,7 @@ class sim_stats(C.Structure):
         ("tile_facets", C.c_int32), ("pulses_per_batch", C.c_int32), ("n_tiles", C.c_int32),
         ("accumulate_block_threads", C.c_int32), ("max_span_samples", C.c_int32),
         ("accumulate_mode", C.c_int32), ("fft_size", C.c_int32), ("kinematics_keyframe", C.c_int32),
-        ("geometry_keyframed", C.c_int32),
+        ("geometry_keyframed", C.c_int32), ("fft_band_size", C.c_int32),
     ]
 
 
@@ -248,7 +248,7 @@ def _marshal(workload):
 
 def sim_create(workload, device: int = 0, *, tile_facets: int = 0, pulses_per_batch: int = 0,
                workspace_bytes: int = 0, accumulate_mode=0, kinematics_keyframe: int = 0,
-               geometry_keyframe: int = 0):
+               geometry_keyframe: int = 0, fft_band: int = 0):
     lib = load_library()
     ci, cg, cs, keep = _marshal(workload)
     opts = sim_options()
@@ -256,6 +256,7 @@ def sim_create(workload, device: int = 0, *, tile_facets: int = 0, pulses_per_ba
     opts.accumulate_mode = _MODES[accumulate_mode]
     opts.kinematics_keyframe = int(kinematics_keyframe)
     opts.geometry_keyframe = int(geometry_keyframe)
+    opts.fft_band = int(fft_band)
     h = C.c_void_p()
     rc = lib.sim_create(C.byref(ci), C.byref(cg), C.byref(cs), C.byref(opts), int(device), C.byref(h))
     del keep

@@ -174,6 +174,10 @@ fftconv_kernel(FftConvArgs a, int p0, int n_pl, int n_samples)
     extern __shared__ __align__(16) float2 xs[];
     const int pl = blockIdx.x, c = blockIdx.y, tid = threadIdx.x;
     const float2 *rows = a.mom + ((size_t)(c * n_pl + pl) * kKt) * a.nb_pad;
+    if (a.nfft2) {                                         // fftconv_band_kernel takes empty and narrow vectors
+        const int lo = __ldg(a.band_lo + (c * n_pl + pl)), hi = __ldg(a.band_hi + (c * n_pl + pl));
+        if (hi <= lo || hi - lo + a.replica - 1 <= a.nfft2) return;
+    }
 
     float2 acc[E];
 #pragma unroll
@@ -207,6 +211,64 @@ fftconv_kernel(FftConvArgs a, int p0, int n_pl, int n_samples)
     const float2 q = make_float2((float)qd.x, (float)qd.y);
     float2 *dst = a.out + ((size_t)c * a.n_out_pulses + a.out_pulse0 + pl) * n_samples;
     for (int n = tid; n < n_samples; n += T) dst[n] = cmul(xs[pad(n + a.replica - 1)], q);
+}
+
+// The same convolution on the vector's occupied band alone.  K2k records the slice range [lo, hi) its echoes fall in
+// (a scene spans a fraction of the sampling window: 450 of 5295 slices on ATI); when hi - lo + L - 1 <= N2 the linear
+// convolution of the band with the L-tap kernels fits an N2-point circular one, four to eight times less transform work
+// and moment-row traffic than the NFFT-point transform of the whole row.  With M'[i] = M[i + lo + L - 1] and
+// y' = sum_k c_k * M'_k:  out[n] = y'[n - lo] for 0 <= n - lo < hi - lo + L - 1, zero elsewhere.  Vectors with a wider
+// band are left to fftconv_kernel (launched beside this one); empty vectors are zero-filled here.
+template <int N2>
+__global__ void __launch_bounds__(FftShape<N2>::kThreads)
+fftconv_band_kernel(FftConvArgs a, int p0, int n_pl, int n_samples)
+{
+    constexpr int T = FftShape<N2>::kThreads, E = FftShape<N2>::kPerThread;
+    extern __shared__ __align__(16) float2 xs[];
+    const int pl = blockIdx.x, c = blockIdx.y, tid = threadIdx.x;
+    const int lo = __ldg(a.band_lo + (c * n_pl + pl)), hi = __ldg(a.band_hi + (c * n_pl + pl));
+    float2 *dst = a.out + ((size_t)c * a.n_out_pulses + a.out_pulse0 + pl) * n_samples;
+    if (hi <= lo) {
+        for (int n = tid; n < n_samples; n += T) dst[n] = make_float2(0.f, 0.f);
+        return;
+    }
+    const int W = hi - lo, L = a.replica;
+    if (W + L - 1 > N2) return;
+    const float2 *rows = a.mom + ((size_t)(c * n_pl + pl) * kKt) * a.nb_pad + (lo + L - 1);
+
+    float2 acc[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) acc[e] = make_float2(0.f, 0.f);
+    for (int k = 0; k < kKt; ++k) {
+        const float2 *row = rows + (size_t)k * a.nb_pad;
+#pragma unroll 4
+        for (int e = 0; e < E; ++e) {
+            const int i = tid + e * T;
+            xs[pad(i)] = (i < W) ? __ldg(row + i) : make_float2(0.f, 0.f);
+        }
+        __syncthreads();
+        fft_forward<N2, T>(xs, a.tw2);
+        const float2 *ck = a.cspec2 + (size_t)k * N2;
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int i = tid + e * T;
+            const float2 u = cmul(xs[pad(i)], __ldg(ck + i));
+            acc[e].x += u.x; acc[e].y += u.y;
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int e = 0; e < E; ++e) xs[pad(tid + e * T)] = acc[e];
+    __syncthreads();
+    fft_inverse<N2, T>(xs, a.tw2);
+
+    const double2 qd = __ldg(a.carrier_p + p0 + pl);
+    const float2 q = make_float2((float)qd.x, (float)qd.y);
+    const unsigned n_out = (unsigned)(W + L - 1);
+    for (int n = tid; n < n_samples; n += T) {
+        const int i = n - lo;
+        dst[n] = ((unsigned)i < n_out) ? cmul(xs[pad(i)], q) : make_float2(0.f, 0.f);
+    }
 }
 
 // Spectra of the waveform kernels: cspec[k] = FFT(zero-padded c_k) / NFFT, in the forward pass's order.
@@ -243,6 +305,18 @@ cudaError_t launch_conv(const FftConvArgs &a, int p0, int n_pl, int n_channels, 
     return cudaGetLastError();
 }
 
+template <int N2>
+cudaError_t launch_conv_band(const FftConvArgs &a, int p0, int n_pl, int n_channels, int n_samples, cudaStream_t s)
+{
+    constexpr size_t smem = FftShape<N2>::kSmem;
+    if (smem > 48 * 1024) {
+        cudaError_t rc = cudaFuncSetAttribute(fftconv_band_kernel<N2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (rc != cudaSuccess) return rc;
+    }
+    fftconv_band_kernel<N2><<<dim3(n_pl, n_channels), FftShape<N2>::kThreads, smem, s>>>(a, p0, n_pl, n_samples);
+    return cudaGetLastError();
+}
+
 template <int NFFT>
 cudaError_t launch_spec(const float2 *ck, int replica, const float2 *tw, float2 *cspec, cudaStream_t s)
 {
@@ -261,6 +335,17 @@ cudaError_t launch_spec(const float2 *ck, int replica, const float2 *tw, float2 
 
 cudaError_t launch_fftconv(const DevParams &prm, const FftConvArgs &a, int p0, int n_pl, cudaStream_t s)
 {
+    if (a.nfft2) {
+        if (!a.band_lo || !a.band_hi || !a.cspec2 || !a.tw2 || a.nfft2 >= a.nfft) return cudaErrorInvalidValue;
+        cudaError_t rc;
+        switch (a.nfft2) {
+#define HEEPS_CASE(N) case N: rc = launch_conv_band<N>(a, p0, n_pl, prm.n_channels, prm.n_samples, s); break;
+            HEEPS_FFT_SIZES(HEEPS_CASE)
+#undef HEEPS_CASE
+            default: return cudaErrorInvalidValue;
+        }
+        if (rc != cudaSuccess) return rc;
+    }
     switch (a.nfft) {
 #define HEEPS_CASE(N) case N: return launch_conv<N>(a, p0, n_pl, prm.n_channels, prm.n_samples, s);
         HEEPS_FFT_SIZES(HEEPS_CASE)

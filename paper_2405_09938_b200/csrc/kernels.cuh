@@ -119,6 +119,9 @@ struct MomentArgs {
     int32_t span_cap;           // slices of a tile's shared-memory window
     int32_t replica;            // L = T fs (integer on this path)
     unsigned long long *counters;
+    // K2k only, may be null: occupied slice range [band_lo, band_hi) of every vector [C][n_pl], by atomicMin / atomicMax
+    // (the caller presets lo to a large and hi to a small value); lets K3s transform only the band (fftconv.cu)
+    int32_t *band_lo, *band_hi;
 };
 size_t moments_smem_bytes(const DevParams &prm, int span_cap);
 cudaError_t launch_moments(const DevParams &prm, const MomentArgs &a, int p0, int n_pl, cudaStream_t s);
@@ -143,6 +146,13 @@ struct FftConvArgs {
     int32_t nb;                 // Ns + L - 1 valid slices
     int32_t nb_pad;
     int32_t replica;            // L
+    // Band transform (optional, nfft2 = 0: off).  A vector whose occupied slices [band_lo, band_hi) satisfy
+    // band_hi - band_lo + L - 1 <= nfft2 is convolved with an nfft2-point transform of the band alone (its echoes span a
+    // fraction of the window: ATI 450 of 5295 slices), the others with the full nfft-point one.
+    const int32_t *band_lo, *band_hi;   // [C][n_pl] from K2k
+    const float2 *cspec2;       // [Kt][nfft2]
+    const float2 *tw2;          // [nfft2]
+    int32_t nfft2;
 };
 cudaError_t launch_fftconv(const DevParams &prm, const FftConvArgs &a, int p0, int n_pl, cudaStream_t s);
 // cspec[k] = FFT(zero-padded ck[k][0..L)) / nfft for k < Kt (run once at sim_create).

@@ -132,6 +132,8 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     __shared__ unsigned long long s_samples;
     __shared__ int s_kept;
     __shared__ int s_rng[kMaxKeyChannels][2];
+    __shared__ int s_band[kMaxKeyPulses][kMaxKeyChannels][2];   // occupied slices of this tile per pulse and channel
+    __shared__ int s_wide;                                       // an echo fell outside the tile's slice window
 
     const int span = a.span_cap, hstride = span + 1;
     const int cap = prm.tile_cap;
@@ -157,7 +159,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         double *d0 = reinterpret_cast<double *>(&pc2[0]), *d1 = reinterpret_cast<double *>(&pc2[1]);
         for (int k = tid; k < (int)(sizeof(PulseConst) / sizeof(double)); k += kThreads) { d0[k] = s0[k]; d1[k] = s1[k]; }
     }
-    if (tid == 0) { s_samples = 0ull; s_kept = 0; }
+    if (tid == 0) { s_samples = 0ull; s_kept = 0; s_wide = 0; }
     for (int k = tid; k < 2 * C * hstride; k += kThreads) hist[k] = 0;
     __syncthreads();
 
@@ -388,6 +390,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                         t0 = t1; t1 = t2;
                     }
                     my_samples += (unsigned)(min(b + L, prm.n_samples) - max(b, 0));
+                    s_wide = 1;
                 }
             }
         }
@@ -428,7 +431,10 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
             }
             smin = __reduce_min_sync(0xffffffffu, smin);
             smax = __reduce_max_sync(0xffffffffu, smax);
-            if (lane == 0) { s_rng[warp][0] = smin; s_rng[warp][1] = smax; }     // occupied slices [smin, smax)
+            if (lane == 0) {
+                s_rng[warp][0] = smin; s_rng[warp][1] = smax;                      // occupied slices [smin, smax)
+                s_band[ip][warp][0] = smin; s_band[ip][warp][1] = smax;            // kept for the band update at the end
+            }
         }
         __syncthreads();                                 // hs[c][s] = first sorted position of slice s
 #pragma unroll
@@ -532,6 +538,16 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     if (tid == 0 && a.counters) {
         if (s_kept) atomicAdd(a.counters + 0, (unsigned long long)s_kept * C);
         if (s_samples) atomicAdd(a.counters + 1, s_samples);
+    }
+    // ---- the band every vector occupies, for K3s (fftconv.cu): outside the pulse loop, whose code must stay as it is
+    //      (two atomics inside it cost 4 % of the kernel); a tile with an out-of-window echo claims the whole row ----
+    if (a.band_lo) {
+        for (int k = tid; k < (hi - lo) * C; k += kThreads) {
+            const int ip = k / C, c = k - ip * C, v = c * n_pl + (lo + ip - p0);
+            const int smin = s_band[ip][c][0], smax = s_band[ip][c][1];
+            if (s_wide) { atomicMin(a.band_lo + v, -(L - 1)); atomicMax(a.band_hi + v, prm.n_samples); }
+            else if (smax > smin) { atomicMin(a.band_lo + v, s_kp[ip].base[c] + smin); atomicMax(a.band_hi + v, s_kp[ip].base[c] + smax); }
+        }
     }
 }
 

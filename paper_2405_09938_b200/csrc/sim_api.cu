@@ -90,7 +90,9 @@ struct sim_handle {
     DevBuf<unsigned long long> counters;
     DevBuf<float2> out_staging;
     // spectral path
-    DevBuf<float2> mom, cspec, tw;
+    DevBuf<float2> mom, cspec, tw, cspec2, tw2;
+    DevBuf<int32_t> band;               // [2][C * pulses_per_batch]: occupied slice range of every vector (K2k -> K3s)
+    int nfft2 = 0;                      // band transform size, 0 = off
 
     // bookkeeping
     sim_stats stats{};
@@ -233,6 +235,36 @@ int validate(const sim_instrument *in, const sim_geometry *g, const sim_scene *s
 
 // Horizontal gradient magnitude bound of the bistatic path at the scene centre, mid dwell
 // (flat surface): |d(r_t+r_r)/dx| + |d(r_t+r_r)/dy|, used only to size tiles and CTAs.
+// Extent of the scene in bistatic path length [m] at a pulse, largest over the dwell and the channels: 9 x 9 lattice of
+// rest positions (the path length is convex over the rectangle: its maximum sits at a corner, the lattice bounds its
+// minimum to a cell) plus the vertical excursion of the waves on both legs.  Sizes the band transform; not a guarantee.
+double scene_slice_extent(const sim_instrument *in, const sim_geometry *g, const sim_scene *sc, double wave_sum)
+{
+    double worst = 0;
+    const int P = g->n_pulses, step = std::max(1, P / 64);
+    for (int p = 0; p < P; p = (p + step < P || p == P - 1) ? p + step : P - 1) {
+        const double *tx = g->tx_pos_m + 3 * p, *rx = g->rx_pos_m + 3 * p, *rv = g->rx_vel_mps + 3 * p;
+        const double vn = std::sqrt(rv[0] * rv[0] + rv[1] * rv[1] + rv[2] * rv[2]);
+        const double tdrift = g->t_pulse_s[p];
+        for (int c = 0; c < in->n_channels; ++c) {
+            const double o = in->channel_offset_m[c];
+            const double rc[3] = {rx[0] + o * rv[0] / vn, rx[1] + o * rv[1] / vn, rx[2] + o * rv[2] / vn};
+            double lo = 1e300, hi = -1e300;
+            for (int a = 0; a <= 8; ++a)
+                for (int b = 0; b <= 8; ++b) {
+                    const double x = sc->centre_m[0] + (a / 8.0 - 0.5) * (sc->nx - 1) * sc->spacing_m + sc->current_uniform[0] * tdrift;
+                    const double y = sc->centre_m[1] + (b / 8.0 - 0.5) * (sc->ny - 1) * sc->spacing_m + sc->current_uniform[1] * tdrift;
+                    const double z = sc->centre_m[2];
+                    const double r = std::sqrt((x - tx[0]) * (x - tx[0]) + (y - tx[1]) * (y - tx[1]) + (z - tx[2]) * (z - tx[2])) +
+                                     std::sqrt((x - rc[0]) * (x - rc[0]) + (y - rc[1]) * (y - rc[1]) + (z - rc[2]) * (z - rc[2]));
+                    lo = std::min(lo, r); hi = std::max(hi, r);
+                }
+            worst = std::max(worst, hi - lo);
+        }
+    }
+    return worst + 4.0 * wave_sum;
+}
+
 double path_gradient_l1(const sim_geometry *g, const sim_scene *sc)
 {
     double worst = 0;
@@ -557,7 +589,7 @@ void sim_destroy(sim_handle *h)
     h->z.release(); h->slope.release(); h->dxy.release();
     h->zt.release(); h->dxy_t.release(); h->omega.release(); h->recs.release(); h->tinfo.release();
     h->tspan.release(); h->acc.release(); h->counters.release(); h->out_staging.release();
-    h->mom.release(); h->cspec.release(); h->tw.release();
+    h->mom.release(); h->cspec.release(); h->tw.release(); h->cspec2.release(); h->tw2.release(); h->band.release();
     delete h;
 }
 
@@ -575,6 +607,10 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     if (opts && (opts->accumulate_mode < 0 || opts->accumulate_mode > 2)) return SIM_EINVAL;
     if (opts && (opts->kinematics_keyframe < 0 || opts->kinematics_keyframe > 4096)) return SIM_EINVAL;
     if (opts && (opts->geometry_keyframe < 0 || opts->geometry_keyframe > 1)) return SIM_EINVAL;
+    if (opts && opts->fft_band != 0 && opts->fft_band != 1) {
+        const int n = opts->fft_band;
+        if (n < 256 || n > 8192 || (n & (n - 1))) return SIM_EINVAL;
+    }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
         cudaGetLastError();
@@ -885,6 +921,32 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
         CKC(cudaMemcpy(h->tw.p, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice));
         cudaError_t e_spec = launch_kernel_spectra(nfft, d_ck.p, L, h->tw.p, h->cspec.p, nullptr);
         if (e_spec == cudaSuccess) e_spec = cudaDeviceSynchronize();
+        // band transform (fftconv.cu): K2k records the slice range every vector occupies; size from the scene's extent
+        // in slices -- only an estimate, a vector with a wider band takes the full transform
+        h->nfft2 = 0;
+        const int band_opt = opts ? opts->fft_band : 0;
+        if (e_spec == cudaSuccess && h->geo_keyframed && band_opt != 1) {
+            int n2 = 256;
+            if (band_opt > 1) n2 = band_opt;
+            else {
+                const double need = scene_slice_extent(in, g, sc, wave_sum) * prm.fs_over_c0 + 16.0 + (L - 1);
+                while (n2 < need && n2 < nfft) n2 <<= 1;
+            }
+            if (n2 < nfft && n2 >= L) {                  // else: no smaller transform holds a band plus the replica
+                std::vector<float2> tw2((size_t)n2);
+                for (int k = 0; k < n2; ++k) {
+                    const double a = -2.0 * M_PI * (double)k / (double)n2;
+                    tw2[k] = make_float2((float)std::cos(a), (float)std::sin(a));
+                }
+                e_spec = h->tw2.alloc(tw2.size());
+                if (e_spec == cudaSuccess) e_spec = h->cspec2.alloc((size_t)kMomentOrder * n2);
+                if (e_spec == cudaSuccess) e_spec = h->band.alloc((size_t)2 * C * pb);
+                if (e_spec == cudaSuccess) e_spec = cudaMemcpy(h->tw2.p, tw2.data(), tw2.size() * sizeof(float2), cudaMemcpyHostToDevice);
+                if (e_spec == cudaSuccess) e_spec = launch_kernel_spectra(n2, d_ck.p, L, h->tw2.p, h->cspec2.p, nullptr);
+                if (e_spec == cudaSuccess) e_spec = cudaDeviceSynchronize();
+                if (e_spec == cudaSuccess) h->nfft2 = n2;
+            }
+        }
         d_ck.release();
         CKC(e_spec);
         CKC(h->mom.alloc((size_t)C * pb * kMomentOrder * h->nb_pad));
@@ -898,6 +960,7 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     h->stats.fft_size = h->spectral ? nfft : 0;
     h->stats.kinematics_keyframe = h->key_H;
     h->stats.geometry_keyframed = h->geo_keyframed ? 1 : 0;
+    h->stats.fft_band_size = h->spectral ? h->nfft2 : 0;
     *out = h;
     return SIM_OK;
 }
@@ -955,6 +1018,12 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         { int rc = run_speckle(h, p0, n_pl, s, &ma.xi_polar, &ma.xi_pulse_stride); if (rc != SIM_OK) return rc; }
         ma.mom = h->mom.p; ma.nb_pad = h->nb_pad; ma.span_cap = h->span_cap_m; ma.replica = h->replica;
         ma.counters = h->counters.p;
+        const size_t n_vec = (size_t)prm.n_channels * n_pl;
+        if (h->nfft2) {                                  // lo preset to 0x7f7f7f7f, hi to 0x80808080
+            ma.band_lo = h->band.p; ma.band_hi = h->band.p + n_vec;
+            CK(h, cudaMemsetAsync(ma.band_lo, 0x7f, n_vec * sizeof(int32_t), s));
+            CK(h, cudaMemsetAsync(ma.band_hi, 0x80, n_vec * sizeof(int32_t), s));
+        }
         if (h->geo_keyframed) CK(h, launch_moments_keyframed(prm, ma, p0, n_pl, s));
         else CK(h, launch_moments(prm, ma, p0, n_pl, s));
         CK(h, mark());
@@ -962,11 +1031,14 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         fa.mom = h->mom.p; fa.cspec = h->cspec.p; fa.tw = h->tw.p; fa.carrier_p = h->carrier_p.p;
         fa.out = out; fa.n_out_pulses = n_out; fa.out_pulse0 = p0 - pb0;
         fa.nfft = h->nfft; fa.nb = h->nb; fa.nb_pad = h->nb_pad; fa.replica = h->replica;
+        if (h->nfft2) {
+            fa.band_lo = ma.band_lo; fa.band_hi = ma.band_hi; fa.cspec2 = h->cspec2.p; fa.tw2 = h->tw2.p; fa.nfft2 = h->nfft2;
+        }
         CK(h, launch_fftconv(prm, fa, p0, n_pl, s));
         CK(h, mark());
         CK(h, mark());                                   // K4 slot: finalize is fused into K3s
         CK(h, ship(p0, n_pl));
-        launches += 3 + (h->speckle_ar1 ? 1 : 0);
+        launches += 3 + (h->speckle_ar1 ? 1 : 0) + (h->nfft2 ? 1 : 0);
     }
     for (int p0 = pb0; !h->spectral && p0 < pb1; p0 += batch) {
         const int n_pl = std::min(batch, pb1 - p0);

@@ -145,6 +145,46 @@ def test_geometry_keyframes_on_and_off():
     assert abs(kept[0] - expect_kept) <= 4 and abs(kept[1] - expect_kept) <= 4
 
 
+def test_band_transform_and_full_transform():
+    """Spectral path, K3s: a vector whose echoes occupy a narrow band of range slices is convolved by a transform of the
+    band alone (sim_options.fft_band), a wider one by the full Ns + L - 1 transform, an empty one is zero-filled; all
+    against the oracle and against each other."""
+    w = _hetero_small(96, 64, 11)                                    # Ns = 4096, L = 1200: full 8192, band 2048
+    ref = oracle_generate(w)
+    outs = {}
+    for fb in (0, 1, 4096):
+        with _sim(w, accumulate_mode="spectral", fft_band=fb, pulses_per_batch=4) as sim:
+            outs[fb] = sim.generate().cpu().numpy()
+            st = sim.stats()
+            part = sim.generate(3, 10).cpu().numpy()
+        assert st["fft_size"] == 8192 and st["fft_band_size"] == {0: 2048, 1: 0, 4096: 4096}[fb], st
+        _assert_parity(outs[fb], ref, f"fft_band={fb}")
+        _assert_parity(part, ref[:, 3:10], f"fft_band={fb}, pulse range")
+    assert rel_l2_per_vector(outs[0], outs[1].astype(np.complex128)).max() < 2e-6
+    # Tiny (Ns = 256, L = 24: full 512) with a forced 256-point band transform: a 3.8 km patch (about 120 slices) fits
+    # it, a 7.7 km patch (about 240 slices + the replica) does not and takes the full transform; the steered, culling
+    # scene has narrower bands at the ends of the dwell than in the middle
+    for d, steer in ((60.0, 0.0), (120.0, 0.0), (105.0, 3.0)):
+        wt = make_workload("tiny", n_pulses=13)
+        wt.scene["spacing_m"] = d
+        wt.instrument["channel_offset_m"] = np.array([-1.5, 0.0, 1.5])
+        if steer:
+            wt = add_antenna_patterns(wt, nu=2049, nv=257, steer_rate_deg_s=steer)
+            wt.instrument["cull_two_way_db"] = -10.0
+        reft = oracle_generate(wt)
+        for fb in (256, 1):
+            with _sim(wt, accumulate_mode="spectral", fft_band=fb) as sim:
+                got = sim.generate().cpu().numpy()
+                st = sim.stats()
+            assert st["geometry_keyframed"] == 1 and st["fft_band_size"] == (256 if fb == 256 else 0), st
+            _assert_parity(got, reft, f"tiny d={d} steer={steer} fft_band={fb}")
+    from paper_2405_09938_b200 import SimError
+    for bad in (-1, 2, 300, 16384):
+        with pytest.raises(SimError) as e:
+            _sim(w, fft_band=bad)
+        assert e.value.code == -1
+
+
 def test_geometry_keyframes_guard_rejects_rough_state_vectors():
     """Per-pulse platform positions that are not smooth in time (10 cm jitter): the host guard must refuse the
     interpolated geometry, and the exact per-pulse kernel must still match the oracle."""
