@@ -102,6 +102,8 @@ struct sim_handle {
     std::string cuda_err;
     // sim_generate_host: device->host copies of finished batches overlap the next batch's kernels
     cudaStream_t copy_stream = nullptr;
+    cudaStream_t aux_stream = nullptr;  // zeroes the moment rows while K1 runs
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     std::vector<cudaEvent_t> copy_events;
 
     ~sim_handle()
@@ -109,6 +111,9 @@ struct sim_handle {
         for (auto e : events) cudaEventDestroy(e);
         for (auto e : copy_events) cudaEventDestroy(e);
         if (copy_stream) cudaStreamDestroy(copy_stream);
+        if (ev_fork) cudaEventDestroy(ev_fork);
+        if (ev_join) cudaEventDestroy(ev_join);
+        if (aux_stream) cudaStreamDestroy(aux_stream);
     }
 };
 
@@ -1008,7 +1013,17 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
     const SurfBufs bufs{h->z.p, h->zt.p, h->slope.p, h->dxy.p, h->dxy_t.p};
     for (int p0 = pb0; h->spectral && p0 < pb1; p0 += batch) {
         const int n_pl = std::min(batch, pb1 - p0);
-        CK(h, cudaMemsetAsync(h->mom.p, 0, (size_t)prm.n_channels * n_pl * kMomentOrder * h->nb_pad * sizeof(float2), s));
+        // the moment rows are zeroed on a second stream, beside K1 (which does not touch them): forked after whatever
+        // precedes on `s` (the previous batch's K3s reads the rows), joined before K2k
+        if (!h->aux_stream) {
+            CK(h, cudaStreamCreateWithFlags(&h->aux_stream, cudaStreamNonBlocking));
+            CK(h, cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+            CK(h, cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
+        }
+        CK(h, cudaEventRecord(h->ev_fork, s));
+        CK(h, cudaStreamWaitEvent(h->aux_stream, h->ev_fork, 0));
+        CK(h, cudaMemsetAsync(h->mom.p, 0, (size_t)prm.n_channels * n_pl * kMomentOrder * h->nb_pad * sizeof(float2), h->aux_stream));
+        CK(h, cudaEventRecord(h->ev_join, h->aux_stream));
         CK(h, mark());
         MomentArgs ma{};
         { int rc = run_kinematics(h, bufs, p0, n_pl, s, &ma.surf); if (rc != SIM_OK) return rc; }
@@ -1024,6 +1039,7 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
             CK(h, cudaMemsetAsync(ma.band_lo, 0x7f, n_vec * sizeof(int32_t), s));
             CK(h, cudaMemsetAsync(ma.band_hi, 0x80, n_vec * sizeof(int32_t), s));
         }
+        CK(h, cudaStreamWaitEvent(s, h->ev_join, 0));
         if (h->geo_keyframed) CK(h, launch_moments_keyframed(prm, ma, p0, n_pl, s));
         else CK(h, launch_moments(prm, ma, p0, n_pl, s));
         CK(h, mark());
