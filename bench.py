@@ -43,8 +43,8 @@ MOMENT_FP32_OPS_PER_FACET_ECHO = 4.0 * 8 + 30.0
 # From the committed ncu captures (profiles/): executed thread-instructions per facet-echo (context for the
 # roofline fraction: the kernels are issue-bound, not pipe-bound) and dram bytes per facet-echo.
 K2S_EXECUTED_INSTR_PER_FACET_ECHO = 1156.0 / 3      # profiles/r1_v4_k2s_ncu_summary.txt
-K2K_EXECUTED_INSTR_PER_FACET_ECHO = 481.7 / 3       # profiles/r1_v13_k2k_ncu_summary.txt (1.010e9 warp instr / launch)
-K2K_DRAM_BYTES_PER_FACET_ECHO = (96.043e6 + 7.802e6) / (256 * 3 * 262144)   # same capture: dram read + write
+K2K_EXECUTED_INSTR_PER_FACET_ECHO = 487.6 / 3       # profiles/r1_v14_k2k_ncu_summary.txt (1.0225e9 warp instr / launch)
+K2K_DRAM_BYTES_PER_FACET_ECHO = (95.982e6 + 7.736e6) / (256 * 3 * 262144)   # same capture: dram read + write
 # dram bytes per kept facet-echo of a K3 launch, from the committed `ncu --set full` capture
 # profiles/r1_v3_k3_ncu_summary.txt: (2.580977e9 read + 1.1966e7 written) / (100 pulses x 3 ch x 262144).
 K3_DRAM_BYTES_PER_FACET_ECHO = (2.580977e9 + 1.1966e7) / (100 * 3 * 262144)
@@ -378,10 +378,10 @@ def run_cuda(args):
                    "wave_node_spacing_m": _VARIANT["wave_node_spacing"], "speckle_tau_s": _VARIANT["speckle_tau"],
                    "tabulated_patterns": _VARIANT["patterns"],
                    "accumulate_mode": "spectral" if spectral else "direct", "fft_size": stats["fft_size"],
-                   "kinematics_keyframe": stats["kinematics_keyframe"],
+                   "kinematics_keyframe": stats["kinematics_keyframe"], "fft_band_size": stats["fft_band_size"],
                    "tile_facets": stats["tile_facets"], "pulses_per_batch": stats["pulses_per_batch"],
                    "l2": (f"per-step working set: {moment_bytes / 1e6:.0f} MB of range-slice moments (zeroed, "
-                          f"scattered into and read back every step) + {C * P * Ns * 8 / 1e6:.0f} MB of output, "
+                          f"scattered into every step, their occupied bands read back) + {C * P * Ns * 8 / 1e6:.0f} MB of output, "
                           "larger than the 126 MB L2; no flush" if spectral else
                           f"per-step working set (facet-echo records) is {F * C * P * 32 / 1e9:.1f} GB, far larger "
                           "than the 126 MB L2; no flush needed")},
