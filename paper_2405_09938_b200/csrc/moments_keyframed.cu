@@ -85,6 +85,7 @@ __device__ __forceinline__ KeyEval<C> key_eval(const DevParams &prm, const Pulse
     return o;
 }
 
+constexpr int kStrayCap = 96;             // stray echoes of one pulse held in shared memory (more: the tile is sorted again)
 constexpr int kScrRow = 9;                // float2 per thread row of the transposition scratch (8 moments + 1 pad)
 constexpr int kScrTeam = 8 * kScrRow;     // float2 per 8-thread team
 __host__ __device__ constexpr int hist_words(int C, int span) { return (2 * C * (span + 1) + 1) & ~1; }
@@ -132,8 +133,9 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     __shared__ unsigned long long s_samples;
     __shared__ int s_kept;
     __shared__ int s_rng[kMaxKeyChannels][2];
-    __shared__ int s_band[kMaxKeyPulses][kMaxKeyChannels][2];   // occupied slices of this tile per pulse and channel
-    __shared__ int s_wide;                                       // an echo fell outside the tile's slice window
+    __shared__ float4 s_stray[2][kStrayCap];                     // echoes that have left their sorted slice: (w, y, row index)
+    __shared__ int s_nstray[3];
+    __shared__ int s_blo[kMaxKeyChannels], s_bhi[kMaxKeyChannels];   // slices this tile touches during the interval
 
     const int span = a.span_cap, hstride = span + 1;
     const int cap = prm.tile_cap;
@@ -159,8 +161,9 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         double *d0 = reinterpret_cast<double *>(&pc2[0]), *d1 = reinterpret_cast<double *>(&pc2[1]);
         for (int k = tid; k < (int)(sizeof(PulseConst) / sizeof(double)); k += kThreads) { d0[k] = s0[k]; d1[k] = s1[k]; }
     }
-    if (tid == 0) { s_samples = 0ull; s_kept = 0; s_wide = 0; }
-    for (int k = tid; k < 2 * C * hstride; k += kThreads) hist[k] = 0;
+    if (tid == 0) { s_samples = 0ull; s_kept = 0; s_nstray[0] = s_nstray[1] = s_nstray[2] = 0; }
+    if (tid < kMaxKeyChannels) { s_blo[tid] = 0x7fffffff; s_bhi[tid] = (int)0x80000000; }
+    for (int k = tid; k < C * hstride; k += kThreads) hist[k] = 0;
     __syncthreads();
 
     const int ts = prm.tile, lts = 31 - __clz(ts);
@@ -316,27 +319,113 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     const int sub = tid & 7, team = tid >> 3, warp = tid >> 5;
     float2 *scr = scratch + team * kScrTeam;
 
-    for (int ip = 0; ip < hi - lo; ++ip) {
+    // ---- The facet-echoes of the tile are ordered by range slice ONCE (counting sort at the interval's middle pulse:
+    //      histogram by integer ATOMS, scan, slot = first position of the slice + rank), not at every pulse: over the
+    //      few milliseconds of an interval a facet's slice changes only when its sub-slice position crosses 0 or 1
+    //      (the window follows the scene: a percent or two of the echoes per pulse).  At every pulse an echo found in
+    //      its sorted slice writes its weight into its slot; one found elsewhere ("stray") leaves a zero there and goes
+    //      to a short shared-memory list that the CTA works off with global atomics.  A pulse with more strays than the
+    //      list holds sorts the tile again at that pulse and is redone.  Stage C reads each slice's slots
+    //      contiguously: no per-pulse histogram, scan or index list; one barrier per pulse. ----
+    uint32_t *slots = reinterpret_cast<uint32_t *>(idx);           // [C][cap]: slice << 12 | slot, or ~0u (never in the list)
+    int *hs = hist;                                                  // [C][span + 1] first slot of each slice
+    int bref[C];                                                     // first slice of the tile's window at the sorting pulse
+    // Sorted at the middle pulse of the interval the strays at its ends are half as many as when sorted at the first;
+    // a tile far from the scene centre drifts too fast for that (expected strays at the first pulse = half the
+    // interval's pulses x the drift of the tile centre against the sampling window, in slices per pulse, x its echoes):
+    // it is sorted at the first pulse, and again whenever the next pulse's strays (this pulse's plus their growth)
+    // would not fit the list.
+    int ip_sort = (hi - lo) / 2;
+    {
+        const double drift = fabs((s_rc[1][0] - s_rc[0][0]) - (a.pulses[k1].r0 - a.pulses[k0].r0)) * prm.fs_over_c0 /
+                             (double)max(k1 - k0, 1);
+        if (drift * (double)(ts * ts * C) * 0.5 * (double)(hi - lo) > 0.9 * kStrayCap) ip_sort = 0;
+    }
+    bool need_sort = true;
+    int ns_prev = 0;                                                 // strays of the previous pulse (0 after a sort)
+
+    for (int ip = 0; ip < hi - lo;) {
+        if (need_sort) {
+            need_sort = false;
+            const KeyPulse &kp = s_kp[ip_sort];
+            __syncthreads();                                         // nobody reads the old histogram / slots any more
+            for (int k = tid; k < C * hstride; k += kThreads) hs[k] = 0;
+            if (tid == 0) s_nstray[ip % 3] = 0;
+            __syncthreads();
+#pragma unroll
+            for (int c = 0; c < C; ++c) bref[c] = kp.base[c];
+            int pr[FPT][C];
+#pragma unroll
+            for (int q = 0; q < FPT; ++q) {
+                const double dRref = fma(kp.sd, RD[q], R0[q]) + (double)fmaf(kp.u0, ra[q], kp.u1 * rb[q]) - kp.r0;
+                const float la = fmaf(kp.s, dla[q], la0[q]);
+#pragma unroll
+                for (int c = 0; c < C; ++c) {
+                    const float dl = och[c] * fmaf(och[c], lbt, la);
+                    const int rel = __double2int_ru(fma(dRref + (double)dl, prm.fs_over_c0, -prm.half_len)) - bref[c];
+                    pr[q][c] = -1;
+                    if (valid[q] && (unsigned)rel < (unsigned)span)
+                        pr[q][c] = (rel << 12) | atomicAdd(&hs[c * hstride + rel + 1], 1);
+                }
+            }
+            __syncthreads();
+            if (warp < C) {                                          // inclusive scan: hs[c][s] = first slot of slice s
+                int *hc = hs + warp * hstride;
+                int carry = 0, smin = span, smax = 0;
+                for (int k0s = 1; k0s <= span; k0s += 32) {
+                    const int k = k0s + lane;
+                    int v = (k <= span) ? hc[k] : 0;
+                    if (v > 0) { smin = min(smin, k - 1); smax = max(smax, k); }
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int t = __shfl_up_sync(0xffffffffu, v, o);
+                        if (lane >= o) v += t;
+                    }
+                    if (k <= span) hc[k] = v + carry;
+                    carry += __shfl_sync(0xffffffffu, v, 31);
+                }
+                smin = __reduce_min_sync(0xffffffffu, smin);
+                smax = __reduce_max_sync(0xffffffffu, smax);
+                if (lane == 0) {
+                    s_rng[warp][0] = smin; s_rng[warp][1] = smax;                      // occupied slices [smin, smax)
+                    if (smax > smin) {                                                 // the band this tile reports to K3s
+                        atomicMin(&s_blo[warp], bref[warp] + smin - 1); atomicMax(&s_bhi[warp], bref[warp] + smax + 1);
+                    }
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int q = 0; q < FPT; ++q)
+#pragma unroll
+                for (int c = 0; c < C; ++c) {
+                    const int v = pr[q][c];
+                    if (FPT > 1 || q * kThreads + tid < cap)         // (FPT = 1: the tile may be smaller than the CTA)
+                        slots[c * cap + q * kThreads + tid] =
+                            (v >= 0) ? (uint32_t)((v & ~4095) | (hs[c * hstride + (v >> 12)] + (v & 4095))) : 0xffffffffu;
+                }
+            // a thread reads only its own slots; the scan results are read after the barrier of stage A
+        }
         const int buf = ip & 1;
         const int pl = lo + ip - p0;
         const KeyPulse &kp = s_kp[ip];
         float2 *pay = payload + (size_t)buf * C * cap;
         float *pay_y = payload_y + (size_t)buf * C * cap;
-        unsigned short *ix = idx + (size_t)buf * C * cap;
-        int *hs = hist + buf * C * hstride;
         const float s = kp.s;
+        int *n_stray = &s_nstray[ip % 3];
+        if (tid == 0) s_nstray[(ip + 1) % 3] = 0;            // last read two pulses ago, next written after this pulse's barrier
+        int kept_p = 0;
+        unsigned samples_p = 0;
 
-        // ---- A: slice, sub-slice position, complex weight of every facet-echo; rank inside the slice.
+        // ---- A: slice, sub-slice position, complex weight of every facet-echo, written to the echo's slot.
         //      Straight-line code for all FPT x C echoes of the thread (predicated stores), so that the
-        //      independent chains interleave; only the rare out-of-window echo branches.
-        int pr[FPT][C];                                  // (slice << 12 | rank) or -1
+        //      independent chains interleave; only a stray echo branches.
 #pragma unroll
         for (int q = 0; q < FPT; ++q) {
             const float Pv = fmaf(s, fmaf(s, pqb[q], pqa[q]), pq0[q]);
             const float Pi = kLut ? fmaf(s, fmaf(s, qib[kLut ? q : 0], qia[kLut ? q : 0]), qi0[kLut ? q : 0]) : 0.f;
             const bool keep = valid[q] && !(kLut ? (fmaf(Pv, Pv, Pi * Pi) < prm.cull_thr * prm.cull_thr)
                                                  : (fabsf(Pv) < prm.cull_thr));     // O7 (G6)
-            my_kept += keep ? 1 : 0;
+            kept_p += keep ? 1 : 0;
             float am = kTilt ? fmaf(s, fmaf(s, amb[q], ama[q]), am0[q]) : am0[q];
             uint32_t xa = xarg[q];
             if (kSpeckleT && valid[q]) {                  // time-dependent speckle: s_f(t_p) of this pulse (eq. (7), (10))
@@ -370,92 +459,33 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                     wr = am * fmaf(g, cs, -gi * sn); wi = am * fmaf(g, sn, gi * cs);
                 }
                 const float yv = fmaf(2.f, eps, -1.f);
-                const int rel = b - kp.base[c];
-                const bool inspan = (unsigned)rel < (unsigned)span;
-                pr[q][c] = -1;
-                if (inwin && inspan) {
-                    pay[c * cap + k] = make_float2(wr, wi);
-                    pay_y[c * cap + k] = yv;
-                    pr[q][c] = (rel << 12) | atomicAdd(&hs[c * hstride + rel + 1], 1);
+                const uint32_t slot = (FPT > 1 || k < cap) ? slots[c * cap + k] : 0xffffffffu;
+                const int rel = b - bref[c];
+                const bool here = inwin && ((uint32_t)rel == (slot >> 12));       // in its sorted slice
+                if (slot != 0xffffffffu) {
+                    const int pos = c * cap + (int)(slot & 4095u);
+                    pay[pos] = here ? make_float2(wr, wi) : make_float2(0.f, 0.f);
+                    pay_y[pos] = here ? yv : 0.f;
                 }
-                if (inwin && !inspan) {                                    // outside the tile window: rare
-                    const float br = wr, bi = wi;
-                    float2 *row = a.mom + ((size_t)(c * n_pl + pl) * kKt) * a.nb_pad + (b + L - 1);
-                    float t0 = 1.f, t1 = yv;
-                    atomicAdd(row, make_float2(br, bi));
-                    atomicAdd(row + a.nb_pad, make_float2(br * t1, bi * t1));
-                    for (int kk = 2; kk < kKt; ++kk) {
-                        const float t2 = 2.f * yv * t1 - t0;
-                        atomicAdd(row + (size_t)kk * a.nb_pad, make_float2(br * t2, bi * t2));
-                        t0 = t1; t1 = t2;
-                    }
-                    my_samples += (unsigned)(min(b + L, prm.n_samples) - max(b, 0));
-                    s_wide = 1;
+                if (inwin) samples_p += (unsigned)(min(b + L, prm.n_samples) - max(b, 0));
+                if (inwin && !here) {                                      // stray: left its sorted slice, or never had one
+                    const int t = atomicAdd(n_stray, 1);
+                    if (t < kStrayCap) s_stray[buf][t] = make_float4(wr, wi, yv, __int_as_float((c << 28) | (b + L - 1)));
                 }
             }
         }
         __syncthreads();
-
-        // ---- B: exclusive scan of each channel's histogram (one warp per channel), then the index list ----
-        if (warp < C) {
-            int *hc = hs + warp * hstride;
-            int smin = span, smax = 0;
-            if (span <= 64) {
-                // one pass, two adjacent entries per lane: hc[1 + 2 lane], hc[2 + 2 lane]
-                const int k = 1 + 2 * lane;
-                const int v0 = (k <= span) ? hc[k] : 0, v1 = (k + 1 <= span) ? hc[k + 1] : 0;
-                if (v0 > 0) { smin = k - 1; smax = k; }
-                if (v1 > 0) { smin = min(smin, k); smax = k + 1; }
-                int v = v0 + v1;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int t = __shfl_up_sync(0xffffffffu, v, o);
-                    if (lane >= o) v += t;
-                }
-                if (k <= span) hc[k] = v - v1;
-                if (k + 1 <= span) hc[k + 1] = v;
-            } else {
-                int carry = 0;
-                for (int k0s = 1; k0s <= span; k0s += 32) {
-                    const int k = k0s + lane;
-                    int v = (k <= span) ? hc[k] : 0;
-                    if (v > 0) { smin = min(smin, k - 1); smax = max(smax, k); }
-#pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) {
-                        const int t = __shfl_up_sync(0xffffffffu, v, o);
-                        if (lane >= o) v += t;
-                    }
-                    if (k <= span) hc[k] = v + carry;
-                    carry += __shfl_sync(0xffffffffu, v, 31);
-                }
-            }
-            smin = __reduce_min_sync(0xffffffffu, smin);
-            smax = __reduce_max_sync(0xffffffffu, smax);
-            if (lane == 0) {
-                s_rng[warp][0] = smin; s_rng[warp][1] = smax;                      // occupied slices [smin, smax)
-                s_band[ip][warp][0] = smin; s_band[ip][warp][1] = smax;            // kept for the band update at the end
-            }
+        const int ns = *n_stray;
+        if (ns > kStrayCap) {                                // too many have moved on: sort the tile at this pulse, redo it
+            need_sort = true; ip_sort = ip;
+            continue;
         }
-        __syncthreads();                                 // hs[c][s] = first sorted position of slice s
-#pragma unroll
-        for (int q = 0; q < FPT; ++q)
-#pragma unroll
-            for (int c = 0; c < C; ++c)
-            {   // branch-free: the histogram load is unconditional (slice 0 for an echo that is not in the list)
-                const int v = pr[q][c], first = hs[c * hstride + (max(v, 0) >> 12)];
-                if (v >= 0) ix[c * cap + first + (v & 4095)] = (unsigned short)(q * kThreads + tid);
-            }
-        {   // the other histogram is free since the previous pulse's stage C: zero it for the next pulse
-            int *hn = hist + (buf ^ 1) * C * hstride;
-            for (int k = tid; k < C * hstride; k += kThreads) hn[k] = 0;
-        }
-        __syncthreads();
+        my_kept += kept_p; my_samples += samples_p;
 
-        // ---- C: 8 threads per slice: Chebyshev moments, transpose through shared memory, one RED per (slice, k).
-        //      The recurrence runs on a_k = sigma_k T_k, sigma = + + - - + + - -, which needs no negation:
-        //      a_{k+1} = -+ 2y a_k + a_{k-1} (minus for odd k); sigma_k is applied to the slice sum.
-        //      Work items = the occupied slices of all C channels laid end to end (a narrow tile occupies fewer than
-        //      the 32 slices one pass of the CTA's teams takes: per channel, half the teams would idle).
+        // ---- C: 8 threads per slice: Chebyshev moments over the slice's slots, transpose through shared memory, one
+        //      RED per (slice, k).  The recurrence runs on a_k = sigma_k T_k, sigma = + + - - + + - -, which needs no
+        //      negation: a_{k+1} = -+ 2y a_k + a_{k-1} (minus for odd k); sigma_k is applied to the slice sum.
+        //      Work items = the occupied slices of all C channels laid end to end.
         {
             int pre[C + 1];                                                // first item of channel c
             pre[0] = 0;
@@ -468,19 +498,20 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                 int c = 0;
 #pragma unroll
                 for (int cc = 1; cc < C; ++cc) c = (it >= pre[cc]) ? cc : c;
-                int pc0 = 0;
+                int pc0 = 0, bc = bref[0];
 #pragma unroll
-                for (int cc = 1; cc < C; ++cc) pc0 = (c == cc) ? pre[cc] : pc0;
+                for (int cc = 1; cc < C; ++cc) { pc0 = (c == cc) ? pre[cc] : pc0; bc = (c == cc) ? bref[cc] : bc; }
                 const int sidx = s_rng[c][0] + (it - pc0);
                 const int *hc = hs + c * hstride;
                 int first = 0, cnt = 0;
                 if (it < total) { first = hc[sidx]; cnt = hc[sidx + 1] - first; }
-                const float2 *payc = pay + c * cap;
-                const float *payc_y = pay_y + c * cap;
+                const int b = bc + sidx;
+                if ((unsigned)(b + L - 1) >= win_hi) cnt = 0;              // a slice outside the sampling window holds zeros only
+                const float2 *payc = pay + c * cap + first;
+                const float *payc_y = pay_y + c * cap + first;
                 f32x2 m[kKt];
 #pragma unroll
                 for (int k = 0; k < kKt; ++k) m[k] = 0ull;
-                const unsigned short *ixc = ix + c * cap + first;
                 auto add = [&](int src) {
                     const f32x2 w = *reinterpret_cast<const f32x2 *>(payc + src);
                     const float yv = payc_y[src];
@@ -496,11 +527,8 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                     }
                 };
                 int i = sub;
-                for (; i + 8 < cnt; i += 16) {
-                    const int sa = ixc[i], sb = ixc[i + 8];
-                    add(sa); add(sb);
-                }
-                if (i < cnt) add(ixc[i]);
+                for (; i + 8 < cnt; i += 16) { add(i); add(i + 8); }
+                if (i < cnt) add(i);
                 // transpose: thread `sub` of the team ends with the team's sum of moment k = sub
                 f32x2 *scr64 = reinterpret_cast<f32x2 *>(scr);
 #pragma unroll
@@ -513,15 +541,26 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                 float2 h1 = *reinterpret_cast<float2 *>(&hsum);
                 if (cnt > 0) {
                     if (sub & 2) { h1.x = -h1.x; h1.y = -h1.y; }
-                    const int b = kp.base[c] + sidx;
                     float2 *row = a.mom + ((size_t)(c * n_pl + pl) * kKt + sub) * a.nb_pad;
                     atomicAdd(row + (b + L - 1), h1);
-                    if (sub == 0) my_samples += (unsigned long long)cnt * (unsigned)(min(b + L, prm.n_samples) - max(b, 0));
                 }
             }
         }
-        // no barrier here: the next pulse writes the other payload / index / histogram buffers, and this
-        // pulse's buffers are rewritten only two barriers later
+        // ---- the strays of this pulse: thread t takes moment t & 7 of stray t >> 3 ----
+        for (int t = tid; t < ns * kKt; t += kThreads) {
+            const float4 e = s_stray[buf][t >> 3];
+            const int k = t & 7, code = __float_as_int(e.w), c = code >> 28, jb = code & 0x0fffffff;
+            float t0 = 1.f, t1 = e.z;
+            for (int kk = 1; kk < k; ++kk) { const float t2 = 2.f * e.z * t1 - t0; t0 = t1; t1 = t2; }
+            const float tk = k ? t1 : 1.f;
+            atomicAdd(a.mom + ((size_t)(c * n_pl + pl) * kKt + k) * a.nb_pad + jb, make_float2(e.x * tk, e.y * tk));
+            if (k == 0) { const int b = jb - (L - 1); atomicMin(&s_blo[c], b); atomicMax(&s_bhi[c], b + 1); }
+        }
+        ++ip;
+        if (ns + max(ns - ns_prev, 0) > kStrayCap && ip < hi - lo) { need_sort = true; ip_sort = ip; }   // before the list overflows
+        ns_prev = need_sort ? 0 : ns;
+        // no barrier here: the next pulse writes the other payload / stray buffers, and this pulse's are rewritten
+        // only after the next barrier
     }
 
     // ---- counters ----
@@ -542,11 +581,12 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     // ---- the band every vector occupies, for K3s (fftconv.cu): outside the pulse loop, whose code must stay as it is
     //      (two atomics inside it cost 4 % of the kernel); a tile with an out-of-window echo claims the whole row ----
     if (a.band_lo) {
+        __syncthreads();                                     // the last pulse's strays have been merged into s_blo / s_bhi
         for (int k = tid; k < (hi - lo) * C; k += kThreads) {
             const int ip = k / C, c = k - ip * C, v = c * n_pl + (lo + ip - p0);
-            const int smin = s_band[ip][c][0], smax = s_band[ip][c][1];
-            if (s_wide) { atomicMin(a.band_lo + v, -(L - 1)); atomicMax(a.band_hi + v, prm.n_samples); }
-            else if (smax > smin) { atomicMin(a.band_lo + v, s_kp[ip].base[c] + smin); atomicMax(a.band_hi + v, s_kp[ip].base[c] + smax); }
+            // the sorted slices (one more on either side) and the strays, inside the sampling window
+            const int blo = max(s_blo[c], -(L - 1)), bhi = min(s_bhi[c], prm.n_samples);
+            if (bhi > blo) { atomicMin(a.band_lo + v, blo); atomicMax(a.band_hi + v, bhi); }
         }
     }
 }
