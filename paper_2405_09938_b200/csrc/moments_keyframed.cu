@@ -20,11 +20,16 @@
 // geometry_keyframes_ok): non-smooth state vectors never reach this kernel.
 //
 // One CTA = one spatial tile x one keyframe interval.  A thread owns FPT facets, holds their interpolants in
-// registers (18 words per facet) and loops over the interval's pulses; per pulse and for all C channels at
-// once: slice, sub-slice position and complex weight of every facet-echo -> counting sort by slice through a
-// shared-memory histogram (integer ATOMS) and an index list -> 8 threads per slice sum the Kt Chebyshev
-// moments (packed FFMA2), reduce-scatter by shuffles, one RED.ADD.F32x2 per (slice, k).  Histogram, payload
-// are double-buffered: three barriers per pulse.
+// registers (18 words per facet) and loops over the interval's pulses.  The tile's facet-echoes (all C channels) are
+// ordered by range slice ONCE per interval -- counting sort at its middle pulse: shared-memory histogram by integer
+// ATOMS, scan, slot = first position of the slice + rank -- because over a few milliseconds a facet changes slice only
+// when its sub-slice position crosses 0 or 1 (a percent or two of the echoes per pulse).  Per pulse: (A) slice,
+// sub-slice position and complex weight of every facet-echo; an echo found in its sorted slice writes its weight into
+// its slot, one found elsewhere ("stray") leaves a zero there and goes to a short shared-memory list; one barrier;
+// (C) 8 threads per occupied slice (one work list over all channels) sum the Kt Chebyshev moments of the slice's
+// contiguous slots (packed FFMA2), transpose through shared memory, one RED.ADD.F32x2 per (slice, k); the strays are
+// worked off with global atomics, thread t taking moment t & 7 of stray t >> 3.  A pulse whose strays would not fit
+// the list sorts the tile again (and is redone if they did not fit).  Payload and stray list are double-buffered.
 //
 // Bound: issue slots (FP32 + FP64 mix); HBM/L2: four surface rows per facet and INTERVAL, the maps once.
 #include "kernels.cuh"
