@@ -131,7 +131,7 @@ typedef struct {
 typedef struct {
     int32_t tile_facets;           /* spatial tile side in facets (4..64, power of 2; SPECTRAL clamps to 32); 0 = auto */
     int32_t pulses_per_batch;      /* 0 = auto from workspace_bytes */
-    int64_t workspace_bytes;       /* cap for per-batch device workspace; 0 = 4 GiB */
+    int64_t workspace_bytes;       /* cap for per-batch device workspace; 0 = 16 GiB, at most a quarter of the free device memory */
     int32_t accumulate_mode;       /* SIM_ACCUMULATE_*; SPECTRAL where it does not apply -> SIM_EINVAL */
     int32_t kinematics_keyframe;   /* wave sums evaluated exactly every H-th pulse (with time derivatives) and
                                       cubic-Hermite interpolated between: 0 = auto (largest H <= 64 whose error

@@ -734,7 +734,16 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
         (h->spectral ? (int64_t)C * kMomentOrder * h->nb_pad * 8
                      : (int64_t)C * fcap * (int64_t)sizeof(Rec) + (int64_t)C * Ns * 16 +
                            (int64_t)prm.n_tiles * (4 + 16 * C));
-    int64_t ws = (opts && opts->workspace_bytes > 0) ? opts->workspace_bytes : ((int64_t)4 << 30);
+    // default workspace: 16 GiB, at most a quarter of the free device memory, at least 1 GiB (a small cap splits a dwell
+    // of a large scene into many batches, and every batch recomputes the keyframe rows at its ends: on 2^26 facets
+    // a 4 GiB cap made three batches of 64 pulses and K1 computed 12 rows instead of 5)
+    int64_t ws = (opts && opts->workspace_bytes > 0) ? opts->workspace_bytes : ((int64_t)16 << 30);
+    if (!(opts && opts->workspace_bytes > 0)) {
+        size_t mem_free = 0, mem_total = 0;
+        if (cudaMemGetInfo(&mem_free, &mem_total) == cudaSuccess)
+            ws = std::max<int64_t>((int64_t)1 << 30, std::min<int64_t>(ws, (int64_t)(mem_free / 4)));
+        else cudaGetLastError();
+    }
     int pb = (int)std::max<int64_t>(1, std::min<int64_t>(ws / std::max<int64_t>(per_pulse, 1), 256));
     if (opts && opts->pulses_per_batch > 0) pb = opts->pulses_per_batch;
     pb = std::min(pb, P);
