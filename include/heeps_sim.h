@@ -135,12 +135,12 @@ typedef struct {
     int32_t accumulate_mode;       /* SIM_ACCUMULATE_*; SPECTRAL where it does not apply -> SIM_EINVAL */
     int32_t kinematics_keyframe;   /* wave sums evaluated exactly every H-th pulse (with time derivatives) and
                                       cubic-Hermite interpolated between: 0 = auto (largest H <= 64 whose error
-                                      bound sum_w A_w (omega_w h)^4/384 <= 2e-9 m; slopes linear between), 1 = every pulse, n = force H = n */
+                                      bound sum_w A_w (omega_w h)^4/384 <= 4e-8 m; slopes linear between), 1 = every pulse, n = force H = n */
     int32_t geometry_keyframe;     /* SPECTRAL only: 0 = auto -- where kinematics keyframes are in use (H > 1), C <= 4 and
                                       the receive offsets are small, ranges / gains are evaluated exactly at the
                                       keyframe pulses only and interpolated between (Hermite path length, quadratic
                                       gains), after sim_create has verified the interpolants against the exact geometry
-                                      at every pulse on a lattice of scene points (path 2e-8 m, gains 3e-6);
+                                      at every pulse on a lattice of scene points (path 2e-8 m, gains 1e-5);
                                       1 = off (exact geometry at every pulse) */
     int32_t fft_band;              /* SPECTRAL with keyframed geometry: a vector whose echoes occupy a narrow band of range
                                       slices is convolved by a transform of that band alone: 0 = auto (size from the scene's
