@@ -43,8 +43,8 @@ MOMENT_FP32_OPS_PER_FACET_ECHO = 4.0 * 8 + 30.0
 # From the committed ncu captures (profiles/): executed thread-instructions per facet-echo (context for the
 # roofline fraction: the kernels are issue-bound, not pipe-bound) and dram bytes per facet-echo.
 K2S_EXECUTED_INSTR_PER_FACET_ECHO = 1156.0 / 3      # profiles/r1_v4_k2s_ncu_summary.txt
-K2K_EXECUTED_INSTR_PER_FACET_ECHO = 491.5 / 3       # profiles/r1_v15_k2k_ncu_summary.txt (1.0307e9 warp instr / launch)
-K2K_DRAM_BYTES_PER_FACET_ECHO = (95.977e6 + 7.938e6) / (256 * 3 * 262144)   # same capture: dram read + write
+K2K_EXECUTED_INSTR_PER_FACET_ECHO = 474.3 / 3       # profiles/r1_v16_k2k_ncu_summary.txt (9.947e8 warp instr / launch)
+K2K_DRAM_BYTES_PER_FACET_ECHO = (62.420e6 + 1.849e6) / (256 * 3 * 262144)   # same capture: dram read + write
 # dram bytes per kept facet-echo of a K3 launch, from the committed `ncu --set full` capture
 # profiles/r1_v3_k3_ncu_summary.txt: (2.580977e9 read + 1.1966e7 written) / (100 pulses x 3 ch x 262144).
 K3_DRAM_BYTES_PER_FACET_ECHO = (2.580977e9 + 1.1966e7) / (100 * 3 * 262144)
