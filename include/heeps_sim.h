@@ -135,7 +135,7 @@ typedef struct {
     int32_t accumulate_mode;       /* SIM_ACCUMULATE_*; SPECTRAL where it does not apply -> SIM_EINVAL */
     int32_t kinematics_keyframe;   /* wave sums evaluated exactly every H-th pulse (with time derivatives) and
                                       cubic-Hermite interpolated between: 0 = auto (largest H <= 64 whose error
-                                      bound sum_w A_w (omega_w h)^4/384 <= 4e-8 m; slopes linear between), 1 = every pulse, n = force H = n */
+                                      bound sum_w A_w (omega_w h)^4/384 <= 4e-8 m; slopes linear between, their error <= 1.2e-4), 1 = every pulse, n = force H = n */
     int32_t geometry_keyframe;     /* SPECTRAL only: 0 = auto -- where kinematics keyframes are in use (H > 1), C <= 4 and
                                       the receive offsets are small, ranges / gains are evaluated exactly at the
                                       keyframe pulses only and interpolated between (Hermite path length, quadratic
