@@ -748,7 +748,7 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
             ws = std::max<int64_t>((int64_t)1 << 30, std::min<int64_t>(ws, (int64_t)(mem_free / 4)));
         else cudaGetLastError();
     }
-    int pb = (int)std::max<int64_t>(1, std::min<int64_t>(ws / std::max<int64_t>(per_pulse, 1), 256));
+    int pb = (int)std::max<int64_t>(1, std::min<int64_t>(ws / std::max<int64_t>(per_pulse, 1), h->spectral ? 1024 : 256));
     if (opts && opts->pulses_per_batch > 0) pb = opts->pulses_per_batch;
     pb = std::min(pb, P);
     if (!(opts && opts->pulses_per_batch > 0)) {        // balance the batches of a full-dwell call
