@@ -8,7 +8,7 @@ import numpy as np
 import mpmath as mp
 import pytest
 
-from oracle import oracle_generate, oracle_facets
+from oracle import oracle_generate, oracle_facets, oracle_samples
 from workloads import C0, make_workload
 from helpers import custom_workload
 
@@ -177,6 +177,80 @@ def test_brute_force_with_maps_tilt_current_cull():
     for p in range(2):
         ref = _numpy_brute(w, p)
         assert np.max(np.abs(s[:, p] - ref)) < 1e-7 * np.max(np.abs(ref))
+
+
+def test_facet_velocity_is_the_time_derivative_of_the_position():
+    """vel (O2: orbital + current) against a central finite difference of pos over pulse times 1 us apart:
+    all three components, many components, CWM on, current map (G10)."""
+    w = make_workload("tiny", n_pulses=3)
+    sc = w.scene
+    sc["nx"], sc["ny"] = 5, 4
+    sc["xi"] = np.ascontiguousarray(sc["xi"][:4, :5])
+    sc["choppy"] = 1
+    sc["current_mps"] = np.random.default_rng(3).normal(0, 0.5, (4, 5, 2)).astype(np.float32)
+    h = 1e-4
+    w.geometry["t_pulse_s"] = np.array([0.3 - h, 0.3, 0.3 + h])
+    f0, f1, f2 = (oracle_facets(w, p) for p in range(3))
+    fd = (f2["pos"] - f0["pos"]) / (2 * h)
+    assert np.abs(f1["vel"][:, :2]).max() > 0.3 and np.abs(f1["vel"][:, 2]).max() > 0.3
+    assert np.max(np.abs(f1["vel"] - fd)) < 1e-6                  # O(h^2 w^3 A) ~ 1e-7
+
+
+def test_oracle_samples_equals_oracle_generate():
+    """heeps_oracle_samples (the O9 loop restricted to listed samples -- the checker of the full-size parity tests)
+    against heeps_oracle_generate on Tiny with 3 channels: unsorted list, a repeated sample, samples outside every
+    echo window, the first and last sample of the window; and on a culling, map-carrying scene."""
+    w = make_workload("tiny", n_pulses=5)
+    w.instrument["channel_offset_m"] = np.array([-1.5, 0.0, 1.5])
+    full = oracle_generate(w)
+    live = np.nonzero(full[1, 3])[0]
+    dead = np.setdiff1d(np.arange(256), live)
+    assert live.size > 30 and dead.size > 30
+    ns = np.array([live[17], live[0], 255, live[-1], live[17], dead[0], 0, live[5], dead[-1], live[30]], dtype=np.int32)
+    for p in (0, 3, 4):
+        got = oracle_samples(w, p, ns)
+        assert got.shape == (3, ns.size)
+        ref = full[:, p, :][:, ns]
+        assert np.max(np.abs(got - ref)) <= 1e-12 * np.abs(full).max()
+        assert np.all(got[:, [2, 5, 6, 8]] == 0) and np.all(got[:, 0] == got[:, 4])
+    # channels are not interchangeable here: a channel / sample stride slip would show
+    assert np.abs(full[0, 3, live[17]] - full[2, 3, live[17]]) > 1e-3 * np.abs(full).max()
+    # with a cull, maps and tilt: same scene as the brute-force pin
+    rng = np.random.default_rng(5)
+    sc = w.scene
+    sc["nx"], sc["ny"] = 6, 5
+    sc["xi"] = np.ascontiguousarray(sc["xi"][:5, :6])
+    sc["sigma0_lin"] = rng.uniform(0.01, 0.1, (5, 6)).astype(np.float32)
+    sc["tilt_modulation"] = 1
+    sc["current_mps"] = rng.normal(0, 0.5, (5, 6, 2)).astype(np.float32)
+    sc["spacing_m"] = 700.0
+    w.instrument["cull_two_way_db"] = -3.0
+    ns2 = np.arange(255, -1, -3, dtype=np.int32)
+    for p in (1, 2):
+        brute = _numpy_brute(w, p)
+        got = oracle_samples(w, p, ns2)
+        assert np.max(np.abs(got - brute[:, ns2])) < 1e-7 * np.max(np.abs(brute))
+
+
+def test_oracle_samples_single_facet_mpmath_fixture():
+    """heeps_oracle_samples against the stored 50-digit values of the single-facet chirp (tests/golden/
+    single_facet_chirp.txt; eq. (3)): every in-window sample, listed in reverse order, plus the two
+    samples just outside the half-open window."""
+    from pathlib import Path
+    gold = Path(__file__).resolve().parent / "golden" / "single_facet_chirp.txt"
+    lines = gold.read_text().splitlines()
+    t0 = float([ln for ln in lines if ln.startswith("# t0")][0].split("=")[1])
+    rows = [ln.split() for ln in lines if ln and not ln.startswith("#")]
+    ns = np.array([int(r[0]) for r in rows], dtype=np.int32)
+    expect = np.array([float(r[1]) + 1j * float(r[2]) for r in rows])
+    tx, rx, pos = (10.0, -300e3, 700e3), (250e3, -300e3, 700e3), (3.0, -7.0, 0.25)
+    xi = np.array([[[0.6, -0.8]]], dtype=np.float32)
+    w = custom_workload(centre=pos, tx_pos=tx, rx_pos=rx, t0=t0, K=5e12, T=2e-6, fs=12e6, n_samples=256,
+                        sigma0=4.0, d=1.5, xi=xi)
+    order = np.concatenate([ns[::-1], [ns[0] - 1, ns[-1] + 1]]).astype(np.int32)
+    got = oracle_samples(w, 0, order)[0]
+    assert np.max(np.abs(got[:ns.size] - expect[::-1])) < 2e-7 * 3.0
+    assert got[-2] == 0 and got[-1] == 0
 
 
 def test_linearity_and_superposition():
@@ -394,8 +468,9 @@ def test_single_wave_component_closed_form_and_cwm_circle():
     ts = np.linspace(0.0, 2 * np.pi / om, 13)
     P = len(ts)
     tx = np.repeat([[0, -300e3, 700e3]], P, 0)
+    CUR = (0.3, -0.2)
     w = custom_workload(nx=3, ny=2, d=5.0, centre=(10.0, 20.0, 1.0), waves=waves, t_pulse=ts,
-                        tx_pos=tx, rx_pos=tx, t0=0.0)
+                        tx_pos=tx, rx_pos=tx, t0=0.0, current=CUR)
     for choppy in (0, 1):
         w.scene["choppy"] = choppy
         path = []
@@ -408,9 +483,14 @@ def test_single_wave_component_closed_form_and_cwm_circle():
             assert abs(f["pos"][fidx, 2] - (1.0 + A * np.cos(psi))) < 1e-13
             assert np.allclose(f["slope"][fidx], [-A * kx * np.sin(psi), -A * ky * np.sin(psi)], atol=1e-14)
             assert abs(f["vel"][fidx, 2] - A * om * np.sin(psi)) < 1e-13
+            # horizontal facet velocity: the current, plus (CWM) the orbital velocity A w k^ cos(psi) -- the time
+            # derivative of the horizontal displacement -A k^ sin(psi)
+            khat_ = np.array([kx, ky]) / np.hypot(kx, ky)
+            vh = np.array(CUR) + (A * om * np.cos(psi) * khat_ if choppy else 0.0)
+            assert np.allclose(f["vel"][fidx, :2], vh, atol=1e-13)
             if not choppy:
-                assert abs(f["pos"][fidx, 0] - xb) < 1e-13 and abs(f["pos"][fidx, 1] - yb) < 1e-13
-            path.append(f["pos"][fidx] - np.array([xb, yb, 1.0]))
+                assert abs(f["pos"][fidx, 0] - (xb + CUR[0] * t)) < 1e-13 and abs(f["pos"][fidx, 1] - (yb + CUR[1] * t)) < 1e-13
+            path.append(f["pos"][fidx] - np.array([xb + CUR[0] * t, yb + CUR[1] * t, 1.0]))
         if choppy:
             path = np.array(path)
             khat = np.array([kx, ky]) / np.hypot(kx, ky)
@@ -496,3 +576,39 @@ def test_workloads_are_frozen():
     xi = w.scene["xi"].astype(np.float64)
     assert abs((xi ** 2).sum(-1).mean() - 1.0) < 0.05        # E|xi|^2 = 1
     assert abs(xi.mean()) < 0.02
+
+
+@pytest.mark.parametrize("name", ["tiny", "ati", "hetero", "large", "sweep20", "sweep22", "sweep24", "sweep26"])
+def test_workload_digests_match_the_committed_file(name):
+    """G22: every seeded workload against its committed fingerprint (tests/golden/workload_digests.txt, written by
+    tests/golden/make_workload_digests.py from workloads/ alone): same keys, dtypes and shapes, checksums to 1e-9
+    (of the Cauchy-Schwarz scale sqrt(n sum_sq)).  A byte-level (SHA-256) difference with matching checksums is a
+    last-bit libm / FFT difference of the platform and is reported, not failed."""
+    import importlib.util
+    import warnings
+    from pathlib import Path
+    gold_dir = Path(__file__).resolve().parent / "golden"
+    spec = importlib.util.spec_from_file_location("make_workload_digests", gold_dir / "make_workload_digests.py")
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    want = {}
+    for ln in (gold_dir / "workload_digests.txt").read_text().splitlines():
+        if ln and not ln.startswith("#"):
+            cfg, key, dt, shape, s1, s2, s3, sha = ln.split()
+            if cfg == name:
+                want[key] = (dt, shape, float(s1), float(s2), float(s3), sha)
+    assert want, name
+    got = mod.fingerprint(mod.build(name))
+    assert sorted(k for k, *_ in got) == sorted(want)
+    drift = []
+    for key, dt, shape, s1, s2, s3, sha in got:
+        wdt, wshape, w1, w2, w3, wsha = want[key]
+        assert (dt, shape) == (wdt, wshape), key
+        n = max(int(np.prod(eval(shape))) if shape != "()" else 1, 1)
+        scale = np.sqrt(n * w2)
+        assert abs(s2 - w2) <= 1e-9 * w2, key
+        assert abs(s1 - w1) <= 1e-9 * scale and abs(s3 - w3) <= 1e-9 * scale, key
+        if sha != wsha:
+            drift.append(key)
+    if drift:
+        warnings.warn(f"{name}: byte-level differences within 1e-9 in {drift}")
