@@ -15,6 +15,7 @@ from .generator import (  # noqa: F401
     make_workload,
     make_sweep_point,
     add_wave_nodes,
+    crop_rows,
     add_antenna_patterns,
     pm_spectrum,
     workload_digest,

@@ -282,6 +282,25 @@ def make_sweep_point(*, log2_facets: int = 24, spacing_m: float | None = None,
     return w
 
 
+def crop_rows(w: Workload, j0: int, j1: int) -> Workload:
+    """A slab of facet rows [j0, j1) of the same scene as a workload of its own (input slicing only): the maps are
+    sliced, the scene centre moves to the slab's centre so that every kept facet keeps its rest position, and the
+    instrument, geometry and sampling window stay those of the full scene.  Used to time the oracle on a bounded
+    sample of a large configuration (bench.py cpu_baseline / --impl reference)."""
+    sc = dict(w.scene)
+    ny = int(sc["ny"])
+    if not (0 <= j0 < j1 <= ny) or sc.get("wave_nodes") is not None:
+        raise ValueError("crop_rows: bad row range, or a heterogeneous-lattice workload")
+    for k in ("sigma0_lin", "current_mps", "xi"):
+        if sc.get(k) is not None:
+            sc[k] = np.ascontiguousarray(sc[k][j0:j1])
+    centre = np.array(sc["centre_m"], dtype=np.float64)
+    centre[1] += (0.5 * (j0 + j1 - 1) - 0.5 * (ny - 1)) * float(sc["spacing_m"])
+    sc["centre_m"] = centre
+    sc["ny"] = int(j1 - j0)
+    return Workload(name=f"{w.name}[rows {j0}:{j1}]", instrument=w.instrument, geometry=w.geometry, scene=sc)
+
+
 def add_wave_nodes(w: Workload, spacing_m: float, seed: int = MASTER_SEED + 4) -> Workload:
     """Heterogeneous-surface variant of a workload: a lattice of wave tables of step `spacing_m`
     covering the grid, one homogeneous tile T2L per node.  Uniform sea state as the paper describes it:
