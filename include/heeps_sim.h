@@ -192,6 +192,16 @@ int sim_replica(const sim_handle *h, float *host_c64_out, int32_t *n);
 int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, double *tau, double *g_tx,
                      double *g_rx, double *amp, int32_t *keep);
 
+/* Per-facet-echo intermediates of the DEFAULT spectral path with keyframed geometry (moments_keyframed.cu), for one
+ * pulse (host arrays, any may be NULL): range slice b = ceil((tau - t0) fs - T fs / 2) (the first in-window sample of
+ * the echo; eq. (17): slice membership is an integer decision) slice [C][F]; sub-slice position
+ * eps = b - ((tau - t0) fs - T fs / 2) in (0, 1], eps [C][F]; complex weight a G_t G_r,c exp(-j 2 pi f0 (tau - t0[p]))
+ * as the kernel interpolates it, weight [C][F][2]; keep [F].  *n_edge_ambiguous = kept facet-echoes whose
+ * position lies within 1e-6 of an integer: their slice may legitimately differ from an fp64 evaluation's (reading
+ * G18).  SIM_EINVAL unless the handle runs the spectral form with keyframed geometry (sim_stats).  Synchronous. */
+int sim_debug_echoes(sim_handle *h, int32_t pulse, int32_t *slice, float *eps, float *weight, int32_t *keep,
+                     int64_t *n_edge_ambiguous);
+
 /* Counters of the most recent sim_generate* call (after the stream has completed). */
 typedef struct {
     int64_t facet_echoes_nominal;  /* F * pulses * C                                   */

@@ -20,6 +20,7 @@ from .binding import (  # noqa: F401
     sim_update_scene,
     sim_replica,
     sim_debug_facets,
+    sim_debug_echoes,
     sim_get_stats,
     sim_measure_pipe_peaks,
 )

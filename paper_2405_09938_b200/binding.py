@@ -118,6 +118,8 @@ def load_library():
         lib.sim_replica.argtypes = [vp, vp, C.POINTER(i32)]
         lib.sim_debug_facets.restype = C.c_int
         lib.sim_debug_facets.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp]
+        lib.sim_debug_echoes.restype = C.c_int
+        lib.sim_debug_echoes.argtypes = [vp, i32, vp, vp, vp, vp, C.POINTER(C.c_int64)]
         lib.sim_get_stats.restype = C.c_int
         lib.sim_get_stats.argtypes = [vp, C.POINTER(sim_stats)]
         lib.sim_set_profiling.restype = C.c_int
@@ -248,7 +250,7 @@ def _marshal(workload):
 
 def sim_create(workload, device: int = 0, *, tile_facets: int = 0, pulses_per_batch: int = 0,
                workspace_bytes: int = 0, accumulate_mode=0, kinematics_keyframe: int = 0,
-               geometry_keyframe: int = 0, fft_band: int = 0):
+               geometry_keyframe: int = 0, fft_band: int = 0, k2k_tile_cap: int = 0):
     lib = load_library()
     ci, cg, cs, keep = _marshal(workload)
     opts = sim_options()
@@ -257,6 +259,7 @@ def sim_create(workload, device: int = 0, *, tile_facets: int = 0, pulses_per_ba
     opts.kinematics_keyframe = int(kinematics_keyframe)
     opts.geometry_keyframe = int(geometry_keyframe)
     opts.fft_band = int(fft_band)
+    opts.reserved[0] = int(k2k_tile_cap)
     h = C.c_void_p()
     rc = lib.sim_create(C.byref(ci), C.byref(cg), C.byref(cs), C.byref(opts), int(device), C.byref(h))
     del keep
@@ -298,6 +301,18 @@ def sim_debug_facets(handle, pulse: int, n_facets: int, n_channels: int) -> dict
     _check(load_library().sim_debug_facets(handle, pulse, *(res[k].ctypes.data for k in
                                            ("pos", "slope", "tau", "g_tx", "g_rx", "amp", "keep"))), handle)
     res["amp"] = res["amp"][..., 0] + 1j * res["amp"][..., 1]
+    return res
+
+
+def sim_debug_echoes(handle, pulse: int, n_facets: int, n_channels: int) -> dict:
+    F, Cn = n_facets, n_channels
+    res = dict(slice=np.zeros((Cn, F), dtype=np.int32), eps=np.zeros((Cn, F), dtype=np.float32),
+               weight=np.zeros((Cn, F, 2), dtype=np.float32), keep=np.zeros(F, dtype=np.int32))
+    n_edge = C.c_int64(0)
+    _check(load_library().sim_debug_echoes(handle, pulse, res["slice"].ctypes.data, res["eps"].ctypes.data,
+                                           res["weight"].ctypes.data, res["keep"].ctypes.data, C.byref(n_edge)), handle)
+    res["weight"] = res["weight"][..., 0] + 1j * res["weight"][..., 1]
+    res["n_edge_ambiguous"] = int(n_edge.value)
     return res
 
 
@@ -381,6 +396,9 @@ class Simulator:
 
     def debug_facets(self, pulse: int) -> dict:
         return sim_debug_facets(self._h, pulse, self.n_facets, self.n_channels)
+
+    def debug_echoes(self, pulse: int) -> dict:
+        return sim_debug_echoes(self._h, pulse, self.n_facets, self.n_channels)
 
     def stats(self) -> dict:
         return sim_get_stats(self._h)

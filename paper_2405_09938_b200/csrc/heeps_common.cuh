@@ -79,6 +79,14 @@ struct DevParams {
     int32_t series_channels;     // receive-channel legs by series about the un-offset phase centre (geometry_common.cuh)
     int32_t lut_any;             // some antenna pattern is tabulated: gains are complex (geometry_common.cuh)
     PatternLut lut[2];           // [0] Tx, [1] Rx
+    // keyframed geometry (moments_keyframed.cu): f0 / fs [turns of carrier per range slice] in units of 2^-48, split
+    // into two 32-bit words, and the constant phase frac((2^15 - T fs / 2) f0 / fs) in 2^-32 turns
+    uint32_t ratio_hi, ratio_lo, phase_bias32;
+    // sheared tiles of K2k: k2k_h lines of k2k_w facets (k2k_w a power of two, k2k_w k2k_h = tile_cap); line b displaced by
+    // rint(k2k_shear b) facets along the line; axis 0: lines = grid rows, 1: lines = grid columns; k2k_a0 = along-line
+    // index of the first tile's first facet (<= 0); k2k_tiles_a tiles along a line, k2k_n_tiles in all
+    int32_t k2k_w, k2k_h, k2k_cap, k2k_axis, k2k_a0, k2k_tiles_a, k2k_n_tiles;   // k2k_cap = k2k_w k2k_h facets per tile
+    double k2k_shear;
 };
 
 }  // namespace heeps

@@ -122,6 +122,14 @@ struct MomentArgs {
     // K2k only, may be null: occupied slice range [band_lo, band_hi) of every vector [C][n_pl], by atomicMin / atomicMax
     // (the caller presets lo to a large and hi to a small value); lets K3s transform only the band (fftconv.cu)
     int32_t *band_lo, *band_hi;
+    // K2k only, debug (sim_debug_echoes), all null in normal operation: what the kernel computes for the facet-echoes of
+    // pulse dbg_pulse -- slice b [C][F], sub-slice position eps [C][F], complex weight [C][F] (before the reference phase
+    // of the pulse), keep [F]
+    int32_t *dbg_slice;
+    float *dbg_eps;
+    float2 *dbg_w;
+    int32_t *dbg_keep;
+    int32_t dbg_pulse;
 };
 size_t moments_smem_bytes(const DevParams &prm, int span_cap);
 cudaError_t launch_moments(const DevParams &prm, const MomentArgs &a, int p0, int n_pl, cudaStream_t s);
@@ -132,6 +140,7 @@ cudaError_t launch_moments(const DevParams &prm, const MomentArgs &a, int p0, in
 constexpr int kMaxKeyChannels = 4;
 constexpr int kMaxKeyPulses = 66;
 size_t moments_keyframed_smem_bytes(const DevParams &prm, int span_cap);
+bool moments_keyframed_fits(const DevParams &prm, int span_cap);
 cudaError_t launch_moments_keyframed(const DevParams &prm, const MomentArgs &a, int p0, int n_pl, cudaStream_t s);
 
 // K3s -- convolution of the moments with the waveform kernels + finalize (fftconv.cu).

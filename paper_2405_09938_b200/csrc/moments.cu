@@ -9,14 +9,16 @@
 // eps in [0,1) is kept to any order: with b = ceil(nu) (integer slice = first in-window sample),
 // m = n - b, y = 2 eps - 1 and z_m = 2 pi kappa (m - L/2),
 //
-//   exp(j 2 pi kappa (m + eps - L/2)^2) = exp(j 2 pi kappa ((m-L/2)^2 + (m-L/2))) exp(j 2 pi kappa eps^2) exp(j z_m y)
-//   exp(j z y) = sum_k e_k j^k J_k(z) T_k(y)          (Jacobi-Anger; e_0 = 1, e_k = 2; |z| <= pi B/(2 fs))
+//   g_m(y) = exp(j 2 pi kappa (m + eps - L/2)^2) = sum_k c_k[m] T_k(y)        (Chebyshev series in y of the slice response;
+//            = exp(j 2 pi kappa ((m-L/2)^2 + (m-L/2) + eps^2)) exp(j z_m y), whose last factor is the Jacobi-Anger series
+//            sum_k e_k j^k J_k(z_m) T_k(y), |z_m| <= pi B/(2 fs); sim_api.cu computes c_k[m] by quadrature)
 //
 // so  s[n] = sum_{k<Kt} sum_m c_k[m] M_k[n-m]  with the Chebyshev moments of each slice
 //
-//   M_k[b] = sum_{f: b_f = b} |A~_f| exp(j 2 pi (-dR_f/lambda + kappa eps_f^2 + arg A~_f)) T_k(y_f)
+//   M_k[b] = sum_{f: b_f = b} |A~_f| exp(j 2 pi (-dR_f/lambda + arg A~_f)) T_k(y_f)
 //
-// (Kt = 1 is exactly eq. (17); Kt = 8 truncates at J_8(1.31) ~ 1e-6.)  This kernel produces M; the
+// (Kt = 1 is eq. (17) with the slice response at its mean; Kt = 8 truncates at J_8(1.31) ~ 1e-6; sim_create refuses the
+// form when the tail beyond Kt exceeds 5e-6.)  This kernel produces M; the
 // convolution with the Kt waveform kernels c_k is fftconv.cu.
 //
 // One CTA = one spatial tile (<= 32 x 32 facets) of one pulse.  Facet state (fp64 position, Tx leg, cull)
@@ -158,7 +160,7 @@ moments_kernel(DevParams prm, MomentArgs a, int p0, int n_pl)
             const double eps = bd - nu;                                    // [0, 1)
             const float g = gt[q] * g_rx;
             const uint32_t garg = (g < 0.f && !prm.lut_any) ? 0x80000000u : 0u;
-            const uint32_t ph = turns_to_u32_fast(fma(prm.kappa * eps, eps, -dR * prm.inv_lambda)) + xarg[q] + garg;
+            const uint32_t ph = turns_to_u32_fast(-dR * prm.inv_lambda) + xarg[q] + garg;    // (the chirp's kappa eps^2 is part of c_k)
             float sn, cs;
             __sincosf((float)(int32_t)ph * 1.4629180792671596e-9f, &sn, &cs);   // 2 pi / 2^32
             if (prm.lut_any) {                                             // complex gain product times the phasor

@@ -7,31 +7,57 @@
 //
 //   R(t)   = r_t + r_r,ref  bistatic path to the un-offset phase centre: cubic HERMITE from the exact values and
 //            time derivatives at the two keyframes,  dR/dt = u_t.(v_f - V_tx) + u_r.(v_f - V_rx)  with the facet
-//            velocity v_f = (current + dD_h/dt, dz/dt) from K1's rate rows.  Error <= h^4 max|R''''| / 384:
-//            platform term 3 V^4/r^3 ~ 0.02 m/s^4 -> 4e-13 m at h = 9.4 ms; wave term = K1's own bound (2e-9 m).
-//   d_c(t) = r_r,c - r_r,ref  (receive phase centre c, |o_c| <= 1e-4 r) = o_c a(t) + o_c^2 b, a = -(d.v^)/r linear
-//            in t, b = (1 - a^2)/(2 r); fp32 (|d_c| < 1 m).
-//   P(t)   = G_t G_r,ref      quadratic through t0, t_mid, t1 with the sinc arguments at t_mid taken as the mean of
-//            the end values (they are linear in t to ~1e-7); G_r,c = G_r,ref + o_c dG/do with dG/do by one
-//            finite difference at t_mid.  |a_f|(t) (tilt modulation) quadratic the same way.
+//            velocity v_f = (current + dD_h/dt, dz/dt) from K1's rate rows.  Error <= h^4 max|d4R/dt4| / 384:
+//            platform term 3 V^4/r^3 ~ 0.02 m/s^4 -> 4e-13 m at h = 9.4 ms; wave term = K1's own bound.
+//   d_c(t) = r_r,c - r_r,ref  (receive phase centre c, |o_c| <= 16 m) = o_c a(t) + o_c^2 b, a = -(d.v^)/r linear
+//            in t, b = (1 - a^2)/(2 r).
+//   P(t)   = G_t G_r,ref      CUBIC through t0, t0 + h/3, t0 + 2h/3, t1 with the sinc arguments (direction cosines)
+//            between the keyframes interpolated linearly (they are linear in t to ~1e-7): interpolation error ~3e-8
+//            of the peak gain, so that the cull decision |P| >= threshold (G6) differs from the exact one only for
+//            facets within ~1e-7 of the threshold (a quadratic left 4e-6: a handful of flipped facets per pulse on
+//            the Large scene, each worth 2e-5 of relative L2).  G_r,c = G_r,ref + o_c dG/do with dG/do by one finite
+//            difference at mid-interval.  |a_f|(t) (tilt modulation) quadratic through t0, t_mid, t1.
 //
-// sim_create verifies these three interpolants against the exact geometry on a 3 x 3 lattice of scene points
-// at EVERY pulse (host, long double) and falls back to moments.cu when any bound fails (sim_api.cu
-// geometry_keyframes_ok): non-smooth state vectors never reach this kernel.
+// sim_create verifies these interpolants against the exact geometry on a lattice of scene points at EVERY pulse
+// (host, long double) and falls back to moments.cu when any bound fails (sim_api.cu geometry_keyframes_ok):
+// non-smooth state vectors or non-uniform pulse times never reach this kernel.
 //
-// One CTA = one spatial tile x one keyframe interval.  A thread owns FPT facets, holds their interpolants in
-// registers (18 words per facet) and loops over the interval's pulses.  The tile's facet-echoes (all C channels) are
-// ordered by range slice ONCE per interval -- counting sort at its middle pulse: shared-memory histogram by integer
+// ARITHMETIC OF THE PULSE LOOP.  Pulse times inside an interval are uniform (checked on the host), so the cubic R is
+// advanced from pulse to pulse by FORWARD DIFFERENCES in 64-bit fixed point: rho = (R - R_base) fs/c0 - L/2 + 2^15 in
+// units of 2^-48 range slice (R_base = c0 t0 of the first keyframe, a CTA constant): three 64-bit adds per facet and
+// pulse, no fp64 in the loop (the fp64 chain, its conversions and the per-echo sub-slice phase were two thirds of
+// round 1's 100 instructions per facet-echo in this stage).  From the same word come
+//   the slice and the sub-slice position  (rho - w_p + channel term) >> 16 = [integer slice . 32-bit fraction]
+//       (w_p = the sampling window's own start (r0[p] - R_base) fs/c0: an arbitrary per-pulse input, from shared memory),
+//   the carrier phase  -R/lambda = -rho (f0/fs) + const: the 32 fraction bits of the 64 x 64-bit product with f0/fs in
+//       2^-48 units -- two IMAD.HI and one IMAD -- exact to 3 units of 2^-32 turn at any range.
+// The receive-channel path difference o_c a(t) + o_c^2 b enters both words, and to the same accuracy (a facet-echo whose
+// slice position sits within the error of an integer lands in the neighbouring slice, and since the replica's window
+// is a hard edge every such echo costs two samples of its full amplitude: relative L2 sqrt(4 delta / L) for an error of
+// delta slices at ANY scene size -- 1e-5 slices: 1.8e-4; 1e-8: 6e-6): a is split into its value at the tile centre (one
+// exact word per channel and CTA, shared memory) and the facet's small deviation + its drift over the interval, which
+// one FP32 FMA against 1.5 x 2^23 rounds to an integer.
+// The chirp's own sub-slice phase kappa eps^2 is part of the waveform kernels (sim_api.cu builds them as the Chebyshev
+// coefficients of the exact slice response), so the per-echo phase is the carrier phase alone.
+//
+// One CTA = one SHEARED spatial tile x one keyframe interval (256 threads x 4 facets, two CTAs per SM).  A thread holds
+// its facets' interpolants in registers and loops over the interval's pulses.  The tile's facet-echoes (all C channels)
+// are ordered by range slice ONCE per interval -- counting sort at its middle pulse: shared-memory histogram by integer
 // ATOMS, scan, slot = first position of the slice + rank -- because over a few milliseconds a facet changes slice only
 // when its sub-slice position crosses 0 or 1 (a percent or two of the echoes per pulse).  Per pulse: (A) slice,
-// sub-slice position and complex weight of every facet-echo; an echo found in its sorted slice writes its weight into
-// its slot, one found elsewhere ("stray") leaves a zero there and goes to a short shared-memory list; one barrier;
-// (C) 8 threads per occupied slice (one work list over all channels) sum the Kt Chebyshev moments of the slice's
-// contiguous slots (packed FFMA2), transpose through shared memory, one RED.ADD.F32x2 per (slice, k); the strays are
-// worked off with global atomics, thread t taking moment t & 7 of stray t >> 3.  A pulse whose strays would not fit
-// the list sorts the tile again (and is redone if they did not fit).  Payload and stray list are double-buffered.
+// sub-slice position and complex weight of every facet-echo, branch-free; an echo found in its sorted slice writes its
+// weight into its slot, one found elsewhere ("stray") leaves a zero there and goes to a short shared-memory list; one
+// barrier; (C) 8 threads per occupied slice (one work list over all channels) sum the Kt Chebyshev moments of the
+// slice's contiguous slots (packed FFMA2), transpose through shared memory, one RED.ADD.F32x2 per (slice, k); the
+// strays are worked off with global atomics, thread t taking moment t & 7 of stray t >> 3.  A pulse whose strays would
+// not fit the list sorts the tile again (and is redone if they did not fit; after a sort at the pulse itself the
+// overflow -- echoes outside the tile's slice window -- goes straight to global atomics, so the redo happens at most
+// once).  Payload and stray list are double-buffered.
+// Tried and measured in round 2 (profiles/r2_k2k_history.md): 512 threads x 2 facets with one CTA per SM, stage C by
+// one thread per chunk of slots, and producer / consumer warps behind named barriers -- each cut the instruction count
+// and none the time: with one CTA per SM the warps that sum the slices hold the others at the barrier.
 //
-// Bound: issue slots (FP32 + FP64 mix); HBM/L2: four surface rows per facet and INTERVAL, the maps once.
+// Bound: issue slots (FP32 + integer mix); HBM/L2: four surface rows per facet and INTERVAL, the maps once.
 #include "kernels.cuh"
 #include "geometry_common.cuh"
 
@@ -39,61 +65,53 @@ namespace heeps {
 
 namespace {
 
-constexpr int kThreads = 256;
 constexpr int kKt = kMomentOrder;
-static_assert(kKt == 8, "the reduce-scatter below is written for 8 moments / 8 threads per slice");
+static_assert(kKt == 8, "the sign pattern of the moment recurrence below is written for 8 moments");
+
+constexpr int kRhoBias = 32768;           // slices added to rho so that it stays positive (unsigned 64-bit product)
 
 struct __align__(16) KeyPulse {          // per pulse of the interval (shared memory)
-    double sd;                           // (t - t0) / h
-    float u0, u1;                        // s (1-s)^2, -s^2 (1-s): weights of the Hermite cubic's bend (see R below)
-    double r0;                           // c0 t0[p]
-    float s, pad0;                       // (t - t0) / h
+    long long w;                         // (r0[p] - R_base) fs/c0 in 2^-48 slices
+    uint32_t phi;                        // frac((r0[p] - R_base) / lambda) in 2^-32 turns
+    float s;                             // (t - t0) / h
     int32_t base[kMaxKeyChannels];       // first slice of the tile's shared-memory window, per channel
 };
 
 // Exact state of one facet at one keyframe pulse.
-template <int C>
 struct KeyEval {
     double R, Rd;                        // path to the un-offset phase centre and its time derivative
-    float xat, xet, xar, xer;            // sinc arguments: Tx azimuth / elevation, Rx (un-offset) azimuth / elevation
-    float xao, xeo;                      // Rx arguments at the finite-difference offset o_fd
-    float la, lb;                        // r_r,c - r_r,ref = o_c la + o_c^2 lb  (series in o_c / r)
-    double uat, uet, uar, uer, uao, ueo; // the same six as direction cosines (tabulated patterns: grid coordinates in fp64)
+    double la, lb;                       // r_r,c - r_r,ref = o_c la + o_c^2 lb  (series in o_c / r)
+    double uat, uet, uar, uer, uao, ueo; // direction cosines: Tx azimuth / elevation, Rx (un-offset), Rx at the offset o_fd
 };
 
-template <int C>
-__device__ __forceinline__ KeyEval<C> key_eval(const DevParams &prm, const PulseConst &pc, const double pos[3],
-                                               const double vel[3], double o_fd)
+__device__ __forceinline__ KeyEval key_eval(const PulseConst &pc, const double pos[3], const double vel[3], double o_fd)
 {
-    KeyEval<C> o;
+    KeyEval o;
     const LegParts lt = leg_parts(pos, pc.tx_pos, pc.tx_a, pc.tx_e);
     const LegParts lr = leg_parts(pos, pc.rx_ref, pc.rx_a, pc.rx_e);
     o.R = lt.r + lr.r;
     const double at = fma(lt.dx, vel[0] - pc.tx_vel[0], fma(lt.dy, vel[1] - pc.tx_vel[1], lt.dz * (vel[2] - pc.tx_vel[2])));
     const double ar = fma(lr.dx, vel[0] - pc.rx_vel[0], fma(lr.dy, vel[1] - pc.rx_vel[1], lr.dz * (vel[2] - pc.rx_vel[2])));
     o.Rd = fma(at, lt.inv, ar * lr.inv);
-    o.xat = (float)(prm.ap_tx_a * (lt.da * lt.inv)); o.xet = (float)(prm.ap_tx_e * (lt.de * lt.inv));
-    o.xar = (float)(prm.ap_rx_a * (lr.da * lr.inv)); o.xer = (float)(prm.ap_rx_e * (lr.de * lr.inv));
     o.uat = lt.da * lt.inv; o.uet = lt.de * lt.inv; o.uar = lr.da * lr.inv; o.uer = lr.de * lr.inv;
     const double dv = fma(lr.dx, pc.rx_vhat[0], fma(lr.dy, pc.rx_vhat[1], lr.dz * pc.rx_vhat[2]));
     {
         double r_c, inv_c, da_c, de_c;
         channel_leg_series(lr, dv, o_fd, pc.rx_va, pc.rx_ve, r_c, inv_c, da_c, de_c);
-        o.xao = (float)(prm.ap_rx_a * (da_c * inv_c)); o.xeo = (float)(prm.ap_rx_e * (de_c * inv_c));
         o.uao = da_c * inv_c; o.ueo = de_c * inv_c;
     }
     // r_c - r = r (dl/2 - dl^2/8 + ...), dl = (o^2 - 2 o d.v^)/r^2  (geometry_common.cuh)
     //         = -o (d.v^)/r + o^2 (1 - (d.v^/r)^2)/(2 r) + O(o^3/r^2)
     const double cv = dv * lr.inv;
-    o.la = (float)(-cv);
-    o.lb = (float)(0.5 * lr.inv * fma(-cv, cv, 1.0));
+    o.la = -cv;
+    o.lb = 0.5 * lr.inv * fma(-cv, cv, 1.0);
     return o;
 }
 
 constexpr int kStrayCap = 96;             // stray echoes of one pulse held in shared memory (more: the tile is sorted again)
 constexpr int kScrRow = 9;                // float2 per thread row of the transposition scratch (8 moments + 1 pad)
 constexpr int kScrTeam = 8 * kScrRow;     // float2 per 8-thread team
-__host__ __device__ constexpr int hist_words(int C, int span) { return (2 * C * (span + 1) + 1) & ~1; }
+__host__ __device__ constexpr int hist_words(int C, int span) { return (C * (span + 1) + 3) & ~3; }
 
 // Packed f32x2 arithmetic on 64-bit registers (FFMA2 / FADD2): the operands stay register pairs from the
 // shared-memory load to the transposition store, no pack / unpack moves in the moment loop.
@@ -103,6 +121,10 @@ __device__ __forceinline__ f32x2 pk(float x, float y)
     f32x2 d;
     asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(x), "f"(y));
     return d;
+}
+__device__ __forceinline__ void unpk(f32x2 v, float &x, float &y)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(v));
 }
 __device__ __forceinline__ f32x2 ffma2(f32x2 a, f32x2 b, f32x2 c)
 {
@@ -120,37 +142,60 @@ __device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b)
 __device__ __forceinline__ float pattern_x(float xa, float xe) { return sinc_pi_fast(xa) * sinc_pi_fast(xe); }
 
 // Complex gain of antenna k at direction cosines (ua, ue): the table if there is one, else the analytic aperture.
+template <bool kLut>
 __device__ __forceinline__ float2 gain_at(const DevParams &prm, int k, double ua, double ue)
 {
-    if (prm.lut[k].tab) return lut_gain(prm.lut[k], ua, ue);
+    if (kLut && prm.lut[k].tab) return lut_gain(prm.lut[k], ua, ue);
     const double apa = k ? prm.ap_rx_a : prm.ap_tx_a, ape = k ? prm.ap_rx_e : prm.ap_tx_e;
     return make_float2(pattern_x((float)(apa * ua), (float)(ape * ue)), 0.f);
 }
+
+// Coefficients (c1, c2, c3) of the cubic through (0, v0), (1/3, va), (2/3, vb), (1, v1); c0 = v0.
+__device__ __forceinline__ void cubic_through(float v0, float va, float vb, float v1, float &c1, float &c2, float &c3)
+{
+    c1 = 0.5f * (-11.f * v0 + 18.f * va - 9.f * vb + 2.f * v1);
+    c2 = 4.5f * (2.f * v0 - 5.f * va + 4.f * vb - v1);
+    c3 = 4.5f * (-v0 + 3.f * va - 3.f * vb + v1);
+}
+
+// Slice word of a facet-echo: rho of the reference path at pulse index n ahead of the running state (Newton's forward
+// formula; sort time only).
+__device__ __forceinline__ unsigned long long rho_ahead(unsigned long long f, long long d1, long long d2, int d3, int n)
+{
+    const long long n1 = n, n2 = (long long)n * (n - 1) / 2, n3 = (long long)n * (n - 1) * (n - 2) / 6;
+    return f + (unsigned long long)(n1 * d1 + n2 * d2 + n3 * (long long)d3);
+}
+
+constexpr int kThreads = 256;
 
 template <int FPT, int C, bool kTilt, bool kSpeckleT, bool kLut>
 __global__ void __launch_bounds__(kThreads, 2)
 moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_first)
 {
+    constexpr int NT = kThreads;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ PulseConst pc2[2];
     __shared__ KeyPulse s_kp[kMaxKeyPulses];
     __shared__ double s_rc[2][kMaxKeyChannels];          // path length of the tile centre at the two keyframes
-    __shared__ unsigned long long s_samples;
+    __shared__ double s_la_tile, s_lb_tile;              // a, b of the receive-channel series at the tile centre, first keyframe
     __shared__ int s_kept;
     __shared__ int s_rng[kMaxKeyChannels][2];
     __shared__ float4 s_stray[2][kStrayCap];                     // echoes that have left their sorted slice: (w, y, row index)
     __shared__ int s_nstray[3];
     __shared__ int s_blo[kMaxKeyChannels], s_bhi[kMaxKeyChannels];   // slices this tile touches during the interval
+    __shared__ int s_dlamax;                                     // max |a - a_tile| + |a(t1) - a(t0)| over the tile, as float bits
 
     const int span = a.span_cap, hstride = span + 1;
-    const int cap = prm.tile_cap;
-    // [2][C][cap] float2 weight | [2][C][cap] float y | [2][C][cap] u16 index list | [2][C][span + 1] int histogram |
-    // [kThreads / 8][kScrTeam] float2 transposition scratch of stage C (8-byte aligned: hist is padded)
+    const int cap = prm.k2k_cap;
+    const int capT = C * cap + 2;                        // slots of one payload buffer: C x cap, + the store target of echoes without a slot
+    // [2][capT] float2 weight | [2][capT] float y | [C][cap] u32 slot of every facet-echo | [C][span + 1] int histogram |
+    // [kThreads / 8][kScrTeam] float2 transposition scratch of stage C
     float2 *payload = reinterpret_cast<float2 *>(smem_raw);
-    float *payload_y = reinterpret_cast<float *>(smem_raw + (size_t)2 * C * cap * 8);
-    unsigned short *idx = reinterpret_cast<unsigned short *>(smem_raw + (size_t)2 * C * cap * 12);
-    int *hist = reinterpret_cast<int *>(smem_raw + (size_t)2 * C * cap * 14);
-    float2 *scratch = reinterpret_cast<float2 *>(smem_raw + (size_t)2 * C * cap * 14 + (size_t)hist_words(C, span) * 4);
+    float *payload_y = reinterpret_cast<float *>(smem_raw + (size_t)2 * capT * 8);
+    uint32_t *slots = reinterpret_cast<uint32_t *>(smem_raw + (size_t)2 * capT * 12);
+    int *hist = reinterpret_cast<int *>(smem_raw + (size_t)2 * capT * 12 + (size_t)C * cap * 4);
+    float2 *scratch = reinterpret_cast<float2 *>(smem_raw + (size_t)2 * capT * 12 + (size_t)C * cap * 4 + (size_t)hist_words(C, span) * 4);
+    const uint32_t no_slot = (0x7ffffu << 13) | (uint32_t)(C * cap);      // slice 0x7ffff (never matches), store target = the spare slot
 
     const int tile = blockIdx.x, j = j_first + blockIdx.y;
     const int tid = threadIdx.x, lane = tid & 31;
@@ -164,45 +209,69 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         const double *s0 = reinterpret_cast<const double *>(a.pulses + k0);
         const double *s1 = reinterpret_cast<const double *>(a.pulses + k1);
         double *d0 = reinterpret_cast<double *>(&pc2[0]), *d1 = reinterpret_cast<double *>(&pc2[1]);
-        for (int k = tid; k < (int)(sizeof(PulseConst) / sizeof(double)); k += kThreads) { d0[k] = s0[k]; d1[k] = s1[k]; }
+        for (int k = tid; k < (int)(sizeof(PulseConst) / sizeof(double)); k += NT) { d0[k] = s0[k]; d1[k] = s1[k]; }
     }
-    if (tid == 0) { s_samples = 0ull; s_kept = 0; s_nstray[0] = s_nstray[1] = s_nstray[2] = 0; }
+    if (tid == 0) { s_kept = 0; s_nstray[0] = s_nstray[1] = s_nstray[2] = 0; s_dlamax = 0; }
     if (tid < kMaxKeyChannels) { s_blo[tid] = 0x7fffffff; s_bhi[tid] = (int)0x80000000; }
-    for (int k = tid; k < C * hstride; k += kThreads) hist[k] = 0;
+    for (int k = tid; k < C * hstride; k += NT) hist[k] = 0;
     __syncthreads();
 
-    const int ts = prm.tile, lts = 31 - __clz(ts);
-    const int ti0 = (tile % prm.tiles_x) * ts, tj0 = (tile / prm.tiles_x) * ts;
+    // SHEARED TILES.  A tile is TH lines of TW facets; line b is displaced by rint(shear b) facets along the line
+    // direction so that the lines' facets of equal index sit on one iso-range line (sim_create takes shear from the
+    // path-length gradient at the scene centre): the tile spans TW |gradient along the line| range slices instead
+    // of TW |g_a| + TH |g_b| -- three times fewer, fuller slices on the ATI geometry (8 instead of 27 per channel), so
+    // three times less per-slice work in stage C and as many fewer RED.  axis 0: lines are grid rows (j), displaced in
+    // i; axis 1: lines are grid columns (i), displaced in j.
+    const int TW = prm.k2k_w, TH = prm.k2k_h, ltw = 31 - __clz(TW);
+    const int ta0 = (tile % prm.k2k_tiles_a) * TW + prm.k2k_a0, tb0 = (tile / prm.k2k_tiles_a) * TH;
+    auto facet_of = [&](int la, int lb, int &i, int &jj) {
+        const int a_ = ta0 + la + __double2int_rn(prm.k2k_shear * (double)lb), b_ = tb0 + lb;
+        i = prm.k2k_axis ? b_ : a_; jj = prm.k2k_axis ? a_ : b_;
+    };
     if (tid < 2 * C) {
-        // tile centre (rest, flat) at the two keyframes: positions the slice window of every pulse between
+        // tile centre (rest height, advected by the current at the centre facet) at the two keyframes: positions the
+        // slice window of every pulse between; and the receive-channel series there (a, b at the first keyframe)
         const int e = tid / C, c = tid - e * C;
         const PulseConst &pc = pc2[e];
-        const double ic = ti0 + 0.5 * (min(ts, prm.nx - ti0) - 1), jc = tj0 + 0.5 * (min(ts, prm.ny - tj0) - 1);
-        const double x = prm.cx + (ic - 0.5 * (prm.nx - 1)) * prm.spacing;
-        const double y = prm.cy + (jc - 0.5 * (prm.ny - 1)) * prm.spacing;
+        int ici, jci;
+        facet_of(TW / 2, TH / 2, ici, jci);
+        ici = min(max(ici, 0), prm.nx - 1); jci = min(max(jci, 0), prm.ny - 1);      // (a tile at the grid's edge: nearest facet)
+        double cux = prm.cur_ux, cuy = prm.cur_uy;
+        if (a.current) {
+            const float2 cv = __ldg(a.current + (size_t)jci * prm.nx + ici);
+            cux = cv.x; cuy = cv.y;
+        }
+        const double x = prm.cx + ((double)ici - 0.5 * (prm.nx - 1)) * prm.spacing + cux * pc.t;
+        const double y = prm.cy + ((double)jci - 0.5 * (prm.ny - 1)) * prm.spacing + cuy * pc.t;
         const double ax = x - pc.tx_pos[0], ay = y - pc.tx_pos[1], az = prm.cz - pc.tx_pos[2];
         const double bx = x - pc.rx_pos[c][0], by = y - pc.rx_pos[c][1], bz = prm.cz - pc.rx_pos[c][2];
         s_rc[e][c] = sqrt(ax * ax + ay * ay + az * az) + sqrt(bx * bx + by * by + bz * bz);
+        if (tid == 0) {
+            const double dx = x - pc.rx_ref[0], dy = y - pc.rx_ref[1], dz = prm.cz - pc.rx_ref[2];
+            const double inv = rsqrt(dx * dx + dy * dy + dz * dz);
+            const double cv = (dx * pc.rx_vhat[0] + dy * pc.rx_vhat[1] + dz * pc.rx_vhat[2]) * inv;
+            s_la_tile = -cv; s_lb_tile = 0.5 * inv * (1.0 - cv * cv);
+        }
     }
     __syncthreads();
-    for (int ip = tid; ip < hi - lo; ip += kThreads) {
+    const double Rbase = pc2[0].r0;                              // c0 t0 of the first keyframe
+    const double two48 = 281474976710656.0;
+    for (int ip = tid; ip < hi - lo; ip += NT) {
         const int p = lo + ip;
         const double t0 = pc2[0].t, t1 = pc2[1].t, t = a.pulses[p].t;
         const double h = t1 - t0;
         const double s = (h != 0.0) ? (t - t0) / h : 0.0;
-        const double s2 = s * s, s3 = s2 * s;
+        const double r0 = a.pulses[p].r0;
         KeyPulse kp;
-        kp.sd = s;
-        kp.u0 = (float)(s3 - 2.0 * s2 + s);
-        kp.u1 = (float)(s3 - s2);
-        kp.r0 = a.pulses[p].r0;
-        kp.s = (float)s; kp.pad0 = 0.f;
+        kp.w = __double2ll_rn((r0 - Rbase) * prm.fs_over_c0 * two48);
+        kp.phi = turns_to_u32_fast((r0 - Rbase) * prm.inv_lambda);
+        kp.s = (float)s;
 #pragma unroll
         for (int c = 0; c < kMaxKeyChannels; ++c) {
             int base = 0;
             if (c < C) {
                 const double rc = fma(s, s_rc[1][c] - s_rc[0][c], s_rc[0][c]);
-                double bc = ceil((rc - kp.r0) * prm.fs_over_c0 - prm.half_len) - 0.5 * span;
+                double bc = ceil((rc - r0) * prm.fs_over_c0 - prm.half_len) - 0.5 * span;
                 bc = fmin(fmax(bc, -1.0e9), 1.0e9);
                 base = (int)bc;
             }
@@ -219,37 +288,42 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
 #pragma unroll
     for (int c = 0; c < C; ++c) o_fd = fmax(o_fd, fabs(pc2[0].ch_off[c]));
     const float inv_ofd = (o_fd > 0.0) ? (float)(1.0 / o_fd) : 0.f;
+    const int n_int = max(k1 - k0, 1), i0 = lo - k0;                // pulses of the interval; index of this CTA's first pulse
+    const double la_tile = s_la_tile;
 
-    // Hermite cubic of the path length as chord + bend:  R(s) = R0 + s D + u0(s) ra + u1(s) rb,  D = R1 - R0,
-    // ra = h R0' - D, rb = h R1' - D.  The bend is millimetres (h^2 R''/8), so ra, rb are fp32.
-    double R0[FPT], RD[FPT];
-    float ra[FPT], rb[FPT];
-    float la0[FPT], dla[FPT];                            // r_r,c - r_r,ref = o_c (la0 + s dla) + o_c^2 lb
-    float lb_sum = 0.f;                                  // lb varies by 1e-4 relative over a tile: one value per thread
-    int lb_n = 0;
-    float pq0[FPT], pqa[FPT], pqb[FPT], bq[FPT];         // P(s) = pq0 + s (pqa + s pqb); bq = G_t dG_r/do
-    constexpr int FL = kLut ? FPT : 1;                   // tabulated patterns: P and bq are complex, these are the imaginary parts
-    float qi0[FL], qia[FL], qib[FL], bqi[FL];
-    float am0[FPT], ama[FPT], amb[FPT];                  // |a_f|(s), quadratic when tilt-modulated
+    unsigned long long rho[FPT];                                     // path of the facet at the current pulse (2^-48 slices, < 2^16 slices)
+    long long rd1[FPT], rd2[FPT];                                    // its running forward differences
+    int rd3[FPT];
+    float dla0[FPT], dla[FPT];                                       // a(t0) - a_tile, a(t1) - a(t0)  (set-up: as computed; then scaled, see dG below)
+    float pq0[FPT], pq1[FPT], pq2[FPT], pq3[FPT], bq[FPT];           // P(s) = pq0 + s (pq1 + s (pq2 + s pq3)); bq = G_t dG_r/do
+    constexpr int FL = kLut ? FPT : 1;                               // tabulated patterns: P and bq are complex, the imaginary parts
+    float qi0[FL], qi1[FL], qi2[FL], qi3[FL], bqi[FL];
+    float am0[FPT];
+    constexpr int FT = kTilt ? FPT : 1;
+    float am1[FT], am2[FT];                                          // |a_f|(s) = am0 + s (am1 + s am2) when tilt-modulated
     uint32_t xarg[FPT];
-    bool valid[FPT];
+    int fidx[kSpeckleT ? FPT : 1];                                   // facet index (time-dependent speckle: one load per pulse)
+    unsigned validmask = 0;
+    float my_dla = 0.f;
 #pragma unroll
     for (int q = 0; q < FPT; ++q) {
-        const int k = q * kThreads + tid;
-        const int li = k & (ts - 1), lj = k >> lts;
-        const int i = ti0 + li, jj = tj0 + lj;
-        valid[q] = (k < ts * ts && i < prm.nx && jj < prm.ny);
-        R0[q] = RD[q] = 0.0; ra[q] = rb[q] = 0.f;
-        pq0[q] = pqa[q] = pqb[q] = bq[q] = 0.f; am0[q] = ama[q] = amb[q] = 0.f; xarg[q] = 0u;
-        la0[q] = dla[q] = 0.f;
-        if (kLut) qi0[q] = qia[q] = qib[q] = bqi[q] = 0.f;
-        if (!valid[q]) continue;
+        const int k = q * NT + tid;
+        int i, jj;
+        facet_of(k & (TW - 1), k >> ltw, i, jj);
+        const bool valid = (k < TW * TH && i >= 0 && i < prm.nx && jj >= 0 && jj < prm.ny);
+        if (kSpeckleT) fidx[kSpeckleT ? q : 0] = valid ? jj * prm.nx + i : 0;
+        rho[q] = (unsigned long long)kRhoBias << 48; rd1[q] = rd2[q] = 0; rd3[q] = 0;
+        dla0[q] = dla[q] = 0.f;
+        pq0[q] = pq1[q] = pq2[q] = pq3[q] = bq[q] = 0.f; am0[q] = 0.f; xarg[q] = 0u;
+        if (kLut) qi0[q] = qi1[q] = qi2[q] = qi3[q] = bqi[q] = 0.f;
+        if (kTilt) am1[q] = am2[q] = 0.f;
+        if (!valid) continue;
         const size_t f = (size_t)jj * prm.nx + i;
         const double xb = prm.cx + ((double)i - 0.5 * (prm.nx - 1)) * prm.spacing;
         const double yb = prm.cy + ((double)jj - 0.5 * (prm.ny - 1)) * prm.spacing;
         double cux = prm.cur_ux, cuy = prm.cur_uy;
         if (a.current) { const float2 cv = __ldg(a.current + f); cux = cv.x; cuy = cv.y; }
-        KeyEval<C> ev[2];
+        KeyEval ev[2];
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
             const PulseConst &pc = pc2[e];
@@ -260,36 +334,53 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                 const double2 dd = a.surf.dxy[r], dt = a.surf.dxy_t[r];
                 pos[0] += dd.x; pos[1] += dd.y; vel[0] += dt.x; vel[1] += dt.y;
             }
-            ev[e] = key_eval<C>(prm, pc, pos, vel, o_fd);
+            ev[e] = key_eval(pc, pos, vel, o_fd);
         }
         {
+            // Hermite cubic of the path in the pulse index i (uniform pulse times):  R(i) = R0 + a1 i + a2 i^2 + a3 i^3,
+            // ra = h R0' - D, rb = h R1' - D, D = R1 - R0;  in range slices, and its forward differences at i0
             const double hh = pc2[1].t - pc2[0].t, D = ev[1].R - ev[0].R;
-            R0[q] = ev[0].R; RD[q] = D;
-            ra[q] = (float)fma(hh, ev[0].Rd, -D); rb[q] = (float)fma(hh, ev[1].Rd, -D);
+            const double ra = fma(hh, ev[0].Rd, -D), rb = fma(hh, ev[1].Rd, -D);
+            const double inv_n = 1.0 / (double)n_int, fsc = prm.fs_over_c0;
+            const double c0q = fma(ev[0].R - Rbase, fsc, (double)kRhoBias - prm.half_len);
+            const double c1 = (D + ra) * fsc * inv_n, c2 = (-2.0 * ra - rb) * fsc * inv_n * inv_n;
+            const double c3 = (ra + rb) * fsc * inv_n * inv_n * inv_n;
+            const double x0 = (double)i0;
+            const double f0 = fma(x0, fma(x0, fma(x0, c3, c2), c1), c0q);
+            const double g1 = c1 + c2 * (2.0 * x0 + 1.0) + c3 * (3.0 * x0 * x0 + 3.0 * x0 + 1.0);
+            const double g2 = 2.0 * c2 + c3 * (6.0 * x0 + 6.0), g3 = 6.0 * c3;
+            if (f0 > 64.0 && f0 < 65536.0 - 64.0 && fabs(g1) < 0.5) {   // inside the fixed-point range (else: no echo; the host guard keeps scenes inside)
+                rho[q] = __double2ull_rn(f0 * two48); rd1[q] = __double2ll_rn(g1 * two48);
+                rd2[q] = __double2ll_rn(g2 * two48); rd3[q] = (int)__double2ll_rn(g3 * two48);
+                validmask |= 1u << q;
+            }
         }
-        la0[q] = ev[0].la; dla[q] = ev[1].la - ev[0].la;
-        lb_sum += 0.5f * (ev[0].lb + ev[1].lb); ++lb_n;
-        // gains at s = 0, 1/2, 1 (sinc arguments at the midpoint = mean of the end values)
-        if (kLut) {
-            const float2 P0 = cmulf(gain_at(prm, 0, ev[0].uat, ev[0].uet), gain_at(prm, 1, ev[0].uar, ev[0].uer));
-            const float2 P1 = cmulf(gain_at(prm, 0, ev[1].uat, ev[1].uet), gain_at(prm, 1, ev[1].uar, ev[1].uer));
-            const float2 gtm = gain_at(prm, 0, 0.5 * (ev[0].uat + ev[1].uat), 0.5 * (ev[0].uet + ev[1].uet));
-            const float2 grm = gain_at(prm, 1, 0.5 * (ev[0].uar + ev[1].uar), 0.5 * (ev[0].uer + ev[1].uer));
-            const float2 gom = gain_at(prm, 1, 0.5 * (ev[0].uao + ev[1].uao), 0.5 * (ev[0].ueo + ev[1].ueo));
-            const float2 Pm = cmulf(gtm, grm);
-            const float2 dq = cmulf(gtm, make_float2((gom.x - grm.x) * inv_ofd, (gom.y - grm.y) * inv_ofd));
-            pq0[q] = P0.x; pqa[q] = -3.f * P0.x + 4.f * Pm.x - P1.x; pqb[q] = 2.f * P0.x - 4.f * Pm.x + 2.f * P1.x;
-            qi0[q] = P0.y; qia[q] = -3.f * P0.y + 4.f * Pm.y - P1.y; qib[q] = 2.f * P0.y - 4.f * Pm.y + 2.f * P1.y;
-            bq[q] = dq.x; bqi[q] = dq.y;
-        } else {
-        const float gt0 = pattern_x(ev[0].xat, ev[0].xet), gr0 = pattern_x(ev[0].xar, ev[0].xer);
-        const float gt1 = pattern_x(ev[1].xat, ev[1].xet), gr1 = pattern_x(ev[1].xar, ev[1].xer);
-        const float gtm = pattern_x(0.5f * (ev[0].xat + ev[1].xat), 0.5f * (ev[0].xet + ev[1].xet));
-        const float grm = pattern_x(0.5f * (ev[0].xar + ev[1].xar), 0.5f * (ev[0].xer + ev[1].xer));
-        const float gom = pattern_x(0.5f * (ev[0].xao + ev[1].xao), 0.5f * (ev[0].xeo + ev[1].xeo));
-        const float P0 = gt0 * gr0, Pm = gtm * grm, P1 = gt1 * gr1;
-        pq0[q] = P0; pqa[q] = -3.f * P0 + 4.f * Pm - P1; pqb[q] = 2.f * P0 - 4.f * Pm + 2.f * P1;
-        bq[q] = gtm * (gom - grm) * inv_ofd;
+        dla0[q] = (float)(ev[0].la - la_tile);
+        dla[q] = (float)(ev[1].la - ev[0].la);
+        my_dla = fmaxf(my_dla, fabsf(dla0[q]) + fabsf(dla[q]));
+        // gains at s = 0, 1/3, 2/3, 1 (direction cosines between the keyframes interpolated linearly)
+        {
+            float2 Pn[4];
+#pragma unroll
+            for (int n = 0; n < 4; ++n) {
+                const double sn = n * (1.0 / 3.0);
+                const float2 gt = gain_at<kLut>(prm, 0, fma(sn, ev[1].uat - ev[0].uat, ev[0].uat), fma(sn, ev[1].uet - ev[0].uet, ev[0].uet));
+                const float2 gr = gain_at<kLut>(prm, 1, fma(sn, ev[1].uar - ev[0].uar, ev[0].uar), fma(sn, ev[1].uer - ev[0].uer, ev[0].uer));
+                Pn[n] = kLut ? cmulf(gt, gr) : make_float2(gt.x * gr.x, 0.f);
+            }
+            const float2 gtm = gain_at<kLut>(prm, 0, 0.5 * (ev[0].uat + ev[1].uat), 0.5 * (ev[0].uet + ev[1].uet));
+            const float2 grm = gain_at<kLut>(prm, 1, 0.5 * (ev[0].uar + ev[1].uar), 0.5 * (ev[0].uer + ev[1].uer));
+            const float2 gom = gain_at<kLut>(prm, 1, 0.5 * (ev[0].uao + ev[1].uao), 0.5 * (ev[0].ueo + ev[1].ueo));
+            pq0[q] = Pn[0].x;
+            cubic_through(Pn[0].x, Pn[1].x, Pn[2].x, Pn[3].x, pq1[q], pq2[q], pq3[q]);
+            if (kLut) {
+                qi0[q] = Pn[0].y;
+                cubic_through(Pn[0].y, Pn[1].y, Pn[2].y, Pn[3].y, qi1[q], qi2[q], qi3[q]);
+                const float2 dq = cmulf(gtm, make_float2((gom.x - grm.x) * inv_ofd, (gom.y - grm.y) * inv_ofd));
+                bq[q] = dq.x; bqi[q] = dq.y;
+            } else {
+                bq[q] = gtm.x * (gom.x - grm.x) * inv_ofd;
+            }
         }
         // amplitude (O8): sqrt(sigma0 tilt d^2) |xi|
         const float sig = a.sigma0 ? __ldg(a.sigma0 + f) : (float)prm.sigma0_uniform;
@@ -298,31 +389,62 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         if (!kSpeckleT) { const uint2 xp = __ldg(a.xi_polar + f); xmag = __uint_as_float(xp.x); xarg[q] = xp.y; }
         if (kTilt) {
             const float2 sl0 = a.surf.slope[row0 + f], sl1 = a.surf.slope[row1 + f];
-            const float smx = 0.5f * (sl0.x + sl1.x), smy = 0.5f * (sl0.y + sl1.y);   // slopes are linear between keyframes
+            float2 slm = make_float2(0.5f * (sl0.x + sl1.x), 0.5f * (sl0.y + sl1.y));   // slopes are linear between keyframes ...
+            if (a.surf.slope_t) {                                // ... or cubic Hermite: value at mid-interval = mean + h (s0' - s1') / 8
+                const float2 r0 = a.surf.slope_t[row0 + f], r1 = a.surf.slope_t[row1 + f];
+                const float h8 = 0.125f * (float)(pc2[1].t - pc2[0].t);
+                slm.x = fmaf(h8, r0.x - r1.x, slm.x); slm.y = fmaf(h8, r0.y - r1.y, slm.y);
+            }
             const float lx = (float)prm.look_x, ly = (float)prm.look_y;
             const float A0 = sqrtf(sig * fmaxf(1.f + 2.f * (sl0.x * lx + sl0.y * ly), 0.f) * area) * xmag;
-            const float Am = sqrtf(sig * fmaxf(1.f + 2.f * (smx * lx + smy * ly), 0.f) * area) * xmag;
+            const float Am = sqrtf(sig * fmaxf(1.f + 2.f * (slm.x * lx + slm.y * ly), 0.f) * area) * xmag;
             const float A1 = sqrtf(sig * fmaxf(1.f + 2.f * (sl1.x * lx + sl1.y * ly), 0.f) * area) * xmag;
-            am0[q] = A0; ama[q] = -3.f * A0 + 4.f * Am - A1; amb[q] = 2.f * A0 - 4.f * Am + 2.f * A1;
+            am0[q] = A0; am1[q] = -3.f * A0 + 4.f * Am - A1; am2[q] = 2.f * A0 - 4.f * Am + 2.f * A1;
         } else {
             am0[q] = sqrtf(sig * area) * xmag;
         }
     }
-    __syncthreads();                                     // s_kp complete
+    if (my_dla > 0.f) atomicMax(&s_dlamax, __float_as_int(my_dla));
+    __syncthreads();                                     // s_kp, s_dlamax complete
 
-    // phase of a facet-echo in 2^-32 turns: -dR/lambda + kappa eps^2 (+ speckle argument, + 1/2 if the gain is negative)
-    const double il32 = prm.inv_lambda * 4294967296.0;
-    const float kappa32 = (float)(prm.kappa * 4294967296.0);
+    // ---- per-channel constants ----
     const int L = a.replica;
     const unsigned win_hi = (unsigned)(prm.n_samples + L - 1);
     float och[C];
+    float och_max = 0.f;
 #pragma unroll
-    for (int c = 0; c < C; ++c) och[c] = (float)pc2[0].ch_off[c];
-    const float lbt = lb_n ? lb_sum / (float)lb_n : 0.f;
-    unsigned long long my_samples = 0;
+    for (int c = 0; c < C; ++c) {
+        och[c] = (float)pc2[0].ch_off[c];
+        och_max = fmaxf(och_max, fabsf(och[c]));
+    }
+    // The receive-channel path difference o_c a + o_c^2 b with a = a_tile + (a_f(t0) - a_tile) + s (a_f(t1) - a_f(t0)):
+    // the tile-centre part is one exact word per channel for the phase (2^-32 turns) and one for the slice (2^-32
+    // slices); the facet's part, -o_c (...) / lambda in units of `mult` 2^-32 turns, is kept under 2^21 so that one FFMA
+    // against 1.5 x 2^23 rounds it to an integer in the mantissa (likewise o_c (...) fs/c0 in 2^-32 slices: smaller).
+    const double il32 = prm.inv_lambda * 4294967296.0;
+    uint32_t mult = 1;
+    {
+        const float lin_max = och_max * __int_as_float(s_dlamax) * (float)il32;
+        while ((float)mult * 2097152.f < lin_max && mult < (1u << 20)) mult <<= 1;
+    }
+    uint32_t PSI[C], DNU[C];
+#pragma unroll
+    for (int c = 0; c < C; ++c) {
+        const double o = pc2[0].ch_off[c];
+        const double dl_tile = o * fma(o, s_lb_tile, la_tile);           // r_r,c - r_r,ref at the tile centre, first keyframe [m]
+        PSI[c] = turns_to_u32_fast(-dl_tile * prm.inv_lambda) + prm.phase_bias32 - 0x4B400000u * mult;
+        DNU[c] = (uint32_t)__double2int_rn(dl_tile * prm.fs_over_c0 * 4294967296.0) - 0x4B400000u;
+    }
+    // facet part: g(s) = dG0 + s dGs in units of mult 2^-32 turns per metre of offset; in 2^-32 slices: g(s) x slice_per_g
+    const float to_g = -(float)il32 / (float)mult;
+    const float slice_per_g = -(float)mult * (float)(prm.fs_over_c0 / prm.inv_lambda);
+#pragma unroll
+    for (int q = 0; q < FPT; ++q) { dla0[q] *= to_g; dla[q] *= to_g; }    // now dG0, dGs
+
     int my_kept = 0;
     const int sub = tid & 7, team = tid >> 3, warp = tid >> 5;
     float2 *scr = scratch + team * kScrTeam;
+    const int capS = C * cap;                                            // slots of all channels (the spare one follows)
 
     // ---- The facet-echoes of the tile are ordered by range slice ONCE (counting sort at the interval's middle pulse:
     //      histogram by integer ATOMS, scan, slot = first position of the slice + rank), not at every pulse: over the
@@ -332,44 +454,49 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     //      to a short shared-memory list that the CTA works off with global atomics.  A pulse with more strays than the
     //      list holds sorts the tile again at that pulse and is redone.  Stage C reads each slice's slots
     //      contiguously: no per-pulse histogram, scan or index list; one barrier per pulse. ----
-    uint32_t *slots = reinterpret_cast<uint32_t *>(idx);           // [C][cap]: slice << 12 | slot, or ~0u (never in the list)
     int *hs = hist;                                                  // [C][span + 1] first slot of each slice
-    int bref[C];                                                     // first slice of the tile's window at the sorting pulse
-    // Sorted at the middle pulse of the interval the strays at its ends are half as many as when sorted at the first;
-    // a tile far from the scene centre drifts too fast for that (expected strays at the first pulse = half the
-    // interval's pulses x the drift of the tile centre against the sampling window, in slices per pulse, x its echoes):
-    // it is sorted at the first pulse, and again whenever the next pulse's strays (this pulse's plus their growth)
-    // would not fit the list.
+    int K2[C];                                                       // slice index relative to the tile window = (word >> 32) - K2[c]
+#pragma unroll
+    for (int c = 0; c < C; ++c) K2[c] = 0;
     int ip_sort = (hi - lo) / 2;
     {
         const double drift = fabs((s_rc[1][0] - s_rc[0][0]) - (a.pulses[k1].r0 - a.pulses[k0].r0)) * prm.fs_over_c0 /
                              (double)max(k1 - k0, 1);
-        if (drift * (double)(ts * ts * C) * 0.5 * (double)(hi - lo) > 0.9 * kStrayCap) ip_sort = 0;
+        if (drift * (double)(TW * TH * C) * 0.5 * (double)(hi - lo) > 0.9 * kStrayCap) ip_sort = 0;
     }
     bool need_sort = true;
     int ns_prev = 0;                                                 // strays of the previous pulse (0 after a sort)
+    int sorted_at = -1;
+    int ns_cur = 0;                                                  // which of the three stray counters this pulse uses
+
+    // slice word of facet q, channel c at pulse state (X = reference path, s): [slice + kRhoBias . fraction]
+    auto slice_word = [&](int q, int c, long long X, float nq) -> long long {
+        const float t3 = fmaf(och[c], nq, 12582912.f);
+        return X + (long long)(int32_t)(DNU[c] + __float_as_uint(t3));
+    };
 
     for (int ip = 0; ip < hi - lo;) {
         if (need_sort) {
             need_sort = false;
-            const KeyPulse &kp = s_kp[ip_sort];
+            sorted_at = ip_sort;
+            const KeyPulse &kps = s_kp[ip_sort];
             __syncthreads();                                         // nobody reads the old histogram / slots any more
-            for (int k = tid; k < C * hstride; k += kThreads) hs[k] = 0;
-            if (tid == 0) s_nstray[ip % 3] = 0;
+            for (int k = tid; k < C * hstride; k += NT) hs[k] = 0;
+            if (tid == 0) s_nstray[ns_cur] = 0;
             __syncthreads();
+            int bref[C];
 #pragma unroll
-            for (int c = 0; c < C; ++c) bref[c] = kp.base[c];
+            for (int c = 0; c < C; ++c) { bref[c] = kps.base[c]; K2[c] = bref[c] + kRhoBias - 1; }
             int pr[FPT][C];
 #pragma unroll
             for (int q = 0; q < FPT; ++q) {
-                const double dRref = fma(kp.sd, RD[q], R0[q]) + (double)fmaf(kp.u0, ra[q], kp.u1 * rb[q]) - kp.r0;
-                const float la = fmaf(kp.s, dla[q], la0[q]);
+                const long long X = (long long)((rho_ahead(rho[q], rd1[q], rd2[q], rd3[q], ip_sort - ip) - (unsigned long long)kps.w) >> 16);
+                const float nq = fmaf(kps.s, dla[q], dla0[q]) * slice_per_g;
 #pragma unroll
                 for (int c = 0; c < C; ++c) {
-                    const float dl = och[c] * fmaf(och[c], lbt, la);
-                    const int rel = __double2int_ru(fma(dRref + (double)dl, prm.fs_over_c0, -prm.half_len)) - bref[c];
+                    const int rel = (int)(slice_word(q, c, X, nq) >> 32) - K2[c];
                     pr[q][c] = -1;
-                    if (valid[q] && (unsigned)rel < (unsigned)span)
+                    if (((validmask >> q) & 1u) && (unsigned)rel < (unsigned)span)
                         pr[q][c] = (rel << 12) | atomicAdd(&hs[c * hstride + rel + 1], 1);
                 }
             }
@@ -404,88 +531,149 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
 #pragma unroll
                 for (int c = 0; c < C; ++c) {
                     const int v = pr[q][c];
-                    if (FPT > 1 || q * kThreads + tid < cap)         // (FPT = 1: the tile may be smaller than the CTA)
-                        slots[c * cap + q * kThreads + tid] =
-                            (v >= 0) ? (uint32_t)((v & ~4095) | (hs[c * hstride + (v >> 12)] + (v & 4095))) : 0xffffffffu;
+                    if (FPT > 1 || q * NT + tid < cap)               // (FPT = 1: the tile may be smaller than the CTA)
+                        slots[c * cap + q * NT + tid] =
+                            (v >= 0) ? (uint32_t)(((v >> 12) << 13) | (c * cap + hs[c * hstride + (v >> 12)] + (v & 4095))) : no_slot;
                 }
             // a thread reads only its own slots; the scan results are read after the barrier of stage A
         }
         const int buf = ip & 1;
         const int pl = lo + ip - p0;
-        const KeyPulse &kp = s_kp[ip];
-        float2 *pay = payload + (size_t)buf * C * cap;
-        float *pay_y = payload_y + (size_t)buf * C * cap;
+        const KeyPulse kp = s_kp[ip];
+        float2 *pay = payload + (size_t)buf * capT;
+        float *pay_y = payload_y + (size_t)buf * capT;
         const float s = kp.s;
-        int *n_stray = &s_nstray[ip % 3];
-        if (tid == 0) s_nstray[(ip + 1) % 3] = 0;            // last read two pulses ago, next written after this pulse's barrier
+        int *n_stray = &s_nstray[ns_cur];
+        const int ns_next = (ns_cur == 2) ? 0 : ns_cur + 1;
+        if (tid == 0) s_nstray[ns_next] = 0;                 // last read two pulses ago, next written after this pulse's barrier
         int kept_p = 0;
-        unsigned samples_p = 0;
 
         // ---- A: slice, sub-slice position, complex weight of every facet-echo, written to the echo's slot.
-        //      Straight-line code for all FPT x C echoes of the thread (predicated stores), so that the
-        //      independent chains interleave; only a stray echo branches.
-#pragma unroll
-        for (int q = 0; q < FPT; ++q) {
-            const float Pv = fmaf(s, fmaf(s, pqb[q], pqa[q]), pq0[q]);
-            const float Pi = kLut ? fmaf(s, fmaf(s, qib[kLut ? q : 0], qia[kLut ? q : 0]), qi0[kLut ? q : 0]) : 0.f;
-            const bool keep = valid[q] && !(kLut ? (fmaf(Pv, Pv, Pi * Pi) < prm.cull_thr * prm.cull_thr)
-                                                 : (fabsf(Pv) < prm.cull_thr));     // O7 (G6)
-            kept_p += keep ? 1 : 0;
-            float am = kTilt ? fmaf(s, fmaf(s, amb[q], ama[q]), am0[q]) : am0[q];
+        //      Branch-free straight-line code for all FPT x C echoes of the thread, so that the independent chains
+        //      (integer slice word -> MUFU -> stores) interleave.  Strays only set a bit; the rare ones are worked off
+        //      after the loop by evaluating that echo again.
+        unsigned stray_mask = 0;
+        auto facet = [&](const int q, float &Pv, float &Pi, float &am, uint32_t &ph_ref, long long &X, float &gq, bool &keep) {
+            Pv = fmaf(s, fmaf(s, fmaf(s, pq3[q], pq2[q]), pq1[q]), pq0[q]);
+            Pi = kLut ? fmaf(s, fmaf(s, fmaf(s, qi3[kLut ? q : 0], qi2[kLut ? q : 0]), qi1[kLut ? q : 0]), qi0[kLut ? q : 0]) : 0.f;
+            keep = ((validmask >> q) & 1u) && !(kLut ? (fmaf(Pv, Pv, Pi * Pi) < prm.cull_thr * prm.cull_thr)
+                                                     : (fabsf(Pv) < prm.cull_thr));     // O7 (G6)
+            am = kTilt ? fmaf(s, fmaf(s, am2[kTilt ? q : 0], am1[kTilt ? q : 0]), am0[q]) : am0[q];
             uint32_t xa = xarg[q];
-            if (kSpeckleT && valid[q]) {                  // time-dependent speckle: s_f(t_p) of this pulse (eq. (7), (10))
-                const int kk = q * kThreads + tid;
-                const uint2 xp = __ldg(a.xi_polar + (size_t)pl * a.xi_pulse_stride +
-                                       (size_t)(tj0 + (kk >> lts)) * prm.nx + (ti0 + (kk & (ts - 1))));
+            if (kSpeckleT && ((validmask >> q) & 1u)) {   // time-dependent speckle: s_f(t_p) of this pulse (eq. (7), (10))
+                const uint2 xp = __ldg(a.xi_polar + (size_t)pl * a.xi_pulse_stride + (size_t)fidx[kSpeckleT ? q : 0]);
                 am *= __uint_as_float(xp.x); xa = xp.y;
             }
-            const double R = fma(kp.sd, RD[q], R0[q]) + (double)fmaf(kp.u0, ra[q], kp.u1 * rb[q]);
-            const double dRref = R - kp.r0;
-            const float la = fmaf(s, dla[q], la0[q]);
-            const int k = q * kThreads + tid;
+            am = keep ? am : 0.f;
+            // carrier phase of the reference path: the 32 fraction bits of rho x (f0 / fs)
+            const uint32_t r_lo = (uint32_t)rho[q], r_hi = (uint32_t)(rho[q] >> 32);
+            const uint32_t T = __umulhi(r_lo, prm.ratio_hi) + __umulhi(r_hi, prm.ratio_lo) + r_hi * prm.ratio_hi;
+            ph_ref = kp.phi - T + xa;
+            X = (long long)((rho[q] - (unsigned long long)kp.w) >> 16);   // [slice + kRhoBias . 32-bit fraction], positive
+            gq = fmaf(s, dla[q], dla0[q]);                                 // channel series of this facet at this pulse
+        };
+        auto echo = [&](const int q, const int c, const float Pv, const float Pi, const float am, const uint32_t ph_ref,
+                        const long long X, const float gq, const float nq, float &wr, float &wi, float &yv, int &xh) {
+            const long long Xc = slice_word(q, c, X, nq);
+            xh = (int)(Xc >> 32);
+            const uint32_t fr = (uint32_t)(unsigned long long)Xc;
+            // b = ceil(nu) = xh + 1 - kRhoBias; eps = b - nu = 1 - fr 2^-32; y = 2 eps - 1 = 3 - 2 (1 + fr 2^-32)
+            yv = fmaf(__uint_as_float(0x3F800000u | (fr >> 9)), -2.f, 3.f);
+            const float t2 = fmaf(och[c], gq, 12582912.f);
+            const uint32_t ph = PSI[c] + ph_ref + __float_as_uint(t2) * mult;
+            float sn, cs;
+            __sincosf((float)(int32_t)ph * 1.4629180792671596e-9f, &sn, &cs);   // 2 pi / 2^32
+            const float g = fmaf(och[c], bq[q], Pv);
+            if (kLut) {                                                    // complex gain times the phasor
+                const float gi = fmaf(och[c], bqi[kLut ? q : 0], Pi);
+                wr = am * fmaf(g, cs, -gi * sn); wi = am * fmaf(g, sn, gi * cs);
+            } else {
+                const float mag = g * am;
+                wr = mag * cs; wi = mag * sn;
+            }
+        };
+#pragma unroll
+        for (int q = 0; q < FPT; ++q) {
+            float Pv, Pi, am, gq; uint32_t ph_ref; long long X; bool keep;
+            facet(q, Pv, Pi, am, ph_ref, X, gq, keep);
+            const float nq = gq * slice_per_g;
+            kept_p += keep ? 1 : 0;
+            const int k = q * NT + tid;
 #pragma unroll
             for (int c = 0; c < C; ++c) {
-                const float dl = och[c] * fmaf(och[c], lbt, la);
-                const double dR = dRref + (double)dl;
-                const double nu = fma(dR, prm.fs_over_c0, -prm.half_len);
-                const int b = __double2int_ru(nu);                                // ceil, saturating
-                const bool inwin = keep && ((unsigned)b + (unsigned)(L - 1) < win_hi);   // window meets [0, Ns)
-                const float eps = (float)((double)b - nu);                        // [0, 1)
-                const float g = fmaf(och[c], bq[q], Pv);
-                const uint32_t ph = (uint32_t)(unsigned long long)__double2ll_rn(
-                                        fma(-dR, il32, (double)(kappa32 * eps * eps))) +
-                                    xa + ((g < 0.f && !kLut) ? 0x80000000u : 0u);
-                float sn, cs;
-                __sincosf((float)(int32_t)ph * 1.4629180792671596e-9f, &sn, &cs);   // 2 pi / 2^32
-                const float mag = fabsf(g) * am;
-                float wr = mag * cs, wi = mag * sn;                        // complex weight of the facet-echo
-                if (kLut) {                                                // complex gain times the phasor
-                    const float gi = fmaf(och[c], bqi[kLut ? q : 0], Pi);
-                    wr = am * fmaf(g, cs, -gi * sn); wi = am * fmaf(g, sn, gi * cs);
-                }
-                const float yv = fmaf(2.f, eps, -1.f);
-                const uint32_t slot = (FPT > 1 || k < cap) ? slots[c * cap + k] : 0xffffffffu;
-                const int rel = b - bref[c];
-                const bool here = inwin && ((uint32_t)rel == (slot >> 12));       // in its sorted slice
-                if (slot != 0xffffffffu) {
-                    const int pos = c * cap + (int)(slot & 4095u);
-                    pay[pos] = here ? make_float2(wr, wi) : make_float2(0.f, 0.f);
-                    pay_y[pos] = here ? yv : 0.f;
-                }
-                if (inwin) samples_p += (unsigned)(min(b + L, prm.n_samples) - max(b, 0));
-                if (inwin && !here) {                                      // stray: left its sorted slice, or never had one
+                float wr, wi, yv; int xh;
+                echo(q, c, Pv, Pi, am, ph_ref, X, gq, nq, wr, wi, yv, xh);
+                const uint32_t slot = (FPT > 1 || k < cap) ? slots[c * cap + k] : no_slot;
+                const bool here = (uint32_t)(xh - K2[c]) == (slot >> 13);   // in its sorted slice
+                const uint32_t pos = slot & 8191u;
+                pay[pos] = here ? make_float2(wr, wi) : make_float2(0.f, 0.f);
+                pay_y[pos] = yv;
+                // stray: left its sorted slice, or never had one; its window meets [0, Ns)
+                const bool stray = !here && keep && ((unsigned)(xh + 1 - kRhoBias) + (unsigned)(L - 1) < win_hi);
+                stray_mask |= stray ? (1u << (q * C + c)) : 0u;
+            }
+        }
+        if (stray_mask) {
+#pragma unroll
+            for (int q = 0; q < FPT; ++q) {
+                if (((stray_mask >> (q * C)) & ((1u << C) - 1u)) == 0u) continue;
+                float Pv, Pi, am, gq; uint32_t ph_ref; long long X; bool keep;
+                facet(q, Pv, Pi, am, ph_ref, X, gq, keep);
+                const float nq = gq * slice_per_g;
+#pragma unroll
+                for (int c = 0; c < C; ++c) {
+                    if (!((stray_mask >> (q * C + c)) & 1u)) continue;
+                    float wr, wi, yv; int xh;
+                    echo(q, c, Pv, Pi, am, ph_ref, X, gq, nq, wr, wi, yv, xh);
+                    const int b = xh + 1 - kRhoBias;
                     const int t = atomicAdd(n_stray, 1);
-                    if (t < kStrayCap) s_stray[buf][t] = make_float4(wr, wi, yv, __int_as_float((c << 28) | (b + L - 1)));
+                    if (t < kStrayCap) {
+                        s_stray[buf][t] = make_float4(wr, wi, yv, __int_as_float((c << 28) | (b + L - 1)));
+                    } else if (sorted_at == ip) {                          // sorted at this very pulse and still no room:
+                        float2 *row = a.mom + ((size_t)(c * n_pl + pl) * kKt) * a.nb_pad + (b + L - 1);   // straight to the rows
+                        float t0 = 1.f, t1 = yv;
+                        atomicAdd(row, make_float2(wr, wi));
+                        atomicAdd(row + a.nb_pad, make_float2(wr * t1, wi * t1));
+                        for (int k2 = 2; k2 < kKt; ++k2) {
+                            const float t2k = 2.f * yv * t1 - t0;
+                            atomicAdd(row + (size_t)k2 * a.nb_pad, make_float2(wr * t2k, wi * t2k));
+                            t0 = t1; t1 = t2k;
+                        }
+                        atomicMin(&s_blo[c], b); atomicMax(&s_bhi[c], b + 1);
+                    }
+                }
+            }
+        }
+        if (a.dbg_slice && lo + ip == a.dbg_pulse) {          // sim_debug_echoes: this pulse's facet-echoes as the kernel sees them
+#pragma unroll
+            for (int q = 0; q < FPT; ++q) {
+                const int k = q * NT + tid;
+                int i, jj;
+                facet_of(k & (TW - 1), k >> ltw, i, jj);
+                if (!(k < TW * TH && i >= 0 && i < prm.nx && jj >= 0 && jj < prm.ny)) continue;
+                const size_t f = (size_t)jj * prm.nx + i;
+                float Pv, Pi, am, gq; uint32_t ph_ref; long long X; bool keep;
+                facet(q, Pv, Pi, am, ph_ref, X, gq, keep);
+                const float nq = gq * slice_per_g;
+                a.dbg_keep[f] = keep ? 1 : 0;
+#pragma unroll
+                for (int c = 0; c < C; ++c) {
+                    float wr, wi, yv; int xh;
+                    echo(q, c, Pv, Pi, am, ph_ref, X, gq, nq, wr, wi, yv, xh);
+                    a.dbg_slice[(size_t)c * F + f] = xh + 1 - kRhoBias;
+                    a.dbg_eps[(size_t)c * F + f] = 0.5f * (yv + 1.f);
+                    a.dbg_w[(size_t)c * F + f] = make_float2(wr, wi);
                 }
             }
         }
         __syncthreads();
-        const int ns = *n_stray;
-        if (ns > kStrayCap) {                                // too many have moved on: sort the tile at this pulse, redo it
+        const int ns_all = *n_stray;
+        if (ns_all > kStrayCap && sorted_at != ip) {         // too many have moved on: sort the tile at this pulse, redo it
             need_sort = true; ip_sort = ip;
             continue;
         }
-        my_kept += kept_p; my_samples += samples_p;
+        const int ns = min(ns_all, kStrayCap);
+        my_kept += kept_p;
 
         // ---- C: 8 threads per slice: Chebyshev moments over the slice's slots, transpose through shared memory, one
         //      RED per (slice, k).  The recurrence runs on a_k = sigma_k T_k, sigma = + + - - + + - -, which needs no
@@ -503,14 +691,14 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                 int c = 0;
 #pragma unroll
                 for (int cc = 1; cc < C; ++cc) c = (it >= pre[cc]) ? cc : c;
-                int pc0 = 0, bc = bref[0];
+                int pc0 = 0, bc = K2[0];
 #pragma unroll
-                for (int cc = 1; cc < C; ++cc) { pc0 = (c == cc) ? pre[cc] : pc0; bc = (c == cc) ? bref[cc] : bc; }
+                for (int cc = 1; cc < C; ++cc) { pc0 = (c == cc) ? pre[cc] : pc0; bc = (c == cc) ? K2[cc] : bc; }
                 const int sidx = s_rng[c][0] + (it - pc0);
                 const int *hc = hs + c * hstride;
                 int first = 0, cnt = 0;
                 if (it < total) { first = hc[sidx]; cnt = hc[sidx + 1] - first; }
-                const int b = bc + sidx;
+                const int b = bc + 1 - kRhoBias + sidx;                    // K2 = bref + kRhoBias - 1
                 if ((unsigned)(b + L - 1) >= win_hi) cnt = 0;              // a slice outside the sampling window holds zeros only
                 const float2 *payc = pay + c * cap + first;
                 const float *payc_y = pay_y + c * cap + first;
@@ -552,7 +740,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
             }
         }
         // ---- the strays of this pulse: thread t takes moment t & 7 of stray t >> 3 ----
-        for (int t = tid; t < ns * kKt; t += kThreads) {
+        for (int t = tid; t < ns * kKt; t += NT) {
             const float4 e = s_stray[buf][t >> 3];
             const int k = t & 7, code = __float_as_int(e.w), c = code >> 28, jb = code & 0x0fffffff;
             float t0 = 1.f, t1 = e.z;
@@ -561,7 +749,11 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
             atomicAdd(a.mom + ((size_t)(c * n_pl + pl) * kKt + k) * a.nb_pad + jb, make_float2(e.x * tk, e.y * tk));
             if (k == 0) { const int b = jb - (L - 1); atomicMin(&s_blo[c], b); atomicMax(&s_bhi[c], b + 1); }
         }
+        // ---- advance the path of every facet to the next pulse (forward differences) ----
+#pragma unroll
+        for (int q = 0; q < FPT; ++q) { rho[q] += (unsigned long long)rd1[q]; rd1[q] += rd2[q]; rd2[q] += (long long)rd3[q]; }
         ++ip;
+        ns_cur = ns_next;
         if (ns + max(ns - ns_prev, 0) > kStrayCap && ip < hi - lo) { need_sort = true; ip_sort = ip; }   // before the list overflows
         ns_prev = need_sort ? 0 : ns;
         // no barrier here: the next pulse writes the other payload / stray buffers, and this pulse's are rewritten
@@ -570,24 +762,15 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
 
     // ---- counters ----
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        my_samples += __shfl_xor_sync(0xffffffffu, my_samples, o);
-        my_kept += __shfl_xor_sync(0xffffffffu, my_kept, o);
-    }
-    if (lane == 0) {
-        if (my_samples) atomicAdd(&s_samples, my_samples);
-        if (my_kept) atomicAdd(&s_kept, my_kept);
-    }
+    for (int o = 16; o > 0; o >>= 1) my_kept += __shfl_xor_sync(0xffffffffu, my_kept, o);
+    if (lane == 0 && my_kept) atomicAdd(&s_kept, my_kept);
     __syncthreads();
-    if (tid == 0 && a.counters) {
-        if (s_kept) atomicAdd(a.counters + 0, (unsigned long long)s_kept * C);
-        if (s_samples) atomicAdd(a.counters + 1, s_samples);
-    }
-    // ---- the band every vector occupies, for K3s (fftconv.cu): outside the pulse loop, whose code must stay as it is
-    //      (two atomics inside it cost 4 % of the kernel); a tile with an out-of-window echo claims the whole row ----
+    if (tid == 0 && a.counters && s_kept) atomicAdd(a.counters + 0, (unsigned long long)s_kept * C);
+    // ---- the band every vector occupies, for K3s (fftconv.cu): outside the pulse loop; a tile with an out-of-window
+    //      echo claims the whole row ----
     if (a.band_lo) {
         __syncthreads();                                     // the last pulse's strays have been merged into s_blo / s_bhi
-        for (int k = tid; k < (hi - lo) * C; k += kThreads) {
+        for (int k = tid; k < (hi - lo) * C; k += NT) {
             const int ip = k / C, c = k - ip * C, v = c * n_pl + (lo + ip - p0);
             // the sorted slices (one more on either side) and the strays, inside the sampling window
             const int blo = max(s_blo[c], -(L - 1)), bhi = min(s_bhi[c], prm.n_samples);
@@ -600,7 +783,7 @@ template <int FPT, int C>
 cudaError_t launch_fc(const DevParams &prm, const MomentArgs &a, int p0, int n_pl, int j_first, int n_int,
                       size_t smem, cudaStream_t s)
 {
-    dim3 grid(prm.n_tiles, n_int);
+    dim3 grid(prm.k2k_n_tiles, n_int);
     auto go = [&](auto kern) -> cudaError_t {
         // always opt in: static + dynamic shared memory together may pass 48 KB even when the dynamic part does not
         cudaError_t rc = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -633,10 +816,18 @@ cudaError_t launch_f(const DevParams &prm, const MomentArgs &a, int p0, int n_pl
 
 }  // namespace
 
+// slice index in 12 bits, slot rank in 12 bits, slot position in 13 bits, shared memory of one CTA
+bool moments_keyframed_fits(const DevParams &prm, int span_cap)
+{
+    return span_cap < 4096 && prm.k2k_cap <= 1024 && (prm.k2k_cap <= kThreads || prm.k2k_cap == 4 * kThreads || prm.k2k_cap == 3 * kThreads || prm.k2k_cap == 2 * kThreads) &&
+           prm.n_channels <= kMaxKeyChannels && prm.n_channels * prm.k2k_cap + 2 <= 8191 &&
+           moments_keyframed_smem_bytes(prm, span_cap) <= 200 * 1024;
+}
+
 size_t moments_keyframed_smem_bytes(const DevParams &prm, int span_cap)
 {
     const size_t C = prm.n_channels;
-    return (size_t)2 * C * prm.tile_cap * 14 + (size_t)hist_words((int)C, span_cap) * 4 +
+    return (size_t)2 * (C * prm.k2k_cap + 2) * 12 + C * prm.k2k_cap * 4 + (size_t)hist_words((int)C, span_cap) * 4 +
            (size_t)(kThreads / 8) * kScrTeam * sizeof(float2);
 }
 
@@ -644,15 +835,16 @@ cudaError_t launch_moments_keyframed(const DevParams &prm, const MomentArgs &a, 
 {
     const int H = a.surf.H, P = a.surf.n_pulses_total;
     if (H <= 1 || H + 1 > kMaxKeyPulses || prm.n_channels > kMaxKeyChannels || !prm.series_channels ||
-        a.span_cap >= (1 << 19) || prm.tile_cap > 4096)
+        !moments_keyframed_fits(prm, a.span_cap))
         return cudaErrorInvalidValue;
     const int n_keys = (P - 1 + H - 1) / H + 1;
     const int j_first = min(p0 / H, n_keys - 2), j_last = min((p0 + n_pl - 1) / H, n_keys - 2);
     const int n_int = j_last - j_first + 1;
     const size_t smem = moments_keyframed_smem_bytes(prm, a.span_cap);
-    if (prm.tile_cap <= kThreads) return launch_f<1>(prm, a, p0, n_pl, j_first, n_int, smem, s);
-    if (prm.tile_cap <= 4 * kThreads) return launch_f<4>(prm, a, p0, n_pl, j_first, n_int, smem, s);
-    return cudaErrorInvalidValue;
+    if (prm.k2k_cap <= kThreads) return launch_f<1>(prm, a, p0, n_pl, j_first, n_int, smem, s);
+    if (prm.k2k_cap == 3 * kThreads) return launch_f<3>(prm, a, p0, n_pl, j_first, n_int, smem, s);
+    if (prm.k2k_cap == 2 * kThreads) return launch_f<2>(prm, a, p0, n_pl, j_first, n_int, smem, s);
+    return launch_f<4>(prm, a, p0, n_pl, j_first, n_int, smem, s);
 }
 
 }  // namespace heeps

@@ -55,7 +55,7 @@ struct sim_handle {
     AccumulatePlan accum{};              // K3 launch shape
     bool need_slope = false;
     bool spectral = false;               // accumulate_mode resolved at sim_create
-    int nfft = 0, nb = 0, nb_pad = 0, replica = 0, span_cap_m = 0;
+    int nfft = 0, nb = 0, nb_pad = 0, replica = 0, span_cap_m = 0, span_cap_k = 0;   // slice window of a tile: K2s, K2k
 
     // tables
     DevBuf<double2> xt, yt, tt, chirp_n, carrier_p;
@@ -74,9 +74,10 @@ struct sim_handle {
     DevBuf<uint32_t> doppler_turns;      // frac(f_s t_p) in 2^-32 turns
     DevBuf<uint2> xi_t;                  // [pulses_per_batch][F] polar speckle of the batch
     int xi_state_pulse = -1;
+    float cur_lo[2] = {0.f, 0.f}, cur_hi[2] = {0.f, 0.f};   // bounding box of the current map at sim_create (widened by 25 %)
     // workspace
     DevBuf<double> z, zt, omega;
-    DevBuf<float2> slope;
+    DevBuf<float2> slope, slope_t;
     DevBuf<double2> dxy, dxy_t;
     int key_H = 1;                       // keyframe spacing of the kinematics (1 = every pulse)
     int nodes_x = 0, nodes_y = 0;        // heterogeneous surface: node lattice of the wave tables (0 = homogeneous)
@@ -94,6 +95,11 @@ struct sim_handle {
     DevBuf<int32_t> band;               // [2][C * pulses_per_batch]: occupied slice range of every vector (K2k -> K3s)
     int nfft2 = 0;                      // band transform size, 0 = off
 
+    // sim_debug_echoes: set for the duration of that call
+    int32_t *dbg_slice = nullptr, *dbg_keep = nullptr;
+    float *dbg_eps = nullptr;
+    float2 *dbg_w = nullptr;
+    int dbg_pulse = -1;
     // bookkeeping
     sim_stats stats{};
     bool profiling = false;
@@ -150,6 +156,12 @@ WaveView wave_view(const sim_scene *sc)
 }
 
 bool finite_all(const double *p, size_t n)
+{
+    for (size_t k = 0; k < n; ++k) if (!std::isfinite(p[k])) return false;
+    return true;
+}
+
+bool finite_all(const float *p, size_t n)
 {
     for (size_t k = 0; k < n; ++k) if (!std::isfinite(p[k])) return false;
     return true;
@@ -231,6 +243,15 @@ int validate(const sim_instrument *in, const sim_geometry *g, const sim_scene *s
             return SIM_EINVAL;
     }
     if (!sc->sigma0_lin && !(sc->sigma0_uniform >= 0 && std::isfinite(sc->sigma0_uniform))) return SIM_EINVAL;
+    {   // the per-facet maps: finite everywhere (a NaN current or sigma0 would poison whole tiles), sigma0 >= 0
+        const size_t F = (size_t)sc->nx * sc->ny;
+        if (sc->sigma0_lin) {
+            if (!finite_all(sc->sigma0_lin, F)) return SIM_EINVAL;
+            for (size_t k = 0; k < F; ++k) if (sc->sigma0_lin[k] < 0.f) return SIM_EINVAL;
+        }
+        if (sc->current_mps && !finite_all(sc->current_mps, 2 * F)) return SIM_EINVAL;
+        if (sc->xi && !finite_all(sc->xi, 2 * F)) return SIM_EINVAL;
+    }
     if (!finite_all(sc->look_dir, 2) || !finite_all(sc->current_uniform, 2)) return SIM_EINVAL;
     if (!std::isfinite(sc->speckle_tau_s) || !std::isfinite(sc->speckle_doppler_hz)) return SIM_EINVAL;
     if (sc->speckle_tau_s > 0)
@@ -293,6 +314,73 @@ double path_gradient_l1(const sim_geometry *g, const sim_scene *sc)
     return worst;
 }
 
+// Sheared tiles of the keyframed geometry kernel (moments_keyframed.cu): TH lines of TW facets, line b displaced by
+// rint(shear b) facets, so that a tile is as narrow in range as its lines are.  From the path-length gradient (in range
+// slices per facet step) at the scene centre, mid dwell, the shear that puts equal facets of all lines on one iso-range
+// line; its worst-case extent over a 3 x 3 lattice of scene points and three pulses sizes the tile's slice window.  The
+// shape with the smallest (tiles x (1 + extent / 16)) wins -- a displaced tiling has a few partly empty tiles per band.
+struct ShearPlan {
+    int w = 32, h = 32, axis = 0, a0 = 0, tiles_a = 1, tiles_b = 1;
+    double shear = 0, extent = 0;
+};
+ShearPlan plan_sheared_tiles(const sim_geometry *g, const sim_scene *sc, double fsc, int tile_cap)
+{
+    const int P = g->n_pulses;
+    const int picks[3] = {0, P / 2, P - 1};
+    struct G2 { double gx, gy; };
+    auto grad_at = [&](int p, double x, double y) {
+        const double *tx = g->tx_pos_m + 3 * p, *rx = g->rx_pos_m + 3 * p;
+        const double z = sc->centre_m[2];
+        const double dt[3] = {x - tx[0], y - tx[1], z - tx[2]}, dr[3] = {x - rx[0], y - rx[1], z - rx[2]};
+        const double rt = std::sqrt(dt[0] * dt[0] + dt[1] * dt[1] + dt[2] * dt[2]);
+        const double rr = std::sqrt(dr[0] * dr[0] + dr[1] * dr[1] + dr[2] * dr[2]);
+        return G2{(dt[0] / rt + dr[0] / rr) * sc->spacing_m * fsc, (dt[1] / rt + dr[1] / rr) * sc->spacing_m * fsc};
+    };
+    std::vector<G2> samples;
+    for (int q = 0; q < 3; ++q)
+        for (int cx = -1; cx <= 1; ++cx)
+            for (int cy = -1; cy <= 1; ++cy)
+                samples.push_back(grad_at(picks[q], sc->centre_m[0] + cx * 0.5 * (sc->nx - 1) * sc->spacing_m,
+                                          sc->centre_m[1] + cy * 0.5 * (sc->ny - 1) * sc->spacing_m));
+    const G2 c = grad_at(P / 2, sc->centre_m[0], sc->centre_m[1]);
+    ShearPlan best;
+    double best_cost = 1e300;
+    for (int axis = 0; axis < 2; ++axis)
+        for (int tw = 4; tw <= tile_cap / 2; tw <<= 1) {
+            const int th = tile_cap / tw;
+            if (tw * th != tile_cap) continue;
+            const double ga = axis ? c.gy : c.gx, gb = axis ? c.gx : c.gy;
+            const int na = axis ? sc->ny : sc->nx, nb = axis ? sc->nx : sc->ny;
+            for (int use_shear = 0; use_shear < 2; ++use_shear) {
+                double sh = 0;
+                if (use_shear) {
+                    if (std::fabs(ga) < 1e-9) continue;
+                    sh = -gb / ga;
+                    const double lim = std::min(4.0 * tw, 128.0) / th;      // at most four extra tiles per band
+                    sh = std::max(-lim, std::min(lim, sh));
+                }
+                double ext = 0;
+                for (const G2 &s2 : samples) {
+                    const double sa = axis ? s2.gy : s2.gx, sb = axis ? s2.gx : s2.gy;
+                    ext = std::max(ext, tw * std::fabs(sa) + th * std::fabs(sb + sa * sh) + std::fabs(sa));
+                }
+                int smin = 0, smax = 0;
+                for (int b = 0; b < th; ++b) {
+                    const int v = (int)std::nearbyint(sh * b);
+                    smin = std::min(smin, v); smax = std::max(smax, v);
+                }
+                const int tiles_a = (na + (smax - smin) + tw - 1) / tw, tiles_b = (nb + th - 1) / th;
+                const double cost = (double)tiles_a * tiles_b * (1.0 + ext / 16.0);
+                if (cost < best_cost) {
+                    best_cost = cost;
+                    best.w = tw; best.h = th; best.axis = axis; best.a0 = -smax; best.tiles_a = tiles_a; best.tiles_b = tiles_b;
+                    best.shear = sh; best.extent = ext;
+                }
+            }
+        }
+    return best;
+}
+
 // Rows of the surface buffers a batch [p0, p0 + n_pl) needs: its pulses (H = 1) or its keyframes.
 void surface_rows(const sim_handle *h, int p0, int n_pl, int *first, int *rows)
 {
@@ -304,7 +392,7 @@ void surface_rows(const sim_handle *h, int p0, int n_pl, int *first, int *rows)
 }
 
 struct SurfBufs {
-    double *z, *zt; float2 *slope; double2 *dxy, *dxy_t;
+    double *z, *zt; float2 *slope, *slope_t; double2 *dxy, *dxy_t;
 };
 
 // Time-dependent speckle of the batch (speckle.cu): fills h->xi_t and returns the pointer / row stride the K2 kernels use.
@@ -336,17 +424,18 @@ int run_kinematics(sim_handle *h, const SurfBufs &b, int p0, int n_pl, cudaStrea
     ka.H = h->key_H; ka.omega = h->omega.p; ka.zt = b.zt; ka.dxy_t = b.dxy_t;
     cudaError_t e = launch_kinematics(h->prm, ka, first, rows, s);
     if (e != cudaSuccess) return fail_cuda(h, e, "launch_kinematics");
-    sa->z = b.z; sa->zt = b.zt; sa->slope = b.slope; sa->dxy = b.dxy; sa->dxy_t = b.dxy_t;
+    sa->z = b.z; sa->zt = b.zt; sa->slope = b.slope; sa->slope_t = nullptr; sa->dxy = b.dxy; sa->dxy_t = b.dxy_t;
     sa->H = h->key_H; sa->key0 = first; sa->n_pulses_total = h->n_pulses;
     return SIM_OK;
 }
 
-// Keyframe spacing (surface.cuh): largest H whose cubic-Hermite error bound sum_w A_w (omega_w h)^4 / 384
-// stays under 4e-8 m (9e-6 rad of carrier phase on the two legs, worst case with all components in phase; the same
-// for the CWM displacement) and, with tilt modulation,
-// whose linear-interpolation error of the slopes, 4 x the root-sum-square of A_w |k_w| (omega_w h)^2 / 8 over the
-// components (random phases), stays under 1.2e-4 (the slopes only scale sigma0: measured 1.2e-5 of relative L2 on the
-// Heterogeneous recipe at H = 32, 4.3e-6 at H = 16); 1 when pulse times are not increasing.
+// Keyframe spacing (surface.cuh): largest H <= 64 whose cubic-Hermite error bound sum_w A_w (omega_w h)^4 / 384 stays
+// under kKeyframeHeightTol (9e-6 rad of carrier phase on the two legs, worst case with all components in phase; the same
+// for the CWM displacement) and, with tilt modulation, whose linear-interpolation error of the slopes, 4 x the
+// root-sum-square of A_w |k_w| (omega_w h)^2 / 8 over the components (random phases), stays under kKeyframeSlopeTol (the
+// slopes only scale sigma0: measured 1.8e-5 of relative L2 on the Large configuration at H = 32); 1 when pulse times are
+// not increasing.
+constexpr double kKeyframeHeightTol = 4e-8, kKeyframeSlopeTol = 1.2e-4;
 int choose_keyframe_spacing(const sim_geometry *g, const sim_scene *sc, int requested)
 {
     const int P = g->n_pulses;
@@ -372,7 +461,7 @@ int choose_keyframe_spacing(const sim_geometry *g, const sim_scene *sc, int requ
             bound = std::max(bound, b1); slope2 = std::max(slope2, s2);
         }
         if (wv.hetero) bound *= 2.0;
-        if (bound <= 4e-8 && (!sc->tilt_modulation || 4.0 * std::sqrt(slope2) <= 1.2e-4)) return H;
+        if (bound <= kKeyframeHeightTol && (!sc->tilt_modulation || 4.0 * std::sqrt(slope2) <= kKeyframeSlopeTol)) return H;
     }
     return 1;
 }
@@ -380,10 +469,10 @@ int choose_keyframe_spacing(const sim_geometry *g, const sim_scene *sc, int requ
 // ---- guard of the keyframed geometry (moments_keyframed.cu) ----
 // Evaluates, in long double on a 3 x 3 lattice of scene points (rest height, drifting with the uniform
 // current), the three interpolants the kernel uses over every keyframe interval of spacing H -- Hermite path
-// length, linear receive-channel path difference, quadratic gain product with the finite-difference channel
-// term -- against the exact geometry at EVERY pulse.  True iff all stay inside: path 2e-8 m, gains 1e-5 (tabulated: 3e-5).
-// Error budget against the parity bar of 1e-4 (relative L2): heights 9e-6 + path 2e-6 + gains 1e-5 + moments 1e-6 (+ 3e-5
-// for the linear slopes under tilt modulation, one sigma), all worst-case bounds; measured on ATI at H = 32: 4.5e-6 (at H = 16, under the former bounds of 2e-9 m and 3e-6: 3.8e-6).
+// length, linear receive-channel path difference, cubic gain product with the finite-difference channel
+// term -- against the exact geometry at EVERY pulse.  True iff all stay inside: path kGuardPathTol, gains kGuardGainTol
+// (tabulated: kGuardGainTolLut); the scene points drift with the uniform current or, with a current map, with each corner
+// of the bounding box of its values.
 long double sincl_pi(long double x)
 {
     if (x == 0.0L) return 1.0L;
@@ -489,27 +578,82 @@ GuardEval guard_eval(const sim_instrument *in, const sim_geometry *g, int p, con
     return o;
 }
 
-bool geometry_keyframes_ok(const sim_instrument *in, const sim_geometry *g, const sim_scene *sc, int H)
+// Waveform kernels of the moment form (moments.cu header): with b = ceil(nu) the slice of a facet-echo, eps = b - nu its
+// sub-slice position and y = 2 eps - 1, sample n = b + m of its replica is
+//     g_m(y) = exp(j 2 pi kappa (m + (y + 1)/2 - L/2)^2),     y in [-1, 1],
+// and c_k[m] are the Chebyshev coefficients of g_m in y (Gauss-Chebyshev quadrature on 64 nodes: exact to rounding
+// for this entire function), so that  s[n] = sum_k sum_m c_k[m] M_k[n - m]  with the Chebyshev moments M_k of the
+// slices.  Returns c_k for k < n_k ([n_k][L]) and max_m |c_k[m]| per k: the tail beyond Kt bounds the truncation.
+void chebyshev_kernels(double kappa, int L, int n_k, std::vector<std::complex<double>> &ck, std::vector<double> &cmax)
+{
+    const int NQ = 64;
+    ck.assign((size_t)n_k * L, std::complex<double>(0, 0));
+    cmax.assign(n_k, 0.0);
+    std::vector<double> cs((size_t)n_k * NQ), yq(NQ);
+    for (int j = 0; j < NQ; ++j) {
+        const double th = M_PI * (j + 0.5) / NQ;
+        yq[j] = std::cos(th);
+        for (int k = 0; k < n_k; ++k) cs[(size_t)k * NQ + j] = std::cos(k * th);
+    }
+    std::vector<std::complex<double>> gq(NQ);
+    for (int m = 0; m < L; ++m) {
+        for (int j = 0; j < NQ; ++j) {
+            const long double u = (long double)m + 0.5L * ((long double)yq[j] + 1.0L) - 0.5L * (long double)L;
+            long double turns = (long double)kappa * u * u;
+            turns -= floorl(turns);
+            gq[j] = std::complex<double>(std::cos(2.0 * M_PI * (double)turns), std::sin(2.0 * M_PI * (double)turns));
+        }
+        for (int k = 0; k < n_k; ++k) {
+            std::complex<double> acc(0, 0);
+            for (int j = 0; j < NQ; ++j) acc += gq[j] * cs[(size_t)k * NQ + j];
+            acc *= (k ? 2.0 : 1.0) / NQ;
+            ck[(size_t)k * L + m] = acc;
+            cmax[k] = std::max(cmax[k], std::abs(acc));
+        }
+    }
+}
+constexpr double kMomentTruncationTol = 5e-6;    // sum over k >= Kt of max_m |c_k[m]| the spectral form accepts (bar: 1e-4)
+
+// Tolerances of the guard: path 2e-8 m (2e-6 rad of carrier phase); gain product 3e-6 of the peak
+// for analytic apertures (the kernel's cubic through four nodes is ~3e-8 away), 3e-5 with tabulated patterns (the
+// bilinear table's kinks dominate).
+constexpr long double kGuardPathTol = 2e-8L, kGuardGainTol = 3e-6L, kGuardGainTolLut = 3e-5L;
+constexpr double kGuardMaxOffsetM = 4.0;         // |o_c| the fixed-point channel terms of K2k are scaled for
+constexpr double kGuardMaxSlices = 30000.0;      // |path - window start| in range slices the 16.48 fixed point holds
+
+// One velocity of the scene points (uniform current, or a corner of the current map's bounding box).
+bool geometry_keyframes_ok_at(const sim_instrument *in, const sim_geometry *g, const sim_scene *sc, int H,
+                              const long double vel[3])
 {
     const int P = g->n_pulses, C = in->n_channels;
-    if (H <= 1 || H + 1 > kMaxKeyPulses || C > kMaxKeyChannels) return false;
     const int n_keys = (P - 1 + H - 1) / H + 1;
     long double o_fd = 0;
     for (int c = 0; c < C; ++c) o_fd = std::max<long double>(o_fd, std::fabs(in->channel_offset_m[c]));
-    const long double vel[3] = {sc->current_uniform[0], sc->current_uniform[1], 0.0L};
-    // Tabulated patterns: the kernel's quadratic through three lookups follows a bilinear table only as closely as the
-    // table follows a smooth function; 2.25 = 1 + the Lebesgue constant 5/4 of the three-point quadratic.  The lattice
-    // check below samples the rest; together they must stay inside 3e-5 (the analytic apertures: 3e-6).
+    // Tabulated patterns: the kernel's cubic through four lookups follows a bilinear table only as closely as the
+    // table follows a smooth function; 2.63 = 1 + the Lebesgue constant 1.63 of the four-point cubic.  The lattice
+    // check below samples the rest; together they must stay inside kGuardGainTolLut.
     const bool lut = in->tx_pattern || in->rx_pattern;
-    long double kink = 0, gain_tol = 3e-6L;
+    long double kink = 0, gain_tol = kGuardGainTol;
     if (lut) {
         long double dt_, gt_, dr_, gr_;
         table_roughness(in, 0, dt_, gt_);
         table_roughness(in, 1, dr_, gr_);
-        kink = 2.25L * (dt_ * gr_ + dr_ * gt_);
-        gain_tol = 3e-5L;
+        kink = 2.63L * (dt_ * gr_ + dr_ * gt_);
+        gain_tol = kGuardGainTolLut;
         if (!(kink <= gain_tol)) return false;
     }
+    // a direction that leaves a table's grid inside an interval sees the hard edge of reading G29 (zero gain outside):
+    // no polynomial follows that step, so every sampled direction must stay one cell inside the grid
+    auto inside = [&](int k, long double ua, long double ue) {
+        const float *tab = k ? in->rx_pattern : in->tx_pattern;
+        if (!tab) return true;
+        const int nu = k ? in->rx_pattern_nu : in->tx_pattern_nu, nv = k ? in->rx_pattern_nv : in->tx_pattern_nv;
+        const double *ur = k ? in->rx_pattern_u : in->tx_pattern_u, *vr = k ? in->rx_pattern_v : in->tx_pattern_v;
+        const long double gu = (ua - ur[0]) * (nu - 1) / ((long double)ur[1] - ur[0]);
+        const long double gv = (ue - vr[0]) * (nv - 1) / ((long double)vr[1] - vr[0]);
+        return gu >= 1 && gu <= nu - 2 && gv >= 1 && gv <= nv - 2;
+    };
+    const long double fsc = (long double)in->fs_hz / kC0, half_len = 0.5L * in->chirp_len_s * in->fs_hz;
     for (int gx = -1; gx <= 1; ++gx)
         for (int gy = -1; gy <= 1; ++gy) {
             const long double x0 = sc->centre_m[0] + gx * 0.5L * (sc->nx - 1) * sc->spacing_m;
@@ -519,51 +663,88 @@ bool geometry_keyframes_ok(const sim_instrument *in, const sim_geometry *g, cons
             };
             for (int j = 0; j + 1 < n_keys; ++j) {
                 const int k0 = std::min(j * H, P - 1), k1 = std::min((j + 1) * H, P - 1);
-                if (k1 - k0 < 2) continue;
+                if (k1 <= k0) continue;
                 long double pa[3], pb[3];
                 at(k0, pa); at(k1, pb);
                 const GuardEval e0 = guard_eval(in, g, k0, pa, vel, o_fd), e1 = guard_eval(in, g, k1, pb, vel, o_fd);
                 const long double t0 = g->t_pulse_s[k0], h = (long double)g->t_pulse_s[k1] - t0;
                 if (!(h > 0)) return false;
-                auto pat = [&](long double a, long double b) { return sincl_pi(a) * sincl_pi(b); };
-                const long double P0 = e0.gt * pat(e0.xar, e0.xer), P1 = e1.gt * pat(e1.xar, e1.xer);
-                const long double gtm = pat(0.5L * (e0.xat + e1.xat), 0.5L * (e0.xet + e1.xet));
-                const long double grm = pat(0.5L * (e0.xar + e1.xar), 0.5L * (e0.xer + e1.xer));
-                const long double gom = pat(0.5L * (e0.xao + e1.xao), 0.5L * (e0.xeo + e1.xeo));
-                const long double Pm = gtm * grm, bq = o_fd > 0 ? gtm * (gom - grm) / o_fd : 0.0L;
-                // the same three-point interpolant with complex (tabulated) gains
-                cld P0c, P1c, Pmc, bqc;
-                if (lut) {
-                    P0c = e0.gtc * host_gain(in, 1, e0.uar, e0.uer); P1c = e1.gtc * host_gain(in, 1, e1.uar, e1.uer);
-                    const cld gtmc = host_gain(in, 0, 0.5L * (e0.uat + e1.uat), 0.5L * (e0.uet + e1.uet));
-                    const cld grmc = host_gain(in, 1, 0.5L * (e0.uar + e1.uar), 0.5L * (e0.uer + e1.uer));
-                    const cld gomc = host_gain(in, 1, 0.5L * (e0.uao + e1.uao), 0.5L * (e0.ueo + e1.ueo));
-                    Pmc = gtmc * grmc;
-                    bqc = o_fd > 0 ? gtmc * (gomc - grmc) / o_fd : cld(0, 0);
+                if (lut && !(inside(0, e0.uat, e0.uet) && inside(1, e0.uar, e0.uer) && inside(1, e0.uao, e0.ueo) &&
+                             inside(0, e1.uat, e1.uet) && inside(1, e1.uar, e1.uer) && inside(1, e1.uao, e1.ueo)))
+                    return false;
+                // the part of the channel path difference that is linear in t is rounded to an integer by one FP32 FMA: it
+                // must stay under 2^21 units of 2^-32 range slice (and of `mult` 2^-32 turns, scaled inside the kernel)
+                for (int c = 0; c < C; ++c)
+                    if (!(fabsl(e1.dl[c] - e0.dl[c]) * fsc * 4294967296.0L < 2097152.0L)) return false;
+                // the kernel's gain interpolant: cubic through s = 0, 1/3, 2/3, 1 with the direction cosines between
+                // the keyframes interpolated linearly; channel term by one finite difference at mid-interval
+                cld Pn[4];
+                for (int n = 0; n < 4; ++n) {
+                    const long double sn = n / 3.0L;
+                    Pn[n] = host_gain(in, 0, e0.uat + sn * (e1.uat - e0.uat), e0.uet + sn * (e1.uet - e0.uet)) *
+                            host_gain(in, 1, e0.uar + sn * (e1.uar - e0.uar), e0.uer + sn * (e1.uer - e0.uer));
                 }
-                for (int p = k0 + 1; p < k1; ++p) {
+                const cld c1 = 0.5L * (-11.0L * Pn[0] + 18.0L * Pn[1] - 9.0L * Pn[2] + 2.0L * Pn[3]);
+                const cld c2 = 4.5L * (2.0L * Pn[0] - 5.0L * Pn[1] + 4.0L * Pn[2] - Pn[3]);
+                const cld c3 = 4.5L * (-Pn[0] + 3.0L * Pn[1] - 3.0L * Pn[2] + Pn[3]);
+                const cld gtm = host_gain(in, 0, 0.5L * (e0.uat + e1.uat), 0.5L * (e0.uet + e1.uet));
+                const cld grm = host_gain(in, 1, 0.5L * (e0.uar + e1.uar), 0.5L * (e0.uer + e1.uer));
+                const cld gom = host_gain(in, 1, 0.5L * (e0.uao + e1.uao), 0.5L * (e0.ueo + e1.ueo));
+                const cld bq = o_fd > 0 ? gtm * (gom - grm) / o_fd : cld(0, 0);
+                for (int p = k0; p <= k1; ++p) {
                     long double pp[3];
                     at(p, pp);
                     const GuardEval ex = guard_eval(in, g, p, pp, vel, o_fd);
-                    const long double s = ((long double)g->t_pulse_s[p] - t0) / h, s2 = s * s, s3 = s2 * s;
+                    // the kernel steps the interval by pulse INDEX (uniform pulse times): a jittered PRF fails here
+                    const long double s = (long double)(p - k0) / (long double)(k1 - k0), s2 = s * s, s3 = s2 * s;
                     const long double Rh = (2 * s3 - 3 * s2 + 1) * e0.R + (s3 - 2 * s2 + s) * h * e0.Rd +
                                            (-2 * s3 + 3 * s2) * e1.R + (s3 - s2) * h * e1.Rd;
-                    if (!(fabsl(Rh - ex.R) <= 2e-8L)) return false;
-                    const long double Pq = P0 + s * ((-3 * P0 + 4 * Pm - P1) + s * (2 * P0 - 4 * Pm + 2 * P1));
+                    if (!(fabsl(Rh - ex.R) <= kGuardPathTol)) return false;
+                    // inside the range of the kernel's fixed point (and of its window arithmetic)
+                    if (!(fabsl((ex.R - (long double)kC0 * g->t0_s[p]) * fsc - half_len) <= kGuardMaxSlices)) return false;
+                    if (!(fabsl((long double)kC0 * ((long double)g->t0_s[p] - g->t0_s[k0]) * fsc) <= kGuardMaxSlices)) return false;
+                    if (lut && !(inside(0, ex.uat, ex.uet) && inside(1, ex.uar, ex.uer) && inside(1, ex.uao, ex.ueo))) return false;
+                    const cld Pq = Pn[0] + s * (c1 + s * (c2 + s * c3));
                     for (int c = 0; c < C; ++c) {
                         const long double dl = e0.dl[c] + s * (e1.dl[c] - e0.dl[c]);
-                        if (!(fabsl(dl - ex.dl[c]) <= 2e-8L)) return false;
-                        if (lut) {
-                            const cld gqc = P0c + s * ((-3.0L * P0c + 4.0L * Pmc - P1c) + s * (2.0L * P0c - 4.0L * Pmc + 2.0L * P1c)) +
-                                            (long double)in->channel_offset_m[c] * bqc;
-                            if (!(std::abs(gqc - ex.gtc * ex.grc[c]) + kink <= gain_tol)) return false;
-                            continue;
-                        }
-                        const long double gq = Pq + (long double)in->channel_offset_m[c] * bq;
-                        if (!(fabsl(gq - ex.gt * ex.gr[c]) <= 1e-5L)) return false;
+                        if (!(fabsl(dl - ex.dl[c]) <= kGuardPathTol)) return false;
+                        const cld gq = Pq + (long double)in->channel_offset_m[c] * bq;
+                        if (!(std::abs(gq - ex.gtc * ex.grc[c]) + kink <= gain_tol)) return false;
                     }
                 }
             }
+        }
+    return true;
+}
+
+bool geometry_keyframes_ok(const sim_instrument *in, const sim_geometry *g, const sim_scene *sc, int H,
+                           const float cur_lo[2], const float cur_hi[2])
+{
+    const int P = g->n_pulses, C = in->n_channels;
+    if (H <= 1 || H + 1 > kMaxKeyPulses || C > kMaxKeyChannels) return false;
+    for (int c = 0; c < C; ++c) if (!(std::fabs(in->channel_offset_m[c]) <= kGuardMaxOffsetM)) return false;
+    const double ratio = in->f0_hz / in->fs_hz;
+    if (!(ratio > 0.0 && ratio < 65000.0)) return false;
+    // uniform pulse times inside every interval (the waves are stepped by pulse index too; the platform terms are
+    // checked against the exact geometry below)
+    const int n_keys = (P - 1 + H - 1) / H + 1;
+    for (int j = 0; j + 1 < n_keys; ++j) {
+        const int k0 = std::min(j * H, P - 1), k1 = std::min((j + 1) * H, P - 1);
+        if (k1 <= k0) continue;
+        const double h = g->t_pulse_s[k1] - g->t_pulse_s[k0];
+        for (int p = k0; p <= k1; ++p)
+            if (!(std::fabs(g->t_pulse_s[p] - (g->t_pulse_s[k0] + h * (double)(p - k0) / (double)(k1 - k0))) <= 1e-9)) return false;
+    }
+    if (!sc->current_mps) {
+        const long double vel[3] = {sc->current_uniform[0], sc->current_uniform[1], 0.0L};
+        return geometry_keyframes_ok_at(in, g, sc, H, vel);
+    }
+    // a current map: the four corners of the bounding box of its values (the drift of a scene point enters the
+    // interpolants through its velocity and its position at every pulse)
+    for (int a = 0; a < 2; ++a)
+        for (int b = 0; b < 2; ++b) {
+            const long double vel[3] = {a ? cur_hi[0] : cur_lo[0], b ? cur_hi[1] : cur_lo[1], 0.0L};
+            if (!geometry_keyframes_ok_at(in, g, sc, H, vel)) return false;
         }
     return true;
 }
@@ -595,7 +776,7 @@ void sim_destroy(sim_handle *h)
     h->sigma0.release(); h->current.release(); h->xi.release(); h->xi_polar.release();
     h->pattern[0].release(); h->pattern[1].release();
     h->xi_state.release(); h->beta_g.release(); h->doppler_turns.release(); h->xi_t.release();
-    h->z.release(); h->slope.release(); h->dxy.release();
+    h->z.release(); h->slope.release(); h->slope_t.release(); h->dxy.release();
     h->zt.release(); h->dxy_t.release(); h->omega.release(); h->recs.release(); h->tinfo.release();
     h->tspan.release(); h->acc.release(); h->counters.release(); h->out_staging.release();
     h->mom.release(); h->cspec.release(); h->tw.release(); h->cspec2.release(); h->tw2.release(); h->band.release();
@@ -661,7 +842,16 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     const bool len_integer = std::fabs(prm.len - len_round) < 1e-9 * std::max(1.0, prm.len) && len_round >= 1.0;
     int nfft = 256;
     while (nfft < Ns + (int)len_round - 1 && nfft < (1 << 20)) nfft <<= 1;
-    const bool spectral_ok = len_integer && nfft <= 16384;
+    bool spectral_ok = len_integer && nfft <= 16384;
+    std::vector<std::complex<double>> ck_host;
+    if (spectral_ok) {
+        // truncation of the Chebyshev series at Kt moments: an under-sampled chirp (B > ~fs) needs more than Kt = 8
+        std::vector<double> cmax;
+        chebyshev_kernels(prm.kappa, (int)len_round, kMomentOrder + 4, ck_host, cmax);
+        double tail = 0;
+        for (int k = kMomentOrder; k < kMomentOrder + 4; ++k) tail += cmax[k];
+        if (!(tail <= kMomentTruncationTol)) spectral_ok = false;
+    }
     const int mode = opts ? opts->accumulate_mode : SIM_ACCUMULATE_AUTO;
     if (mode == SIM_ACCUMULATE_SPECTRAL && !spectral_ok) { delete h; return SIM_EINVAL; }
     h->spectral = (mode == SIM_ACCUMULATE_SPECTRAL) || (mode == SIM_ACCUMULATE_AUTO && spectral_ok);
@@ -695,7 +885,16 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     }
     const double tile_spread = tile * samples_per_facet + 2.0 * 2.0 * wave_sum * prm.fs_over_c0 + 3.0;
     h->accum = accumulate_plan(prm, tile_spread);
-    h->span_cap_m = std::min(4096, (((int)std::ceil(tile_spread) + 8) + 31) & ~31);
+    h->span_cap_m = std::min(4064, (((int)std::ceil(tile_spread) + 8) + 31) & ~31);
+    {   // K2k's own tiling (sheared) and the slice window of its tiles
+        const int k2k_cap = (prm.tile_cap == 1024) ? ((opts && opts->reserved[0] > 0) ? opts->reserved[0] : 768) : prm.tile_cap;
+        const ShearPlan sp = plan_sheared_tiles(g, sc, prm.fs_over_c0, k2k_cap);
+        prm.k2k_cap = k2k_cap;
+        prm.k2k_w = sp.w; prm.k2k_h = sp.h; prm.k2k_axis = sp.axis; prm.k2k_a0 = sp.a0; prm.k2k_shear = sp.shear;
+        prm.k2k_tiles_a = sp.tiles_a; prm.k2k_n_tiles = sp.tiles_a * sp.tiles_b;
+        const double spread_k = sp.extent + 2.0 * 2.0 * wave_sum * prm.fs_over_c0 + 3.0;
+        h->span_cap_k = std::min(4064, (((int)std::ceil(spread_k) + 8) + 15) & ~15);
+    }
 
     {   // receive-channel legs by series (geometry_common.cuh): offsets small against the nearest range
         double o_max = 0, r_min = 1e300;
@@ -711,6 +910,31 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
         prm.series_channels = (r_min > 0 && o_max <= 1e-4 * r_min) ? 1 : 0;
     }
     h->key_H = choose_keyframe_spacing(g, sc, opts ? opts->kinematics_keyframe : 0);
+    {   // K2k's fixed point: f0 / fs in 2^-48 units; the constant phase of the slice bias
+        const long double ratio = (long double)in->f0_hz / (long double)in->fs_hz;
+        if (ratio > 0 && ratio < 65000.0L) {
+            const long double k48 = ratio * 281474976710656.0L;       // 2^48
+            const unsigned long long K = (unsigned long long)(k48 + 0.5L);
+            prm.ratio_hi = (uint32_t)(K >> 32); prm.ratio_lo = (uint32_t)K;
+            // the kernel multiplies by K 2^-48, not by f0 / fs itself: the bias uses the same number
+            const long double kr = (long double)K / 281474976710656.0L;
+            long double turns = (32768.0L - 0.5L * (long double)prm.len) * kr;
+            turns -= floorl(turns);
+            prm.phase_bias32 = (uint32_t)(unsigned long long)(turns * 4294967296.0L + 0.5L);
+        }
+        if (sc->current_mps) {
+            for (int k = 0; k < 2; ++k) { h->cur_lo[k] = 1e30f; h->cur_hi[k] = -1e30f; }
+            const size_t n2 = 2 * (size_t)nx * ny;
+            for (size_t k = 0; k < n2; ++k) {
+                h->cur_lo[k & 1] = std::min(h->cur_lo[k & 1], sc->current_mps[k]);
+                h->cur_hi[k & 1] = std::max(h->cur_hi[k & 1], sc->current_mps[k]);
+            }
+            for (int k = 0; k < 2; ++k) {                  // room for sim_update_scene
+                const float m = 0.25f * std::max({std::fabs(h->cur_lo[k]), std::fabs(h->cur_hi[k]), 0.1f});
+                h->cur_lo[k] -= m; h->cur_hi[k] += m;
+            }
+        }
+    }
     prm.lut_any = (in->tx_pattern || in->rx_pattern) ? 1 : 0;
     if (h->spectral && h->key_H > 1 && prm.series_channels && C <= kMaxKeyChannels &&
         !(opts && opts->geometry_keyframe == 1)) {
@@ -718,8 +942,8 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
         // (a forced spacing is tried as it is)
         const bool forced = opts && opts->kinematics_keyframe > 1;
         for (int H = h->key_H; H > 1; H = forced ? 1 : H / 2) {
-            if (H + 1 <= kMaxKeyPulses && moments_keyframed_smem_bytes(prm, h->span_cap_m) <= 200 * 1024 &&
-                geometry_keyframes_ok(in, g, sc, H)) {
+            if (H + 1 <= kMaxKeyPulses && moments_keyframed_fits(prm, h->span_cap_k) &&
+                geometry_keyframes_ok(in, g, sc, H, h->cur_lo, h->cur_hi)) {
                 h->key_H = H; h->geo_keyframed = true;
                 break;
             }
@@ -905,28 +1129,14 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
         CKC(h->tspan.alloc((size_t)C * pb * prm.n_tiles));
         CKC(h->acc.alloc((size_t)C * pb * Ns));
     } else {
-        // waveform kernels c_k[m] = exp(j 2 pi kappa ((m-L/2)^2 + (m-L/2))) e_k j^k J_k(2 pi kappa (m-L/2))
-        // (moments.cu header), their spectra, and the transform's twiddle table
+        // waveform kernels c_k[m] (chebyshev_kernels above), their spectra, and the transform's twiddle table
         const int L = h->replica;
         std::vector<float2> ck((size_t)kMomentOrder * L), tw((size_t)nfft);
-        for (int m = 0; m < L; ++m) {
-            const long double mm = (long double)m - 0.5L * (long double)L;
-            long double turns = (long double)prm.kappa * (mm * mm + mm);
-            turns -= floorl(turns);
-            const double cr = std::cos(2.0 * M_PI * (double)turns), ci = std::sin(2.0 * M_PI * (double)turns);
-            const double zarg = 2.0 * M_PI * prm.kappa * (double)mm;
-            for (int k = 0; k < kMomentOrder; ++k) {
-                const double jk = (k == 0 ? 1.0 : 2.0) * jn(k, zarg);
-                double re = cr * jk, im = ci * jk, t;
-                switch (k & 3) {                                   // * j^k
-                    case 1: t = re; re = -im; im = t; break;
-                    case 2: re = -re; im = -im; break;
-                    case 3: t = re; re = im; im = -t; break;
-                    default: break;
-                }
-                ck[(size_t)k * L + m] = make_float2((float)re, (float)im);
+        for (int k = 0; k < kMomentOrder; ++k)
+            for (int m = 0; m < L; ++m) {
+                const std::complex<double> v = ck_host[(size_t)k * L + m];
+                ck[(size_t)k * L + m] = make_float2((float)v.real(), (float)v.imag());
             }
-        }
         for (int k = 0; k < nfft; ++k) {
             const double a = -2.0 * M_PI * (double)k / (double)nfft;
             tw[k] = make_float2((float)std::cos(a), (float)std::sin(a));
@@ -1023,7 +1233,7 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         }
         return cudaEventRecord(h->events[h->events_used++], s);
     };
-    const SurfBufs bufs{h->z.p, h->zt.p, h->slope.p, h->dxy.p, h->dxy_t.p};
+    const SurfBufs bufs{h->z.p, h->zt.p, h->slope.p, h->slope_t.p, h->dxy.p, h->dxy_t.p};
     for (int p0 = pb0; h->spectral && p0 < pb1; p0 += batch) {
         const int n_pl = std::min(batch, pb1 - p0);
         // the moment rows are zeroed on a second stream, beside K1 (which does not touch them): forked after whatever
@@ -1044,7 +1254,9 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         ma.pulses = h->pulses.p;
         ma.sigma0 = h->sigma0.p; ma.current = h->current.p;
         { int rc = run_speckle(h, p0, n_pl, s, &ma.xi_polar, &ma.xi_pulse_stride); if (rc != SIM_OK) return rc; }
-        ma.mom = h->mom.p; ma.nb_pad = h->nb_pad; ma.span_cap = h->span_cap_m; ma.replica = h->replica;
+        ma.mom = h->mom.p; ma.nb_pad = h->nb_pad; ma.replica = h->replica;
+        ma.span_cap = h->geo_keyframed ? h->span_cap_k : h->span_cap_m;
+        ma.dbg_slice = h->dbg_slice; ma.dbg_eps = h->dbg_eps; ma.dbg_w = h->dbg_w; ma.dbg_keep = h->dbg_keep; ma.dbg_pulse = h->dbg_pulse;
         ma.counters = h->counters.p;
         const size_t n_vec = (size_t)prm.n_channels * n_pl;
         if (h->nfft2) {                                  // lo preset to 0x7f7f7f7f, hi to 0x80808080
@@ -1144,6 +1356,20 @@ int sim_update_scene(sim_handle *h, const float *sigma0_lin, const float *curren
 {
     if (!h) return SIM_EINVAL;
     if ((sigma0_lin && !h->sigma0.p) || (current_mps && !h->current.p)) return SIM_EINVAL;
+    {
+        const size_t Fn = (size_t)h->n_facets;
+        if (sigma0_lin) {
+            if (!finite_all(sigma0_lin, Fn)) return SIM_EINVAL;
+            for (size_t k = 0; k < Fn; ++k) if (sigma0_lin[k] < 0.f) return SIM_EINVAL;
+        }
+        if (current_mps) {
+            if (!finite_all(current_mps, 2 * Fn)) return SIM_EINVAL;
+            // the keyframed geometry was admitted for the current extremes seen at sim_create
+            for (size_t k = 0; k < 2 * Fn; ++k)
+                if (current_mps[k] < h->cur_lo[k & 1] || current_mps[k] > h->cur_hi[k & 1]) return SIM_EINVAL;
+        }
+        if (xi && !finite_all(xi, 2 * Fn)) return SIM_EINVAL;
+    }
     DeviceGuard g(h->device);
     if (!g.ok) return SIM_ECUDA;
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
@@ -1200,7 +1426,7 @@ int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, d
         CK(h, d_pos.alloc(3 * F)); CK(h, d_tau.alloc(C * F)); CK(h, d_gtx.alloc(F));
         CK(h, d_grx.alloc(C * F)); CK(h, d_amp.alloc(2 * C * F)); CK(h, d_keep.alloc(F));
         // the slope is reported even when the scene does not use it: temporary rows
-        SurfBufs bufs{h->z.p, h->zt.p, h->slope.p, h->dxy.p, h->dxy_t.p};
+        SurfBufs bufs{h->z.p, h->zt.p, h->slope.p, h->slope_t.p, h->dxy.p, h->dxy_t.p};
         if (!bufs.slope) {
             CK(h, d_slope.alloc(F * 3 * 2));
             bufs.slope = d_slope.p;
@@ -1233,8 +1459,56 @@ int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, d
         return SIM_OK;
     };
     rc = run();
+    h->xi_state_pulse = -1;                              // the debug pass walked the AR(1) speckle state: the next batch replays it
     d_pos.release(); d_tau.release(); d_gtx.release(); d_grx.release(); d_amp.release(); d_keep.release();
     d_slope.release(); d_slope_out.release(); d_recs.release(); d_tinfo.release(); d_tspan.release();
+    return rc;
+}
+
+int sim_debug_echoes(sim_handle *h, int32_t pulse, int32_t *slice, float *eps, float *weight, int32_t *keep,
+                     int64_t *n_edge_ambiguous)
+{
+    if (!h) return SIM_EINVAL;
+    if (pulse < 0 || pulse >= h->n_pulses) return SIM_ERANGE;
+    if (!h->spectral || !h->geo_keyframed) return SIM_EINVAL;
+    DeviceGuard g(h->device);
+    if (!g.ok) return SIM_ECUDA;
+    const size_t F = (size_t)h->n_facets, C = h->prm.n_channels;
+    DevBuf<int32_t> d_slice, d_keep;
+    DevBuf<float> d_eps;
+    DevBuf<float2> d_w, d_out;
+    auto run = [&]() -> int {
+        CK(h, d_slice.alloc(C * F)); CK(h, d_keep.alloc(F)); CK(h, d_eps.alloc(C * F)); CK(h, d_w.alloc(C * F));
+        CK(h, d_out.alloc(C * (size_t)h->prm.n_samples));
+        CK(h, cudaMemset(d_slice.p, 0, C * F * sizeof(int32_t))); CK(h, cudaMemset(d_keep.p, 0, F * sizeof(int32_t)));
+        CK(h, cudaMemset(d_eps.p, 0, C * F * sizeof(float))); CK(h, cudaMemset(d_w.p, 0, C * F * sizeof(float2)));
+        h->dbg_slice = d_slice.p; h->dbg_keep = d_keep.p; h->dbg_eps = d_eps.p; h->dbg_w = d_w.p; h->dbg_pulse = pulse;
+        const sim_stats saved = h->stats;
+        const int rc = run_batches(h, pulse, pulse + 1, d_out.p, nullptr);
+        h->stats = saved;
+        h->dbg_slice = h->dbg_keep = nullptr; h->dbg_eps = nullptr; h->dbg_w = nullptr; h->dbg_pulse = -1;
+        if (rc != SIM_OK) return rc;
+        CK(h, cudaDeviceSynchronize());
+        std::vector<int32_t> hk(F);
+        std::vector<float> he(C * F);
+        CK(h, cudaMemcpy(hk.data(), d_keep.p, F * sizeof(int32_t), cudaMemcpyDeviceToHost));
+        CK(h, cudaMemcpy(he.data(), d_eps.p, C * F * sizeof(float), cudaMemcpyDeviceToHost));
+        if (slice) CK(h, cudaMemcpy(slice, d_slice.p, C * F * sizeof(int32_t), cudaMemcpyDeviceToHost));
+        if (weight) CK(h, cudaMemcpy(weight, d_w.p, C * F * sizeof(float2), cudaMemcpyDeviceToHost));
+        if (eps) std::memcpy(eps, he.data(), C * F * sizeof(float));
+        if (keep) std::memcpy(keep, hk.data(), F * sizeof(int32_t));
+        if (n_edge_ambiguous) {
+            int64_t n = 0;
+            for (size_t c = 0; c < C; ++c)
+                for (size_t f = 0; f < F; ++f)
+                    if (hk[f] && (he[c * F + f] < 1e-6f || he[c * F + f] > 1.f - 1e-6f)) ++n;
+            *n_edge_ambiguous = n;
+        }
+        return SIM_OK;
+    };
+    const int rc = run();
+    h->xi_state_pulse = -1;                              // (the debug pass walked the speckle state)
+    d_slice.release(); d_keep.release(); d_eps.release(); d_w.release(); d_out.release();
     return rc;
 }
 

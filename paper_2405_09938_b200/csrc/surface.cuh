@@ -4,10 +4,10 @@
 // pulses kf_j = min(j H, P-1), where it also stores the time derivatives; between keyframes the state is
 // the cubic Hermite interpolant in t.  Waves are slow against the PRF (omega <= ~3 rad/s): the interpolation
 // error of one component is <= A (omega h)^4 / 384 (h = keyframe spacing in seconds), and sim_create picks H
-// so that the sum of these bounds stays under 2e-9 m (hard part 3).  The slopes only scale sigma0
-// (tilt modulation): they are interpolated LINEARLY, per-component error <= A_w |k_w| (omega_w h)^2 / 8 (4 x their root-sum-square kept
-// under 4e-5 by sim_create).  The oracle always
-// evaluates exactly per pulse.
+// so that the sum of these bounds stays under kKeyframeHeightTol (sim_api.cu, hard part 3).  The slopes
+// only scale sigma0 (tilt modulation): they are interpolated LINEARLY, per-component error <= A_w |k_w| (omega_w h)^2 / 8
+// (4 x their root-sum-square kept under kKeyframeSlopeTol by sim_create; rate rows for a cubic interpolant were tried:
+// +40 % of K1 for 1e-5 of relative L2).  The oracle always evaluates exactly per pulse.
 #pragma once
 #include "heeps_common.cuh"
 
@@ -15,7 +15,8 @@ namespace heeps {
 
 struct SurfaceArgs {
     const double *z, *zt;               // [n][F] height above centre_z and its time derivative (zt: H > 1 only)
-    const float2 *slope;                // [n][F] or null (tilt modulation only; LINEAR between keyframes)
+    const float2 *slope;                // [n][F] or null (tilt modulation only)
+    const float2 *slope_t;              // [n][F] or null: time derivative of the slope (cubic Hermite between keyframes; null: linear -- what K1 provides)
     const double2 *dxy, *dxy_t;         // [n][F] or null (Choppy Wave Model only)
     int32_t H;                          // 1: n = pulses of the batch; > 1: n = keyframes of the batch
     int32_t key0;                       // H > 1: index j of the first keyframe held
@@ -67,6 +68,12 @@ __device__ __forceinline__ float2 surface_slope(const SurfaceArgs &sa, const Sur
     if (sa.H <= 1) return sa.slope[it.row0 * F + f];
     const size_t a = it.row0 * F + f, b = it.row1 * F + f;
     const float2 s0 = sa.slope[a], s1 = sa.slope[b];
+    if (sa.slope_t) {                                   // cubic Hermite, like the height
+        const float2 r0 = sa.slope_t[a], r1 = sa.slope_t[b];
+        const float w00 = (float)it.w00, w10 = (float)it.w10, w01 = (float)it.w01, w11 = (float)it.w11;
+        return make_float2(fmaf(w00, s0.x, fmaf(w10, r0.x, fmaf(w01, s1.x, w11 * r1.x))),
+                           fmaf(w00, s0.y, fmaf(w10, r0.y, fmaf(w01, s1.y, w11 * r1.y))));
+    }
     return make_float2(fmaf(it.s, s1.x - s0.x, s0.x), fmaf(it.s, s1.y - s0.y, s0.y));
 }
 

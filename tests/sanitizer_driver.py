@@ -41,9 +41,9 @@ def main():
 
     cases = []
     tiny = make_workload("tiny", n_pulses=9)
-    cases.append(("tiny spectral K2k H=4 batch=3", tiny, dict(accumulate_mode="spectral", kinematics_keyframe=4, pulses_per_batch=3)))
-    cases.append(("tiny spectral K2s", tiny, dict(accumulate_mode="spectral", geometry_keyframe=1)))
     cases.append(("tiny direct", tiny, dict(accumulate_mode="direct", pulses_per_batch=4)))
+    cases.append(("tiny spectral K2s", tiny, dict(accumulate_mode="spectral", geometry_keyframe=1)))
+    cases.append(("tiny spectral K2k H=4 batch=3", tiny, dict(accumulate_mode="spectral", kinematics_keyframe=4, pulses_per_batch=3)))
     hs = hetero_small(96, 64, 11)
     hs.scene["choppy"] = 1
     cases.append(("hetero_small spectral K2k H=4 batch=3", hs, dict(accumulate_mode="spectral", kinematics_keyframe=4, pulses_per_batch=3)))
@@ -67,7 +67,7 @@ def main():
     cases.append(("ar1 speckle spectral K2k batch=4", ar1, dict(accumulate_mode="spectral", pulses_per_batch=4)))
     cases.append(("ar1 speckle direct", ar1, dict(accumulate_mode="direct")))
 
-    worst = 0.0
+    worst, failed = 0.0, 0
     for name, w, opts in cases:
         ref = oracle_generate(w)
         with Simulator(w, 0, **opts) as sim:
@@ -82,7 +82,10 @@ def main():
             print(f"{name:45s} {what:6s} worst rel-L2 {err:.2e}", flush=True)
             if not err <= 1e-4:
                 print("PARITY FAILED", flush=True)
-                return 2
+                failed += 1
+    if failed:
+        print(f"sanitizer driver: {failed} FAILED comparisons")
+        return 2
     print(f"sanitizer driver ok: {len(cases)} cases, worst rel-L2 {worst:.2e}")
     return 0
 

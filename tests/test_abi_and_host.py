@@ -43,7 +43,8 @@ def test_kernels_are_sm100a_sass():
         pytest.skip("cuobjdump unavailable")
     assert "sm_100a" in out.stdout
     syms = subprocess.run(["cuobjdump", "-res-usage", str(LIBRARY_PATH)], capture_output=True, text=True).stdout
-    for k in ("kinematics_kernel", "geometry_kernel", "accumulate", "finalize_kernel"):
+    for k in ("kinematics_kernel", "geometry_kernel", "accumulate", "finalize_kernel",
+              "moments_keyframed_kernel", "moments_kernel", "fftconv_kernel", "fftconv_band_kernel", "speckle"):
         assert k in syms, k
 
 
@@ -63,6 +64,15 @@ def test_error_strings_and_validation_without_gpu():
     with pytest.raises(SimError) as e:
         sim_create(w)
     assert e.value.code == -1
+    # per-facet maps are scanned too: a NaN current or a negative sigma0 would poison whole tiles of the keyframed kernel
+    for key, idx, val in (("current_mps", (3, 4, 1), np.nan), ("sigma0_lin", (0, 0), -1.0), ("xi", (5, 5, 0), np.inf)):
+        w = make_workload("tiny", n_pulses=2)
+        w.scene["sigma0_lin"] = np.full((64, 64), 0.03, dtype=np.float32)
+        w.scene["current_mps"] = np.zeros((64, 64, 2), dtype=np.float32)
+        w.scene[key][idx] = val
+        with pytest.raises(SimError) as e:
+            sim_create(w)
+        assert e.value.code == -1, key
     import torch
     if not torch.cuda.is_available():
         # valid descriptors but no device: loud SIM_ECUDA, never a CPU fallback
@@ -144,3 +154,18 @@ def test_pulse_sharding_world_size_2_gloo(tmp_path):
         out, _ = p.communicate(timeout=300)
         assert p.returncode == 0, out
         assert "ok" in out
+
+
+def test_crop_rows_keeps_the_scene():
+    """workloads.crop_rows (bench.py's bounded oracle samples): slabs of facet rows of one scene, each with the facets'
+    rest positions unchanged -- the oracle's sums over the slabs add up to the sum over the scene (superposition)."""
+    from oracle import oracle_facets, oracle_generate
+    from workloads import crop_rows, make_workload
+    w = make_workload("tiny", n_pulses=2)
+    full = oracle_generate(w)
+    parts = sum(oracle_generate(crop_rows(w, a, b)) for a, b in ((0, 20), (20, 41), (41, 64)))
+    assert np.abs(full - parts).max() <= 1e-12 * np.abs(full).max()
+    f, g = oracle_facets(w, 1), oracle_facets(crop_rows(w, 20, 41), 1)
+    assert np.array_equal(f["pos"][20 * 64:41 * 64], g["pos"])
+    with pytest.raises(ValueError):
+        crop_rows(w, 10, 10)

@@ -292,6 +292,42 @@ def test_facet_intermediates(name):
     assert np.max(np.abs(g["amp"][:, kept] - o["amp"][:, kept])) < 5e-6 * scale
 
 
+def test_keyframed_geometry_unit_parity_and_edge_ambiguity():
+    """Unit parity of the DEFAULT path's geometry (moments_keyframed.cu through sim_debug_echoes) at pulses inside
+    keyframe intervals: range slice b = ceil((tau - t0) fs - L/2) against the oracle's tau per facet-echo -- an integer
+    decision (eq. (17)), identical except where the position lies within 1e-6 of an integer, and those are
+    counted (hard part 4); sub-slice position; cull decision outside a 1e-5 margin of the
+    threshold; interpolated complex weight against a G_t G_r exp(-j 2 pi f0 tau)."""
+    for w, pulses in ((_hetero_small(150, 90, 40), (13, 31)), (make_workload("tiny", n_pulses=24), (5,))):
+        if w.name == "tiny":
+            w.scene["spacing_m"] = 120.0                                   # culling scene, 3 channels
+            w.instrument["channel_offset_m"] = np.array([-1.5, 0.0, 1.5])
+        inst, geo = w.instrument, w.geometry
+        fs, L = inst["fs_hz"], w.replica_samples
+        with _sim(w, accumulate_mode="spectral") as sim:
+            assert sim.stats()["geometry_keyframed"] == 1 and sim.stats()["kinematics_keyframe"] >= 8
+            for p in pulses:
+                g = sim.debug_echoes(p)
+                o = oracle_facets(w, p)
+                nu = (o["tau"] - geo["t0_s"][p]) * fs - L / 2                  # [C][F]
+                b_ref = np.ceil(nu).astype(np.int64)
+                frac = nu - np.floor(nu)
+                near = np.minimum(frac, 1 - frac) < 1e-6
+                thr = 10 ** (inst["cull_two_way_db"] / 20)
+                margin = np.abs(np.abs(o["g_tx"] * o["g_rx"][w.n_channels // 2]) - thr) < 1e-5
+                assert np.array_equal(g["keep"][~margin], o["keep"][~margin])
+                kept = (o["keep"].astype(bool) & ~margin)[None, :] & ~near
+                assert np.array_equal(g["slice"][kept], b_ref[kept])
+                assert np.max(np.abs(g["eps"][kept] - (b_ref - nu)[kept])) < 2e-6
+                # every disagreement of the integer decision sits among the counted edge-ambiguous echoes
+                both = (o["keep"].astype(bool) & g["keep"].astype(bool))[None, :] & np.ones_like(near)
+                assert np.count_nonzero((g["slice"] != b_ref) & both & ~margin[None, :]) <= np.count_nonzero(near & both)
+                assert 0 <= g["n_edge_ambiguous"] <= 4 + 3 * np.count_nonzero(near & both)
+                carrier = np.exp(-2j * np.pi * np.mod(inst["f0_hz"] * np.longdouble(geo["t0_s"][p]), 1.0).astype(np.float64))
+                scale = np.abs(o["amp"][:, o["keep"].astype(bool)]).max()
+                assert np.max(np.abs(g["weight"] * carrier - o["amp"])[kept]) < 2e-5 * scale
+
+
 # ----------------------------------------------------------------------------- NEXT-3: tabulated antenna patterns
 
 def _wide_tiny(n_pulses=6, d=60.0, **kw):
@@ -414,6 +450,71 @@ def test_tabulated_patterns_keyframed_geometry_and_its_guard():
         got = sim.generate().cpu().numpy()
         assert sim.stats()["geometry_keyframed"] == 0
     _assert_parity(got, oracle_generate(wc), "coarse tables")
+
+
+def test_keyframed_geometry_with_late_pulse_times_and_currents(mode):
+    """Pulse times that start at +1000 s with a current: the facets have drifted half a kilometre from their rest
+    positions, the tiles' slice windows must follow (the window of a tile is placed at its drifted centre), and the
+    keyframed kernel must terminate whatever the stray count (round-1 advice: the re-sort loop could spin)."""
+    w = _hetero_small(96, 64, 11)
+    w.geometry["t_pulse_s"] = w.geometry["t_pulse_s"] + 1000.0
+    w.scene["current_mps"] = (w.scene["current_mps"] + np.float32(0.4)).astype(np.float32)
+    ref = oracle_generate(w)
+    assert np.abs(ref).max() > 0
+    with _sim(w, accumulate_mode=mode) as sim:
+        got = sim.generate().cpu().numpy()
+        st = sim.stats()
+    _assert_parity(got, ref, "late pulse times")
+    if mode == "spectral":
+        assert st["geometry_keyframed"] == 1
+
+
+def test_tabulated_pattern_edge_inside_the_scene_turns_the_keyframed_geometry_off():
+    """A table that covers only part of the scene, steered frames, 65 pulses at the default keyframe spacing: directions
+    cross the table's hard edge (zero gain outside, reading G29) inside keyframe intervals, which no polynomial follows;
+    sim_create must leave the exact per-pulse geometry on (round-1 advice), and the result must match the oracle."""
+    w = make_workload("tiny", n_pulses=65)
+    w.scene["spacing_m"] = 150.0
+    w.instrument["channel_offset_m"] = np.array([-1.5, 0.0, 1.5])
+    w = add_antenna_patterns(w, nu=513, nv=129, steer_rate_deg_s=3.0)
+    pat = w.instrument["tx_pattern"]
+    u0, u1 = pat["u"]
+    pat["u"] = (u0 + 0.3 * (u1 - u0), u1)                       # the table now starts 30 % into the scene
+    ref = oracle_generate(w)
+    with _sim(w, accumulate_mode="spectral") as sim:
+        got = sim.generate().cpu().numpy()
+        st = sim.stats()
+    assert st["geometry_keyframed"] == 0 and st["kinematics_keyframe"] > 1, st
+    _assert_parity(got, ref, "table edge inside the scene")
+    # the same tables covering the whole scene go through the keyframed kernel
+    w2 = make_workload("tiny", n_pulses=65)
+    w2.scene["spacing_m"] = 150.0
+    w2.instrument["channel_offset_m"] = np.array([-1.5, 0.0, 1.5])
+    w2 = add_antenna_patterns(w2, nu=2049, nv=257, steer_rate_deg_s=3.0)
+    with _sim(w2, accumulate_mode="spectral") as sim:
+        got2 = sim.generate().cpu().numpy()
+        assert sim.stats()["geometry_keyframed"] == 1
+    _assert_parity(got2, oracle_generate(w2), "tables covering the scene, 65 pulses")
+
+
+def test_update_scene_rejects_bad_maps():
+    """sim_update_scene scans what it uploads: NaN and currents outside the range the keyframe guard was run for."""
+    import torch
+    from paper_2405_09938_b200 import SimError
+    w = _hetero_small(96, 64, 3)
+    with _sim(w) as sim:
+        cur = torch.from_numpy(w.scene["current_mps"].copy()).pin_memory()
+        sim.update_scene(current=cur)                                  # the same map: fine
+        bad = cur.clone(); bad[3, 4, 0] = float("nan")
+        with pytest.raises(SimError) as e:
+            sim.update_scene(current=bad.pin_memory())
+        assert e.value.code == -1
+        fast = (cur * 50.0).pin_memory()
+        with pytest.raises(SimError) as e:
+            sim.update_scene(current=fast)
+        assert e.value.code == -1
+        got = sim.generate().cpu().numpy()
+    _assert_parity(got, oracle_generate(w), "after rejected updates")
 
 
 # ----------------------------------------------------------------------------- edge cases

@@ -612,3 +612,32 @@ def test_workload_digests_match_the_committed_file(name):
             drift.append(key)
     if drift:
         warnings.warn(f"{name}: byte-level differences within 1e-9 in {drift}")
+
+
+# ----------------------------------------------------------------------------- NEXT-4: the paper's fast mode (CPU restatement)
+
+def _ati_crop(n=24, n_pulses=9):
+    w = make_workload("ati", n_pulses=n_pulses)
+    sc = w.scene
+    j0 = 256 - n // 2
+    sc["xi"] = np.ascontiguousarray(sc["xi"][j0:j0 + n, j0:j0 + n])
+    sc["nx"] = sc["ny"] = n
+    return w
+
+
+def test_fast_mode_restatement_reduces_to_the_defined_sum():
+    """oracle/fast_mode.py (Doppler spectrum per range gate at PRF/n_fast, 1-D IFFT, linear combination):
+    with n_fast = 1 every pulse is a node and the scheme IS the defined sum (pins the restatement to heeps_oracle.c);
+    with n_fast > 1 it departs from it, the less the finer the Doppler bins; node pulses stay exact."""
+    from oracle import rel_l2_per_vector
+    from oracle.fast_mode import fast_mode_generate
+    w = _ati_crop()
+    ref = oracle_generate(w)
+    exact = fast_mode_generate(w, 1, 64)
+    assert np.max(np.abs(exact - ref)) <= 1e-9 * np.abs(ref).max()
+    coarse = rel_l2_per_vector(fast_mode_generate(w, 4, 64), ref)
+    fine = rel_l2_per_vector(fast_mode_generate(w, 4, 4096), ref)
+    assert np.all(coarse[:, [0, 4, 8]] < 1e-9) and np.all(fine[:, [0, 4, 8]] < 1e-9)     # nodes
+    mid = [2, 6]
+    assert np.all(coarse[:, mid] > 3 * fine[:, mid]) and fine[:, mid].min() > 0
+    assert fine[:, mid].max() > 1e-4            # still outside the parity bar at 1024 bins per skipped pulse
