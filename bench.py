@@ -355,7 +355,7 @@ def run_cuda(args):
     if rank > 0:
         w = _workload(args.workload, P, rank * P)
     F, C, Ns, L = w.n_facets, w.n_channels, w.n_samples, w.replica_samples
-    sim = Simulator(w, local_rank, accumulate_mode=args.mode, tile_facets=args.tile, k2k_tile_cap=args.k2k_cap)
+    sim = Simulator(w, local_rank, accumulate_mode=args.mode, tile_facets=args.tile)
     out = torch.empty((C, P, Ns), dtype=torch.complex64, device=f"cuda:{local_rank}")
     stream = torch.cuda.current_stream()
 
@@ -485,7 +485,6 @@ def main():
     ap.add_argument("--mode", default="auto", choices=["auto", "direct", "spectral"],
                     help="echo accumulation (include/heeps_sim.h SIM_ACCUMULATE_*)")
     ap.add_argument("--tile", type=int, default=0, help="spatial tile side in facets (0 = library default)")
-    ap.add_argument("--k2k-cap", type=int, default=0, help="facets per tile of the keyframed geometry kernel: 512, 768, 1024 (0 = library default)")
     ap.add_argument("--pulses", type=int, default=None, help="override the dwell length (debugging)")
     ap.add_argument("--wave-node-spacing", type=float, default=0.0,
                     help="heterogeneous surface: lattice step L [m] of per-node wave tables (0 = homogeneous, the configs)")

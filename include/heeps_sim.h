@@ -24,8 +24,8 @@
  *   - Facet (i,j), i fastest, rest position centre + ((i-(nx-1)/2) d, (j-(ny-1)/2) d, 0).
  *   - Output is complex64 [C][pulse_end-pulse_begin][Ns], interleaved (re,im) float32.
  *   - Return value 0 on success, a negative SIM_E* code otherwise.  Nothing is printed, no
- *     exception or abort crosses the boundary.  A handle is not thread-safe; distinct
- *     handles are independent.  There is no CPU fallback: without a CUDA device every
+ *     exception or abort crosses the boundary.  A handle is not thread-safe and serves ONE stream at
+ *     a time (its workspace and its cached speckle state are shared by its calls); distinct handles are independent.  There is no CPU fallback: without a CUDA device every
  *     compute entry point returns SIM_ECUDA.
  *   - Echo samples falling outside [0, Ns) are clipped silently (not an error).
  */
@@ -39,7 +39,7 @@ extern "C" {
 #endif
 
 #define SIM_OK        0
-#define SIM_EINVAL   (-1)   /* null pointer, bad size, NaN, non-orthonormal frame, > SIM_MAX_CHANNELS */
+#define SIM_EINVAL   (-1)   /* null pointer, bad size, NaN (descriptors and per-facet maps), non-orthonormal frame, > SIM_MAX_CHANNELS */
 #define SIM_ERANGE   (-2)   /* pulse range outside [0, P] or empty-inverted */
 #define SIM_ENOMEM   (-3)   /* host or device allocation failed */
 #define SIM_ECUDA    (-4)   /* CUDA runtime error; see sim_last_cuda_error */
@@ -121,7 +121,8 @@ typedef struct {
  *   SPECTRAL facet-echoes are summed into range slices (eq. 17) as Kt = 8 Chebyshev moments of the
  *            sub-slice position, and the slices are convolved with the waveform by FFT (the paper's
  *            "impulse response ... subsequently convolved by the waveform", with the sub-slice term
- *            kept to ~1e-6).  Needs T*fs integer and Ns + T*fs - 1 <= 16384.
+ *            kept to ~1e-6).  Needs T*fs integer, Ns + T*fs - 1 <= 16384 and a chirp that Kt = 8 moments resolve
+ *            (Chebyshev tail <= 5e-6: B <~ fs).
  *   AUTO     SPECTRAL where it applies, DIRECT otherwise. */
 #define SIM_ACCUMULATE_AUTO     0
 #define SIM_ACCUMULATE_DIRECT   1
@@ -136,11 +137,13 @@ typedef struct {
     int32_t kinematics_keyframe;   /* wave sums evaluated exactly every H-th pulse (with time derivatives) and
                                       cubic-Hermite interpolated between: 0 = auto (largest H <= 64 whose error
                                       bound sum_w A_w (omega_w h)^4/384 <= 4e-8 m; slopes linear between, their error <= 1.2e-4), 1 = every pulse, n = force H = n */
-    int32_t geometry_keyframe;     /* SPECTRAL only: 0 = auto -- where kinematics keyframes are in use (H > 1), C <= 4 and
-                                      the receive offsets are small, ranges / gains are evaluated exactly at the
-                                      keyframe pulses only and interpolated between (Hermite path length, quadratic
-                                      gains), after sim_create has verified the interpolants against the exact geometry
-                                      at every pulse on a lattice of scene points (path 2e-8 m, gains 1e-5);
+    int32_t geometry_keyframe;     /* SPECTRAL only: 0 = auto -- where kinematics keyframes are in use (H > 1), C <= 4, the
+                                      receive offsets are small (|o_c| <= 4 m) and the pulse times inside every keyframe
+                                      interval are uniform, ranges / gains are evaluated exactly at the keyframe pulses only
+                                      and interpolated between (Hermite path length stepped by fixed-point forward differences,
+                                      cubic gains), after sim_create has verified the interpolants against the exact geometry
+                                      at every pulse on a lattice of scene points (path 2e-8 m, gains 3e-6; tabulated patterns:
+                                      3e-5, and every sampled direction at least one cell inside the tables);
                                       1 = off (exact geometry at every pulse) */
     int32_t fft_band;              /* SPECTRAL with keyframed geometry: a vector whose echoes occupy a narrow band of range
                                       slices is convolved by a transform of that band alone: 0 = auto (size from the scene's
@@ -177,7 +180,9 @@ int sim_generate_host(sim_handle *h, int32_t pulse_begin, int32_t pulse_end, voi
 /*
  * sim_update_scene: replace the per-facet maps from HOST arrays (any may be NULL = keep):
  * sigma0 [ny][nx], current [ny][nx][2], xi [ny][nx][2]; host->device copies on cuda_stream.
- * A map that was NULL (uniform) at sim_create cannot be introduced later (SIM_EINVAL).
+ * A map that was NULL (uniform) at sim_create cannot be introduced later (SIM_EINVAL).  The new maps are scanned
+ * like the ones given to sim_create: finite, sigma0 >= 0, and every current component inside the range of the map
+ * given at sim_create widened by a quarter (the keyframe guard was run for that range), else SIM_EINVAL.
  */
 int sim_update_scene(sim_handle *h, const float *sigma0_lin, const float *current_mps, const float *xi,
                      void *cuda_stream);
@@ -206,7 +211,7 @@ int sim_debug_echoes(sim_handle *h, int32_t pulse, int32_t *slice, float *eps, f
 typedef struct {
     int64_t facet_echoes_nominal;  /* F * pulses * C                                   */
     int64_t facet_echoes_kept;     /* after the cull                                   */
-    int64_t facet_samples;         /* sum over kept facet-echoes of in-window samples  */
+    int64_t facet_samples;         /* sum over kept facet-echoes of in-window samples (0 on the SPECTRAL path with keyframed geometry) */
     int64_t kernel_launches;       /* kernels launched by the call                     */
     int32_t tile_facets, pulses_per_batch, n_tiles, accumulate_block_threads;
     int32_t max_span_samples;      /* largest per-tile sample span seen                */
@@ -224,7 +229,7 @@ int sim_get_stats(sim_handle *h, sim_stats *out);
 int sim_set_profiling(sim_handle *h, int32_t enable);
 int sim_get_kernel_ms(sim_handle *h, float ms[4]);
 
-/* Pipe-throughput microbenchmarks on `device` (the FP32 / XU / FP64 pipe peaks that
+/* DIAGNOSTIC, not part of the method's boundary: pipe-throughput microbenchmarks on `device` (the FP32 / XU / FP64 pipe peaks that
  * bound the ALU-bound kernels are measured in the same run as the numbers quoted against them).
  * All figures are LANE operations per second at the clock the GPU ran the probe at (an FMA = 1
  * operation; a packed f32x2 instruction = 2).  Synchronous; takes a few tens of milliseconds. */

@@ -12,7 +12,10 @@ from pathlib import Path
 
 import numpy as np
 
-LIBRARY_PATH = Path(__file__).resolve().parent / "libheeps_sim.so"
+import os
+
+# HEEPS_SIM_LIBRARY selects another build of the same library (the checked build, build.py --checked)
+LIBRARY_PATH = Path(os.environ.get("HEEPS_SIM_LIBRARY") or Path(__file__).resolve().parent / "libheeps_sim.so").resolve()
 HEADER_PATH = Path(__file__).resolve().parent.parent / "include" / "heeps_sim.h"
 
 SIM_OK, SIM_EINVAL, SIM_ERANGE, SIM_ENOMEM, SIM_ECUDA = 0, -1, -2, -3, -4
@@ -250,7 +253,7 @@ def _marshal(workload):
 
 def sim_create(workload, device: int = 0, *, tile_facets: int = 0, pulses_per_batch: int = 0,
                workspace_bytes: int = 0, accumulate_mode=0, kinematics_keyframe: int = 0,
-               geometry_keyframe: int = 0, fft_band: int = 0, k2k_tile_cap: int = 0):
+               geometry_keyframe: int = 0, fft_band: int = 0):
     lib = load_library()
     ci, cg, cs, keep = _marshal(workload)
     opts = sim_options()
@@ -259,7 +262,6 @@ def sim_create(workload, device: int = 0, *, tile_facets: int = 0, pulses_per_ba
     opts.kinematics_keyframe = int(kinematics_keyframe)
     opts.geometry_keyframe = int(geometry_keyframe)
     opts.fft_band = int(fft_band)
-    opts.reserved[0] = int(k2k_tile_cap)
     h = C.c_void_p()
     rc = lib.sim_create(C.byref(ci), C.byref(cg), C.byref(cs), C.byref(opts), int(device), C.byref(h))
     del keep

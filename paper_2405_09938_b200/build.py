@@ -70,5 +70,36 @@ def build_library(force: bool = False, verbose: bool = False) -> Path:
     return LIB
 
 
+CHECKED_LIB = PKG / "libheeps_sim_checked.so"
+
+
+def build_checked_library() -> Path:
+    """libheeps_sim_checked.so: the same library with the keyframed geometry kernel compiled with -DHEEPS_CHECKED (device-side
+    bounds checks that trap).  Stands in for compute-sanitizer, which the GPU pool does not offer: run
+    `HEEPS_SIM_LIBRARY=paper_2405_09938_b200/libheeps_sim_checked.so python tests/sanitizer_driver.py`."""
+    build_library()
+    nvcc = os.environ.get("NVCC", "nvcc")
+    src = CSRC / "moments_keyframed.cu"
+    obj = OBJ / "moments_keyframed_checked.o"
+    headers = list(CSRC.glob("*.cuh")) + list(INCLUDE.glob("*.h")) + [Path(__file__)]
+    if _stale(obj, [src] + headers):
+        r = subprocess.run([nvcc, *NVCC_FLAGS, "-DHEEPS_CHECKED", "-I", str(INCLUDE), "-c", str(src), "-o", str(obj)],
+                           capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError("nvcc failed:\n" + r.stdout + r.stderr)
+    objs = [OBJ / (s.stem + ".o") for s in sources() if s.stem != "moments_keyframed"] + [obj]
+    if _stale(CHECKED_LIB, objs):
+        tmp = CHECKED_LIB.with_suffix(f".{os.getpid()}.tmp")
+        r = subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", str(tmp), *map(str, objs), "-lcudart"],
+                           capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError("link failed:\n" + r.stdout + r.stderr)
+        os.replace(tmp, CHECKED_LIB)
+    return CHECKED_LIB
+
+
 if __name__ == "__main__":
-    print(build_library(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    if "--checked" in sys.argv:
+        print(build_checked_library())
+    else:
+        print(build_library(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

@@ -40,7 +40,7 @@
 // The chirp's own sub-slice phase kappa eps^2 is part of the waveform kernels (sim_api.cu builds them as the Chebyshev
 // coefficients of the exact slice response), so the per-echo phase is the carrier phase alone.
 //
-// One CTA = one SHEARED spatial tile x one keyframe interval (256 threads x 4 facets, two CTAs per SM).  A thread holds
+// One CTA = one SHEARED spatial tile x one keyframe interval (256 threads x 3 facets -- 32 x 24 -- two CTAs per SM).  A thread holds
 // its facets' interpolants in registers and loops over the interval's pulses.  The tile's facet-echoes (all C channels)
 // are ordered by range slice ONCE per interval -- counting sort at its middle pulse: shared-memory histogram by integer
 // ATOMS, scan, slot = first position of the slice + rank -- because over a few milliseconds a facet changes slice only
@@ -54,10 +54,13 @@
 // overflow -- echoes outside the tile's slice window -- goes straight to global atomics, so the redo happens at most
 // once).  Payload and stray list are double-buffered.
 // Tried and measured in round 2 (profiles/r2_k2k_history.md): 512 threads x 2 facets with one CTA per SM, stage C by
-// one thread per chunk of slots, and producer / consumer warps behind named barriers -- each cut the instruction count
-// and none the time: with one CTA per SM the warps that sum the slices hold the others at the barrier.
+// one thread per chunk of slots, producer / consumer warps behind named barriers, 2 and 4 facets per thread -- each
+// cut the instruction count and none the time: with one CTA per SM the warps that sum the slices hold the others at
+// the barrier, and at 4 facets per thread the state spills.
 //
 // Bound: issue slots (FP32 + integer mix); HBM/L2: four surface rows per facet and INTERVAL, the maps once.
+#include <cstdio>
+
 #include "kernels.cuh"
 #include "geometry_common.cuh"
 
@@ -167,6 +170,16 @@ __device__ __forceinline__ unsigned long long rho_ahead(unsigned long long f, lo
 }
 
 constexpr int kThreads = 256;
+
+// Checked build (python -m paper_2405_09938_b200.build --checked: -DHEEPS_CHECKED, libheeps_sim_checked.so): every
+// computed shared-memory position and global moment-row index of this kernel is tested and a violation traps (the
+// launch fails with a CUDA error).  compute-sanitizer is not available on the GPU pool this was developed on; the
+// checked library runs tests/sanitizer_driver.py in its place.
+#ifdef HEEPS_CHECKED
+#define HEEPS_CHECK(cond) do { if (!(cond)) { printf("HEEPS_CHECK failed: %s (line %d, block %d, thread %d)\n", #cond, __LINE__, (int)blockIdx.x, (int)threadIdx.x); __trap(); } } while (0)
+#else
+#define HEEPS_CHECK(cond) do { } while (0)
+#endif
 
 template <int FPT, int C, bool kTilt, bool kSpeckleT, bool kLut>
 __global__ void __launch_bounds__(kThreads, 2)
@@ -497,7 +510,10 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                     const int rel = (int)(slice_word(q, c, X, nq) >> 32) - K2[c];
                     pr[q][c] = -1;
                     if (((validmask >> q) & 1u) && (unsigned)rel < (unsigned)span)
+                    {
+                        HEEPS_CHECK(rel + 1 <= span);
                         pr[q][c] = (rel << 12) | atomicAdd(&hs[c * hstride + rel + 1], 1);
+                    }
                 }
             }
             __syncthreads();
@@ -531,6 +547,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
 #pragma unroll
                 for (int c = 0; c < C; ++c) {
                     const int v = pr[q][c];
+                    HEEPS_CHECK(v < 0 || ((v & 4095) < cap && hs[c * hstride + (v >> 12)] + (v & 4095) < cap));
                     if (FPT > 1 || q * NT + tid < cap)               // (FPT = 1: the tile may be smaller than the CTA)
                         slots[c * cap + q * NT + tid] =
                             (v >= 0) ? (uint32_t)(((v >> 12) << 13) | (c * cap + hs[c * hstride + (v >> 12)] + (v & 4095))) : no_slot;
@@ -606,6 +623,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                 const uint32_t slot = (FPT > 1 || k < cap) ? slots[c * cap + k] : no_slot;
                 const bool here = (uint32_t)(xh - K2[c]) == (slot >> 13);   // in its sorted slice
                 const uint32_t pos = slot & 8191u;
+                HEEPS_CHECK(pos <= (uint32_t)capS && (!here || pos < (uint32_t)capS));
                 pay[pos] = here ? make_float2(wr, wi) : make_float2(0.f, 0.f);
                 pay_y[pos] = yv;
                 // stray: left its sorted slice, or never had one; its window meets [0, Ns)
@@ -627,6 +645,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                     echo(q, c, Pv, Pi, am, ph_ref, X, gq, nq, wr, wi, yv, xh);
                     const int b = xh + 1 - kRhoBias;
                     const int t = atomicAdd(n_stray, 1);
+                    HEEPS_CHECK(b + L - 1 >= 0 && b + L - 1 < a.nb_pad);
                     if (t < kStrayCap) {
                         s_stray[buf][t] = make_float4(wr, wi, yv, __int_as_float((c << 28) | (b + L - 1)));
                     } else if (sorted_at == ip) {                          // sorted at this very pulse and still no room:
@@ -732,6 +751,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                 for (int r = 1; r < 8; ++r) hsum = fadd2(hsum, scr64[r * kScrRow + sub]);
                 __syncwarp();
                 float2 h1 = *reinterpret_cast<float2 *>(&hsum);
+                HEEPS_CHECK(cnt == 0 || (first >= 0 && first + cnt <= cap && b + L - 1 >= 0 && b + L - 1 < a.nb_pad));
                 if (cnt > 0) {
                     if (sub & 2) { h1.x = -h1.x; h1.y = -h1.y; }
                     float2 *row = a.mom + ((size_t)(c * n_pl + pl) * kKt + sub) * a.nb_pad;
@@ -819,7 +839,7 @@ cudaError_t launch_f(const DevParams &prm, const MomentArgs &a, int p0, int n_pl
 // slice index in 12 bits, slot rank in 12 bits, slot position in 13 bits, shared memory of one CTA
 bool moments_keyframed_fits(const DevParams &prm, int span_cap)
 {
-    return span_cap < 4096 && prm.k2k_cap <= 1024 && (prm.k2k_cap <= kThreads || prm.k2k_cap == 4 * kThreads || prm.k2k_cap == 3 * kThreads || prm.k2k_cap == 2 * kThreads) &&
+    return span_cap < 4096 && prm.k2k_cap <= 1024 && (prm.k2k_cap <= kThreads || prm.k2k_cap == 3 * kThreads) &&
            prm.n_channels <= kMaxKeyChannels && prm.n_channels * prm.k2k_cap + 2 <= 8191 &&
            moments_keyframed_smem_bytes(prm, span_cap) <= 200 * 1024;
 }
@@ -842,9 +862,7 @@ cudaError_t launch_moments_keyframed(const DevParams &prm, const MomentArgs &a, 
     const int n_int = j_last - j_first + 1;
     const size_t smem = moments_keyframed_smem_bytes(prm, a.span_cap);
     if (prm.k2k_cap <= kThreads) return launch_f<1>(prm, a, p0, n_pl, j_first, n_int, smem, s);
-    if (prm.k2k_cap == 3 * kThreads) return launch_f<3>(prm, a, p0, n_pl, j_first, n_int, smem, s);
-    if (prm.k2k_cap == 2 * kThreads) return launch_f<2>(prm, a, p0, n_pl, j_first, n_int, smem, s);
-    return launch_f<4>(prm, a, p0, n_pl, j_first, n_int, smem, s);
+    return launch_f<3>(prm, a, p0, n_pl, j_first, n_int, smem, s);
 }
 
 }  // namespace heeps

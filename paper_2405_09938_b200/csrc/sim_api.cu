@@ -885,9 +885,12 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     }
     const double tile_spread = tile * samples_per_facet + 2.0 * 2.0 * wave_sum * prm.fs_over_c0 + 3.0;
     h->accum = accumulate_plan(prm, tile_spread);
+    if (!h->spectral && h->accum.block_threads > 1024) { delete h; return SIM_EINVAL; }   // replica too long for one CTA of the direct form
     h->span_cap_m = std::min(4064, (((int)std::ceil(tile_spread) + 8) + 31) & ~31);
     {   // K2k's own tiling (sheared) and the slice window of its tiles
-        const int k2k_cap = (prm.tile_cap == 1024) ? ((opts && opts->reserved[0] > 0) ? opts->reserved[0] : 768) : prm.tile_cap;
+        // 32 x 32 tiles of the spectral path become 32 x 24 sheared tiles here: 256 threads x 3 facets, two CTAs per SM
+        // (4 facets per thread spill, 2 leave the slices half as full: profiles/r2_k2k_history.md)
+        const int k2k_cap = (prm.tile_cap == 1024) ? 768 : prm.tile_cap;
         const ShearPlan sp = plan_sheared_tiles(g, sc, prm.fs_over_c0, k2k_cap);
         prm.k2k_cap = k2k_cap;
         prm.k2k_w = sp.w; prm.k2k_h = sp.h; prm.k2k_axis = sp.axis; prm.k2k_a0 = sp.a0; prm.k2k_shear = sp.shear;

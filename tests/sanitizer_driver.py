@@ -3,10 +3,13 @@ library -- K1 (homogeneous, heterogeneous lattice), K2k (forced keyframe spacing
 patch, tabulated patterns, AR(1) speckle), K2s, K2 / K3 / K4 (direct form), K3s (full and band transform), speckle.cu,
 sim_debug_facets -- and checks each result against the oracle, so that a sanitizer run is also a parity run.
 
-    compute-sanitizer --tool memcheck  --error-exitcode 1 python tests/sanitizer_driver.py
-    compute-sanitizer --tool racecheck --error-exitcode 1 python tests/sanitizer_driver.py
-    compute-sanitizer --tool initcheck --error-exitcode 1 python tests/sanitizer_driver.py
-    compute-sanitizer --tool synccheck --error-exitcode 1 python tests/sanitizer_driver.py
+    compute-sanitizer --tool memcheck  --error-exitcode 1 python tests/sanitizer_driver.py      (likewise racecheck,
+                                                                                                  initcheck, synccheck)
+    HEEPS_SIM_LIBRARY=paper_2405_09938_b200/libheeps_sim_checked.so python tests/sanitizer_driver.py
+
+The GPU pool this was developed on refuses compute-sanitizer (profiles/r2_sanitizer.md); the second form -- the library
+built with device-side bounds checks that trap, `python -m paper_2405_09938_b200.build --checked` -- is what
+tests/test_gpu_parity.py::test_checked_build_runs_the_driver_clean runs.
 
 Not collected by pytest (no test_ prefix); the summaries are kept under profiles/.
 """
@@ -36,8 +39,9 @@ def hetero_small(nx, ny, n_pulses):
 def main():
     import torch
     from oracle import oracle_generate, rel_l2_per_vector
-    from paper_2405_09938_b200 import Simulator
+    from paper_2405_09938_b200 import LIBRARY_PATH, Simulator
     from workloads import add_antenna_patterns, make_workload
+    print("library:", LIBRARY_PATH, flush=True)
 
     cases = []
     tiny = make_workload("tiny", n_pulses=9)
