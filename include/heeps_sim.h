@@ -203,7 +203,8 @@ int sim_debug_facets(sim_handle *h, int32_t pulse, double *pos, double *slope, d
  * eps = b - ((tau - t0) fs - T fs / 2) in (0, 1], eps [C][F]; complex weight a G_t G_r,c exp(-j 2 pi f0 (tau - t0[p]))
  * as the kernel interpolates it, weight [C][F][2]; keep [F].  *n_edge_ambiguous = kept facet-echoes whose
  * position lies within 1e-6 of an integer: their slice may legitimately differ from an fp64 evaluation's (reading
- * G18).  SIM_EINVAL unless the handle runs the spectral form with keyframed geometry (sim_stats).  Synchronous. */
+ * G18).  SIM_EINVAL unless the handle runs the spectral form with keyframed geometry (sim_stats), analytic antenna
+ * patterns and static speckle.  Synchronous. */
 int sim_debug_echoes(sim_handle *h, int32_t pulse, int32_t *slice, float *eps, float *weight, int32_t *keep,
                      int64_t *n_edge_ambiguous);
 

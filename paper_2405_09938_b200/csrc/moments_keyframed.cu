@@ -181,7 +181,10 @@ constexpr int kThreads = 256;
 #define HEEPS_CHECK(cond) do { } while (0)
 #endif
 
-template <int FPT, int C, bool kTilt, bool kSpeckleT, bool kLut>
+// kDbg: the instantiation behind sim_debug_echoes, which also reports one pulse's facet-echoes.  A template flag and not
+// a run-time test: the extra copy of the echo code inside the pulse loop cost the normal kernel 12 % (register
+// allocation: 748 -> 854 ms on the Large configuration).
+template <int FPT, int C, bool kTilt, bool kSpeckleT, bool kLut, bool kDbg>
 __global__ void __launch_bounds__(kThreads, 2)
 moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_first)
 {
@@ -663,7 +666,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                 }
             }
         }
-        if (a.dbg_slice && lo + ip == a.dbg_pulse) {          // sim_debug_echoes: this pulse's facet-echoes as the kernel sees them
+        if (kDbg && a.dbg_slice && lo + ip == a.dbg_pulse) {  // sim_debug_echoes: this pulse's facet-echoes as the kernel sees them
 #pragma unroll
             for (int q = 0; q < FPT; ++q) {
                 const int k = q * NT + tid;
@@ -811,14 +814,19 @@ cudaError_t launch_fc(const DevParams &prm, const MomentArgs &a, int p0, int n_p
         kern<<<grid, kThreads, smem, s>>>(prm, a, p0, n_pl, j_first);
         return cudaGetLastError();
     };
+    if (a.dbg_slice) {                                   // sim_debug_echoes (analytic patterns, static speckle only)
+        if (prm.lut_any || a.xi_pulse_stride) return cudaErrorInvalidValue;
+        return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, false, false, true>)
+                        : go(moments_keyframed_kernel<FPT, C, false, false, false, true>);
+    }
     if (prm.lut_any) {
         if (a.xi_pulse_stride)
-            return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, true, true>) : go(moments_keyframed_kernel<FPT, C, false, true, true>);
-        return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, false, true>) : go(moments_keyframed_kernel<FPT, C, false, false, true>);
+            return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, true, true, false>) : go(moments_keyframed_kernel<FPT, C, false, true, true, false>);
+        return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, false, true, false>) : go(moments_keyframed_kernel<FPT, C, false, false, true, false>);
     }
     if (a.xi_pulse_stride)
-        return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, true, false>) : go(moments_keyframed_kernel<FPT, C, false, true, false>);
-    return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, false, false>) : go(moments_keyframed_kernel<FPT, C, false, false, false>);
+        return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, true, false, false>) : go(moments_keyframed_kernel<FPT, C, false, true, false, false>);
+    return prm.tilt ? go(moments_keyframed_kernel<FPT, C, true, false, false, false>) : go(moments_keyframed_kernel<FPT, C, false, false, false, false>);
 }
 
 template <int FPT>

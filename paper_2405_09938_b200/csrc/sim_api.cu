@@ -1473,7 +1473,7 @@ int sim_debug_echoes(sim_handle *h, int32_t pulse, int32_t *slice, float *eps, f
 {
     if (!h) return SIM_EINVAL;
     if (pulse < 0 || pulse >= h->n_pulses) return SIM_ERANGE;
-    if (!h->spectral || !h->geo_keyframed) return SIM_EINVAL;
+    if (!h->spectral || !h->geo_keyframed || h->prm.lut_any || h->speckle_ar1) return SIM_EINVAL;
     DeviceGuard g(h->device);
     if (!g.ok) return SIM_ECUDA;
     const size_t F = (size_t)h->n_facets, C = h->prm.n_channels;
