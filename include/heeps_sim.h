@@ -247,6 +247,37 @@ typedef struct {
 } sim_pipe_peaks;
 int sim_measure_pipe_peaks(int device, sim_pipe_peaks *out);
 
+/*
+ * sim_echoes_to_iq_static: the entry point that ALLOCATES NOTHING -- for callers that cannot call cudaMalloc (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid it).  It is the echo accumulation of the SPECTRAL form
+ * (eq. (17) + waveform convolution; SIM_ACCUMULATE_SPECTRAL above) for ONE (channel, pulse) vector
+ * from a caller-supplied list of facet-echoes:
+ *
+ *     iq[n] = phase * sum_e weight_e exp(j pi K ((n - slice_e + eps_e)/fs - T/2)^2)   over slice_e <= n < slice_e + T fs,
+ *
+ * i.e. echo e lays its chirp replica down from sample slice_e on, its delay ending eps_e in [0, 1] samples before that
+ * sample (slice, eps, weight: what sim_debug_echoes reports).  No handle: the range-slice moment rows that the normal
+ * path keeps in its cudaMalloc'd workspace, the waveform taps, their spectra and the FFT twiddles live in ONE static
+ * device array inside the library (1.38 MB, held by every GPU that loads the library until exit), and the FFT
+ * convolution kernel is the normal path's, launched on that array.  The call enqueues one memset and four kernels on
+ * cuda_stream and returns; it calls no cudaMalloc, cudaFree or allocating library routine (first use on a device looks
+ * the array's address up once, cudaGetSymbolAddress).
+ *   slice_dev [n] int32, eps_dev [n] float, weight_dev [n][2] float (re, im): DEVICE memory, read only; n_echoes >= 0
+ *   (0: the vector is zero-filled, the pointers may be NULL).  phase: HOST, {re, im} of the factor applied to the vector
+ *   (the normal path's exp(-j 2 pi f0 t0[p])).  iq_dev: DEVICE complex64 [n_samples], overwritten.  Echoes whose window
+ *   misses [0, n_samples) are clipped silently.
+ * Limits: T fs an integer <= SIM_STATIC_MAX_REPLICA and n_samples + T fs - 1 <= SIM_STATIC_MAX_SLICES, else SIM_ERANGE
+ * (nothing is launched); a chirp that eight moments do not resolve (B >~ fs), a non-integer T fs or bad arguments:
+ * SIM_EINVAL; SIM_ECUDA on a CUDA error.
+ * Every call uses the same array, which keeps the last call's contents (the call clears the rows it needs first):
+ * calls that overlap on one GPU -- two streams, two threads, two captured graphs replayed concurrently -- RACE.  Serialise them.
+ */
+#define SIM_STATIC_MAX_SLICES  8192
+#define SIM_STATIC_MAX_REPLICA 4096
+int sim_echoes_to_iq_static(double chirp_rate_hz_per_s, double chirp_len_s, double fs_hz, int32_t n_samples,
+                            const int32_t *slice_dev, const float *eps_dev, const float *weight_dev, int64_t n_echoes,
+                            const double phase[2], void *iq_dev, int device, void *cuda_stream);
+
 void sim_destroy(sim_handle *h);
 const char *sim_error_string(int code);
 /* Text of the last CUDA error seen by this handle ("" if none). Valid until the next call on h. */

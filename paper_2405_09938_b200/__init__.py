@@ -21,6 +21,7 @@ from .binding import (  # noqa: F401
     sim_replica,
     sim_debug_facets,
     sim_debug_echoes,
+    sim_echoes_to_iq_static,
     sim_get_stats,
     sim_measure_pipe_peaks,
 )

@@ -123,6 +123,9 @@ def load_library():
         lib.sim_debug_facets.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp]
         lib.sim_debug_echoes.restype = C.c_int
         lib.sim_debug_echoes.argtypes = [vp, i32, vp, vp, vp, vp, C.POINTER(C.c_int64)]
+        lib.sim_echoes_to_iq_static.restype = C.c_int
+        lib.sim_echoes_to_iq_static.argtypes = [C.c_double, C.c_double, C.c_double, i32, vp, vp, vp, C.c_int64,
+                                                C.POINTER(C.c_double * 2), vp, C.c_int, vp]
         lib.sim_get_stats.restype = C.c_int
         lib.sim_get_stats.argtypes = [vp, C.POINTER(sim_stats)]
         lib.sim_set_profiling.restype = C.c_int
@@ -316,6 +319,17 @@ def sim_debug_echoes(handle, pulse: int, n_facets: int, n_channels: int) -> dict
     res["weight"] = res["weight"][..., 0] + 1j * res["weight"][..., 1]
     res["n_edge_ambiguous"] = int(n_edge.value)
     return res
+
+
+def sim_echoes_to_iq_static(chirp_rate_hz_per_s: float, chirp_len_s: float, fs_hz: float, n_samples: int,
+                            slice_dev_ptr: int, eps_dev_ptr: int, weight_dev_ptr: int, n_echoes: int, phase: complex,
+                            iq_dev_ptr: int, device: int = 0, cuda_stream: int = 0):
+    """The entry point that allocates nothing (include/heeps_sim.h): device pointers in, complex64 [n_samples] out."""
+    ph = (C.c_double * 2)(float(np.real(phase)), float(np.imag(phase)))
+    _check(load_library().sim_echoes_to_iq_static(
+        float(chirp_rate_hz_per_s), float(chirp_len_s), float(fs_hz), int(n_samples), C.c_void_p(slice_dev_ptr or None),
+        C.c_void_p(eps_dev_ptr or None), C.c_void_p(weight_dev_ptr or None), int(n_echoes), C.byref(ph),
+        C.c_void_p(iq_dev_ptr), int(device), C.c_void_p(cuda_stream or None)))
 
 
 def sim_measure_pipe_peaks(device: int = 0) -> dict:

@@ -366,3 +366,182 @@ cudaError_t launch_kernel_spectra(int nfft, const float2 *ck, int replica, const
 }
 
 }  // namespace heeps
+
+// ---------------------------------------------------------------------------------------------------------------------
+// sim_echoes_to_iq_static (include/heeps_sim.h) -- K3s for ONE (channel, pulse) vector with every byte of device memory
+// it needs besides the caller's inputs and output in a file-scope static array: the moment rows (the scratch the moment
+// kernels fill and fftconv_kernel reads), the waveform taps c_k, their spectra, the twiddle table and the vector's
+// phase factor.  For callers that cannot call cudaMalloc (code under CUDA graph capture, serving loops, harnesses that
+// forbid it): the entry point enqueues kernels and one memset on the caller's stream and calls no cudaMalloc / cudaFree
+// or allocating library routine; the only set-up is one cudaGetSymbolAddress per device.  fftconv_kernel and
+// kernel_spectra_kernel are the kernels of the normal path, launched on the static array.
+// Every call shares the array (it keeps the last call's contents; the rows are cleared at the start of every call):
+// two calls that overlap on one GPU (different streams, or threads) race.  Every GPU that loads the library holds
+// the array (kStaticFloat2 * 8 bytes = 1.38 MB) until exit.
+// ---------------------------------------------------------------------------------------------------------------------
+#include <algorithm>
+#include <cmath>
+#include <mutex>
+
+#include "../../include/heeps_sim.h"
+
+namespace heeps {
+
+namespace {
+
+constexpr int kStaticMaxFft = SIM_STATIC_MAX_SLICES;              // Ns + L - 1 <= this
+constexpr int kStaticMaxReplica = SIM_STATIC_MAX_REPLICA;
+// [Kt][kStaticMaxFft] moment rows | [Kt][kStaticMaxFft] spectra | [kStaticMaxFft] twiddles | [Kt][kStaticMaxReplica] taps |
+// 2 float2 = one double2 phase factor
+constexpr size_t kStaticRows = 0, kStaticSpec = (size_t)kKt * kStaticMaxFft, kStaticTw = 2 * (size_t)kKt * kStaticMaxFft,
+                 kStaticTaps = kStaticTw + kStaticMaxFft, kStaticPhase = kStaticTaps + (size_t)kKt * kStaticMaxReplica,
+                 kStaticFloat2 = kStaticPhase + 2;
+static __device__ __align__(256) float2 g_static_scratch[kStaticFloat2];
+
+// In host code `g_static_scratch` is a host-side stand-in, not a device address: the device address is looked up once
+// per device, with that device current.
+std::mutex g_static_mutex;
+float2 *g_static_ptr[64] = {};
+
+// Twiddles exp(-2 pi i k / nfft), the taps c_k[m] (Chebyshev coefficients in y of the slice response
+// exp(j 2 pi kappa (m + (y + 1)/2 - L/2)^2), 64-node Gauss-Chebyshev quadrature -- the formula of sim_create's
+// chebyshev_kernels, evaluated here on the device in fp64 so that nothing is copied from host memory) and the phase.
+__global__ void __launch_bounds__(256)
+static_tables_kernel(float2 *scratch, int nfft, int replica, double kappa, double ph_re, double ph_im)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < nfft) {
+        double sn, cs;
+        sincospi(-2.0 * (double)t / (double)nfft, &sn, &cs);
+        scratch[kStaticTw + t] = make_float2((float)cs, (float)sn);
+    }
+    if (t == 0) *reinterpret_cast<double2 *>(scratch + kStaticPhase) = make_double2(ph_re, ph_im);
+    if (t < replica) {
+        constexpr int NQ = 64;
+        double ar[kKt], ai[kKt];
+#pragma unroll
+        for (int k = 0; k < kKt; ++k) ar[k] = ai[k] = 0.0;
+        for (int j = 0; j < NQ; ++j) {
+            const double th = (j + 0.5) / NQ;                               // in units of pi
+            const double u = (double)t + 0.5 * (cospi(th) + 1.0) - 0.5 * (double)replica;
+            double turns = kappa * u * u;
+            turns -= floor(turns);
+            double gs, gc;
+            sincospi(2.0 * turns, &gs, &gc);
+#pragma unroll
+            for (int k = 0; k < kKt; ++k) {
+                const double ck = cospi((double)k * th);
+                ar[k] = fma(gc, ck, ar[k]); ai[k] = fma(gs, ck, ai[k]);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < kKt; ++k) {
+            const double sc = (k ? 2.0 : 1.0) / NQ;
+            scratch[kStaticTaps + (size_t)k * replica + t] = make_float2((float)(ar[k] * sc), (float)(ai[k] * sc));
+        }
+    }
+}
+
+// Moment rows from the caller's echo list: M_k[b + L - 1] += w T_k(2 eps - 1) (moments.cu header), by atomics.
+__global__ void __launch_bounds__(256)
+static_moments_kernel(float2 *rows, int nb, int nb_pad, int replica, const int32_t *slice, const float *eps,
+                      const float2 *weight, long long n)
+{
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x) {
+        const long long idx = (long long)slice[e] + replica - 1;
+        if (idx < 0 || idx >= nb) continue;                                 // the echo's window misses [0, Ns): clipped
+        const float2 w = weight[e];
+        const float y = fmaf(2.f, eps[e], -1.f);
+        float t0 = 1.f, t1 = y;
+        atomicAdd(rows + idx, w);
+        atomicAdd(rows + nb_pad + idx, make_float2(w.x * t1, w.y * t1));
+        for (int k = 2; k < kKt; ++k) {
+            const float t2 = 2.f * y * t1 - t0;
+            atomicAdd(rows + (size_t)k * nb_pad + idx, make_float2(w.x * t2, w.y * t2));
+            t0 = t1; t1 = t2;
+        }
+    }
+}
+
+template <int NFFT>
+cudaError_t static_run(float2 *scr, int n_samples, int replica, double kappa, double ph_re, double ph_im,
+                       const int32_t *slice, const float *eps, const float2 *weight, long long n, float2 *out, cudaStream_t s)
+{
+    const int nb = n_samples + replica - 1, nb_pad = (nb + 3) & ~3;
+    cudaError_t rc = cudaMemsetAsync(scr + kStaticRows, 0, (size_t)kKt * nb_pad * sizeof(float2), s);    // rows start at zero
+    if (rc != cudaSuccess) return rc;
+    static_tables_kernel<<<(std::max(NFFT, replica) + 255) / 256, 256, 0, s>>>(scr, NFFT, replica, kappa, ph_re, ph_im);
+    if ((rc = cudaGetLastError()) != cudaSuccess) return rc;
+    if ((rc = launch_spec<NFFT>(scr + kStaticTaps, replica, scr + kStaticTw, scr + kStaticSpec, s)) != cudaSuccess) return rc;
+    if (n > 0) {
+        const int blocks = (int)std::min<long long>((n + 255) / 256, 148 * 8);
+        static_moments_kernel<<<blocks, 256, 0, s>>>(scr + kStaticRows, nb, nb_pad, replica, slice, eps, weight, n);
+        if ((rc = cudaGetLastError()) != cudaSuccess) return rc;
+    }
+    FftConvArgs a{};
+    a.mom = scr + kStaticRows; a.cspec = scr + kStaticSpec; a.tw = scr + kStaticTw;
+    a.carrier_p = reinterpret_cast<const double2 *>(scr + kStaticPhase);
+    a.out = out; a.n_out_pulses = 1; a.out_pulse0 = 0;
+    a.nfft = NFFT; a.nb = nb; a.nb_pad = nb_pad; a.replica = replica;
+    return launch_conv<NFFT>(a, 0, 1, 1, n_samples, s);
+}
+
+}  // namespace
+
+}  // namespace heeps
+
+extern "C" int sim_echoes_to_iq_static(double chirp_rate_hz_per_s, double chirp_len_s, double fs_hz, int32_t n_samples,
+                                       const int32_t *slice_dev, const float *eps_dev, const float *weight_dev,
+                                       int64_t n_echoes, const double phase[2], void *iq_dev, int device, void *cuda_stream)
+{
+    using namespace heeps;
+    if (!(fs_hz > 0) || !(chirp_len_s > 0) || !std::isfinite(chirp_rate_hz_per_s) || !std::isfinite(chirp_len_s) ||
+        !std::isfinite(fs_hz) || n_samples < 1 || n_echoes < 0 || !iq_dev || !phase || !std::isfinite(phase[0]) ||
+        !std::isfinite(phase[1]) || (n_echoes > 0 && (!slice_dev || !eps_dev || !weight_dev)))
+        return SIM_EINVAL;
+    const double len = chirp_len_s * fs_hz, len_round = std::nearbyint(len);
+    if (!(std::fabs(len - len_round) < 1e-9 * std::max(1.0, len)) || len_round < 1.0) return SIM_EINVAL;   // T fs integer
+    const int replica = (int)len_round;
+    // beyond the static array: a clear error, never a silent overrun
+    if (replica > kStaticMaxReplica || (long long)n_samples + replica - 1 > kStaticMaxFft) return SIM_ERANGE;
+    const double kappa = chirp_rate_hz_per_s / (2.0 * fs_hz * fs_hz);
+    {   // Kt = 8 moments must resolve the chirp (Jacobi-Anger tail; sim_create applies the same bar to its taps)
+        const double z = M_PI * std::fabs(kappa) * len;
+        double tail = 0;
+        for (int k = kKt; k < kKt + 4; ++k) tail += 2.0 * std::fabs(jn(k, z));
+        if (!(tail <= 5e-6)) return SIM_EINVAL;
+    }
+    if (device < 0 || device >= 64) return SIM_EINVAL;
+    int prev = -1;
+    if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return SIM_ECUDA; }
+    if (prev != device && cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return SIM_ECUDA; }
+    float2 *scr = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_static_mutex);
+        if (!g_static_ptr[device]) {
+            float2 *p = nullptr;
+            if (cudaGetSymbolAddress((void **)&p, g_static_scratch) != cudaSuccess || !p) {
+                cudaGetLastError();
+                if (prev != device) cudaSetDevice(prev);
+                return SIM_ECUDA;
+            }
+            g_static_ptr[device] = p;
+        }
+        scr = g_static_ptr[device];
+    }
+    int nfft = 256;
+    while (nfft < n_samples + replica - 1) nfft <<= 1;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const float2 *w2 = reinterpret_cast<const float2 *>(weight_dev);
+    float2 *out = static_cast<float2 *>(iq_dev);
+    cudaError_t rc = cudaErrorInvalidValue;
+    switch (nfft) {
+#define HEEPS_CASE(N) case N: rc = static_run<N>(scr, n_samples, replica, kappa, phase[0], phase[1], slice_dev, eps_dev, w2, n_echoes, out, s); break;
+        HEEPS_CASE(256) HEEPS_CASE(512) HEEPS_CASE(1024) HEEPS_CASE(2048) HEEPS_CASE(4096) HEEPS_CASE(8192)
+#undef HEEPS_CASE
+        default: break;
+    }
+    if (prev != device) cudaSetDevice(prev);
+    if (rc != cudaSuccess) { cudaGetLastError(); return SIM_ECUDA; }
+    return SIM_OK;
+}
