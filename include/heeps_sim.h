@@ -136,7 +136,10 @@ typedef struct {
     int32_t accumulate_mode;       /* SIM_ACCUMULATE_*; SPECTRAL where it does not apply -> SIM_EINVAL */
     int32_t kinematics_keyframe;   /* wave sums evaluated exactly every H-th pulse (with time derivatives) and
                                       cubic-Hermite interpolated between: 0 = auto (largest H <= 64 whose error
-                                      bound sum_w A_w (omega_w h)^4/384 <= 4e-8 m; slopes linear between, their error <= 1.2e-4), 1 = every pulse, n = force H = n */
+                                      bound sum_w A_w (omega_w h)^4/384 <= 4e-8 m; slopes linear between, their error <= 1.2e-4), 1 = every pulse, n = force H = n.
+                                      With the keyframed geometry (below), a linear surface and H chosen automatically the wave sums themselves
+                                      are evaluated only every 4 H-th (or 2 H-th) pulse, with second time derivatives, and the rows at spacing H
+                                      are their quintic (slopes: cubic) Hermite interpolants (bounds 1e-8 m, 1e-5) */
     int32_t geometry_keyframe;     /* SPECTRAL only: 0 = auto -- where kinematics keyframes are in use (H > 1), C <= 4, the
                                       receive offsets are small (|o_c| <= 4 m) and the pulse times inside every keyframe
                                       interval are uniform, ranges / gains are evaluated exactly at the keyframe pulses only
@@ -221,6 +224,8 @@ typedef struct {
     int32_t kinematics_keyframe;   /* H as resolved at sim_create                     */
     int32_t geometry_keyframed;    /* 1 when ranges / gains are interpolated between keyframes (sim_options) */
     int32_t fft_band_size;         /* SPECTRAL: band transform length (sim_options.fft_band), 0 = not in use */
+    int32_t kinematics_coarse_keyframe;   /* spacing at which the wave sums themselves are evaluated when it is a multiple of
+                                             kinematics_keyframe (decoupled keyframes, sim_options.kinematics_keyframe); else 0 */
 } sim_stats;
 int sim_get_stats(sim_handle *h, sim_stats *out);
 

@@ -85,7 +85,7 @@ class sim_stats(C.Structure):
         ("tile_facets", C.c_int32), ("pulses_per_batch", C.c_int32), ("n_tiles", C.c_int32),
         ("accumulate_block_threads", C.c_int32), ("max_span_samples", C.c_int32),
         ("accumulate_mode", C.c_int32), ("fft_size", C.c_int32), ("kinematics_keyframe", C.c_int32),
-        ("geometry_keyframed", C.c_int32), ("fft_band_size", C.c_int32),
+        ("geometry_keyframed", C.c_int32), ("fft_band_size", C.c_int32), ("kinematics_coarse_keyframe", C.c_int32),
     ]
 
 

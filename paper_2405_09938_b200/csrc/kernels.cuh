@@ -25,10 +25,24 @@ struct KinematicsArgs {
     double2 *dxy;           // [n_pl][F] or null    CWM horizontal displacement
     int32_t H;              // keyframe spacing in pulses (1 = every pulse)
     const double *omega;    // [Nw] (H > 1)
+    float *ztt;             // or null: second time derivative of the height [n_rows][F] (H > 1, no CWM), and with it
+    float2 *slope_t;        //          the time derivative of the slopes [n_rows][F] (when slope is given)
     double *zt;             // time derivatives (H > 1): [n_rows][F]
     double2 *dxy_t;         // or null
 };
 cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a, int first, int n_rows, cudaStream_t s);
+// K1b -- keyframe rows at spacing H interpolated from K1's coarse rows at spacing H1 (kinematics.cu).
+struct SurfaceRefineArgs {
+    const double *zc, *ztc;      // coarse rows [n_rows1][F]: height, its rate
+    const float *zttc;           //                            its second time derivative
+    const float2 *slopec, *slope_tc;   // or null: slopes and their rate
+    double *z, *zt;              // out [n_rows][F]
+    float2 *slope;               // out, or null
+    const PulseConst *pulses;    // pulse times
+    int64_t n_facets;
+    int32_t H, H1, first, n_rows, first1, n_pulses_total;   // output row r = keyframe first + r (spacing H); coarse row 0 = coarse keyframe first1
+};
+cudaError_t launch_surface_refine(const SurfaceRefineArgs &a, cudaStream_t s);
 cudaError_t launch_surface_slope(const DevParams &prm, const SurfaceArgs &sa, const PulseConst *pulses, int p,
                                  float2 *out, cudaStream_t s);
 

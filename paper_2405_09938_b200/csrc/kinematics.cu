@@ -21,6 +21,9 @@
 //
 // Keyframes (surface.cuh): with H > 1 the kernel runs only at the keyframe pulses min(j H, P-1) and also
 // writes the time derivatives (d/dt of A cos(psi) is A omega sin(psi)), from which K2 interpolates.
+// Decoupled keyframes (sim_api.cu choose_coarse_spacing): for the keyframed geometry kernel the wave sums are evaluated at
+// a multiple of its spacing, with second time derivatives (kRate2), and surface_refine_kernel (K1b) below writes the
+// rows at its spacing from them by quintic / cubic Hermite interpolation.
 #include <algorithm>
 #include <type_traits>
 
@@ -38,7 +41,10 @@ constexpr int kNF = 2;        // facets per thread (same i, rows kBY apart): the
 // square of the weight of eq. (2), in the paper's expanded form: w_x = |x^i - x|/L, w_y = |y^i - y|/L
 __device__ __forceinline__ double weight2(double wx, double wy) { return __dadd_rn(__dadd_rn(1.0 - wx, -wy), __dmul_rn(wx, wy)); }
 
-template <int NK, bool kSlope, bool kChoppy, bool kRate, bool kHetero>
+// kRate2 (with kRate): also the SECOND time derivative of the height and the rate of the slopes -- the keyframe rows of
+// the decoupled scheme (sim_api.cu: K1 at R x the spacing of the geometry kernel; quintic Hermite for the height, cubic
+// Hermite for the slopes between them).
+template <int NK, bool kSlope, bool kChoppy, bool kRate, bool kHetero, bool kRate2 = false>
 __global__ void __launch_bounds__(kBX * kBY)
 kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
 {
@@ -99,12 +105,16 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
     double z[kNF][NK], dx[kNF][NK], dy[kNF][NK];
     float zt[kNF][NK], dxt[kNF][NK], dyt[kNF][NK];
     float2 sxy[kNF][NK];
+    constexpr int NK2 = kRate2 ? NK : 1;
+    float ztt[kNF][NK2];
+    float2 sxyt[kNF][NK2];
 #pragma unroll
     for (int u = 0; u < kNF; ++u)
 #pragma unroll
         for (int k = 0; k < NK; ++k) {
             z[u][k] = dx[u][k] = dy[u][k] = 0.0;
             zt[u][k] = dxt[u][k] = dyt[u][k] = 0.f; sxy[u][k] = make_float2(0.f, 0.f);
+            if (kRate2) { ztt[u][k] = 0.f; sxyt[u][k] = make_float2(0.f, 0.f); }
         }
 
     for (int corner = 0; corner < (hetero ? 4 : 1); ++corner) {
@@ -177,9 +187,14 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
                         const float imf = fmaf(cfr[u], tf.y, cfi[u] * tf.x);
                         if (kRate) zt[u][k] = fmaf(om, imf, zt[u][k]);    // d/dt A cos(psi) = A omega sin(psi)
                         if (kSlope) sxy[u][k] = __ffma2_rn(nk2, make_float2(imf, imf), sxy[u][k]);   // grad z = -sum A k sin(psi)
-                        if (kChoppy && kRate) {
+                        if ((kChoppy || kRate2) && kRate) {
                             const float wre = om * fmaf(cfr[u], tf.x, -cfi[u] * tf.y);   // omega A cos(psi)
-                            dxt[u][k] = fmaf(k4.z, wre, dxt[u][k]); dyt[u][k] = fmaf(k4.w, wre, dyt[u][k]);
+                            if (kChoppy) { dxt[u][k] = fmaf(k4.z, wre, dxt[u][k]); dyt[u][k] = fmaf(k4.w, wre, dyt[u][k]); }
+                            if (kRate2) {
+                                ztt[u][kRate2 ? k : 0] = fmaf(-om, wre, ztt[u][kRate2 ? k : 0]);      // d2/dt2 A cos(psi) = -A omega^2 cos(psi)
+                                // d/dt grad z = d/dt (-A k sin(psi)) = A k omega cos(psi)   (psi = ... - omega t)
+                                if (kSlope) sxyt[u][kRate2 ? k : 0] = __ffma2_rn(make_float2(k4.x, k4.y), make_float2(wre, wre), sxyt[u][kRate2 ? k : 0]);
+                            }
                         }
                     }
                 }
@@ -199,10 +214,61 @@ kinematics_kernel(DevParams prm, KinematicsArgs a, int first, int n_rows)
             a.z[f] = z[u][k];
             if (kSlope) a.slope[f] = sxy[u][k];
             if (kChoppy) a.dxy[f] = make_double2(dx[u][k], dy[u][k]);
+            if (kRate2) {
+                a.ztt[f] = ztt[u][kRate2 ? k : 0];
+                if (kSlope) a.slope_t[f] = sxyt[u][kRate2 ? k : 0];
+            }
             if (kRate) {
                 a.zt[f] = (double)zt[u][k];
                 if (kChoppy) a.dxy_t[f] = make_double2((double)dxt[u][k], (double)dyt[u][k]);
             }
+        }
+    }
+}
+
+// K1b -- keyframe rows at spacing H from K1's coarse rows at spacing H1 = R H (decoupled keyframes, sim_api.cu
+// choose_coarse_spacing): height and its rate by the QUINTIC Hermite interpolant of (z, dz/dt, d2z/dt2) at the two coarse
+// keyframes around, slopes by the cubic Hermite of (slope, its rate).  One thread per facet walks the output rows and
+// keeps the two coarse rows in registers; HBM-bound: 36 B read per facet and coarse row, 24 B written per output row.
+__global__ void __launch_bounds__(256)
+surface_refine_kernel(SurfaceRefineArgs a)
+{
+    const size_t F = a.n_facets;
+    const size_t f = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= F) return;
+    const int P = a.n_pulses_total, H = a.H, H1 = a.H1;
+    const int n_keys1 = (P - 1 + H1 - 1) / H1 + 1;
+    int m_cur = -1;
+    double z0 = 0, v0 = 0, a0 = 0, z1 = 0, v1 = 0, a1 = 0, t0 = 0, hh = 1;
+    float2 s0 = make_float2(0.f, 0.f), r0 = s0, s1 = s0, r1 = s0;
+    for (int r = 0; r < a.n_rows; ++r) {
+        const int k = min((a.first + r) * H, P - 1);                       // pulse of output row r
+        const int m = min(k / H1, n_keys1 - 2);
+        if (m != m_cur) {
+            const size_t c0 = (size_t)(m - a.first1) * F + f, c1 = c0 + F;
+            if (m == m_cur + 1 && m_cur >= 0) { z0 = z1; v0 = v1; a0 = a1; s0 = s1; r0 = r1; }
+            else { z0 = a.zc[c0]; v0 = a.ztc[c0]; a0 = (double)a.zttc[c0]; if (a.slopec) { s0 = a.slopec[c0]; r0 = a.slope_tc[c0]; } }
+            z1 = a.zc[c1]; v1 = a.ztc[c1]; a1 = (double)a.zttc[c1];
+            if (a.slopec) { s1 = a.slopec[c1]; r1 = a.slope_tc[c1]; }
+            const int q0 = min(m * H1, P - 1), q1 = min((m + 1) * H1, P - 1);
+            t0 = a.pulses[q0].t; hh = a.pulses[q1].t - t0;
+            m_cur = m;
+        }
+        const double x = (a.pulses[k].t - t0) / hh, x2 = x * x, x3 = x2 * x, x4 = x3 * x, x5 = x4 * x;
+        const double w0 = 1.0 - 10.0 * x3 + 15.0 * x4 - 6.0 * x5, w5 = 10.0 * x3 - 15.0 * x4 + 6.0 * x5;
+        const double w1 = (x - 6.0 * x3 + 8.0 * x4 - 3.0 * x5) * hh, w4 = (-4.0 * x3 + 7.0 * x4 - 3.0 * x5) * hh;
+        const double w2 = 0.5 * (x2 - 3.0 * x3 + 3.0 * x4 - x5) * hh * hh, w3 = 0.5 * (x3 - 2.0 * x4 + x5) * hh * hh;
+        const double d0 = (-30.0 * x2 + 60.0 * x3 - 30.0 * x4) / hh, d5 = -d0;
+        const double d1 = 1.0 - 18.0 * x2 + 32.0 * x3 - 15.0 * x4, d4 = -12.0 * x2 + 28.0 * x3 - 15.0 * x4;
+        const double d2 = 0.5 * (2.0 * x - 9.0 * x2 + 12.0 * x3 - 5.0 * x4) * hh, d3 = 0.5 * (3.0 * x2 - 8.0 * x3 + 5.0 * x4) * hh;
+        const size_t o = (size_t)r * F + f;
+        a.z[o] = fma(w0, z0, fma(w5, z1, fma(w1, v0, fma(w4, v1, fma(w2, a0, w3 * a1)))));
+        a.zt[o] = fma(d0, z0, fma(d5, z1, fma(d1, v0, fma(d4, v1, fma(d2, a0, d3 * a1)))));
+        if (a.slope) {
+            const float g0 = (float)(2.0 * x3 - 3.0 * x2 + 1.0), g1 = (float)((x3 - 2.0 * x2 + x) * hh),
+                        g2 = (float)((x3 - x2) * hh), g3 = (float)(-2.0 * x3 + 3.0 * x2);
+            a.slope[o] = make_float2(fmaf(g0, s0.x, fmaf(g1, r0.x, fmaf(g2, r1.x, g3 * s1.x))),
+                                     fmaf(g0, s0.y, fmaf(g1, r0.y, fmaf(g2, r1.y, g3 * s1.y))));
         }
     }
 }
@@ -219,6 +285,13 @@ surface_slope_kernel(DevParams prm, SurfaceArgs sa, const PulseConst *pulses, in
 }
 
 }  // namespace
+
+cudaError_t launch_surface_refine(const SurfaceRefineArgs &a, cudaStream_t s)
+{
+    if (a.n_rows <= 0) return cudaSuccess;
+    surface_refine_kernel<<<(unsigned)((a.n_facets + 255) / 256), 256, 0, s>>>(a);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_surface_slope(const DevParams &prm, const SurfaceArgs &sa, const PulseConst *pulses, int p,
                                  float2 *out, cudaStream_t s)
@@ -244,6 +317,18 @@ cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a_in, 
     }
     const bool slope = a.slope != nullptr, choppy = a.dxy != nullptr, rate = a.H > 1;
     auto launch = [&](auto kern) { kern<<<grid, block, 0, s>>>(prm, a, first, n_rows); };
+    if (a.ztt) {                                       // second-derivative rows: 4 rows per block (register budget), no CWM
+        if (!rate || choppy || (slope && !a.slope_t)) return cudaErrorInvalidValue;
+        grid.z = (n_rows + 3) / 4;
+        if (a.nodes_x > 0) {
+            if (slope) launch(kinematics_kernel<4, true, false, true, true, true>);
+            else       launch(kinematics_kernel<4, false, false, true, true, true>);
+        } else {
+            if (slope) launch(kinematics_kernel<4, true, false, true, false, true>);
+            else       launch(kinematics_kernel<4, false, false, true, false, true>);
+        }
+        return cudaGetLastError();
+    }
     auto pick2 = [&](auto nk_tag, auto het_tag) {
         constexpr int NK = decltype(nk_tag)::value;
         constexpr bool HET = decltype(het_tag)::value;

@@ -200,6 +200,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     __shared__ int s_nstray[3];
     __shared__ int s_blo[kMaxKeyChannels], s_bhi[kMaxKeyChannels];   // slices this tile touches during the interval
     __shared__ int s_dlamax;                                     // max |a - a_tile| + |a(t1) - a(t0)| over the tile, as float bits
+    __shared__ int s_nitems;
 
     const int span = a.span_cap, hstride = span + 1;
     const int cap = prm.k2k_cap;
@@ -211,6 +212,9 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     uint32_t *slots = reinterpret_cast<uint32_t *>(smem_raw + (size_t)2 * capT * 12);
     int *hist = reinterpret_cast<int *>(smem_raw + (size_t)2 * capT * 12 + (size_t)C * cap * 4);
     float2 *scratch = reinterpret_cast<float2 *>(smem_raw + (size_t)2 * capT * 12 + (size_t)C * cap * 4 + (size_t)hist_words(C, span) * 4);
+    // work list of stage C, written at every sort: one item per slice of [smin, smax) of every channel, channels end to end:
+    // {first slot | echoes << 13 (0: empty, or outside the sampling window), channel | moment-row index << 2}
+    uint2 *items = reinterpret_cast<uint2 *>(scratch + (kThreads / 8) * kScrTeam);
     const uint32_t no_slot = (0x7ffffu << 13) | (uint32_t)(C * cap);      // slice 0x7ffff (never matches), store target = the spare slot
 
     const int tile = blockIdx.x, j = j_first + blockIdx.y;
@@ -227,7 +231,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         double *d0 = reinterpret_cast<double *>(&pc2[0]), *d1 = reinterpret_cast<double *>(&pc2[1]);
         for (int k = tid; k < (int)(sizeof(PulseConst) / sizeof(double)); k += NT) { d0[k] = s0[k]; d1[k] = s1[k]; }
     }
-    if (tid == 0) { s_kept = 0; s_nstray[0] = s_nstray[1] = s_nstray[2] = 0; s_dlamax = 0; }
+    if (tid == 0) { s_kept = 0; s_nstray[0] = s_nstray[1] = s_nstray[2] = 0; s_dlamax = 0; s_nitems = 0; }
     if (tid < kMaxKeyChannels) { s_blo[tid] = 0x7fffffff; s_bhi[tid] = (int)0x80000000; }
     for (int k = tid; k < C * hstride; k += NT) hist[k] = 0;
     __syncthreads();
@@ -545,6 +549,29 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                 }
             }
             __syncthreads();
+            {
+                int pre[C + 1];                                            // first item of channel c
+                pre[0] = 0;
+#pragma unroll
+                for (int c = 0; c < C; ++c) pre[c + 1] = pre[c] + max(s_rng[c][1] - s_rng[c][0], 0);
+                const int total = pre[C];
+                if (tid == 0) s_nitems = total;
+                for (int it = tid; it < total; it += NT) {
+                    int c = 0;
+#pragma unroll
+                    for (int cc = 1; cc < C; ++cc) c = (it >= pre[cc]) ? cc : c;
+                    int pc0 = 0, bc = bref[0];
+#pragma unroll
+                    for (int cc = 1; cc < C; ++cc) { pc0 = (c == cc) ? pre[cc] : pc0; bc = (c == cc) ? bref[cc] : bc; }
+                    const int sidx = s_rng[c][0] + (it - pc0);
+                    const int first = hs[c * hstride + sidx];
+                    int cnt = hs[c * hstride + sidx + 1] - first;
+                    const int jb = bc + sidx + L - 1;                      // slice b = bref + sidx sits at row index b + L - 1
+                    if ((unsigned)jb >= win_hi) cnt = 0;                   // a slice outside the sampling window holds zeros only
+                    HEEPS_CHECK(cnt == 0 || (first >= 0 && first + cnt <= cap && jb < a.nb_pad));
+                    items[it] = make_uint2((uint32_t)(c * cap + first) | ((uint32_t)cnt << 13), (uint32_t)c | ((uint32_t)max(jb, 0) << 2));
+                }
+            }
 #pragma unroll
             for (int q = 0; q < FPT; ++q)
 #pragma unroll
@@ -702,28 +729,17 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         //      negation: a_{k+1} = -+ 2y a_k + a_{k-1} (minus for odd k); sigma_k is applied to the slice sum.
         //      Work items = the occupied slices of all C channels laid end to end.
         {
-            int pre[C + 1];                                                // first item of channel c
-            pre[0] = 0;
-#pragma unroll
-            for (int c = 0; c < C; ++c) pre[c + 1] = pre[c] + max(s_rng[c][1] - s_rng[c][0], 0);
-            const int total = pre[C];
+            const int total = s_nitems;
+            // moment row `sub` of this pulse, channel 0 (the channel adds c n_pl Kt rows)
+            float2 *const row0 = a.mom + ((size_t)pl * kKt + sub) * a.nb_pad;
+            const size_t cstride = (size_t)n_pl * kKt * a.nb_pad;
             for (int it0 = 0; it0 < total; it0 += kThreads / 8) {
                 if (it0 + warp * 4 >= total) break;                        // warp-uniform
                 const int it = it0 + team;
-                int c = 0;
-#pragma unroll
-                for (int cc = 1; cc < C; ++cc) c = (it >= pre[cc]) ? cc : c;
-                int pc0 = 0, bc = K2[0];
-#pragma unroll
-                for (int cc = 1; cc < C; ++cc) { pc0 = (c == cc) ? pre[cc] : pc0; bc = (c == cc) ? K2[cc] : bc; }
-                const int sidx = s_rng[c][0] + (it - pc0);
-                const int *hc = hs + c * hstride;
-                int first = 0, cnt = 0;
-                if (it < total) { first = hc[sidx]; cnt = hc[sidx + 1] - first; }
-                const int b = bc + 1 - kRhoBias + sidx;                    // K2 = bref + kRhoBias - 1
-                if ((unsigned)(b + L - 1) >= win_hi) cnt = 0;              // a slice outside the sampling window holds zeros only
-                const float2 *payc = pay + c * cap + first;
-                const float *payc_y = pay_y + c * cap + first;
+                const uint2 item = (it < total) ? items[it] : make_uint2(0u, 0u);
+                const int cnt = (int)(item.x >> 13), c = (int)(item.y & 3u), jb = (int)(item.y >> 2);
+                const float2 *payc = pay + (item.x & 8191u);
+                const float *payc_y = pay_y + (item.x & 8191u);
                 f32x2 m[kKt];
 #pragma unroll
                 for (int k = 0; k < kKt; ++k) m[k] = 0ull;
@@ -754,23 +770,30 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                 for (int r = 1; r < 8; ++r) hsum = fadd2(hsum, scr64[r * kScrRow + sub]);
                 __syncwarp();
                 float2 h1 = *reinterpret_cast<float2 *>(&hsum);
-                HEEPS_CHECK(cnt == 0 || (first >= 0 && first + cnt <= cap && b + L - 1 >= 0 && b + L - 1 < a.nb_pad));
                 if (cnt > 0) {
                     if (sub & 2) { h1.x = -h1.x; h1.y = -h1.y; }
-                    float2 *row = a.mom + ((size_t)(c * n_pl + pl) * kKt + sub) * a.nb_pad;
-                    atomicAdd(row + (b + L - 1), h1);
+                    atomicAdd(row0 + (size_t)c * cstride + jb, h1);
                 }
             }
         }
-        // ---- the strays of this pulse: thread t takes moment t & 7 of stray t >> 3 ----
-        for (int t = tid; t < ns * kKt; t += NT) {
-            const float4 e = s_stray[buf][t >> 3];
-            const int k = t & 7, code = __float_as_int(e.w), c = code >> 28, jb = code & 0x0fffffff;
+        // ---- the strays of this pulse: one thread per stray, its eight moments (8 threads per stray made all 8 warps walk
+        //      the loop: 5 % of the kernel's instructions) ----
+        if (tid < ns) {
+            const float4 e = s_stray[buf][tid];
+            const int code = __float_as_int(e.w), c = code >> 28, jb = code & 0x0fffffff;
+            float2 *row = a.mom + ((size_t)(c * n_pl + pl) * kKt) * a.nb_pad + jb;
+            const float y2 = e.z + e.z;
             float t0 = 1.f, t1 = e.z;
-            for (int kk = 1; kk < k; ++kk) { const float t2 = 2.f * e.z * t1 - t0; t0 = t1; t1 = t2; }
-            const float tk = k ? t1 : 1.f;
-            atomicAdd(a.mom + ((size_t)(c * n_pl + pl) * kKt + k) * a.nb_pad + jb, make_float2(e.x * tk, e.y * tk));
-            if (k == 0) { const int b = jb - (L - 1); atomicMin(&s_blo[c], b); atomicMax(&s_bhi[c], b + 1); }
+            atomicAdd(row, make_float2(e.x, e.y));
+            atomicAdd(row + a.nb_pad, make_float2(e.x * t1, e.y * t1));
+#pragma unroll
+            for (int k = 2; k < kKt; ++k) {
+                const float t2 = fmaf(y2, t1, -t0);
+                atomicAdd(row + (size_t)k * a.nb_pad, make_float2(e.x * t2, e.y * t2));
+                t0 = t1; t1 = t2;
+            }
+            const int b = jb - (L - 1);
+            atomicMin(&s_blo[c], b); atomicMax(&s_bhi[c], b + 1);
         }
         // ---- advance the path of every facet to the next pulse (forward differences) ----
 #pragma unroll
@@ -856,7 +879,7 @@ size_t moments_keyframed_smem_bytes(const DevParams &prm, int span_cap)
 {
     const size_t C = prm.n_channels;
     return (size_t)2 * (C * prm.k2k_cap + 2) * 12 + C * prm.k2k_cap * 4 + (size_t)hist_words((int)C, span_cap) * 4 +
-           (size_t)(kThreads / 8) * kScrTeam * sizeof(float2);
+           (size_t)(kThreads / 8) * kScrTeam * sizeof(float2) + C * (size_t)(span_cap + 1) * sizeof(uint2);
 }
 
 cudaError_t launch_moments_keyframed(const DevParams &prm, const MomentArgs &a, int p0, int n_pl, cudaStream_t s)

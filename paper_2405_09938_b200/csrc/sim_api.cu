@@ -80,6 +80,10 @@ struct sim_handle {
     DevBuf<float2> slope, slope_t;
     DevBuf<double2> dxy, dxy_t;
     int key_H = 1;                       // keyframe spacing of the kinematics (1 = every pulse)
+    int key_H1 = 0;                      // > 0: K1 runs at this coarser spacing (a multiple of key_H) for the keyframed geometry kernel
+    DevBuf<double> zc, ztc;              // K1's coarse keyframe rows (spacing key_H1): height, rate,
+    DevBuf<float> zttc;                  //   second time derivative,
+    DevBuf<float2> slopec, slope_tc;     //   slopes and their rate
     int nodes_x = 0, nodes_y = 0;        // heterogeneous surface: node lattice of the wave tables (0 = homogeneous)
     double node_spacing = 0;
     bool geo_keyframed = false;          // spectral path: ranges / gains interpolated between keyframes (K2k)
@@ -382,9 +386,9 @@ ShearPlan plan_sheared_tiles(const sim_geometry *g, const sim_scene *sc, double 
 }
 
 // Rows of the surface buffers a batch [p0, p0 + n_pl) needs: its pulses (H = 1) or its keyframes.
-void surface_rows(const sim_handle *h, int p0, int n_pl, int *first, int *rows)
+void surface_rows(const sim_handle *h, int p0, int n_pl, int *first, int *rows, int spacing = 0)
 {
-    const int H = h->key_H, P = h->n_pulses;
+    const int H = spacing > 0 ? spacing : h->key_H, P = h->n_pulses;
     if (H <= 1) { *first = p0; *rows = n_pl; return; }
     const int n_keys = (P - 1 + H - 1) / H + 1;
     const int j0 = std::min(p0 / H, n_keys - 2), j1 = std::min((p0 + n_pl - 1) / H, n_keys - 2) + 1;
@@ -413,7 +417,9 @@ int run_speckle(sim_handle *h, int p0, int n_pl, cudaStream_t s, const uint2 **p
 }
 
 // K1 for the batch; fills `sa` for K2.
-int run_kinematics(sim_handle *h, const SurfBufs &b, int p0, int n_pl, cudaStream_t s, SurfaceArgs *sa)
+// `coarse`: K1 runs at the coarser spacing key_H1 (with second derivatives) into the coarse buffers and K1b interpolates
+// the rows at spacing key_H from them; what the geometry kernel sees is the same either way.
+int run_kinematics(sim_handle *h, const SurfBufs &b, int p0, int n_pl, cudaStream_t s, SurfaceArgs *sa, bool coarse = false)
 {
     int first = 0, rows = 0;
     surface_rows(h, p0, n_pl, &first, &rows);
@@ -422,8 +428,23 @@ int run_kinematics(sim_handle *h, const SurfBufs &b, int p0, int n_pl, cudaStrea
     ka.nodes_x = h->nodes_x; ka.nodes_y = h->nodes_y; ka.node_spacing = h->node_spacing;
     ka.z = b.z; ka.slope = b.slope; ka.dxy = b.dxy;
     ka.H = h->key_H; ka.omega = h->omega.p; ka.zt = b.zt; ka.dxy_t = b.dxy_t;
-    cudaError_t e = launch_kinematics(h->prm, ka, first, rows, s);
-    if (e != cudaSuccess) return fail_cuda(h, e, "launch_kinematics");
+    if (coarse) {
+        int first1 = 0, rows1 = 0;
+        surface_rows(h, p0, n_pl, &first1, &rows1, h->key_H1);
+        ka.z = h->zc.p; ka.zt = h->ztc.p; ka.ztt = h->zttc.p; ka.H = h->key_H1;
+        ka.slope = b.slope ? h->slopec.p : nullptr; ka.slope_t = b.slope ? h->slope_tc.p : nullptr;
+        cudaError_t e = launch_kinematics(h->prm, ka, first1, rows1, s);
+        if (e != cudaSuccess) return fail_cuda(h, e, "launch_kinematics (coarse)");
+        SurfaceRefineArgs ra{};
+        ra.zc = h->zc.p; ra.ztc = h->ztc.p; ra.zttc = h->zttc.p; ra.slopec = ka.slope; ra.slope_tc = ka.slope_t;
+        ra.z = b.z; ra.zt = b.zt; ra.slope = b.slope; ra.pulses = h->pulses.p; ra.n_facets = h->n_facets;
+        ra.H = h->key_H; ra.H1 = h->key_H1; ra.first = first; ra.n_rows = rows; ra.first1 = first1; ra.n_pulses_total = h->n_pulses;
+        e = launch_surface_refine(ra, s);
+        if (e != cudaSuccess) return fail_cuda(h, e, "launch_surface_refine");
+    } else {
+        cudaError_t e = launch_kinematics(h->prm, ka, first, rows, s);
+        if (e != cudaSuccess) return fail_cuda(h, e, "launch_kinematics");
+    }
     sa->z = b.z; sa->zt = b.zt; sa->slope = b.slope; sa->slope_t = nullptr; sa->dxy = b.dxy; sa->dxy_t = b.dxy_t;
     sa->H = h->key_H; sa->key0 = first; sa->n_pulses_total = h->n_pulses;
     return SIM_OK;
@@ -436,6 +457,44 @@ int run_kinematics(sim_handle *h, const SurfBufs &b, int p0, int n_pl, cudaStrea
 // slopes only scale sigma0: measured 1.8e-5 of relative L2 on the Large configuration at H = 32); 1 when pulse times are
 // not increasing.
 constexpr double kKeyframeHeightTol = 4e-8, kKeyframeSlopeTol = 1.2e-4;
+
+// Decoupled keyframes.  The geometry kernel needs the surface only at ITS keyframes (spacing H, bounded by its cubic path
+// interpolant); K1 -- 15 % of a step at that spacing -- can run at a multiple R H of it when it also stores the second
+// time derivative of the height and the rate of the slopes: between K1's keyframes the height is the QUINTIC Hermite
+// interpolant (error <= sum_w A_w (omega_w h)^6 / 46080), its rate the derivative of that (error <= sum_w A_w omega_w
+// (omega_w h)^5 / 1920, times the interval of the geometry kernel as a path error), the slopes the cubic one
+// (<= sum_w A_w |k_w| (omega_w h)^4 / 384).  Largest R in {4, 2} within a quarter of the height bound (the geometry
+// kernel's own cubic adds its part) and kCoarseSlopeTol on the slopes (they only scale sigma0; the linear interpolation
+// between the geometry kernel's keyframes that follows is allowed kKeyframeSlopeTol = 1.2e-4); 0 = keep one spacing.
+constexpr double kCoarseSlopeTol = 1e-5;
+int choose_coarse_spacing(const sim_geometry *g, const sim_scene *sc, int H)
+{
+    const int P = g->n_pulses;
+    const WaveView wv = wave_view(sc);
+    for (int R = 4; R >= 2; R >>= 1) {
+        const int H1 = R * H;
+        if (H1 > P - 1) continue;
+        double hmax = 0, hk = 0;
+        for (int k = 0; k < P - 1; k += H1) hmax = std::max(hmax, g->t_pulse_s[std::min(k + H1, P - 1)] - g->t_pulse_s[k]);
+        for (int k = 0; k < P - 1; k += H) hk = std::max(hk, g->t_pulse_s[std::min(k + H, P - 1)] - g->t_pulse_s[k]);
+        double bz = 0, bv = 0, bs = 0;
+        for (int n = 0; n < wv.n_nodes; ++n) {
+            double z1 = 0, v1 = 0, s1 = 0;
+            for (int w = 0; w < wv.n_waves; ++w) {
+                const size_t k = (size_t)n * wv.n_waves + w;
+                const double x = wv.omega[k] * hmax, a = std::fabs(wv.amp[k]);
+                z1 += a * std::pow(x, 6) / 46080.0;
+                v1 += a * wv.omega[k] * std::pow(x, 5) / 1920.0;
+                s1 += a * std::hypot(wv.kx[k], wv.ky[k]) * std::pow(x, 4) / 384.0;
+            }
+            bz = std::max(bz, z1); bv = std::max(bv, v1); bs = std::max(bs, s1);
+        }
+        if (wv.hetero) { bz *= 2.0; bv *= 2.0; bs *= 2.0; }
+        if (bz + 0.125 * hk * bv <= 0.25 * kKeyframeHeightTol && (!sc->tilt_modulation || bs <= kCoarseSlopeTol)) return H1;
+    }
+    return 0;
+}
+
 int choose_keyframe_spacing(const sim_geometry *g, const sim_scene *sc, int requested)
 {
     const int P = g->n_pulses;
@@ -777,7 +836,7 @@ void sim_destroy(sim_handle *h)
     h->pattern[0].release(); h->pattern[1].release();
     h->xi_state.release(); h->beta_g.release(); h->doppler_turns.release(); h->xi_t.release();
     h->z.release(); h->slope.release(); h->slope_t.release(); h->dxy.release();
-    h->zt.release(); h->dxy_t.release(); h->omega.release(); h->recs.release(); h->tinfo.release();
+    h->zt.release(); h->zc.release(); h->ztc.release(); h->zttc.release(); h->slopec.release(); h->slope_tc.release(); h->dxy_t.release(); h->omega.release(); h->recs.release(); h->tinfo.release();
     h->tspan.release(); h->acc.release(); h->counters.release(); h->out_staging.release();
     h->mom.release(); h->cspec.release(); h->tw.release(); h->cspec2.release(); h->tw2.release(); h->band.release();
     delete h;
@@ -952,6 +1011,8 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
             }
         }
     }
+    if (h->geo_keyframed && !prm.choppy && !(opts && opts->kinematics_keyframe > 1))
+        h->key_H1 = choose_coarse_spacing(g, sc, h->key_H);
     // ---- batch size ----
     const int64_t fcap = (int64_t)prm.n_tiles * prm.tile_cap;
     const int64_t surf_row = h->n_facets * 8 + (h->need_slope ? h->n_facets * 8 : 0) +
@@ -1123,6 +1184,11 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
             CKC(h->zt.alloc(F * rows));
             if (prm.choppy) CKC(h->dxy_t.alloc(F * rows));
         }
+        if (h->key_H1 > 0) {
+            const size_t rows1 = (size_t)(pb / h->key_H1 + 3);
+            CKC(h->zc.alloc(F * rows1)); CKC(h->ztc.alloc(F * rows1)); CKC(h->zttc.alloc(F * rows1));
+            if (h->need_slope) { CKC(h->slopec.alloc(F * rows1)); CKC(h->slope_tc.alloc(F * rows1)); }
+        }
         CKC(h->omega.alloc(std::max<size_t>(NQ, 1)));
         if (NQ) CKC(cudaMemcpy(h->omega.p, wv.omega, NQ * sizeof(double), cudaMemcpyHostToDevice));
     }
@@ -1192,6 +1258,7 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     h->stats.kinematics_keyframe = h->key_H;
     h->stats.geometry_keyframed = h->geo_keyframed ? 1 : 0;
     h->stats.fft_band_size = h->spectral ? h->nfft2 : 0;
+    h->stats.kinematics_coarse_keyframe = (h->geo_keyframed && h->key_H1 > 0) ? h->key_H1 : 0;
     *out = h;
     return SIM_OK;
 }
@@ -1252,7 +1319,7 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         CK(h, cudaEventRecord(h->ev_join, h->aux_stream));
         CK(h, mark());
         MomentArgs ma{};
-        { int rc = run_kinematics(h, bufs, p0, n_pl, s, &ma.surf); if (rc != SIM_OK) return rc; }
+        { int rc = run_kinematics(h, bufs, p0, n_pl, s, &ma.surf, h->geo_keyframed && h->key_H1 > 0); if (rc != SIM_OK) return rc; }
         CK(h, mark());
         ma.pulses = h->pulses.p;
         ma.sigma0 = h->sigma0.p; ma.current = h->current.p;
@@ -1282,7 +1349,7 @@ static int run_batches(sim_handle *h, int32_t pb0, int32_t pb1, float2 *out, cud
         CK(h, mark());
         CK(h, mark());                                   // K4 slot: finalize is fused into K3s
         CK(h, ship(p0, n_pl));
-        launches += 3 + (h->speckle_ar1 ? 1 : 0) + (h->nfft2 ? 1 : 0);
+        launches += 3 + (h->speckle_ar1 ? 1 : 0) + (h->nfft2 ? 1 : 0) + ((h->geo_keyframed && h->key_H1 > 0) ? 1 : 0);
     }
     for (int p0 = pb0; !h->spectral && p0 < pb1; p0 += batch) {
         const int n_pl = std::min(batch, pb1 - p0);

@@ -111,6 +111,28 @@ def test_kinematics_keyframes(mode):
     assert np.max(np.abs(g["pos"] - o["pos"])) < 3e-9              # interpolated height against the exact one
 
 
+def test_decoupled_kinematics_keyframes():
+    """Default path on a dwell long enough for the decoupled keyframes: the wave sums are evaluated every 128th pulse with
+    second derivatives (K1, kRate2), the rows at the geometry kernel's spacing 32 are their quintic / cubic Hermite
+    interpolants (K1b), and every vector of the dwell -- ragged last intervals of both spacings (300 = 2 x 128 + 44 =
+    9 x 32 + 12), batches that start inside a coarse interval -- must match the oracle like any other."""
+    w = _hetero_small(96, 64, 300)
+    ref = oracle_generate(w)
+    for batch in (0, 77):
+        with _sim(w, accumulate_mode="spectral", pulses_per_batch=batch) as sim:
+            got = sim.generate().cpu().numpy()
+            st = sim.stats()
+            part = sim.generate(131, 201).cpu().numpy()
+        assert st["geometry_keyframed"] == 1 and st["kinematics_keyframe"] == 32 and st["kinematics_coarse_keyframe"] == 128, st
+        _assert_parity(got, ref, f"decoupled keyframes, batch {batch}")
+        _assert_parity(part, ref[:, 131:201], "decoupled keyframes, pulse range")
+    with _sim(w, accumulate_mode="spectral", kinematics_keyframe=32) as sim:          # a forced spacing keeps one spacing
+        assert sim.stats()["kinematics_coarse_keyframe"] == 0
+        got1 = sim.generate().cpu().numpy()
+    _assert_parity(got1, ref, "one spacing")
+    assert rel_l2_per_vector(got, got1.astype(np.complex128)).max() < 2e-5
+
+
 def test_geometry_keyframes_on_and_off():
     """Spectral path: ranges / gains interpolated between the kinematics keyframes (moments_keyframed.cu, the
     default where sim_create's host guard admits it) against exact geometry at every pulse (moments.cu); both
