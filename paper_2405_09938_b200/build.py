@@ -36,11 +36,15 @@ def _stale(target: Path, deps) -> bool:
     return any(d.stat().st_mtime > t for d in deps)
 
 
-def build_library(force: bool = False, verbose: bool = False) -> Path:
+def build_library(force: bool = False, verbose: bool = False, with_checked_object: bool = False) -> Path:
     nvcc = os.environ.get("NVCC", "nvcc")
     headers = list(CSRC.glob("*.cuh")) + list(INCLUDE.glob("*.h")) + [Path(__file__)]
     OBJ.mkdir(exist_ok=True)
     jobs = []
+    if with_checked_object:                            # compiled beside the others (it is the longest job of the build)
+        src, obj = CSRC / "moments_keyframed.cu", OBJ / "moments_keyframed_checked.o"
+        if force or _stale(obj, [src] + headers):
+            jobs.append([nvcc, *NVCC_FLAGS, "-DHEEPS_CHECKED", "-I", str(INCLUDE), "-c", str(src), "-o", str(obj)])
     for src in sources():
         obj = OBJ / (src.stem + ".o")
         if force or _stale(obj, [src] + headers):
@@ -77,7 +81,7 @@ def build_checked_library() -> Path:
     """libheeps_sim_checked.so: the same library with the keyframed geometry kernel compiled with -DHEEPS_CHECKED (device-side
     bounds checks that trap).  Stands in for compute-sanitizer, which the GPU pool does not offer: run
     `HEEPS_SIM_LIBRARY=paper_2405_09938_b200/libheeps_sim_checked.so python tests/sanitizer_driver.py`."""
-    build_library()
+    build_library(with_checked_object=True)
     nvcc = os.environ.get("NVCC", "nvcc")
     src = CSRC / "moments_keyframed.cu"
     obj = OBJ / "moments_keyframed_checked.o"
