@@ -206,7 +206,9 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     const int cap = prm.k2k_cap;
     const int capT = C * cap + 2;                        // slots of one payload buffer: C x cap, + the store target of echoes without a slot
     // [2][capT] float2 weight | [2][capT] float y | [C][cap] u32 slot of every facet-echo | [C][span + 1] int histogram |
-    // [kThreads / 8][kScrTeam] float2 transposition scratch of stage C
+    // [kThreads / 8][kScrTeam] float2 transposition scratch of stage C (+ the threads' stray stashes) | stage C work list |
+    // [3][kThreads] float2 (am1, am2) | [3][kThreads] float2 (pq2, pq3): per-facet polynomial coefficients that are read
+    // once per facet and pulse and would otherwise be spilled (128 registers at 2 CTAs per SM)
     float2 *payload = reinterpret_cast<float2 *>(smem_raw);
     float *payload_y = reinterpret_cast<float *>(smem_raw + (size_t)2 * capT * 8);
     uint32_t *slots = reinterpret_cast<uint32_t *>(smem_raw + (size_t)2 * capT * 12);
@@ -215,6 +217,8 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     // work list of stage C, written at every sort: one item per slice of [smin, smax) of every channel, channels end to end:
     // {first slot | echoes << 13 (0: empty, or outside the sampling window), channel | moment-row index << 2}
     uint2 *items = reinterpret_cast<uint2 *>(scratch + (kThreads / 8) * kScrTeam);
+    float2 *amc = reinterpret_cast<float2 *>(items + C * (span + 1));    // [FPT][kThreads] tilt-modulation coefficients
+    float2 *pqc = amc + 3 * kThreads;                                    // [FPT][kThreads] (pq2, pq3) of the gain cubic
     const uint32_t no_slot = (0x7ffffu << 13) | (uint32_t)(C * cap);      // slice 0x7ffff (never matches), store target = the spare slot
 
     const int tile = blockIdx.x, j = j_first + blockIdx.y;
@@ -319,8 +323,8 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     constexpr int FL = kLut ? FPT : 1;                               // tabulated patterns: P and bq are complex, the imaginary parts
     float qi0[FL], qi1[FL], qi2[FL], qi3[FL], bqi[FL];
     float am0[FPT];
-    constexpr int FT = kTilt ? FPT : 1;
-    float am1[FT], am2[FT];                                          // |a_f|(s) = am0 + s (am1 + s am2) when tilt-modulated
+    // |a_f|(s) = am0 + s (am1 + s am2) when tilt-modulated: (am1, am2) of the thread's facets live in shared memory
+    // (amc[q][tid], one LDS.64 per facet and pulse; six registers less in the pulse loop)
     uint32_t xarg[FPT];
     int fidx[kSpeckleT ? FPT : 1];                                   // facet index (time-dependent speckle: one load per pulse)
     unsigned validmask = 0;
@@ -336,7 +340,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
         dla0[q] = dla[q] = 0.f;
         pq0[q] = pq1[q] = pq2[q] = pq3[q] = bq[q] = 0.f; am0[q] = 0.f; xarg[q] = 0u;
         if (kLut) qi0[q] = qi1[q] = qi2[q] = qi3[q] = bqi[q] = 0.f;
-        if (kTilt) am1[q] = am2[q] = 0.f;
+        if (kTilt) amc[q * NT + tid] = make_float2(0.f, 0.f);
         if (!valid) continue;
         const size_t f = (size_t)jj * prm.nx + i;
         const double xb = prm.cx + ((double)i - 0.5 * (prm.nx - 1)) * prm.spacing;
@@ -419,7 +423,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
             const float A0 = sqrtf(sig * fmaxf(1.f + 2.f * (sl0.x * lx + sl0.y * ly), 0.f) * area) * xmag;
             const float Am = sqrtf(sig * fmaxf(1.f + 2.f * (slm.x * lx + slm.y * ly), 0.f) * area) * xmag;
             const float A1 = sqrtf(sig * fmaxf(1.f + 2.f * (sl1.x * lx + sl1.y * ly), 0.f) * area) * xmag;
-            am0[q] = A0; am1[q] = -3.f * A0 + 4.f * Am - A1; am2[q] = 2.f * A0 - 4.f * Am + 2.f * A1;
+            am0[q] = A0; amc[q * NT + tid] = make_float2(-3.f * A0 + 4.f * Am - A1, 2.f * A0 - 4.f * Am + 2.f * A1);
         } else {
             am0[q] = sqrtf(sig * area) * xmag;
         }
@@ -461,9 +465,15 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
 #pragma unroll
     for (int q = 0; q < FPT; ++q) { dla0[q] *= to_g; dla[q] *= to_g; }    // now dG0, dGs
 
+#pragma unroll
+    for (int q = 0; q < FPT; ++q) pqc[q * NT + tid] = make_float2(pq2[q], pq3[q]);
     int my_kept = 0;
     const int sub = tid & 7, team = tid >> 3, warp = tid >> 5;
     float2 *scr = scratch + team * kScrTeam;
+    // the thread's stray stash: C float4 inside its team's transposition scratch (stage C of the same warp uses the
+    // scratch only after this pulse's barrier, the stash is written and read before it); quarter-warp conflict-free
+    static_assert((size_t)kScrTeam * sizeof(float2) >= 8 * (size_t)C * sizeof(float4) + 16, "stash does not fit the team scratch");
+    float4 *stash = reinterpret_cast<float4 *>((reinterpret_cast<uintptr_t>(scr) + 15) & ~(uintptr_t)15) + sub * C;
     const int capS = C * cap;                                            // slots of all channels (the spare one follows)
 
     // ---- The facet-echoes of the tile are ordered by range slice ONCE (counting sort at the interval's middle pulse:
@@ -597,15 +607,34 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
 
         // ---- A: slice, sub-slice position, complex weight of every facet-echo, written to the echo's slot.
         //      Branch-free straight-line code for all FPT x C echoes of the thread, so that the independent chains
-        //      (integer slice word -> MUFU -> stores) interleave.  Strays only set a bit; the rare ones are worked off
-        //      after the loop by evaluating that echo again.
-        unsigned stray_mask = 0;
+        //      (integer slice word -> MUFU -> stores) interleave.  A stray is written (one predicated STS.128) to the
+        //      thread's stash and appended to the pulse's list after the loop; a thread's second stray of one channel
+        //      in one pulse only sets a bit and is worked off after the loop by evaluating that echo again.  (Round 2:
+        //      re-evaluating every stray was 11 % of the kernel's instructions on the Large configuration.)
+        unsigned stray_mask = 0, stashed = 0;
+        // sorted at this very pulse and still no room in the list: the stray's eight moments straight to the rows
+        auto straight_to_the_rows = [&](const float4 e) {
+            const int code = __float_as_int(e.w), c = code >> 28, jb = code & 0x0fffffff;
+            float2 *row = a.mom + ((size_t)(c * n_pl + pl) * kKt) * a.nb_pad + jb;
+            float t0 = 1.f, t1 = e.z;
+            atomicAdd(row, make_float2(e.x, e.y));
+            atomicAdd(row + a.nb_pad, make_float2(e.x * t1, e.y * t1));
+            for (int k2 = 2; k2 < kKt; ++k2) {
+                const float t2k = 2.f * e.z * t1 - t0;
+                atomicAdd(row + (size_t)k2 * a.nb_pad, make_float2(e.x * t2k, e.y * t2k));
+                t0 = t1; t1 = t2k;
+            }
+            const int b = jb - (L - 1);
+            atomicMin(&s_blo[c], b); atomicMax(&s_bhi[c], b + 1);
+        };
         auto facet = [&](const int q, float &Pv, float &Pi, float &am, uint32_t &ph_ref, long long &X, float &gq, bool &keep) {
-            Pv = fmaf(s, fmaf(s, fmaf(s, pq3[q], pq2[q]), pq1[q]), pq0[q]);
+            const float2 p23 = pqc[q * NT + tid];
+            Pv = fmaf(s, fmaf(s, fmaf(s, p23.y, p23.x), pq1[q]), pq0[q]);
             Pi = kLut ? fmaf(s, fmaf(s, fmaf(s, qi3[kLut ? q : 0], qi2[kLut ? q : 0]), qi1[kLut ? q : 0]), qi0[kLut ? q : 0]) : 0.f;
             keep = ((validmask >> q) & 1u) && !(kLut ? (fmaf(Pv, Pv, Pi * Pi) < prm.cull_thr * prm.cull_thr)
                                                      : (fabsf(Pv) < prm.cull_thr));     // O7 (G6)
-            am = kTilt ? fmaf(s, fmaf(s, am2[kTilt ? q : 0], am1[kTilt ? q : 0]), am0[q]) : am0[q];
+            am = am0[q];
+            if (kTilt) { const float2 c12 = amc[q * NT + tid]; am = fmaf(s, fmaf(s, c12.y, c12.x), am); }
             uint32_t xa = xarg[q];
             if (kSpeckleT && ((validmask >> q) & 1u)) {   // time-dependent speckle: s_f(t_p) of this pulse (eq. (7), (10))
                 const uint2 xp = __ldg(a.xi_polar + (size_t)pl * a.xi_pulse_stride + (size_t)fidx[kSpeckleT ? q : 0]);
@@ -656,9 +685,23 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                 HEEPS_CHECK(pos <= (uint32_t)capS && (!here || pos < (uint32_t)capS));
                 pay[pos] = here ? make_float2(wr, wi) : make_float2(0.f, 0.f);
                 pay_y[pos] = yv;
-                // stray: left its sorted slice, or never had one; its window meets [0, Ns)
-                const bool stray = !here && keep && ((unsigned)(xh + 1 - kRhoBias) + (unsigned)(L - 1) < win_hi);
-                stray_mask |= stray ? (1u << (q * C + c)) : 0u;
+                // stray: left its sorted slice, or never had one; its window meets [0, Ns).  The thread's first stray of a
+                // channel goes to its stash (a facet that crosses a slice edge does so in every channel); any other sets a bit
+                const int jb = xh + 1 - kRhoBias + (L - 1);
+                const bool stray = !here && keep && ((unsigned)jb < win_hi);
+                const bool first = stray && !((stashed >> c) & 1u);
+                if (first) stash[c] = make_float4(wr, wi, yv, __int_as_float((c << 28) | jb));
+                stray_mask |= (stray && !first) ? (1u << (q * C + c)) : 0u;
+                stashed |= stray ? (1u << c) : 0u;
+            }
+        }
+        if (stashed) {
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+                if (!((stashed >> c) & 1u)) continue;
+                const int t = atomicAdd(n_stray, 1);
+                if (t < kStrayCap) s_stray[buf][t] = stash[c];
+                else if (sorted_at == ip) straight_to_the_rows(stash[c]);
             }
         }
         if (stray_mask) {
@@ -676,20 +719,9 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                     const int b = xh + 1 - kRhoBias;
                     const int t = atomicAdd(n_stray, 1);
                     HEEPS_CHECK(b + L - 1 >= 0 && b + L - 1 < a.nb_pad);
-                    if (t < kStrayCap) {
-                        s_stray[buf][t] = make_float4(wr, wi, yv, __int_as_float((c << 28) | (b + L - 1)));
-                    } else if (sorted_at == ip) {                          // sorted at this very pulse and still no room:
-                        float2 *row = a.mom + ((size_t)(c * n_pl + pl) * kKt) * a.nb_pad + (b + L - 1);   // straight to the rows
-                        float t0 = 1.f, t1 = yv;
-                        atomicAdd(row, make_float2(wr, wi));
-                        atomicAdd(row + a.nb_pad, make_float2(wr * t1, wi * t1));
-                        for (int k2 = 2; k2 < kKt; ++k2) {
-                            const float t2k = 2.f * yv * t1 - t0;
-                            atomicAdd(row + (size_t)k2 * a.nb_pad, make_float2(wr * t2k, wi * t2k));
-                            t0 = t1; t1 = t2k;
-                        }
-                        atomicMin(&s_blo[c], b); atomicMax(&s_bhi[c], b + 1);
-                    }
+                    const float4 e = make_float4(wr, wi, yv, __int_as_float((c << 28) | (b + L - 1)));
+                    if (t < kStrayCap) s_stray[buf][t] = e;
+                    else if (sorted_at == ip) straight_to_the_rows(e);
                 }
             }
         }
@@ -879,7 +911,8 @@ size_t moments_keyframed_smem_bytes(const DevParams &prm, int span_cap)
 {
     const size_t C = prm.n_channels;
     return (size_t)2 * (C * prm.k2k_cap + 2) * 12 + C * prm.k2k_cap * 4 + (size_t)hist_words((int)C, span_cap) * 4 +
-           (size_t)(kThreads / 8) * kScrTeam * sizeof(float2) + C * (size_t)(span_cap + 1) * sizeof(uint2);
+           (size_t)(kThreads / 8) * kScrTeam * sizeof(float2) + C * (size_t)(span_cap + 1) * sizeof(uint2) +
+           (size_t)6 * kThreads * sizeof(float2);
 }
 
 cudaError_t launch_moments_keyframed(const DevParams &prm, const MomentArgs &a, int p0, int n_pl, cudaStream_t s)
