@@ -111,6 +111,7 @@ __device__ __forceinline__ KeyEval key_eval(const PulseConst &pc, const double p
     return o;
 }
 
+constexpr int kSplitMin = 48;             // stage C: an item with fewer echoes is not split between two teams
 constexpr int kStrayCap = 96;             // stray echoes of one pulse held in shared memory (more: the tile is sorted again)
 constexpr int kScrRow = 9;                // float2 per thread row of the transposition scratch (8 moments + 1 pad)
 constexpr int kScrTeam = 8 * kScrRow;     // float2 per 8-thread team
@@ -170,6 +171,11 @@ __device__ __forceinline__ unsigned long long rho_ahead(unsigned long long f, lo
 }
 
 constexpr int kThreads = 256;
+// entries of stage C's work list: one per slice and channel, at least one per 8-thread team (split slices), even
+__host__ __device__ constexpr int item_words(int C, int span)
+{
+    return ((C * (span + 1) > kThreads / 8 ? C * (span + 1) : kThreads / 8) + 1) & ~1;
+}
 
 // Checked build (python -m paper_2405_09938_b200.build --checked: -DHEEPS_CHECKED, libheeps_sim_checked.so): every
 // computed shared-memory position and global moment-row index of this kernel is tested and a violation traps (the
@@ -217,7 +223,7 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
     // work list of stage C, written at every sort: one item per slice of [smin, smax) of every channel, channels end to end:
     // {first slot | echoes << 13 (0: empty, or outside the sampling window), channel | moment-row index << 2}
     uint2 *items = reinterpret_cast<uint2 *>(scratch + (kThreads / 8) * kScrTeam);
-    float2 *amc = reinterpret_cast<float2 *>(items + C * (span + 1));    // [FPT][kThreads] tilt-modulation coefficients
+    float2 *amc = reinterpret_cast<float2 *>(items + item_words(C, span));   // [FPT][kThreads] tilt-modulation coefficients
     float2 *pqc = amc + 3 * kThreads;                                    // [FPT][kThreads] (pq2, pq3) of the gain cubic
     const uint32_t no_slot = (0x7ffffu << 13) | (uint32_t)(C * cap);      // slice 0x7ffff (never matches), store target = the spare slot
 
@@ -581,6 +587,28 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                     HEEPS_CHECK(cnt == 0 || (first >= 0 && first + cnt <= cap && jb < a.nb_pad));
                     items[it] = make_uint2((uint32_t)(c * cap + first) | ((uint32_t)cnt << 13), (uint32_t)c | ((uint32_t)max(jb, 0) << 2));
                 }
+                // Fewer slices than 8-thread teams (a tile of the Large configuration: 18 slices of up to 220 echoes for 32
+                // teams): the fullest item is halved until every team has one (the halves add into the same moment row; the
+                // second half goes to the end of the list, i.e. to another warp).  The barrier of a pulse waits for the team
+                // with the longest item: 2.0 barrier-stall cycles per issue on Large before this (round 2).  All items were
+                // written by warp 0 when there are at most 32.
+                if (warp == 0 && total < kThreads / 8) {
+                    __syncwarp();
+                    uint2 my = (lane < total) ? items[lane] : make_uint2(0u, 0u);
+                    int n = total;
+                    while (n < kThreads / 8) {
+                        const unsigned best = __reduce_max_sync(0xffffffffu, ((my.x >> 13) << 5) | (unsigned)lane);
+                        const int bc = (int)(best >> 5), bl = (int)(best & 31u);
+                        if (bc < kSplitMin) break;
+                        const int h = ((bc >> 1) + 7) & ~7;                // the first half keeps whole octets
+                        const uint32_t sx = __shfl_sync(0xffffffffu, my.x, bl), sy = __shfl_sync(0xffffffffu, my.y, bl);
+                        if (lane == bl) my.x = (sx & 8191u) | ((uint32_t)h << 13);
+                        if (lane == n) { my.x = ((sx & 8191u) + (uint32_t)h) | ((uint32_t)(bc - h) << 13); my.y = sy; }
+                        ++n;
+                    }
+                    if (lane < n) items[lane] = my;
+                    if (lane == 0) s_nitems = n;
+                }
             }
 #pragma unroll
             for (int q = 0; q < FPT; ++q)
@@ -911,7 +939,7 @@ size_t moments_keyframed_smem_bytes(const DevParams &prm, int span_cap)
 {
     const size_t C = prm.n_channels;
     return (size_t)2 * (C * prm.k2k_cap + 2) * 12 + C * prm.k2k_cap * 4 + (size_t)hist_words((int)C, span_cap) * 4 +
-           (size_t)(kThreads / 8) * kScrTeam * sizeof(float2) + C * (size_t)(span_cap + 1) * sizeof(uint2) +
+           (size_t)(kThreads / 8) * kScrTeam * sizeof(float2) + (size_t)item_words((int)C, span_cap) * sizeof(uint2) +
            (size_t)6 * kThreads * sizeof(float2);
 }
 
