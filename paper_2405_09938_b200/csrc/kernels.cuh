@@ -31,6 +31,7 @@ struct KinematicsArgs {
     double2 *dxy_t;         // or null
 };
 cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a, int first, int n_rows, cudaStream_t s);
+int kinematics_coarse_row_slots(int n_rows);   // row slots a coarse-keyframe launch of n_rows pays for (kinematics.cu)
 // K1b -- keyframe rows at spacing H interpolated from K1's coarse rows at spacing H1 (kinematics.cu).
 struct SurfaceRefineArgs {
     const double *zc, *ztc;      // coarse rows [n_rows1][F]: height, its rate

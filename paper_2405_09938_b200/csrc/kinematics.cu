@@ -301,6 +301,14 @@ cudaError_t launch_surface_slope(const DevParams &prm, const SurfaceArgs &sa, co
     return cudaGetLastError();
 }
 
+// Row slots a launch of the second-derivative (coarse keyframe) rows pays for: blocks of four rows, or of three when
+// that wastes none (a block's spare rows recompute its last one).
+int kinematics_coarse_row_slots(int n_rows)
+{
+    const int groups = (n_rows + 3) / 4;
+    return n_rows <= 3 * groups ? 3 * groups : 4 * groups;
+}
+
 cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a_in, int first, int n_rows, cudaStream_t s)
 {
     if (n_rows <= 0) return cudaSuccess;
@@ -320,7 +328,16 @@ cudaError_t launch_kinematics(const DevParams &prm, const KinematicsArgs &a_in, 
     if (a.ztt) {                                       // second-derivative rows: 4 rows per block (register budget), no CWM
         if (!rate || choppy || (slope && !a.slope_t)) return cudaErrorInvalidValue;
         grid.z = (n_rows + 3) / 4;
-        if (a.nodes_x > 0) {
+        if (kinematics_coarse_row_slots(n_rows) == 3 * (int)grid.z) {   // <= 3, 5, 6 or 9 rows: blocks of three (fewer rows computed twice)
+            grid.z = (n_rows + 2) / 3;
+            if (a.nodes_x > 0) {
+                if (slope) launch(kinematics_kernel<3, true, false, true, true, true>);
+                else       launch(kinematics_kernel<3, false, false, true, true, true>);
+            } else {
+                if (slope) launch(kinematics_kernel<3, true, false, true, false, true>);
+                else       launch(kinematics_kernel<3, false, false, true, false, true>);
+            }
+        } else if (a.nodes_x > 0) {
             if (slope) launch(kinematics_kernel<4, true, false, true, true, true>);
             else       launch(kinematics_kernel<4, false, false, true, true, true>);
         } else {

@@ -1086,8 +1086,30 @@ int sim_create(const sim_instrument *in, const sim_geometry *g, const sim_scene 
     if (opts && opts->pulses_per_batch > 0) pb = opts->pulses_per_batch;
     pb = std::min(pb, P);
     if (!(opts && opts->pulses_per_batch > 0)) {        // balance the batches of a full-dwell call
+        const int pb_max = pb;
         const int nb = (P + pb - 1) / pb;
         pb = (P + nb - 1) / nb;
+        // Decoupled keyframes: every batch evaluates the coarse rows (spacing H1) that span it, four rows per thread block
+        // of K1 (three where that wastes none; a partial group costs a whole one), so batch boundaries on coarse keyframes
+        // save rows: Large, 2048 pulses, at most 900 per batch: 3 x 683 pulses = 3 x 7 rows = 24 row slots; 896 + 896 + 256
+        // = 8 + 8 + 3 rows = 19.
+        if (h->key_H1 > 0 && pb < P) {
+            auto row_slots = [&](int batch) {
+                int slots = 0;
+                for (int p0 = 0; p0 < P; p0 += batch) {
+                    int first = 0, rows = 0;
+                    surface_rows(h, p0, std::min(batch, P - p0), &first, &rows, h->key_H1);
+                    slots += kinematics_coarse_row_slots(rows);
+                }
+                return slots;
+            };
+            int best = pb, best_slots = row_slots(pb);
+            for (int cand = h->key_H1; cand <= pb_max; cand += h->key_H1) {
+                const int sl = row_slots(cand);
+                if (sl < best_slots || (sl == best_slots && cand > best)) { best = cand; best_slots = sl; }
+            }
+            pb = best;
+        }
     }
     h->pulses_per_batch = pb;
 
