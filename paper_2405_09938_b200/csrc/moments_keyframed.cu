@@ -606,7 +606,11 @@ moments_keyframed_kernel(DevParams prm, MomentArgs a, int p0, int n_pl, int j_fi
                         if (lane == n) { my.x = ((sx & 8191u) + (uint32_t)h) | ((uint32_t)(bc - h) << 13); my.y = sy; }
                         ++n;
                     }
-                    if (lane < n) items[lane] = my;
+                    // longest first: the four teams of a warp run their items in step, so a warp should hold items of like length
+                    const unsigned mykey = ((my.x >> 13) << 5) | (unsigned)(31 - lane);
+                    int rank = 0;
+                    for (int o = 0; o < kThreads / 8; ++o) rank += (__shfl_sync(0xffffffffu, mykey, o) > mykey) ? 1 : 0;
+                    if (lane < n) items[rank] = my;
                     if (lane == 0) s_nitems = n;
                 }
             }
