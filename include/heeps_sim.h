@@ -131,7 +131,8 @@ typedef struct {
 /* Tunables; zero-initialise for defaults. */
 typedef struct {
     int32_t tile_facets;           /* spatial tile side in facets (4..64, power of 2; SPECTRAL clamps to 32); 0 = auto */
-    int32_t pulses_per_batch;      /* 0 = auto from workspace_bytes */
+    int32_t pulses_per_batch;      /* 0 = auto from workspace_bytes (balanced over the dwell; with decoupled keyframes the batch
+                                      boundaries are put on coarse keyframes where that saves keyframe rows) */
     int64_t workspace_bytes;       /* cap for per-batch device workspace; 0 = 16 GiB, at most a quarter of the free device memory */
     int32_t accumulate_mode;       /* SIM_ACCUMULATE_*; SPECTRAL where it does not apply -> SIM_EINVAL */
     int32_t kinematics_keyframe;   /* wave sums evaluated exactly every H-th pulse (with time derivatives) and
